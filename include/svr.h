@@ -1,0 +1,140 @@
+/* svr.h - C ABI of the B200-native differentiable sparse-voxel tile rasterizer (libsvr.so).
+ *
+ * The hot path of LiteVoxel's training loop (arXiv 2511.02510; "P:n" = line n of the paper text):
+ * "we project, rasterize, measure a photometric objective, and back-propagate", with the
+ * per-voxel maximum blending weight w_max gathered during rasterization (eq. 5).
+ * The paper states the rasterizer only through eqs. 1-5; everything it is silent on is fixed by
+ * the readings R1-R10 and the binning specification B1-B4 in DESIGN.md, which the CPU oracle follows too.
+ *
+ * Conventions
+ *  - Every array pointer is a DEVICE pointer owned by the caller unless the parameter name ends in
+ *    `_host`. The library never frees caller memory.
+ *  - Every call enqueues its kernels on the context's stream and returns without synchronising, except
+ *    svr_preprocess (one 8-byte device->host read of the entry count, which sizes the sort buffers) and
+ *    the *_host entry points (they return when the host outputs are valid).
+ *  - Calls return an SvrStatus; svr_last_error gives the detail string. On error no output buffer
+ *    holds a valid result.
+ *  - Workspace (rectangles, keys, sorted lists, per-view colours) comes from a stream-ordered pool owned
+ *    by the context; svr_create's `workspace_budget_bytes` (0 = unlimited) bounds it: a request that
+ *    would exceed it fails with SVR_ERR_WORKSPACE before anything is launched for that request.
+ *  - There is no CPU fallback: with no usable CUDA device svr_create fails with SVR_ERR_CUDA.
+ */
+#ifndef SVR_H_
+#define SVR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct SvrContext SvrContext; /* stream, workspace pool, counters, last error */
+typedef struct SvrFrame SvrFrame;     /* one (scene, camera) view: rects, per-view colours, sorted tile lists */
+
+typedef enum {
+    SVR_OK = 0,
+    SVR_ERR_INVALID_ARG = 1,
+    SVR_ERR_CUDA = 2,
+    SVR_ERR_WORKSPACE = 3,  /* workspace budget exceeded */
+    SVR_ERR_UNSUPPORTED = 4 /* e.g. tile bits + 3 + 3*max_level > 64, K > 4, sh_degree > 3 */
+} SvrStatus;
+
+/* Sparse voxel octree leaves. Level-L edge = root_edge / 2^L (R1), lo = root_lo + (ix,iy,iz)*edge.
+ * Leaves must be pairwise interior-disjoint. */
+typedef struct {
+    int64_t n;
+    int32_t sh_degree;        /* 0..3 */
+    int32_t max_level;        /* Lmax >= every level; Morton codes use 3*Lmax bits */
+    float root_lo[3];
+    float root_edge;          /* power of two */
+    const uint16_t* ijkl;     /* [n,4] ix, iy, iz, level */
+    const float* raw_density; /* [n,8] corner c = bx + 2*by + 4*bz; density = exp(trilinear(raw)) (R5) */
+    const float* sh;          /* [n,(D+1)^2,3] real SH coefficients, basis index i = l(l+1)+m (R6) */
+} SvrVoxels;
+
+/* Pinhole camera, OpenCV axes: p_cam = R p_world + t (R2); ray through pixel centre (x+.5, y+.5) (eq. 1). */
+typedef struct {
+    int32_t W, H;             /* <= 65535 */
+    float fx, fy, cx, cy;
+    float R[9];               /* row-major */
+    float t[3];
+    float z_near;             /* B1 straddle rule; typical 0.01 */
+    float bg[3];              /* background colour, composited as T_K * bg (R7) */
+} SvrCamera;
+
+typedef struct {
+    int32_t K;                /* 1..4 midpoint samples per ray segment (R5) */
+    float T_min;              /* a ray stops after the first voxel that leaves T < T_min (R8); 0 = never */
+} SvrRenderOpts;
+
+typedef struct {
+    float eps;                /* eq. 7, 1e-3 */
+    float percentile;         /* q of the percentile-normalised Sobel magnitude (R10), e.g. 0.99 */
+    int32_t sobel_source;     /* 0 = target image (default reading), 1 = render */
+} SvrLossOpts;
+
+SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t workspace_budget_bytes);
+void svr_destroy(SvrContext* ctx);
+const char* svr_last_error(const SvrContext* ctx);
+/* High-water mark of the context's workspace pool, bytes (peak VRAM the library itself held). */
+size_t svr_workspace_peak_bytes(const SvrContext* ctx);
+/* Number of this library's kernels launched on the context so far (bench.py's gpu_launches). */
+int64_t svr_kernel_launches(const SvrContext* ctx);
+
+/* (1)+(2) of the path: per-voxel projection to pixel rectangles and tile-overlap counts (B1), per-view SH
+ * colour c_v (R6), key build (tile | direction octant | direction-flipped Morton code, B3), device radix
+ * sort, per-(tile,octant) ranges (B4). The frame borrows `vox` pointers: keep them alive and the topology
+ * (ijkl) unchanged until svr_frame_release; raw_density / sh VALUES are re-read by forward/backward.
+ * svr_frame_refresh_colors recomputes c_v after sh changed without redoing the lists. */
+SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam, SvrFrame** out);
+SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame);
+void svr_frame_release(SvrContext* ctx, SvrFrame* frame);
+
+/* (3) forward compositing, eqs. 2-4: image[H,W,3] = sum_k w_k c_k + T_K bg; depth[H,W] =
+ * sum_k w_k t_mid,k (R7); T_final[H,W]; w_max[n] (eq. 5) is MAX-accumulated in place (caller zeroes;
+ * never-hit voxels stay 0). depth, T_final, w_max may be NULL. */
+SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts,
+                      float* image, float* depth, float* T_final, float* w_max);
+
+/* (5) LF-weighted photometric loss and its gradient, eqs. 7-10, eq. 18:
+ * dL_dimage[H,W,3] = w~(p) sign(R-I) / (3 |P|); *loss (device float) = L_LF. gamma = gamma(t), eq. 9. */
+SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H,
+                        float gamma, const SvrLossOpts* opts, float* dL_dimage, float* loss);
+
+/* (4) backward compositing: gradients of sum(dL_dimage * image) w.r.t. corner raw densities and SH
+ * coefficients. `image` is svr_forward's output for this frame (the suffix colour is image - prefix).
+ * grad_raw_density[n,8] and grad_sh[n,(D+1)^2,3] ACCUMULATE (+=; caller zeroes) so several views sum
+ * into one buffer; w_max as in svr_forward (may be NULL). */
+SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts,
+                       const float* dL_dimage, const float* image,
+                       float* grad_raw_density, float* grad_sh, float* w_max);
+
+/* One whole training-view step with HOST inputs/outputs (bench.py's e2e leg): copies camera + target image
+ * host->device, runs preprocess -> forward -> loss_grad -> backward on device-resident voxel parameters and
+ * gradient buffers, copies the loss (and, if image_host != NULL, the render) device->host, and returns
+ * when they are valid. target_host / image_host: [H,W,3] floats (pinned memory recommended). */
+SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam_host,
+                              const SvrRenderOpts* ropts, const SvrLossOpts* lopts, float gamma,
+                              const float* target_host, float* grad_raw_density, float* grad_sh, float* w_max,
+                              float* loss_host, float* image_host);
+
+/* Inspection hooks for the bit-exact binning checks (device pointers valid until svr_frame_release):
+ * keys[E] canonical (tile << (3+3Lmax)) | (octant << 3Lmax) | (morton ^ flip), vals[E] voxel ids,
+ * ranges[n_tiles,8,2] = [start,end) ((0,0) if empty), rects[n,4] = x0,y0,x1,y1 pixels inclusive
+ * (culled: 65535,65535,0,0), tile_masks[n_tiles] octant sets. Any out pointer may be NULL. */
+SvrStatus svr_frame_lists(const SvrFrame* frame, const uint64_t** keys, const uint32_t** vals, int64_t* n_entries,
+                          const uint32_t** ranges, const uint16_t** rects, const uint8_t** tile_masks);
+/* Per-view voxel colours [n,4]: r,g,b and the clamp mask bits (as float bits) - debugging / tests. */
+SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm);
+
+/* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
+SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);
+
+/* eq. 9: 0 for t < t0, linear to gamma_max at t1, then gamma_max. Host function. */
+float svr_gamma_schedule(float t, float T, float t0_frac, float t1_frac, float gamma_max);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SVR_H_ */

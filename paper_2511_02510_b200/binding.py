@@ -1,0 +1,285 @@
+"""ctypes binding of libsvr.so - argument marshalling only (include/svr.h is the contract).
+
+PyTorch is used for device memory and streams; every step of the path runs in the library's kernels.
+There is no fallback: if libsvr.so is missing or cannot be loaded, importing this module raises.
+Function names mirror the C ABI (svr_create, svr_preprocess, svr_forward, svr_loss_grad, svr_backward, ...).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libsvr.so")
+
+SVR_OK, SVR_ERR_INVALID_ARG, SVR_ERR_CUDA, SVR_ERR_WORKSPACE, SVR_ERR_UNSUPPORTED = range(5)
+_STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR_WORKSPACE", 4: "SVR_ERR_UNSUPPORTED"}
+
+EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
+           "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
+           "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule"]
+
+
+class SvrError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class SvrVoxels(C.Structure):
+    _fields_ = [("n", C.c_int64), ("sh_degree", C.c_int32), ("max_level", C.c_int32), ("root_lo", C.c_float * 3),
+                ("root_edge", C.c_float), ("ijkl", C.c_void_p), ("raw_density", C.c_void_p), ("sh", C.c_void_p)]
+
+
+class SvrCamera(C.Structure):
+    _fields_ = [("W", C.c_int32), ("H", C.c_int32), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float),
+                ("cy", C.c_float), ("R", C.c_float * 9), ("t", C.c_float * 3), ("z_near", C.c_float), ("bg", C.c_float * 3)]
+
+
+class SvrRenderOpts(C.Structure):
+    _fields_ = [("K", C.c_int32), ("T_min", C.c_float)]
+
+
+class SvrLossOpts(C.Structure):
+    _fields_ = [("eps", C.c_float), ("percentile", C.c_float), ("sobel_source", C.c_int32)]
+
+
+def _load():
+    if not os.path.exists(_SO):
+        raise ImportError(f"{_SO} is missing: build it with `python -m paper_2511_02510_b200._build` "
+                          "(nvcc, sm_100a). There is no CPU or PyTorch fallback.")
+    lib = C.CDLL(_SO)
+    lib.svr_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.c_size_t]
+    lib.svr_destroy.argtypes = [C.c_void_p]
+    lib.svr_destroy.restype = None
+    lib.svr_last_error.argtypes = [C.c_void_p]
+    lib.svr_last_error.restype = C.c_char_p
+    lib.svr_workspace_peak_bytes.argtypes = [C.c_void_p]
+    lib.svr_workspace_peak_bytes.restype = C.c_size_t
+    lib.svr_kernel_launches.argtypes = [C.c_void_p]
+    lib.svr_kernel_launches.restype = C.c_int64
+    lib.svr_preprocess.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.POINTER(SvrCamera), C.POINTER(C.c_void_p)]
+    lib.svr_frame_refresh_colors.argtypes = [C.c_void_p, C.c_void_p]
+    lib.svr_frame_release.argtypes = [C.c_void_p, C.c_void_p]
+    lib.svr_frame_release.restype = None
+    lib.svr_forward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 4
+    lib.svr_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_float,
+                                  C.POINTER(SvrLossOpts), C.c_void_p, C.c_void_p]
+    lib.svr_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 5
+    lib.svr_train_view_host.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.POINTER(SvrCamera), C.POINTER(SvrRenderOpts),
+                                        C.POINTER(SvrLossOpts), C.c_float] + [C.c_void_p] * 6
+    lib.svr_frame_lists.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 2 + [C.POINTER(C.c_int64)] + [C.POINTER(C.c_void_p)] * 3
+    lib.svr_frame_colors.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+    lib.svr_copy_to_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]
+    lib.svr_gamma_schedule.argtypes = [C.c_float] * 5
+    lib.svr_gamma_schedule.restype = C.c_float
+    return lib
+
+
+_lib = _load()
+
+
+def lib():
+    return _lib
+
+
+def _p(t: Optional[torch.Tensor]):
+    return C.c_void_p(0) if t is None else C.c_void_p(t.data_ptr())
+
+
+def _dev(t: torch.Tensor, dtype, name: str):
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise ValueError(f"{name} must be a contiguous CUDA tensor of dtype {dtype}")
+    return t
+
+
+def make_camera(cam) -> SvrCamera:
+    """From any object with W,H,fx,fy,cx,cy,R,t,z_near,bg attributes (e.g. svr_inputs.Camera)."""
+    c = SvrCamera()
+    c.W, c.H = int(cam.W), int(cam.H)
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    c.R = (C.c_float * 9)(*[float(x) for x in np.asarray(cam.R, dtype=np.float32).reshape(-1)])
+    c.t = (C.c_float * 3)(*[float(x) for x in np.asarray(cam.t, dtype=np.float32)])
+    c.z_near = float(cam.z_near)
+    c.bg = (C.c_float * 3)(*[float(x) for x in np.asarray(cam.bg, dtype=np.float32)])
+    return c
+
+
+class Voxels:
+    """Device-resident voxel arrays + the C struct pointing at them."""
+
+    def __init__(self, ijkl: torch.Tensor, raw: torch.Tensor, sh: torch.Tensor, sh_degree: int, max_level: int,
+                 root_lo, root_edge: float):
+        self.ijkl = _dev(ijkl, torch.int16, "ijkl")          # uint16 bit patterns
+        self.raw = _dev(raw, torch.float32, "raw")
+        self.sh = _dev(sh, torch.float32, "sh")
+        self.n = int(ijkl.shape[0])
+        self.sh_degree, self.max_level = int(sh_degree), int(max_level)
+        assert raw.shape == (self.n, 8) and sh.shape == (self.n, (sh_degree + 1) ** 2, 3) and ijkl.shape == (self.n, 4)
+        s = SvrVoxels()
+        s.n, s.sh_degree, s.max_level = self.n, self.sh_degree, self.max_level
+        s.root_lo = (C.c_float * 3)(*[float(x) for x in root_lo])
+        s.root_edge = float(root_edge)
+        s.ijkl, s.raw_density, s.sh = self.ijkl.data_ptr(), self.raw.data_ptr(), self.sh.data_ptr()
+        self.c = s
+
+    @staticmethod
+    def from_scene(scene, device="cuda:0") -> "Voxels":
+        ijkl = torch.from_numpy(np.ascontiguousarray(scene.ijkl).view(np.int16)).to(device)
+        raw = torch.from_numpy(np.ascontiguousarray(scene.raw, dtype=np.float32)).to(device)
+        sh = torch.from_numpy(np.ascontiguousarray(scene.sh, dtype=np.float32)).to(device)
+        return Voxels(ijkl, raw, sh, scene.sh_degree, scene.max_level, scene.root_lo, scene.root_edge)
+
+
+class Frame:
+    def __init__(self, ctx: "Context", handle: int, vox: Voxels, cam: SvrCamera):
+        self.ctx, self.handle, self.vox, self.cam = ctx, handle, vox, cam
+        self.W, self.H = cam.W, cam.H
+
+    def release(self):
+        if self.handle:
+            _lib.svr_frame_release(self.ctx.handle, C.c_void_p(self.handle))
+            self.handle = 0
+
+    def __del__(self):
+        try:
+            self.release()
+        except Exception:
+            pass
+
+    def lists(self):
+        """Copies of the inspection buffers as NumPy arrays (tests)."""
+        keys, vals, ranges, rects, masks = (C.c_void_p() for _ in range(5))
+        n = C.c_int64()
+        self.ctx._check(_lib.svr_frame_lists(C.c_void_p(self.handle), C.byref(keys), C.byref(vals), C.byref(n),
+                                             C.byref(ranges), C.byref(rects), C.byref(masks)))
+        self.ctx.synchronize()
+        E = int(n.value)
+        n_tiles = ((self.W + 15) // 16) * ((self.H + 15) // 16)
+
+        def grab(ptr, count, dtype):
+            out = np.empty(count, dtype=dtype)
+            if count:
+                self.ctx._check(_lib.svr_copy_to_host(self.ctx.handle, out.ctypes.data, ptr, out.nbytes))
+            return out
+        return dict(keys=grab(keys, E, np.uint64), vals=grab(vals, E, np.uint32),
+                    ranges=grab(ranges, n_tiles * 16, np.uint32).reshape(n_tiles, 8, 2),
+                    rects=grab(rects, self.vox.n * 4, np.uint16).reshape(self.vox.n, 4),
+                    tile_masks=grab(masks, n_tiles, np.uint8), n_entries=E)
+
+    def colors(self) -> np.ndarray:
+        p = C.c_void_p()
+        self.ctx._check(_lib.svr_frame_colors(C.c_void_p(self.handle), C.byref(p)))
+        self.ctx.synchronize()
+        out = np.empty(self.vox.n * 4, dtype=np.float32)
+        if self.vox.n:
+            self.ctx._check(_lib.svr_copy_to_host(self.ctx.handle, out.ctypes.data, p, out.nbytes))
+        return out.reshape(self.vox.n, 4)
+
+
+
+
+class Context:
+    """One library context bound to a device and a stream (default: torch's current stream)."""
+
+    def __init__(self, device: int = 0, stream: Optional[torch.cuda.Stream] = None, workspace_budget_bytes: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2511_02510_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        torch.cuda.set_device(device)
+        self.device = device
+        self.stream = stream if stream is not None else torch.cuda.current_stream(device)
+        h = C.c_void_p()
+        st = _lib.svr_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream), workspace_budget_bytes)
+        if st != SVR_OK:
+            raise SvrError(st, "svr_create failed")
+        self.handle = h
+
+    def close(self):
+        if self.handle:
+            _lib.svr_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != SVR_OK:
+            raise SvrError(st, _lib.svr_last_error(self.handle).decode())
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    @property
+    def workspace_peak_bytes(self) -> int:
+        return int(_lib.svr_workspace_peak_bytes(self.handle))
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(_lib.svr_kernel_launches(self.handle))
+
+    # ---- the four calls of the path -------------------------------------------------------------
+    def svr_preprocess(self, vox: Voxels, cam) -> Frame:
+        c = cam if isinstance(cam, SvrCamera) else make_camera(cam)
+        h = C.c_void_p()
+        self._check(_lib.svr_preprocess(self.handle, C.byref(vox.c), C.byref(c), C.byref(h)))
+        return Frame(self, h.value, vox, c)
+
+    def svr_forward(self, frame: Frame, K: int, T_min: float = 1e-5, w_max: Optional[torch.Tensor] = None,
+                    image=None, depth=None, T_final=None, want_aux: bool = True):
+        dev = frame.vox.raw.device
+        if image is None:
+            image = torch.empty((frame.H, frame.W, 3), dtype=torch.float32, device=dev)
+        if want_aux:
+            if depth is None:
+                depth = torch.empty((frame.H, frame.W), dtype=torch.float32, device=dev)
+            if T_final is None:
+                T_final = torch.empty((frame.H, frame.W), dtype=torch.float32, device=dev)
+        o = SvrRenderOpts(K, T_min)
+        self._check(_lib.svr_forward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(image), _p(depth), _p(T_final), _p(w_max)))
+        return image, depth, T_final
+
+    def svr_loss_grad(self, render: torch.Tensor, target: torch.Tensor, gamma: float, eps: float = 1e-3,
+                      percentile: float = 0.99, sobel_source: int = 0, dL=None, loss=None):
+        H, W = int(render.shape[0]), int(render.shape[1])
+        _dev(render, torch.float32, "render")
+        _dev(target, torch.float32, "target")
+        if dL is None:
+            dL = torch.empty_like(render)
+        if loss is None:
+            loss = torch.empty(1, dtype=torch.float32, device=render.device)
+        o = SvrLossOpts(eps, percentile, sobel_source)
+        self._check(_lib.svr_loss_grad(self.handle, _p(render), _p(target), W, H, gamma, C.byref(o), _p(dL), _p(loss)))
+        return dL, loss
+
+    def svr_backward(self, frame: Frame, K: int, dL: torch.Tensor, image: torch.Tensor, grad_raw: torch.Tensor,
+                     grad_sh: torch.Tensor, T_min: float = 1e-5, w_max: Optional[torch.Tensor] = None):
+        _dev(dL, torch.float32, "dL")
+        _dev(image, torch.float32, "image")
+        _dev(grad_raw, torch.float32, "grad_raw")
+        _dev(grad_sh, torch.float32, "grad_sh")
+        o = SvrRenderOpts(K, T_min)
+        self._check(_lib.svr_backward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(image), _p(grad_raw),
+                                      _p(grad_sh), _p(w_max)))
+
+    def svr_train_view_host(self, vox: Voxels, cam, K: int, gamma: float, target_host: torch.Tensor, grad_raw, grad_sh,
+                            w_max=None, T_min: float = 1e-5, eps: float = 1e-3, percentile: float = 0.99,
+                            sobel_source: int = 0, image_host: Optional[torch.Tensor] = None) -> float:
+        c = cam if isinstance(cam, SvrCamera) else make_camera(cam)
+        assert not target_host.is_cuda and target_host.dtype == torch.float32 and target_host.is_contiguous()
+        ro, lo = SvrRenderOpts(K, T_min), SvrLossOpts(eps, percentile, sobel_source)
+        loss = C.c_float()
+        self._check(_lib.svr_train_view_host(self.handle, C.byref(vox.c), C.byref(c), C.byref(ro), C.byref(lo), gamma,
+                                             _p(target_host), _p(grad_raw), _p(grad_sh), _p(w_max),
+                                             C.cast(C.byref(loss), C.c_void_p), _p(image_host)))
+        return float(loss.value)
+
+
+def svr_gamma_schedule(t: float, T: float, t0_frac: float = 0.3, t1_frac: float = 0.6, gamma_max: float = 0.6) -> float:
+    return float(_lib.svr_gamma_schedule(t, T, t0_frac, t1_frac, gamma_max))

@@ -1,0 +1,357 @@
+// Stage (1)+(2) kernels: tile octant masks, per-voxel pixel rectangles and entry counts, key emission,
+// per-(tile,octant) ranges, per-view SH colours. Integer outputs are bit-exact against the binning
+// specification B1-B4 in DESIGN.md: all fp32 arithmetic that decides an integer uses __f*_rn intrinsics
+// (never contracted to FMA) in the specified order.
+#include "svr_internal.cuh"
+
+namespace {
+
+constexpr int BIG_THRESHOLD = 48;   // voxels with more list entries than this are emitted by a whole CTA
+
+// ---- B2: octant set of every tile ---------------------------------------------------------------
+__global__ void __launch_bounds__(256) tile_mask_kernel(CamDev c, uint8_t* __restrict__ masks) {
+    __shared__ unsigned int m;
+    if (threadIdx.x == 0 && threadIdx.y == 0) m = 0;
+    __syncthreads();
+    int x = blockIdx.x * SVR_TILE + threadIdx.x, y = blockIdx.y * SVR_TILE + threadIdx.y;
+    unsigned int mine = 0;
+    if (x < c.W && y < c.H) mine = 1u << pixel_octant_dev(c, x, y);
+    mine = __reduce_or_sync(0xffffffffu, mine);
+    if (((threadIdx.y * SVR_TILE + threadIdx.x) & 31) == 0) atomicOr(&m, mine);
+    __syncthreads();
+    if (threadIdx.x == 0 && threadIdx.y == 0) masks[blockIdx.y * c.tiles_x + blockIdx.x] = (uint8_t)m;
+}
+
+// Summed-area table of popcount(mask): sat[j*(tx+1)+i] = entries of one voxel covering tiles [0,i) x [0,j).
+__global__ void sat_kernel(const uint8_t* __restrict__ masks, uint32_t* __restrict__ sat, int tx, int ty) {
+    int sx = tx + 1;
+    for (int i = threadIdx.x; i <= tx; i += blockDim.x) sat[i] = 0;
+    for (int j = threadIdx.x; j < ty; j += blockDim.x) {      // row prefix sums
+        uint32_t run = 0;
+        sat[(j + 1) * sx] = 0;
+        for (int i = 0; i < tx; ++i) {
+            run += __popc((unsigned)masks[j * tx + i]);
+            sat[(j + 1) * sx + i + 1] = run;
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= tx; i += blockDim.x) {      // column prefix sums
+        uint32_t run = 0;
+        for (int j = 1; j <= ty; ++j) {
+            run += sat[j * sx + i];
+            sat[j * sx + i] = run;
+        }
+    }
+}
+
+__device__ __forceinline__ uint32_t sat_query(const uint32_t* __restrict__ sat, int sx, int i0, int j0, int i1, int j1) {
+    // tiles [i0, i1) x [j0, j1)
+    return sat[j1 * sx + i1] - sat[j0 * sx + i1] - sat[j1 * sx + i0] + sat[j0 * sx + i0];
+}
+
+// ---- B1: pixel rectangle of a voxel ---------------------------------------------------------------
+__device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c, uint2 q) {
+    const ushort4 culled = make_ushort4(0xFFFF, 0xFFFF, 0, 0);
+    int L = q.y >> 16;
+    float e = __fmul_rn(s.root_edge, __int_as_float((127 - L) << 23));
+    float lo[3], hi[3];
+    lo[0] = __fadd_rn(s.root_lo[0], __fmul_rn((float)(q.x & 0xFFFF), e));
+    lo[1] = __fadd_rn(s.root_lo[1], __fmul_rn((float)(q.x >> 16), e));
+    lo[2] = __fadd_rn(s.root_lo[2], __fmul_rn((float)(q.y & 0xFFFF), e));
+#pragma unroll
+    for (int a = 0; a < 3; ++a) hi[a] = __fadd_rn(lo[a], e);
+    float X[8], Y[8], Z[8];
+    float zmin = 0.f, zmax = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        float Px = (k & 1) ? hi[0] : lo[0], Py = (k & 2) ? hi[1] : lo[1], Pz = (k & 4) ? hi[2] : lo[2];
+        X[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.R[0], Px), __fmul_rn(c.R[1], Py)), __fmul_rn(c.R[2], Pz)), c.t[0]);
+        Y[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.R[3], Px), __fmul_rn(c.R[4], Py)), __fmul_rn(c.R[5], Pz)), c.t[1]);
+        Z[k] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(c.R[6], Px), __fmul_rn(c.R[7], Py)), __fmul_rn(c.R[8], Pz)), c.t[2]);
+        if (k == 0) { zmin = zmax = Z[k]; }
+        else { zmin = fminf(zmin, Z[k]); zmax = fmaxf(zmax, Z[k]); }
+    }
+    if (!(zmax > 0.0f)) return culled;
+    float Wf = (float)c.W, Hf = (float)c.H;
+    if (zmin < c.z_near) {
+        float cxw = __fsub_rn(c.cx, Wf), cyh = __fsub_rn(c.cy, Hf);
+        bool allL = true, allR = true, allT = true, allB = true;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            float a0 = __fmul_rn(c.fx, X[k]), b0 = __fmul_rn(c.fy, Y[k]);
+            allL = allL && (__fadd_rn(a0, __fmul_rn(c.cx, Z[k])) < 0.0f);
+            allR = allR && (__fadd_rn(a0, __fmul_rn(cxw, Z[k])) >= 0.0f);
+            allT = allT && (__fadd_rn(b0, __fmul_rn(c.cy, Z[k])) < 0.0f);
+            allB = allB && (__fadd_rn(b0, __fmul_rn(cyh, Z[k])) >= 0.0f);
+        }
+        if (allL || allR || allT || allB) return culled;
+        return make_ushort4(0, 0, (unsigned short)(c.W - 1), (unsigned short)(c.H - 1));
+    }
+    float u0 = 0.f, u1 = 0.f, v0 = 0.f, v1 = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        float u = __fadd_rn(__fmul_rn(c.fx, __fdiv_rn(X[k], Z[k])), c.cx);
+        float w = __fadd_rn(__fmul_rn(c.fy, __fdiv_rn(Y[k], Z[k])), c.cy);
+        if (k == 0) { u0 = u1 = u; v0 = v1 = w; }
+        else { u0 = fminf(u0, u); u1 = fmaxf(u1, u); v0 = fminf(v0, w); v1 = fmaxf(v1, w); }
+    }
+    if (u1 < 0.0f || u0 >= Wf || v1 < 0.0f || v0 >= Hf) return culled;
+    ushort4 r;
+    r.x = (unsigned short)(int)floorf(fmaxf(u0, 0.0f));
+    r.z = (unsigned short)(int)floorf(fminf(u1, __fsub_rn(Wf, 1.0f)));
+    r.y = (unsigned short)(int)floorf(fmaxf(v0, 0.0f));
+    r.w = (unsigned short)(int)floorf(fminf(v1, __fsub_rn(Hf, 1.0f)));
+    return r;
+}
+
+__global__ void __launch_bounds__(256) rect_count_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ sat,
+                                                         ushort4* __restrict__ rects, uint32_t* __restrict__ counts,
+                                                         unsigned long long* __restrict__ totals) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v > s.n) return;
+    if (v == s.n) { counts[v] = 0; return; }
+    uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+    ushort4 r = voxel_rect(s, c, q);
+    rects[v] = r;
+    uint32_t cnt = 0;
+    if (r.x <= r.z)
+        cnt = sat_query(sat, c.tiles_x + 1, r.x >> 4, r.y >> 4, (r.z >> 4) + 1, (r.w >> 4) + 1);
+    counts[v] = cnt;
+    if (cnt > BIG_THRESHOLD) atomicAdd(&totals[1], 1ULL);
+}
+
+// ---- B3: keys ---------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t part1by2(uint64_t x) {
+    x &= 0x1fffffULL;
+    x = (x | x << 32) & 0x1f00000000ffffULL;
+    x = (x | x << 16) & 0x1f0000ff0000ffULL;
+    x = (x | x << 8) & 0x100f00f00f00f00fULL;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ULL;
+    x = (x | x << 2) & 0x1249249249249249ULL;
+    return x;
+}
+
+__device__ __forceinline__ uint64_t voxel_code(uint2 q, int Lm) {
+    int sh = Lm - (int)(q.y >> 16);
+    return part1by2((uint64_t)(q.x & 0xFFFF) << sh) | (part1by2((uint64_t)(q.x >> 16) << sh) << 1) |
+           (part1by2((uint64_t)(q.y & 0xFFFF) << sh) << 2);
+}
+
+__device__ __forceinline__ uint64_t flip_mask(int o, int Lm) {
+    uint64_t xm = 0x1249249249249249ULL & ((Lm >= 21) ? ~0ULL : ((1ULL << (3 * Lm)) - 1ULL));
+    return ((o & 1) ? xm : 0ULL) | ((o & 2) ? xm << 1 : 0ULL) | ((o & 4) ? xm << 2 : 0ULL);
+}
+
+__device__ __forceinline__ void emit_tile(uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, uint32_t pos,
+                                          uint32_t tile, unsigned mask, uint64_t code, int Lm, uint32_t v) {
+    while (mask) {
+        int o = __ffs(mask) - 1;
+        mask &= mask - 1;
+        keys[pos] = ((uint64_t)tile << (3 + 3 * Lm)) | ((uint64_t)o << (3 * Lm)) | (code ^ flip_mask(o, Lm));
+        vals[pos] = v;
+        ++pos;
+    }
+}
+
+__global__ void __launch_bounds__(256) emit_small_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                         const uint32_t* __restrict__ offsets, const uint8_t* __restrict__ masks,
+                                                         uint64_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                         uint32_t* __restrict__ big_list, unsigned int* __restrict__ big_count) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    uint32_t off = offsets[v], cnt = offsets[v + 1] - off;
+    if (cnt == 0) return;
+    if (cnt > BIG_THRESHOLD) { big_list[atomicAdd(big_count, 1u)] = (uint32_t)v; return; }
+    ushort4 r = rects[v];
+    uint64_t code = voxel_code(reinterpret_cast<const uint2*>(s.ijkl)[v], s.max_level);
+    for (int j = r.y >> 4; j <= (r.w >> 4); ++j)
+        for (int i = r.x >> 4; i <= (r.z >> 4); ++i) {
+            uint32_t tile = j * c.tiles_x + i;
+            unsigned m = masks[tile];
+            emit_tile(keys, vals, off, tile, m, code, s.max_level, (uint32_t)v);
+            off += __popc(m);
+        }
+}
+
+__global__ void __launch_bounds__(256) emit_big_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                       const uint32_t* __restrict__ offsets, const uint8_t* __restrict__ masks,
+                                                       const uint32_t* __restrict__ sat, uint64_t* __restrict__ keys,
+                                                       uint32_t* __restrict__ vals, const uint32_t* __restrict__ big_list,
+                                                       const unsigned int* __restrict__ big_count) {
+    int sx = c.tiles_x + 1;
+    unsigned int nb = *big_count;
+    for (unsigned int b = blockIdx.x; b < nb; b += gridDim.x) {
+        uint32_t v = big_list[b];
+        ushort4 r = rects[v];
+        uint32_t off = offsets[v];
+        uint64_t code = voxel_code(reinterpret_cast<const uint2*>(s.ijkl)[v], s.max_level);
+        int i0 = r.x >> 4, j0 = r.y >> 4, w = (r.z >> 4) - i0 + 1, h = (r.w >> 4) - j0 + 1;
+        for (int k = threadIdx.x; k < w * h; k += blockDim.x) {
+            int j = k / w, i = k - j * w;
+            uint32_t before = sat_query(sat, sx, i0, j0, i0 + w, j0 + j) + sat_query(sat, sx, i0, j0 + j, i0 + i, j0 + j + 1);
+            uint32_t tile = (j0 + j) * c.tiles_x + i0 + i;
+            emit_tile(keys, vals, off + before, tile, masks[tile], code, s.max_level, v);
+        }
+    }
+}
+
+// ---- B4: ranges -------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ranges_kernel(const uint64_t* __restrict__ keys, int64_t n, int shift,
+                                                     uint32_t* __restrict__ ranges) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint64_t p = keys[i] >> shift;
+    if (i == 0 || (keys[i - 1] >> shift) != p) ranges[2 * p] = (uint32_t)i;
+    if (i + 1 == n || (keys[i + 1] >> shift) != p) ranges[2 * p + 1] = (uint32_t)(i + 1);
+}
+
+// ---- a3: per-view voxel colour (R6) -------------------------------------------------------------------
+// c_v = max(0, 0.5 + sum_i Y_i(dir_v) sh[v,i,:]); rgbm[v] = (r, g, b, clamp-mask bits).
+template <int DEG>
+__global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                          float4* __restrict__ rgbm) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    ushort4 r = rects[v];
+    if (r.x > r.z) return;                                   // not visible in this view: never read
+    constexpr int NB = (DEG + 1) * (DEG + 1);
+    float dx, dy, dz, Y[NB];
+    voxel_dir_dev(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v], dx, dy, dz);
+    sh_basis_dev(DEG, dx, dy, dz, Y);
+    const float* p = s.sh + v * (NB * 3);
+    float acc[3] = {0.5f, 0.5f, 0.5f};
+    if (NB * 3 % 4 == 0) {
+        const float4* p4 = reinterpret_cast<const float4*>(p);
+#pragma unroll
+        for (int k = 0; k < NB * 3 / 4; ++k) {
+            float4 t = __ldg(p4 + k);
+            float tv[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                int idx = 4 * k + e;
+                acc[idx % 3] = fmaf(Y[idx / 3], tv[e], acc[idx % 3]);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int idx = 0; idx < NB * 3; ++idx) acc[idx % 3] = fmaf(Y[idx / 3], __ldg(p + idx), acc[idx % 3]);
+    }
+    unsigned mask = (acc[0] > 0.f ? 1u : 0u) | (acc[1] > 0.f ? 2u : 0u) | (acc[2] > 0.f ? 4u : 0u);
+    rgbm[v] = make_float4(fmaxf(acc[0], 0.f), fmaxf(acc[1], 0.f), fmaxf(acc[2], 0.f), __uint_as_float(mask));
+}
+
+// ---- a10: SH backward ----------------------------------------------------------------------------------
+// grad_sh[v,i,ch] += Y_i(dir_v) * grad_rgb[v,ch] * [c_v,ch > 0]; consumed grad_rgb entries are re-zeroed.
+template <int DEG>
+__global__ void __launch_bounds__(256) sh_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                          const float4* __restrict__ rgbm, float4* __restrict__ grad_rgb,
+                                                          float* __restrict__ grad_sh) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    ushort4 r = rects[v];
+    if (r.x > r.z) return;
+    float4 g = grad_rgb[v];
+    if (g.x == 0.f && g.y == 0.f && g.z == 0.f) return;
+    grad_rgb[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+    unsigned mask = __float_as_uint(rgbm[v].w);
+    float gv[3] = {(mask & 1u) ? g.x : 0.f, (mask & 2u) ? g.y : 0.f, (mask & 4u) ? g.z : 0.f};
+    constexpr int NB = (DEG + 1) * (DEG + 1);
+    float dx, dy, dz, Y[NB];
+    voxel_dir_dev(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v], dx, dy, dz);
+    sh_basis_dev(DEG, dx, dy, dz, Y);
+    float* p = grad_sh + v * (NB * 3);
+    if (NB * 3 % 4 == 0) {
+        float4* p4 = reinterpret_cast<float4*>(p);
+#pragma unroll
+        for (int k = 0; k < NB * 3 / 4; ++k) {
+            float4 t = p4[k];
+            float tv[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                int idx = 4 * k + e;
+                tv[e] = fmaf(Y[idx / 3], gv[idx % 3], tv[e]);
+            }
+            p4[k] = make_float4(tv[0], tv[1], tv[2], tv[3]);
+        }
+    } else {
+#pragma unroll
+        for (int idx = 0; idx < NB * 3; ++idx) p[idx] = fmaf(Y[idx / 3], gv[idx % 3], p[idx]);
+    }
+}
+
+inline unsigned int blocks_for(int64_t n, int bs) { return (unsigned int)((n + bs - 1) / bs); }
+
+}  // namespace
+
+SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f) {
+    dim3 grid(f->cam.tiles_x, f->cam.tiles_y), block(SVR_TILE, SVR_TILE);
+    tile_mask_kernel<<<grid, block, 0, ctx->stream>>>(f->cam, f->tile_masks);
+    sat_kernel<<<1, 256, 0, ctx->stream>>>(f->tile_masks, f->sat, f->cam.tiles_x, f->cam.tiles_y);
+    ctx->launches += 2;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+// totals[1] = number of "big" voxels (caller zeroes); totals[0] is filled by the caller from the scan.
+SvrStatus launch_rects_counts(SvrContext* ctx, SvrFrame* f, uint32_t* counts, unsigned long long* totals) {
+    rect_count_kernel<<<blocks_for(f->scene.n + 1, 256), 256, 0, ctx->stream>>>(
+        f->scene, f->cam, f->sat, reinterpret_cast<ushort4*>(f->rects), counts, totals);
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_emit_keys(SvrContext* ctx, SvrFrame* f, uint64_t* keys, uint32_t* vals, uint32_t* big_list,
+                                unsigned int* big_count) {
+    emit_small_kernel<<<blocks_for(f->scene.n, 256), 256, 0, ctx->stream>>>(
+        f->scene, f->cam, reinterpret_cast<const ushort4*>(f->rects), f->offsets, f->tile_masks, keys, vals, big_list, big_count);
+    emit_big_kernel<<<148 * 4, 256, 0, ctx->stream>>>(f->scene, f->cam, reinterpret_cast<const ushort4*>(f->rects), f->offsets,
+                                                      f->tile_masks, f->sat, keys, vals, big_list, big_count);
+    ctx->launches += 2;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
+    SVR_CUDA(ctx, cudaMemsetAsync(f->ranges, 0, sizeof(uint32_t) * 16 * (size_t)f->n_tiles, ctx->stream));
+    if (f->n_entries > 0) {
+        ranges_kernel<<<blocks_for(f->n_entries, 256), 256, 0, ctx->stream>>>(f->keys, f->n_entries, 3 * f->scene.max_level,
+                                                                              f->ranges);
+        ctx->launches += 1;
+    }
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
+    if (f->scene.n == 0) return SVR_OK;
+    unsigned int g = blocks_for(f->scene.n, 256);
+    const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
+    float4* out = reinterpret_cast<float4*>(f->rgbm);
+    switch (f->scene.sh_degree) {
+        case 0: voxel_color_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, out); break;
+        case 1: voxel_color_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, out); break;
+        case 2: voxel_color_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, out); break;
+        default: voxel_color_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, out); break;
+    }
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_rgb, float* grad_sh) {
+    if (f->scene.n == 0) return SVR_OK;
+    unsigned int g = blocks_for(f->scene.n, 256);
+    const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
+    const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
+    float4* gr = reinterpret_cast<float4*>(grad_rgb);
+    switch (f->scene.sh_degree) {
+        case 0: sh_backward_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
+        case 1: sh_backward_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
+        case 2: sh_backward_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
+        default: sh_backward_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
+    }
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}

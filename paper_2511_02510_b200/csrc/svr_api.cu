@@ -1,0 +1,352 @@
+// C-ABI entry points of libsvr.so (include/svr.h): context, workspace pool, and the orchestration of
+// svr_preprocess / svr_forward / svr_loss_grad / svr_backward. No torch types, no CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "svr_internal.cuh"
+
+SvrStatus svr_fail(SvrContext* ctx, SvrStatus st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf;
+    return st;
+}
+
+SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 256;
+    bytes = (bytes + 255) & ~(size_t)255;
+    if (ctx->budget && ctx->in_use + bytes > ctx->budget)
+        return svr_fail(ctx, SVR_ERR_WORKSPACE, "workspace budget exceeded: in use %zu + request %zu > budget %zu", ctx->in_use,
+                        bytes, ctx->budget);
+    SVR_CUDA(ctx, cudaMallocAsync(p, bytes, ctx->stream));
+    ctx->in_use += bytes;
+    if (ctx->in_use > ctx->peak) ctx->peak = ctx->in_use;
+    return SVR_OK;
+}
+
+void svr_free(SvrContext* ctx, void* p, size_t bytes) {
+    if (!p) return;
+    if (bytes == 0) bytes = 256;
+    bytes = (bytes + 255) & ~(size_t)255;
+    cudaFreeAsync(p, ctx->stream);
+    ctx->in_use -= bytes;
+}
+
+namespace {
+
+struct FrameAlloc {
+    SvrContext* ctx;
+    SvrFrame* f;
+    SvrStatus get(void** p, size_t bytes) {
+        SvrStatus st = svr_alloc(ctx, p, bytes);
+        if (st == SVR_OK) f->bytes += (bytes == 0 ? 256 : (bytes + 255) & ~(size_t)255);
+        return st;
+    }
+};
+
+int bits_for(int64_t n) {
+    int b = 0;
+    while (((int64_t)1 << b) < n) ++b;
+    return b;
+}
+
+void fill_cam(const SvrCamera* cam, CamDev* c) {
+    c->W = cam->W; c->H = cam->H;
+    c->tiles_x = (cam->W + SVR_TILE - 1) / SVR_TILE;
+    c->tiles_y = (cam->H + SVR_TILE - 1) / SVR_TILE;
+    c->fx = cam->fx; c->fy = cam->fy; c->cx = cam->cx; c->cy = cam->cy;
+    for (int i = 0; i < 9; ++i) c->R[i] = cam->R[i];
+    for (int i = 0; i < 3; ++i) { c->t[i] = cam->t[i]; c->bg[i] = cam->bg[i]; }
+    c->z_near = cam->z_near;
+    for (int a = 0; a < 3; ++a)   // o = -R^T t in fp64 (R3)
+        c->o[a] = -((double)cam->R[a] * cam->t[0] + (double)cam->R[3 + a] * cam->t[1] + (double)cam->R[6 + a] * cam->t[2]);
+}
+
+SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
+    // sizes are tracked in aggregate: free pointers, then give the bytes back in one go
+    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges};
+    for (void* p : ptrs)
+        if (p) cudaFreeAsync(p, ctx->stream);
+    ctx->in_use -= f->bytes;
+    f->bytes = 0;
+    return SVR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t workspace_budget_bytes) {
+    if (!out) return SVR_ERR_INVALID_ARG;
+    *out = nullptr;
+    SvrContext* ctx = new (std::nothrow) SvrContext();
+    if (!ctx) return SVR_ERR_CUDA;
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->budget = workspace_budget_bytes;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) {
+        cudaMemPool_t pool;
+        e = cudaDeviceGetDefaultMemPool(&pool, device);
+        if (e == cudaSuccess) {
+            uint64_t thr = UINT64_MAX;   // keep freed workspace cached in the pool between frames
+            e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+    }
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->host_pinned), 64);
+    if (e != cudaSuccess) {
+        // no usable CUDA device: fail loudly, there is no other path
+        fprintf(stderr, "svr_create: CUDA error: %s\n", cudaGetErrorString(e));
+        delete ctx;
+        return SVR_ERR_CUDA;
+    }
+    *out = ctx;
+    return SVR_OK;
+}
+
+void svr_destroy(SvrContext* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->grad_rgb) cudaFreeAsync(ctx->grad_rgb, ctx->stream);
+    if (ctx->loss_ws) cudaFreeAsync(ctx->loss_ws, ctx->stream);
+    if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
+    cudaStreamSynchronize(ctx->stream);
+    delete ctx;
+}
+
+const char* svr_last_error(const SvrContext* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+size_t svr_workspace_peak_bytes(const SvrContext* ctx) { return ctx ? ctx->peak : 0; }
+int64_t svr_kernel_launches(const SvrContext* ctx) { return ctx ? ctx->launches : 0; }
+
+SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam, SvrFrame** out) {
+    if (!ctx || !vox || !cam || !out) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    *out = nullptr;
+    if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    if (vox->sh_degree < 0 || vox->sh_degree > 3) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "sh_degree must be 0..3");
+    if (cam->W <= 0 || cam->H <= 0 || cam->W > 65535 || cam->H > 65535)
+        return svr_fail(ctx, SVR_ERR_INVALID_ARG, "image size must be 1..65535");
+    if (vox->max_level < 1 || vox->max_level > 16) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "max_level must be 1..16");
+    if (vox->n > 0 && (!vox->ijkl || !vox->raw_density || !vox->sh)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null voxel arrays");
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+
+    SvrFrame* f = new (std::nothrow) SvrFrame();
+    if (!f) return svr_fail(ctx, SVR_ERR_CUDA, "out of host memory");
+    f->scene.n = vox->n;
+    f->scene.sh_degree = vox->sh_degree;
+    f->scene.n_basis = (vox->sh_degree + 1) * (vox->sh_degree + 1);
+    f->scene.max_level = vox->max_level;
+    for (int a = 0; a < 3; ++a) f->scene.root_lo[a] = vox->root_lo[a];
+    f->scene.root_edge = vox->root_edge;
+    f->scene.ijkl = vox->ijkl;
+    f->scene.raw = vox->raw_density;
+    f->scene.sh = vox->sh;
+    fill_cam(cam, &f->cam);
+    f->n_tiles = f->cam.tiles_x * f->cam.tiles_y;
+    f->tile_bits = bits_for(f->n_tiles);
+    f->key_bits = f->tile_bits + 3 + 3 * vox->max_level;
+    if (f->key_bits > 64) {
+        const int kb = f->key_bits;
+        delete f;
+        return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "key needs %d bits (> 64): reduce max_level or image size", kb);
+    }
+
+    FrameAlloc A{ctx, f};
+    const int64_t n = vox->n;
+    uint32_t* counts = nullptr;
+    unsigned long long* totals = nullptr;
+    uint32_t* big_list = nullptr;
+    uint64_t *keys_a = nullptr, *keys_b = nullptr;
+    uint32_t *vals_a = nullptr, *vals_b = nullptr;
+    size_t counts_bytes = sizeof(uint32_t) * (size_t)(n + 1), big_bytes = 0, ka = 0, va = 0;
+    SvrStatus st = SVR_OK;
+    auto fail = [&](SvrStatus s) {
+        if (counts) svr_free(ctx, counts, counts_bytes);
+        if (totals) svr_free(ctx, totals, 64);
+        if (big_list) svr_free(ctx, big_list, big_bytes);
+        if (keys_a) svr_free(ctx, keys_a, ka);
+        if (keys_b) svr_free(ctx, keys_b, ka);
+        if (vals_a) svr_free(ctx, vals_a, va);
+        if (vals_b) svr_free(ctx, vals_b, va);
+        f->keys = nullptr; f->vals = nullptr;
+        release_frame_buffers(ctx, f);
+        delete f;
+        return s;
+    };
+#define TRYF(call) do { st = (call); if (st != SVR_OK) return fail(st); } while (0)
+#define CUDAF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(svr_fail(ctx, SVR_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e__))); } while (0)
+
+    TRYF(A.get((void**)&f->rects, sizeof(uint16_t) * 4 * (size_t)n));
+    TRYF(A.get((void**)&f->tile_masks, (size_t)f->n_tiles));
+    TRYF(A.get((void**)&f->sat, sizeof(uint32_t) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1)));
+    TRYF(A.get((void**)&f->offsets, sizeof(uint32_t) * (size_t)(n + 1)));
+    TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
+    TRYF(A.get((void**)&f->ranges, sizeof(uint32_t) * 16 * (size_t)f->n_tiles));
+    TRYF(svr_alloc(ctx, (void**)&counts, counts_bytes));
+    TRYF(svr_alloc(ctx, (void**)&totals, 64));
+    CUDAF(cudaMemsetAsync(totals, 0, 64, ctx->stream));
+
+    TRYF(launch_tile_masks(ctx, f));
+    TRYF(launch_rects_counts(ctx, f, counts, totals));
+    TRYF(launch_exclusive_scan(ctx, counts, f->offsets, n + 1));
+    // E = offsets[n]; number of big voxels = totals[1]: one small readback sizes the sort buffers
+    CUDAF(cudaMemcpyAsync(totals, f->offsets + n, sizeof(uint32_t), cudaMemcpyDeviceToDevice, ctx->stream));
+    CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 16, cudaMemcpyDeviceToHost, ctx->stream));
+    // per-view colours do not depend on E: enqueue before the sync so they overlap the readback
+    TRYF(launch_voxel_colors(ctx, f));
+    CUDAF(cudaStreamSynchronize(ctx->stream));
+    const int64_t E = (int64_t)(ctx->host_pinned[0] & 0xFFFFFFFFull);
+    const int64_t n_big = (int64_t)ctx->host_pinned[1];
+    svr_free(ctx, counts, counts_bytes);
+    counts = nullptr;
+    if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));
+    f->n_entries = E;
+
+    if (E > 0) {
+        ka = sizeof(uint64_t) * (size_t)E;
+        va = sizeof(uint32_t) * (size_t)E;
+        big_bytes = sizeof(uint32_t) * (size_t)(n_big + 1);
+        TRYF(svr_alloc(ctx, (void**)&keys_a, ka));
+        TRYF(svr_alloc(ctx, (void**)&keys_b, ka));
+        TRYF(svr_alloc(ctx, (void**)&vals_a, va));
+        TRYF(svr_alloc(ctx, (void**)&vals_b, va));
+        TRYF(svr_alloc(ctx, (void**)&big_list, big_bytes));
+        unsigned int* big_count = reinterpret_cast<unsigned int*>(totals + 2);
+        TRYF(launch_emit_keys(ctx, f, keys_a, vals_a, big_list, big_count));
+        uint64_t* ks = nullptr;
+        uint32_t* vs = nullptr;
+        TRYF(launch_sort_pairs(ctx, keys_a, keys_b, vals_a, vals_b, E, f->key_bits, &ks, &vs));
+        // keep the buffers holding the sorted result, return the others to the pool
+        svr_free(ctx, ks == keys_a ? keys_b : keys_a, ka);
+        svr_free(ctx, vs == vals_a ? vals_b : vals_a, va);
+        svr_free(ctx, big_list, big_bytes);
+        big_list = nullptr;
+        f->keys = ks; f->vals = vs;
+        f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
+        keys_a = keys_b = nullptr;
+        vals_a = vals_b = nullptr;
+    }
+    svr_free(ctx, totals, 64);
+    totals = nullptr;
+    TRYF(launch_ranges(ctx, f));
+#undef TRYF
+#undef CUDAF
+    *out = f;
+    return SVR_OK;
+}
+
+SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame) {
+    if (!ctx || !frame) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    return launch_voxel_colors(ctx, frame);
+}
+
+void svr_frame_release(SvrContext* ctx, SvrFrame* frame) {
+    if (!ctx || !frame) return;
+    release_frame_buffers(ctx, frame);
+    delete frame;
+}
+
+SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* image, float* depth,
+                      float* T_final, float* w_max) {
+    if (!ctx || !frame || !opts || !image) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
+    return launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max);
+}
+
+SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H, float gamma,
+                        const SvrLossOpts* opts, float* dL_dimage, float* loss) {
+    if (!ctx || !render || !target || !opts || !dL_dimage || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (W <= 0 || H <= 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "empty image");
+    if (!(opts->percentile > 0.f && opts->percentile <= 1.f)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "percentile must be in (0,1]");
+    return launch_loss_grad(ctx, render, target, W, H, gamma, opts->eps, opts->percentile, opts->sobel_source, dL_dimage, loss);
+}
+
+SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
+                       const float* image, float* grad_raw_density, float* grad_sh, float* w_max) {
+    if (!ctx || !frame || !opts || !dL_dimage || !image || !grad_raw_density || !grad_sh)
+        return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
+    const int64_t n = frame->scene.n;
+    if (n == 0) return SVR_OK;
+    if (ctx->grad_rgb_cap < n) {
+        if (ctx->grad_rgb) svr_free(ctx, ctx->grad_rgb, sizeof(float) * 4 * (size_t)ctx->grad_rgb_cap);
+        ctx->grad_rgb = nullptr;
+        ctx->grad_rgb_cap = 0;
+        SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_rgb, sizeof(float) * 4 * (size_t)n));
+        ctx->grad_rgb_cap = n;
+        SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_rgb, 0, sizeof(float) * 4 * (size_t)n, ctx->stream));
+    }
+    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, grad_raw_density, ctx->grad_rgb, w_max));
+    return launch_sh_backward(ctx, frame, ctx->grad_rgb, grad_sh);
+}
+
+SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam_host, const SvrRenderOpts* ropts,
+                              const SvrLossOpts* lopts, float gamma, const float* target_host, float* grad_raw_density,
+                              float* grad_sh, float* w_max, float* loss_host, float* image_host) {
+    if (!ctx || !vox || !cam_host || !ropts || !lopts || !target_host || !loss_host)
+        return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    const size_t npix = (size_t)cam_host->W * cam_host->H;
+    float* buf = nullptr;   // target | image | dL | loss
+    const size_t bytes = sizeof(float) * (npix * 9 + 64);
+    SVR_TRY(svr_alloc(ctx, (void**)&buf, bytes));
+    float *target = buf, *image = buf + npix * 3, *dL = buf + npix * 6, *loss = buf + npix * 9;
+    SvrFrame* f = nullptr;
+    SvrStatus st = SVR_OK;
+    cudaError_t e = cudaMemcpyAsync(target, target_host, sizeof(float) * npix * 3, cudaMemcpyHostToDevice, ctx->stream);
+    if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "H2D copy: %s", cudaGetErrorString(e));
+    if (st == SVR_OK) st = svr_preprocess(ctx, vox, cam_host, &f);
+    if (st == SVR_OK) st = svr_forward(ctx, f, ropts, image, nullptr, nullptr, nullptr);
+    if (st == SVR_OK) st = svr_loss_grad(ctx, image, target, cam_host->W, cam_host->H, gamma, lopts, dL, loss);
+    if (st == SVR_OK) st = svr_backward(ctx, f, ropts, dL, image, grad_raw_density, grad_sh, w_max);
+    if (st == SVR_OK) {
+        e = cudaMemcpyAsync(loss_host, loss, sizeof(float), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess && image_host)
+            e = cudaMemcpyAsync(image_host, image, sizeof(float) * npix * 3, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "D2H copy: %s", cudaGetErrorString(e));
+    }
+    if (f) svr_frame_release(ctx, f);
+    svr_free(ctx, buf, bytes);
+    return st;
+}
+
+SvrStatus svr_frame_lists(const SvrFrame* frame, const uint64_t** keys, const uint32_t** vals, int64_t* n_entries,
+                          const uint32_t** ranges, const uint16_t** rects, const uint8_t** tile_masks) {
+    if (!frame) return SVR_ERR_INVALID_ARG;
+    if (keys) *keys = frame->keys;
+    if (vals) *vals = frame->vals;
+    if (n_entries) *n_entries = frame->n_entries;
+    if (ranges) *ranges = frame->ranges;
+    if (rects) *rects = frame->rects;
+    if (tile_masks) *tile_masks = frame->tile_masks;
+    return SVR_OK;
+}
+
+SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm) {
+    if (!frame || !rgbm) return SVR_ERR_INVALID_ARG;
+    *rgbm = frame->rgbm;
+    return SVR_OK;
+}
+
+SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes) {
+    if (!ctx || !dst_host || !src_device) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    SVR_CUDA(ctx, cudaMemcpyAsync(dst_host, src_device, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    SVR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SVR_OK;
+}
+
+float svr_gamma_schedule(float t, float T, float t0_frac, float t1_frac, float gamma_max) {
+    float t0 = t0_frac * T, t1 = t1_frac * T;
+    if (t < t0) return 0.0f;
+    if (t < t1) return gamma_max * (t - t0) / (t1 - t0);
+    return gamma_max;
+}
+
+}  // extern "C"

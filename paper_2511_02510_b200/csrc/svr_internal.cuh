@@ -1,0 +1,156 @@
+// Internal declarations shared by the .cu files of libsvr.so (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+#include "svr.h"
+
+#define SVR_TILE 16
+#define SVR_MAX_K 4
+
+struct SvrContext {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    size_t budget = 0;            // 0 = unlimited
+    size_t in_use = 0, peak = 0;
+    int64_t launches = 0;
+    std::string err;
+    // persistent scratch
+    float* grad_rgb = nullptr;    // [n_cap,4] per-voxel colour-gradient scratch, kept all-zero between calls
+    int64_t grad_rgb_cap = 0;
+    void* loss_ws = nullptr;      // loss workspace (see loss.cu)
+    size_t loss_ws_bytes = 0;
+    uint64_t* host_pinned = nullptr;  // 64-byte pinned readback slot
+};
+
+// Device-side copy of the camera with everything derived on the host in fp64.
+struct CamDev {
+    int W, H, tiles_x, tiles_y;
+    float fx, fy, cx, cy;
+    float R[9], t[3];
+    float z_near;
+    float bg[3];
+    double o[3];                  // camera centre -R^T t (fp64)
+};
+
+struct SceneDev {
+    int64_t n;
+    int sh_degree, n_basis, max_level;
+    float root_lo[3];
+    float root_edge;
+    const uint16_t* ijkl;
+    const float* raw;
+    const float* sh;
+};
+
+struct SvrFrame {
+    SceneDev scene;
+    CamDev cam;
+    int n_tiles = 0;
+    int tile_bits = 0, key_bits = 0;
+    int64_t n_entries = 0;
+    // device buffers (pool-allocated)
+    uint16_t* rects = nullptr;       // [n,4]
+    uint8_t* tile_masks = nullptr;   // [n_tiles]
+    uint32_t* sat = nullptr;         // [(tiles_y+1)*(tiles_x+1)] summed-area table of popcount(mask)
+    uint32_t* offsets = nullptr;     // [n+1] exclusive scan of counts
+    float* rgbm = nullptr;           // [n,4]
+    uint64_t* keys = nullptr;        // [E] sorted
+    uint32_t* vals = nullptr;        // [E] sorted
+    uint32_t* ranges = nullptr;      // [n_tiles*8*2]
+    size_t bytes = 0;
+};
+
+// ---- error handling -------------------------------------------------------------------------
+SvrStatus svr_fail(SvrContext* ctx, SvrStatus st, const char* fmt, ...);
+#define SVR_CUDA(ctx, call)                                                                      \
+    do {                                                                                         \
+        cudaError_t e__ = (call);                                                                \
+        if (e__ != cudaSuccess)                                                                  \
+            return svr_fail((ctx), SVR_ERR_CUDA, "%s failed: %s (%s:%d)", #call,                 \
+                            cudaGetErrorString(e__), __FILE__, __LINE__);                        \
+    } while (0)
+#define SVR_TRY(call)                          \
+    do {                                       \
+        SvrStatus s__ = (call);                \
+        if (s__ != SVR_OK) return s__;         \
+    } while (0)
+
+// ---- workspace pool --------------------------------------------------------------------------
+SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes);
+void svr_free(SvrContext* ctx, void* p, size_t bytes);
+
+// ---- stage launchers (each counts its kernel launches into ctx->launches) --------------------
+SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_rects_counts(SvrContext* ctx, SvrFrame* f, uint32_t* counts, unsigned long long* totals);
+SvrStatus launch_exclusive_scan(SvrContext* ctx, const uint32_t* in, uint32_t* out, int64_t n_plus_1);
+SvrStatus launch_emit_keys(SvrContext* ctx, SvrFrame* f, uint64_t* keys, uint32_t* vals, uint32_t* big_list,
+                           unsigned int* big_count);
+SvrStatus launch_sort_pairs(SvrContext* ctx, uint64_t* keys, uint64_t* keys_alt, uint32_t* vals, uint32_t* vals_alt,
+                            int64_t n, int bits, uint64_t** keys_sorted, uint32_t** vals_sorted);
+SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
+                         float* T_final, float* w_max);
+SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
+                          float* grad_raw, float* grad_rgb, float* w_max);
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_rgb, float* grad_sh);
+SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma,
+                           float eps, float q, int sobel_source, float* dL, float* loss);
+
+// ---- small device helpers ---------------------------------------------------------------------
+#ifdef __CUDACC__
+// Real SH basis up to degree 3, no Condon-Shortley phase, i = l(l+1)+m (R6).
+__device__ __forceinline__ void sh_basis_dev(int degree, float x, float y, float z, float* Y) {
+    Y[0] = 0.28209479177387814f;
+    if (degree < 1) return;
+    Y[1] = 0.4886025119029199f * y;
+    Y[2] = 0.4886025119029199f * z;
+    Y[3] = 0.4886025119029199f * x;
+    if (degree < 2) return;
+    float xx = x * x, yy = y * y, zz = z * z;
+    Y[4] = 1.0925484305920792f * x * y;
+    Y[5] = 1.0925484305920792f * y * z;
+    Y[6] = 0.31539156525252005f * (3.0f * zz - 1.0f);
+    Y[7] = 1.0925484305920792f * x * z;
+    Y[8] = 0.5462742152960396f * (xx - yy);
+    if (degree < 3) return;
+    Y[9] = 0.5900435899266435f * y * (3.0f * xx - yy);
+    Y[10] = 2.890611442640554f * x * y * z;
+    Y[11] = 0.4570457994644658f * y * (5.0f * zz - 1.0f);
+    Y[12] = 0.3731763325901154f * z * (5.0f * zz - 3.0f);
+    Y[13] = 0.4570457994644658f * x * (5.0f * zz - 1.0f);
+    Y[14] = 1.445305721320277f * z * (xx - yy);
+    Y[15] = 0.5900435899266435f * x * (xx - 3.0f * yy);
+}
+
+__device__ __forceinline__ void voxel_dir_dev(const SceneDev& s, const CamDev& c, uint2 q, float& dx, float& dy, float& dz) {
+    int L = q.y >> 16;
+    double e = (double)s.root_edge * (double)__int_as_float((127 - L) << 23);
+    double gx = (double)s.root_lo[0] + ((double)(q.x & 0xFFFF) + 0.5) * e - c.o[0];
+    double gy = (double)s.root_lo[1] + ((double)(q.x >> 16) + 0.5) * e - c.o[1];
+    double gz = (double)s.root_lo[2] + ((double)(q.y & 0xFFFF) + 0.5) * e - c.o[2];
+    float fx = (float)gx, fy = (float)gy, fz = (float)gz;
+    float n2 = fx * fx + fy * fy + fz * fz;
+    if (n2 == 0.0f) { dx = 0.f; dy = 0.f; dz = 1.f; return; }
+    float inv = rsqrtf(n2);
+    dx = fx * inv; dy = fy * inv; dz = fz * inv;
+}
+#endif
+
+#ifdef __CUDACC__
+// Direction-sign octant of a pixel's ray (B2): individually rounded binary32 operations in this
+// exact order, so the compositing kernels select the same (tile, octant) list the binning built.
+__device__ __forceinline__ int pixel_octant_dev(const CamDev& c, int x, int y) {
+    float u = __fdiv_rn(__fsub_rn(__fadd_rn((float)x, 0.5f), c.cx), c.fx);
+    float v = __fdiv_rn(__fsub_rn(__fadd_rn((float)y, 0.5f), c.cy), c.fy);
+    int s = 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float d = __fadd_rn(__fadd_rn(__fmul_rn(c.R[a], u), __fmul_rn(c.R[3 + a], v)), c.R[6 + a]);
+        if (d < 0.0f) s |= 1 << a;
+    }
+    return s;
+}
+#endif

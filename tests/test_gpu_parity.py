@@ -1,0 +1,259 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: -m gpu).
+
+Bars (BASELINE.json north_star; metric readings C1/C2 in DESIGN.md):
+  * rectangles, tile masks, entry count, sorted keys + voxel ids, ranges: bit-exact;
+  * image / T_final / w_max: max |x - r| / max(|r|, 1) <= 1e-4; depth: same with scale = orbit radius;
+  * gradients: relative L2 per parameter tensor <= 1e-3 (both sides fed the same dL/dimage);
+  * loss gradient: relative L2 <= 1e-5, loss scalar relative 1e-5.
+"""
+import numpy as np
+import pytest
+
+from svr_inputs import look_at_camera, make_config, tiny_scene
+from svr_inputs.scenes import noisy_target, random_image_grad, uniform_target
+
+pytestmark = pytest.mark.gpu
+
+IMG_TOL = 1e-4
+GRAD_TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def svr():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2511_02510_b200 as pkg
+    ctx = pkg.Context(0)
+    yield pkg, ctx, torch
+    ctx.close()
+
+
+def max_rel(x, r, scale=1.0):
+    x, r = np.asarray(x, dtype=np.float64), np.asarray(r, dtype=np.float64)
+    return float(np.max(np.abs(x - r) / np.maximum(np.abs(r), scale))) if r.size else 0.0
+
+
+def rel_l2(x, r):
+    x, r = np.asarray(x, dtype=np.float64), np.asarray(r, dtype=np.float64)
+    return float(np.linalg.norm(x - r) / max(np.linalg.norm(r), 1e-300))
+
+
+def gpu_forward(svr, scene, cam, K, T_min=1e-5):
+    pkg, ctx, torch = svr
+    vox = pkg.Voxels.from_scene(scene)
+    frame = ctx.svr_preprocess(vox, cam)
+    w_max = torch.zeros(scene.n, dtype=torch.float32, device="cuda")
+    image, depth, Tf = ctx.svr_forward(frame, K, T_min, w_max=w_max)
+    ctx.synchronize()
+    return vox, frame, image, depth, Tf, w_max
+
+
+def check_lists(orc, svr, scene, cam):
+    pkg, ctx, torch = svr
+    vox = pkg.Voxels.from_scene(scene)
+    frame = ctx.svr_preprocess(vox, cam)
+    got = frame.lists()
+    want = orc.bin_lists(scene, cam)
+    np.testing.assert_array_equal(got["rects"], want["rects"])
+    np.testing.assert_array_equal(got["tile_masks"], want["tile_masks"])
+    assert got["n_entries"] == want["keys"].size
+    np.testing.assert_array_equal(got["keys"], want["keys"])
+    np.testing.assert_array_equal(got["vals"], want["vals"])
+    np.testing.assert_array_equal(got["ranges"], want["ranges"])
+    frame.release()
+    return got["n_entries"]
+
+
+def check_forward(orc, svr, cfg, cam, mode="bucketed"):
+    vox, frame, image, depth, Tf, w_max = gpu_forward(svr, cfg.scene, cam, cfg.K, cfg.T_min)
+    ref = orc.render(cfg.scene, cam, cfg.K, mode=mode)
+    errs = dict(image=max_rel(image.cpu().numpy(), ref["image"]), T=max_rel(Tf.cpu().numpy(), ref["T_final"]),
+                depth=max_rel(depth.cpu().numpy(), ref["depth"], cfg.orbit_radius),
+                w_max=max_rel(w_max.cpu().numpy(), ref["w_max"]))
+    for k, v in errs.items():
+        assert v <= IMG_TOL, (k, errs)
+    # eq. 5: never-hit voxels stay exactly 0 (unless their only hits came after the T_min cut)
+    wm = w_max.cpu().numpy()
+    assert np.all(wm[ref["w_max"] == 0] <= 1e-6)
+    return vox, frame, image, ref, errs
+
+
+def check_backward(orc, svr, cfg, cam, vox, frame, image, G, mode="bucketed"):
+    pkg, ctx, torch = svr
+    sc = cfg.scene
+    g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+    g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+    w_max = torch.zeros(sc.n, dtype=torch.float32, device="cuda")
+    dL = torch.from_numpy(np.ascontiguousarray(G, dtype=np.float32)).cuda()
+    ctx.svr_backward(frame, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=w_max)
+    ctx.synchronize()
+    r_raw, r_sh = orc.backward(sc, cam, cfg.K, dL.cpu().numpy().astype(np.float64), mode=mode)
+    e_raw, e_sh = rel_l2(g_raw.cpu().numpy(), r_raw), rel_l2(g_sh.cpu().numpy(), r_sh)
+    assert e_raw <= GRAD_TOL and e_sh <= GRAD_TOL, (e_raw, e_sh)
+    return e_raw, e_sh, w_max
+
+
+# ---------------------------------------------------------------------------------------------
+# bit-exact binning
+# ---------------------------------------------------------------------------------------------
+def test_lists_bit_exact_C1(orc, svr):
+    cfg = make_config("C1")
+    assert check_lists(orc, svr, cfg.scene, cfg.cameras[0]) > 500
+
+
+def test_lists_bit_exact_C2_all_cameras(orc, svr):
+    cfg = make_config("C2")
+    for cam in cfg.cameras:
+        assert check_lists(orc, svr, cfg.scene, cam) > 10_000
+
+
+def test_lists_bit_exact_camera_inside_and_ragged(orc, svr):
+    cfg = make_config("C2", n_voxels=20_000)
+    cam = look_at_camera((0.31, 0.27, 0.13), (-0.5, 0.4, -0.1), 203, 117)     # ragged tiles, straddling voxels
+    assert check_lists(orc, svr, cfg.scene, cam) > 1000
+    cfg4 = make_config("C4", n_voxels=60_000, res_scale=0.2, n_cams=2)          # cameras inside background cells
+    for cam in cfg4.cameras:
+        check_lists(orc, svr, cfg4.scene, cam)
+
+
+# ---------------------------------------------------------------------------------------------
+# forward + backward + loss on C1, C2
+# ---------------------------------------------------------------------------------------------
+def test_C1_end_to_end(orc, svr):
+    pkg, ctx, torch = svr
+    cfg = make_config("C1")
+    cam = cfg.cameras[0]
+    vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam, mode="pure")
+    target = uniform_target(cam, cfg.seed + 7)
+    tgt = torch.from_numpy(target).cuda()
+    dL, loss = ctx.svr_loss_grad(image, tgt, cfg.gamma)
+    ctx.synchronize()
+    L_ref, dL_ref, _ = orc.lf_loss_and_grad(image.cpu().numpy(), target, cfg.gamma)
+    assert rel_l2(dL.cpu().numpy(), dL_ref) <= 1e-5
+    assert abs(float(loss.item()) - L_ref) <= 1e-5 * abs(L_ref)
+    check_backward(orc, svr, cfg, cam, vox, frame, image, dL.cpu().numpy(), mode="pure")
+    frame.release()
+
+
+def test_C2_forward_backward(orc, svr):
+    pkg, ctx, torch = svr
+    cfg = make_config("C2")
+    for i, cam in enumerate(cfg.cameras[:2]):
+        vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam)
+        G = random_image_grad(cam, 100 + i)
+        check_backward(orc, svr, cfg, cam, vox, frame, image, G)
+        frame.release()
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 4])
+def test_K_variants_and_sh_degrees(orc, svr, K):
+    deg = K - 1
+    sc = tiny_scene(40 + K, n=8, sh_degree=deg)
+    cam = look_at_camera((2.1, 0.7, 1.3), (0.05, -0.1, 0.0), 37, 21)
+    cfg = make_config("C1")
+    cfg.scene, cfg.K = sc, K
+    vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam, mode="pure")
+    check_backward(orc, svr, cfg, cam, vox, frame, image, random_image_grad(cam, K), mode="pure")
+    frame.release()
+
+
+def test_loss_grad_parity_and_gamma0(orc, svr):
+    pkg, ctx, torch = svr
+    rng = np.random.default_rng(5)
+    H, W = 75, 133
+    base = np.zeros((H, W, 3), dtype=np.float32)
+    base[:, W // 2:] = 0.8
+    base[H // 3:, :] += 0.1
+    target = np.clip(base + rng.normal(0, 0.01, size=base.shape), 0, 1).astype(np.float32)
+    render = np.clip(target + rng.normal(0, 0.05, size=base.shape), 0, 1).astype(np.float32)
+    for gamma, src in [(0.6, 0), (0.3, 1), (0.0, 0)]:
+        dL, loss = ctx.svr_loss_grad(torch.from_numpy(render).cuda(), torch.from_numpy(target).cuda(), gamma, sobel_source=src)
+        ctx.synchronize()
+        L_ref, dL_ref, _ = orc.lf_loss_and_grad(render, target, gamma, sobel_source=src)
+        assert rel_l2(dL.cpu().numpy(), dL_ref) <= 1e-5, (gamma, src)
+        assert abs(float(loss.item()) - L_ref) <= 1e-5 * abs(L_ref)
+    # gamma = 0 reduces exactly to the unweighted L1 gradient sign(r)/(3|P|)
+    np.testing.assert_allclose(dL.cpu().numpy(), np.sign(render - target) / (3.0 * H * W), rtol=1e-6, atol=0)
+    assert abs(pkg.svr_gamma_schedule(9000, 20000) - orc.gamma_schedule(9000, 20000)) < 1e-7
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------------
+def test_empty_and_invisible_scenes(orc, svr):
+    pkg, ctx, torch = svr
+    from dataclasses import replace
+    sc = tiny_scene(3, n=4, sh_degree=0)
+    empty = replace(sc, ijkl=sc.ijkl[:0], raw=sc.raw[:0], sh=sc.sh[:0])
+    cam = look_at_camera((3.0, 1.0, 0.5), (0, 0, 0), 50, 30)
+    vox, frame, image, depth, Tf, w_max = gpu_forward(svr, empty, cam, 2)
+    assert frame.lists()["n_entries"] == 0
+    np.testing.assert_array_equal(image.cpu().numpy(), np.broadcast_to(cam.bg, (30, 50, 3)))
+    assert float(depth.abs().max()) == 0.0 and float((Tf - 1).abs().max()) == 0.0
+    cam_away = look_at_camera((3.0, 0.0, 0.0), (6.0, 0.0, 0.0), 50, 30)
+    vox, frame, image, depth, Tf, w_max = gpu_forward(svr, sc, cam_away, 2)
+    assert frame.lists()["n_entries"] == 0 and float(w_max.max()) == 0.0
+    np.testing.assert_array_equal(image.cpu().numpy(), np.broadcast_to(cam.bg, (30, 50, 3)))
+
+
+def test_determinism(orc, svr):
+    cfg = make_config("C2", n_voxels=20_000)
+    cam = cfg.cameras[1]
+    a = gpu_forward(svr, cfg.scene, cam, cfg.K)
+    b = gpu_forward(svr, cfg.scene, cam, cfg.K)
+    assert np.array_equal(a[2].cpu().numpy(), b[2].cpu().numpy())            # image
+    assert np.array_equal(a[5].cpu().numpy(), b[5].cpu().numpy())            # w_max
+    la, lb = a[1].lists(), b[1].lists()
+    assert np.array_equal(la["keys"], lb["keys"]) and np.array_equal(la["vals"], lb["vals"])
+
+
+def test_workspace_budget_error(svr):
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    small = pkg.Context(0, workspace_budget_bytes=64 << 10)
+    vox = pkg.Voxels.from_scene(cfg.scene)
+    with pytest.raises(pkg.SvrError) as ei:
+        small.svr_preprocess(vox, cfg.cameras[0])
+    assert ei.value.status == 3
+    small.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# reduced copies of C3..C5 in full (all pixels), full-size C3/C4 on sampled rays
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,n,scale", [("C3", 150_000, 0.3), ("C4", 200_000, 0.3), ("C5", 250_000, 0.25)])
+def test_reduced_configs_full_images(orc, svr, name, n, scale):
+    cfg = make_config(name, n_voxels=n, res_scale=scale, n_cams=2)
+    for i, cam in enumerate(cfg.cameras):
+        check_lists(orc, svr, cfg.scene, cam)
+        vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam)
+        target = noisy_target(ref["image"], cfg.seed + i, cfg.target_noise)
+        pkg, ctx, torch = svr
+        dL, _ = ctx.svr_loss_grad(image, torch.from_numpy(target).cuda(), cfg.gamma)
+        ctx.synchronize()
+        check_backward(orc, svr, cfg, cam, vox, frame, image, dL.cpu().numpy())
+        frame.release()
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_full_size_sampled_rays(orc, svr, name):
+    """Full-size scene in the launch configuration bench.py times; the oracle brute-forces 384 sampled rays."""
+    pkg, ctx, torch = svr
+    cfg = make_config(name, n_cams=1)
+    cam = cfg.cameras[0]
+    vox, frame, image, depth, Tf, w_max = gpu_forward(svr, cfg.scene, cam, cfg.K, cfg.T_min)
+    rng = np.random.default_rng(77)
+    xy = np.stack([rng.integers(0, cam.W, 384), rng.integers(0, cam.H, 384)], axis=1).astype(np.int32)
+    ref = orc.render(cfg.scene, cam, cfg.K, mode="pure", xy=xy)
+    img = image.cpu().numpy()[xy[:, 1], xy[:, 0]]
+    assert max_rel(img, ref["image"]) <= IMG_TOL
+    assert max_rel(Tf.cpu().numpy()[xy[:, 1], xy[:, 0]], ref["T_final"]) <= IMG_TOL
+    assert max_rel(depth.cpu().numpy()[xy[:, 1], xy[:, 0]], ref["depth"], cfg.orbit_radius) <= IMG_TOL
+    # properties that hold at any size
+    wm = w_max.cpu().numpy()
+    assert np.all((wm >= 0) & (wm <= 1.0 + 1e-6)) and np.all(np.isfinite(img))
+    # w_max is a max over ALL rays: at least the sampled rays' weights
+    assert np.all(wm + 1e-4 >= ref["w_max"])
+    assert ref["n_hits"].max() > 3
+    frame.release()
