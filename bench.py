@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py - forward+backward Mrays/s of the sparse-voxel tile rasterizer on config C4 (BASELINE.json
+configs[3], the Mip-NeRF-360-shaped 4M-voxel scene the metric is quoted on), one process per GPU.
+
+A "step" is one training view through the whole hot path: svr_preprocess (project, key build, sort, ranges,
+per-view colours) -> svr_forward -> svr_loss_grad -> svr_backward (+ SH backward, w_max), cameras taken
+round-robin from the config's 8 views. Inputs are seeded synthetic (svr_inputs), resident in HBM for `value`;
+`e2e` goes through svr_train_view_host with the step's inputs (camera + target image) in pinned HOST memory and
+the loss read back to the host inside the timed region. The scene parameters (928 MB) and the sorted lists
+are far larger than the 126 MB L2, so no explicit L2 flush is needed between iterations.
+
+--impl reference times the CPU oracle (oracle/, fp64, OpenMP) on a bounded sample of the same workload.
+N > 1 (torchrun): independent replicas (the path has no exchange step: DESIGN.md "Multi-GPU"), weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# algorithmic work per ray-voxel hit: forward 125 flop, backward 250 flop
+FLOP_PER_FWD_HIT = 125.0
+FLOP_PER_BWD_HIT = 250.0
+FP32_LANES_PER_SM = 128
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return d, "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.idx = device_index
+        self.lines = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.idx)], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample_run(cfg, cam, n_rays: int, seed: int):
+    """The CPU oracle as it stands (bucketed mode, fp64, OpenMP) on n_rays seeded rays: forward + backward."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    xy = np.stack([rng.integers(0, cam.W, n_rays), rng.integers(0, cam.H, n_rays)], axis=1).astype(np.int32)
+    G = rng.normal(0, 1.0 / (3 * cam.W * cam.H), size=(n_rays, 3))
+    t0 = time.perf_counter()
+    oracle.render(cfg.scene, cam, cfg.K, mode="bucketed", xy=xy)
+    oracle.backward(cfg.scene, cam, cfg.K, G, mode="bucketed", xy=xy)
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    """--impl reference: the oracle on this box's host cores, same metric/config; each step is a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from svr_inputs import make_config
+    oracle.build()
+    cfg = make_config(args.workload, n_voxels=args.n_voxels, res_scale=args.res_scale)
+    n_rays = args.ref_rays
+    for i in range(args.warmup if args.warmup < 2 else 1):
+        oracle_sample_run(cfg, cfg.cameras[i % len(cfg.cameras)], min(n_rays, 2000), 900 + i)
+    total = 0.0
+    for i in range(args.steps):
+        total += oracle_sample_run(cfg, cfg.cameras[i % len(cfg.cameras)], n_rays, 1000 + i)
+    value = n_rays * args.steps / total / 1e6
+    cores = oracle.num_threads()
+    sample = f"{n_rays} seeded rays per step (of {cfg.cameras[0].W * cfg.cameras[0].H} per view), bucketed fp64 oracle, forward+backward"
+    line = {"impl": "reference", "metric": "fwd+bwd Mrays/s", "value": value, "unit": "Mrays/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, args),
+            "cpu_baseline": {"value": value, "unit": "Mrays/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "Mrays/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(cfg, args):
+    cam = cfg.cameras[0]
+    return {"workload": f"{cfg.name}: {cfg.scene.n} voxels, {cam.W}x{cam.H}, {len(cfg.cameras)} cameras round-robin, K={cfg.K}, "
+                        f"SH degree {cfg.scene.sh_degree}, T_min={cfg.T_min}, gamma={cfg.gamma}, backward emits w_max",
+            "seed": cfg.seed, "rays_per_step": cam.W * cam.H,
+            "l2": "inputs larger than L2 (scene parameters 928 MB at full size); no explicit flush",
+            "parallelism": f"replicas x{args.gpus} (no data-path collective)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=16)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4")
+    ap.add_argument("--n-voxels", type=int, default=None, help="reduced copy of the workload (debugging only)")
+    ap.add_argument("--res-scale", type=float, default=1.0)
+    ap.add_argument("--ref-rays", type=int, default=100_000, help="rays per step of the CPU oracle sample")
+    ap.add_argument("--cpu-baseline-rays", type=int, default=100_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import paper_2511_02510_b200 as pkg          # raises if libsvr.so is missing: no fallback
+    from svr_inputs import make_config
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+
+    cfg = make_config(args.workload, n_voxels=args.n_voxels, res_scale=args.res_scale)
+    sc, cams = cfg.scene, cfg.cameras
+    W, H = cams[0].W, cams[0].H
+    rays = W * H
+    ctx = pkg.Context(local_rank, workspace_budget_bytes=cfg.workspace_budget_bytes)
+    stream = ctx.stream
+    vox = pkg.Voxels.from_scene(sc, device=dev)
+    ccams = [pkg.make_camera(c) for c in cams]
+    g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device=dev)
+    g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device=dev)
+    w_max = torch.zeros(sc.n, dtype=torch.float32, device=dev)
+    image = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
+    depth = torch.empty((H, W), dtype=torch.float32, device=dev)
+    Tf = torch.empty((H, W), dtype=torch.float32, device=dev)
+    dL = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
+    loss = torch.empty(1, dtype=torch.float32, device=dev)
+
+    # targets: seeded noise-perturbed renders (config recipe), one per camera, device + pinned host copies
+    targets, targets_host = [], []
+    for i, c in enumerate(ccams):
+        fr = ctx.svr_preprocess(vox, c)
+        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False)
+        ctx.synchronize()
+        fr.release()
+        rng = np.random.Generator(np.random.PCG64(cfg.seed * 100 + i))
+        noise = torch.from_numpy(rng.normal(0, cfg.target_noise, size=(H, W, 3)).astype(np.float32))
+        t_host = torch.clamp(image.cpu() + noise, 0.0, 1.0).contiguous().pin_memory()
+        targets_host.append(t_host)
+        targets.append(t_host.to(dev))
+
+    def step(i):
+        k = (i + rank) % len(ccams)
+        fr = ctx.svr_preprocess(vox, ccams[k])
+        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, depth=depth, T_final=Tf)
+        ctx.svr_loss_grad(image, targets[k], cfg.gamma, dL=dL, loss=loss)
+        ctx.svr_backward(fr, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=w_max if cfg.emit_wmax_in_backward else None)
+        fr.release()
+
+    def render_step(i):
+        k = (i + rank) % len(ccams)
+        fr = ctx.svr_preprocess(vox, ccams[k])
+        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False)
+        fr.release()
+
+    def e2e_step(i):
+        k = (i + rank) % len(ccams)
+        return ctx.svr_train_view_host(vox, ccams[k], cfg.K, cfg.gamma, targets_host[k], g_raw, g_sh,
+                                       w_max=w_max if cfg.emit_wmax_in_backward else None, T_min=cfg.T_min)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, sampler=None):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        if sampler:
+            sampler.start()
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for i in range(steps):
+                fn(i)
+            e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        clocks = sampler.stop() if sampler else None
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, clocks
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    torch.cuda.reset_peak_memory_stats(dev)
+
+    # ---- timed region: K steps of the whole path, stage timers on (CUDA events on the library's stream) ----
+    launches0 = ctx.kernel_launches
+    ctx.svr_get_stage_times(reset=True)
+    ctx.svr_set_stage_timing(True)
+    ms_total, clocks = timed(step, args.steps, ClockSampler(local_rank))
+    stage = ctx.svr_get_stage_times(reset=True)
+    ctx.svr_set_stage_timing(False)
+    launches = ctx.kernel_launches - launches0
+    value = rays * args.steps * world / (ms_total * 1e-3) / 1e6
+
+    # ---- render-only FPS (preprocess + forward, w_max off) ----
+    for i in range(3):
+        render_step(i)
+    ms_render, _ = timed(render_step, args.steps)
+    render_fps = args.steps * world / (ms_render * 1e-3)
+
+    # ---- end to end through the host-buffer entry point ----
+    for i in range(3):
+        e2e_step(i)
+    ms_e2e, _ = timed(e2e_step, args.steps)
+    e2e_value = rays * args.steps * world / (ms_e2e * 1e-3) / 1e6
+
+    peak_vram = int(torch.cuda.max_memory_allocated(dev)) + int(ctx.workspace_peak_bytes)
+
+    # ---- work counters (outside the timed region): hits / tests per view ----
+    stats = []
+    for k in sorted({(i + rank) % len(ccams) for i in range(args.steps)}):
+        fr = ctx.svr_preprocess(vox, ccams[k])
+        st = ctx.svr_forward_stats(fr, cfg.K, cfg.T_min)
+        st["entries"] = fr.n_entries
+        fr.release()
+        stats.append(st)
+    hits = float(np.mean([s["hits"] for s in stats]))
+    tests = float(np.mean([s["slab_tests"] for s in stats]))
+    staged = float(np.mean([s["entries_staged"] for s in stats]))
+
+    peaks, peak_src = measured_peaks()
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    fp32_peak = n_sm * FP32_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12    # TFLOP/s
+    stage_ms = {k: v[0] / max(v[1], 1) for k, v in stage.items() if v[1] > 0}
+    dom = max(stage_ms, key=stage_ms.get)
+    flop = {"forward_composite": FLOP_PER_FWD_HIT, "backward_composite": FLOP_PER_BWD_HIT}
+    if dom in flop:
+        achieved = hits * flop[dom] / (stage_ms[dom] * 1e-3) / 1e12
+        roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+                    "frac": achieved / fp32_peak, "traffic": None,
+                    "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x sm_max_mhz, clocks {peak_src}",
+                    "algorithmic": f"{hits:.4g} ray-voxel hits/view x {flop[dom]:.0f} flop",
+                    "kernel_ms": stage_ms[dom], "slab_tests_per_hit": tests / max(hits, 1.0)}
+    else:   # an HBM-bound stage dominates (not expected): report bytes moved by the sort
+        bytes_ = staged * 170.0
+        achieved = bytes_ / (stage_ms[dom] * 1e-3) / 1e9
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": None, "kernel_ms": stage_ms[dom]}
+
+    line = {"metric": "fwd+bwd Mrays/s", "value": value, "unit": "Mrays/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, args),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "Mrays/s", "ms_per_step": ms_e2e / args.steps,
+                    "h2d_bytes_per_step": int(targets_host[0].numel() * 4 + 92), "d2h_bytes_per_step": 4,
+                    "note": "svr_train_view_host: camera + target image from pinned host memory, loss read back"},
+            "gpu_launches": int(launches),
+            "render_fps": render_fps,
+            "roofline": roofline,
+            "stage_ms_per_step": stage_ms,
+            "work_per_view": {"hits": hits, "slab_tests": tests, "entries_staged": staged,
+                              "list_entries": float(np.mean([s["entries"] for s in stats])),
+                              "warp_voxel_pairs": float(np.mean([s["warp_voxel_pairs"] for s in stats]))},
+            "peak_vram_bytes": peak_vram}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        n_rays = args.cpu_baseline_rays
+        dt = oracle_sample_run(cfg, cams[0], n_rays, 4242)
+        line["cpu_baseline"] = {"value": n_rays / dt / 1e6, "unit": "Mrays/s", "cores": oracle.num_threads(), "kind": "oracle",
+                                "sample": f"{n_rays} seeded rays of camera 0 (of {rays}), bucketed fp64 oracle, forward+backward, "
+                                          f"{dt:.1f} s"}
+    if rank == 0:
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

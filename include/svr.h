@@ -128,6 +128,18 @@ SvrStatus svr_frame_lists(const SvrFrame* frame, const uint64_t** keys, const ui
 /* Per-view voxel colours [n,4]: r,g,b and the clamp mask bits (as float bits) - debugging / tests. */
 SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm);
 
+/* Measurement hooks (bench.py). svr_forward_stats runs the forward pass with counters compiled in and
+ * returns stats_host[4] = ray-voxel hits composited, per-lane slab tests, (warp, voxel) pairs walked after the
+ * warp-level rectangle cull, list entries staged. It synchronises. svr_set_stage_timing(1) brackets every
+ * stage's kernels with CUDA events on the context's stream; svr_get_stage_times synchronises and returns the
+ * accumulated milliseconds and call counts per stage (svr_num_stages() entries, named by svr_stage_name). */
+SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* image,
+                            uint64_t* stats_host);
+void svr_set_stage_timing(SvrContext* ctx, int enabled);
+int svr_num_stages(void);
+const char* svr_stage_name(int stage);
+SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset);
+
 /* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);
 

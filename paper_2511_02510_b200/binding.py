@@ -21,7 +21,8 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
-           "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule"]
+           "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
+           "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times"]
 
 
 class SvrError(RuntimeError):
@@ -75,6 +76,13 @@ def _load():
     lib.svr_frame_lists.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 2 + [C.POINTER(C.c_int64)] + [C.POINTER(C.c_void_p)] * 3
     lib.svr_frame_colors.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
     lib.svr_copy_to_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]
+    lib.svr_forward_stats.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts), C.c_void_p, C.c_void_p]
+    lib.svr_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
+    lib.svr_set_stage_timing.restype = None
+    lib.svr_num_stages.restype = C.c_int
+    lib.svr_stage_name.argtypes = [C.c_int]
+    lib.svr_stage_name.restype = C.c_char_p
+    lib.svr_get_stage_times.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
     lib.svr_gamma_schedule.argtypes = [C.c_float] * 5
     lib.svr_gamma_schedule.restype = C.c_float
     return lib
@@ -151,6 +159,12 @@ class Frame:
         except Exception:
             pass
 
+    @property
+    def n_entries(self) -> int:
+        n = C.c_int64()
+        self.ctx._check(_lib.svr_frame_lists(C.c_void_p(self.handle), None, None, C.byref(n), None, None, None))
+        return int(n.value)
+
     def lists(self):
         """Copies of the inspection buffers as NumPy arrays (tests)."""
         keys, vals, ranges, rects, masks = (C.c_void_p() for _ in range(5))
@@ -223,6 +237,23 @@ class Context:
     @property
     def kernel_launches(self) -> int:
         return int(_lib.svr_kernel_launches(self.handle))
+
+    # ---- measurement hooks -----------------------------------------------------------------------
+    def svr_forward_stats(self, frame: "Frame", K: int, T_min: float = 1e-5) -> dict:
+        image = torch.empty((frame.H, frame.W, 3), dtype=torch.float32, device=frame.vox.raw.device)
+        out = (C.c_uint64 * 4)()
+        o = SvrRenderOpts(K, T_min)
+        self._check(_lib.svr_forward_stats(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(image), C.cast(out, C.c_void_p)))
+        return dict(hits=int(out[0]), slab_tests=int(out[1]), warp_voxel_pairs=int(out[2]), entries_staged=int(out[3]))
+
+    def svr_set_stage_timing(self, enabled: bool):
+        _lib.svr_set_stage_timing(self.handle, 1 if enabled else 0)
+
+    def svr_get_stage_times(self, reset: bool = True) -> dict:
+        n = _lib.svr_num_stages()
+        ms, calls = (C.c_double * n)(), (C.c_int64 * n)()
+        self._check(_lib.svr_get_stage_times(self.handle, C.cast(ms, C.c_void_p), C.cast(calls, C.c_void_p), 1 if reset else 0))
+        return {_lib.svr_stage_name(i).decode(): (float(ms[i]), int(calls[i])) for i in range(n)}
 
     # ---- the four calls of the path -------------------------------------------------------------
     def svr_preprocess(self, vox: Voxels, cam) -> Frame:

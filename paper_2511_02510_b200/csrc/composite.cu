@@ -170,14 +170,15 @@ __device__ __forceinline__ float transpose_reduce11(float* v, int lane) {
     return v[0] + __shfl_xor_sync(FULL, v[0], 1);
 }
 
-template <int K, bool BWD>
+template <int K, bool BWD, bool STATS>
 __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ vals,
                                                         const uint32_t* __restrict__ ranges, const ushort4* __restrict__ rects,
                                                         const float4* __restrict__ rgbm, float T_min,
                                                         float* __restrict__ image, float* __restrict__ depth,
                                                         float* __restrict__ T_final, unsigned int* __restrict__ w_max,
                                                         const float* __restrict__ dL, const float* __restrict__ image_in,
-                                                        float* __restrict__ grad_raw, float* __restrict__ grad_rgb) {
+                                                        float* __restrict__ grad_raw, float* __restrict__ grad_rgb,
+                                                        unsigned long long* __restrict__ stats) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Staged& S = *reinterpret_cast<Staged*>(smem_raw);
     float* acc = reinterpret_cast<float*>(smem_raw + sizeof(Staged));   // [CHUNK*12], BWD only
@@ -200,6 +201,7 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
         for (int a = 0; a < 3; ++a) { ray.dh[a] = 0.f; ray.dl[a] = 0.f; ray.inv[a] = 0.f; ray.ainv[a] = 0.f; }
     }
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dep = 0.f;
+    unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_staged = 0;   // STATS only
     float G0 = 0.f, G1 = 0.f, G2 = 0.f, F0 = 0.f, F1 = 0.f, F2 = 0.f;
     if (BWD) {
         if (inimg) {
@@ -220,6 +222,7 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
                 bool valid = idx < end;
                 uint32_t vid = valid ? __ldg(vals + idx) : 0u;
                 stage_entry(S, tid, valid, vid, s, c, rects, rgbm);
+                if (STATS && valid) ++n_staged;
             }
             __syncthreads();
             const int nchunk = min((uint32_t)CHUNK, end - base);
@@ -238,6 +241,7 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
                                         py >= (int)(rx >> 16) && py <= (int)(ry >> 16);
                     float w = 0.f;
                     float gv[11];
+                    if (STATS) { n_surv += (lane == 0); n_test += inside; }
                     if (BWD) {
 #pragma unroll
                         for (int i = 0; i < 11; ++i) gv[i] = 0.f;
@@ -250,6 +254,7 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
                             float dtau[8];
                             float tau = integrate<K, BWD>(ray, D, a.w, s0, s1, ra, rb, dtau);
                             float E = __expf(-tau);
+                            if (STATS) ++n_hit;
                             w = T * (1.f - E);
                             T *= E;
                             C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
@@ -293,6 +298,14 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
             if (!any_alive) break;
         }
     }
+    if (STATS) {
+        unsigned int v4[4] = {n_hit, n_test, n_surv, n_staged};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            unsigned int t = __reduce_add_sync(FULL, v4[i]);
+            if (lane == 0 && t) atomicAdd(stats + i, (unsigned long long)t);
+        }
+    }
     if (!BWD && inimg) {
         image[pix * 3] = fmaf(T, c.bg[0], C0);
         image[pix * 3 + 1] = fmaf(T, c.bg[1], C1);
@@ -304,15 +317,20 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
 
 template <bool BWD>
 SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
-                           float* w_max, const float* dL, const float* image_in, float* grad_raw, float* grad_rgb) {
+                           float* w_max, const float* dL, const float* image_in, float* grad_raw, float* grad_rgb,
+                           unsigned long long* stats) {
     if (f->n_tiles == 0) return SVR_OK;
+    StageScope scope__(ctx, BWD ? ST_BACKWARD : ST_FORWARD);
     size_t smem = sizeof(Staged) + (BWD ? CHUNK * 12 * sizeof(float) : 0);
     const ushort4* rects = reinterpret_cast<const ushort4*>(f->rects);
     const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
-#define SVR_LAUNCH(KK)                                                                                                     \
-    composite_kernel<KK, BWD><<<f->n_tiles, 256, smem, ctx->stream>>>(f->scene, f->cam, f->vals, f->ranges, rects, rgbm, T_min, \
-                                                                      image, depth, T_final, wm, dL, image_in, grad_raw, grad_rgb)
+#define SVR_ARGS f->scene, f->cam, f->vals, f->ranges, rects, rgbm, T_min, image, depth, T_final, wm, dL, image_in, grad_raw, grad_rgb, stats
+#define SVR_LAUNCH(KK)                                                                             \
+    do {                                                                                           \
+        if (!BWD && stats) composite_kernel<KK, false, true><<<f->n_tiles, 256, smem, ctx->stream>>>(SVR_ARGS); \
+        else composite_kernel<KK, BWD, false><<<f->n_tiles, 256, smem, ctx->stream>>>(SVR_ARGS);   \
+    } while (0)
     switch (K) {
         case 1: SVR_LAUNCH(1); break;
         case 2: SVR_LAUNCH(2); break;
@@ -321,6 +339,7 @@ SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_mi
         default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     }
 #undef SVR_LAUNCH
+#undef SVR_ARGS
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
@@ -329,11 +348,11 @@ SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_mi
 }  // namespace
 
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
-                         float* w_max) {
-    return launch_composite<false>(ctx, f, K, T_min, image, depth, T_final, w_max, nullptr, nullptr, nullptr, nullptr);
+                         float* w_max, unsigned long long* stats) {
+    return launch_composite<false>(ctx, f, K, T_min, image, depth, T_final, w_max, nullptr, nullptr, nullptr, nullptr, stats);
 }
 
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
                           float* grad_raw, float* grad_rgb, float* w_max) {
-    return launch_composite<true>(ctx, f, K, T_min, nullptr, nullptr, nullptr, w_max, dL, image, grad_raw, grad_rgb);
+    return launch_composite<true>(ctx, f, K, T_min, nullptr, nullptr, nullptr, w_max, dL, image, grad_raw, grad_rgb, nullptr);
 }

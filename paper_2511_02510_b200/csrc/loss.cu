@@ -155,6 +155,7 @@ __global__ void __launch_bounds__(256) grad_kernel(const float* __restrict__ mag
 
 SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma, float eps,
                            float q, int sobel_source, float* dL, float* loss) {
+    StageScope scope__(ctx, ST_LOSS);
     const int64_t n = (int64_t)W * H;
     size_t need = sizeof(LossWs) + sizeof(float) * (size_t)n + 256;
     if (ctx->loss_ws_bytes < need) {

@@ -284,6 +284,7 @@ inline unsigned int blocks_for(int64_t n, int bs) { return (unsigned int)((n + b
 }  // namespace
 
 SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f) {
+    StageScope scope__(ctx, ST_TILE_MASKS);
     dim3 grid(f->cam.tiles_x, f->cam.tiles_y), block(SVR_TILE, SVR_TILE);
     tile_mask_kernel<<<grid, block, 0, ctx->stream>>>(f->cam, f->tile_masks);
     sat_kernel<<<1, 256, 0, ctx->stream>>>(f->tile_masks, f->sat, f->cam.tiles_x, f->cam.tiles_y);
@@ -294,6 +295,7 @@ SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f) {
 
 // totals[1] = number of "big" voxels (caller zeroes); totals[0] is filled by the caller from the scan.
 SvrStatus launch_rects_counts(SvrContext* ctx, SvrFrame* f, uint32_t* counts, unsigned long long* totals) {
+    StageScope scope__(ctx, ST_RECTS);
     rect_count_kernel<<<blocks_for(f->scene.n + 1, 256), 256, 0, ctx->stream>>>(
         f->scene, f->cam, f->sat, reinterpret_cast<ushort4*>(f->rects), counts, totals);
     ctx->launches += 1;
@@ -303,6 +305,7 @@ SvrStatus launch_rects_counts(SvrContext* ctx, SvrFrame* f, uint32_t* counts, un
 
 SvrStatus launch_emit_keys(SvrContext* ctx, SvrFrame* f, uint64_t* keys, uint32_t* vals, uint32_t* big_list,
                                 unsigned int* big_count) {
+    StageScope scope__(ctx, ST_EMIT);
     emit_small_kernel<<<blocks_for(f->scene.n, 256), 256, 0, ctx->stream>>>(
         f->scene, f->cam, reinterpret_cast<const ushort4*>(f->rects), f->offsets, f->tile_masks, keys, vals, big_list, big_count);
     emit_big_kernel<<<148 * 4, 256, 0, ctx->stream>>>(f->scene, f->cam, reinterpret_cast<const ushort4*>(f->rects), f->offsets,
@@ -313,6 +316,7 @@ SvrStatus launch_emit_keys(SvrContext* ctx, SvrFrame* f, uint64_t* keys, uint32_
 }
 
 SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
+    StageScope scope__(ctx, ST_RANGES);
     SVR_CUDA(ctx, cudaMemsetAsync(f->ranges, 0, sizeof(uint32_t) * 16 * (size_t)f->n_tiles, ctx->stream));
     if (f->n_entries > 0) {
         ranges_kernel<<<blocks_for(f->n_entries, 256), 256, 0, ctx->stream>>>(f->keys, f->n_entries, 3 * f->scene.max_level,
@@ -324,6 +328,7 @@ SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
 }
 
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
+    StageScope scope__(ctx, ST_COLORS);
     if (f->scene.n == 0) return SVR_OK;
     unsigned int g = blocks_for(f->scene.n, 256);
     const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
@@ -340,6 +345,7 @@ SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
 }
 
 SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_rgb, float* grad_sh) {
+    StageScope scope__(ctx, ST_SH_BACKWARD);
     if (f->scene.n == 0) return SVR_OK;
     unsigned int g = blocks_for(f->scene.n, 256);
     const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);

@@ -5,6 +5,7 @@
 #include <cub/cub.cuh>
 
 SvrStatus launch_exclusive_scan(SvrContext* ctx, const uint32_t* in, uint32_t* out, int64_t n_plus_1) {
+    StageScope scope__(ctx, ST_SCAN);
     size_t tmp_bytes = 0;
     SVR_CUDA(ctx, cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, in, out, n_plus_1, ctx->stream));
     void* tmp = nullptr;
@@ -18,6 +19,7 @@ SvrStatus launch_exclusive_scan(SvrContext* ctx, const uint32_t* in, uint32_t* o
 
 SvrStatus launch_sort_pairs(SvrContext* ctx, uint64_t* keys, uint64_t* keys_alt, uint32_t* vals, uint32_t* vals_alt,
                             int64_t n, int bits, uint64_t** keys_sorted, uint32_t** vals_sorted) {
+    StageScope scope__(ctx, ST_SORT);
     cub::DoubleBuffer<uint64_t> dk(keys, keys_alt);
     cub::DoubleBuffer<uint32_t> dv(vals, vals_alt);
     size_t tmp_bytes = 0;

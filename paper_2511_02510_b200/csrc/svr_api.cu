@@ -119,6 +119,8 @@ void svr_destroy(SvrContext* ctx) {
     if (ctx->loss_ws) cudaFreeAsync(ctx->loss_ws, ctx->stream);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     cudaStreamSynchronize(ctx->stream);
+    for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
+    for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
     delete ctx;
 }
 
@@ -257,7 +259,7 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
                       float* T_final, float* w_max) {
     if (!ctx || !frame || !opts || !image) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
-    return launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max);
+    return launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max, nullptr);
 }
 
 SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H, float gamma,
@@ -332,6 +334,56 @@ SvrStatus svr_frame_lists(const SvrFrame* frame, const uint64_t** keys, const ui
 SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm) {
     if (!frame || !rgbm) return SVR_ERR_INVALID_ARG;
     *rgbm = frame->rgbm;
+    return SVR_OK;
+}
+
+SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* image,
+                            uint64_t* stats_host) {
+    if (!ctx || !frame || !opts || !image || !stats_host) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
+    unsigned long long* d = nullptr;
+    SVR_TRY(svr_alloc(ctx, (void**)&d, 64));
+    cudaMemsetAsync(d, 0, 64, ctx->stream);
+    SvrStatus st = launch_forward(ctx, frame, opts->K, opts->T_min, image, nullptr, nullptr, nullptr, d);
+    if (st == SVR_OK) {
+        cudaError_t e = cudaMemcpyAsync(stats_host, d, 32, cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "stats readback: %s", cudaGetErrorString(e));
+    }
+    svr_free(ctx, d, 64);
+    return st;
+}
+
+void svr_set_stage_timing(SvrContext* ctx, int enabled) {
+    if (ctx) ctx->timing = enabled != 0;
+}
+
+int svr_num_stages(void) { return ST_COUNT; }
+
+const char* svr_stage_name(int stage) {
+    static const char* names[ST_COUNT] = {"tile_masks", "rects_counts", "scan", "emit_keys", "sort", "ranges", "voxel_colors",
+                                          "forward_composite", "loss_grad", "backward_composite", "sh_backward"};
+    return (stage >= 0 && stage < ST_COUNT) ? names[stage] : "";
+}
+
+SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset) {
+    if (!ctx) return SVR_ERR_INVALID_ARG;
+    SVR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (const StagePending& p : ctx->pending) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, p.e0, p.e1) == cudaSuccess) {
+            ctx->stage_ms[p.stage] += (double)t;
+            ctx->stage_calls[p.stage] += 1;
+        }
+        ctx->event_pool.push_back(p.e0);
+        ctx->event_pool.push_back(p.e1);
+    }
+    ctx->pending.clear();
+    for (int i = 0; i < ST_COUNT; ++i) {
+        if (ms) ms[i] = ctx->stage_ms[i];
+        if (calls) calls[i] = ctx->stage_calls[i];
+        if (reset) { ctx->stage_ms[i] = 0.0; ctx->stage_calls[i] = 0; }
+    }
     return SVR_OK;
 }
 

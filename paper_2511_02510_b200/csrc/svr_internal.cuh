@@ -4,12 +4,25 @@
 #include <stdint.h>
 #include <stddef.h>
 #include <string>
+#include <vector>
 #include "svr.h"
 
 #define SVR_TILE 16
 #define SVR_MAX_K 4
 
+enum SvrStage {
+    ST_TILE_MASKS = 0, ST_RECTS, ST_SCAN, ST_EMIT, ST_SORT, ST_RANGES, ST_COLORS, ST_FORWARD, ST_LOSS, ST_BACKWARD,
+    ST_SH_BACKWARD, ST_COUNT
+};
+
+struct StagePending { int stage; cudaEvent_t e0, e1; };
+
 struct SvrContext {
+    bool timing = false;
+    std::vector<StagePending> pending;
+    std::vector<cudaEvent_t> event_pool;
+    double stage_ms[ST_COUNT] = {0};
+    int64_t stage_calls[ST_COUNT] = {0};
     int device = 0;
     cudaStream_t stream = nullptr;
     size_t budget = 0;            // 0 = unlimited
@@ -77,6 +90,21 @@ SvrStatus svr_fail(SvrContext* ctx, SvrStatus st, const char* fmt, ...);
         if (s__ != SVR_OK) return s__;         \
     } while (0)
 
+// Brackets the kernels of one stage with CUDA events on the context's stream when timing is enabled.
+struct StageScope {
+    SvrContext* ctx; int stage; cudaEvent_t e0 = nullptr, e1 = nullptr;
+    static cudaEvent_t get(SvrContext* c) {
+        if (!c->event_pool.empty()) { cudaEvent_t e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+        cudaEvent_t e; cudaEventCreate(&e); return e;
+    }
+    StageScope(SvrContext* c, int st) : ctx(c), stage(st) {
+        if (ctx->timing) { e0 = get(ctx); e1 = get(ctx); cudaEventRecord(e0, ctx->stream); }
+    }
+    ~StageScope() {
+        if (e0) { cudaEventRecord(e1, ctx->stream); ctx->pending.push_back({stage, e0, e1}); }
+    }
+};
+
 // ---- workspace pool --------------------------------------------------------------------------
 SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes);
 void svr_free(SvrContext* ctx, void* p, size_t bytes);
@@ -92,7 +120,7 @@ SvrStatus launch_sort_pairs(SvrContext* ctx, uint64_t* keys, uint64_t* keys_alt,
 SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
-                         float* T_final, float* w_max);
+                         float* T_final, float* w_max, unsigned long long* stats);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
                           float* grad_raw, float* grad_rgb, float* w_max);
 SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_rgb, float* grad_sh);
