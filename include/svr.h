@@ -137,6 +137,8 @@ SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRen
                             uint64_t* stats_host);
 void svr_set_stage_timing(SvrContext* ctx, int enabled);
 int svr_num_stages(void);
+/* Experiments only: bit 0 makes svr_backward skip its gradient reductions (timing the arithmetic alone). */
+void svr_set_debug_flags(SvrContext* ctx, int flags);
 const char* svr_stage_name(int stage);
 SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset);
 

@@ -22,7 +22,7 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
            "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
-           "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times"]
+           "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags"]
 
 
 class SvrError(RuntimeError):
@@ -80,6 +80,8 @@ def _load():
     lib.svr_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.svr_set_stage_timing.restype = None
     lib.svr_num_stages.restype = C.c_int
+    lib.svr_set_debug_flags.argtypes = [C.c_void_p, C.c_int]
+    lib.svr_set_debug_flags.restype = None
     lib.svr_stage_name.argtypes = [C.c_int]
     lib.svr_stage_name.restype = C.c_char_p
     lib.svr_get_stage_times.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]

@@ -1,38 +1,52 @@
 // Stage (3) forward compositing and stage (4) backward compositing (DESIGN.md rows a7, a9).
 //
-// One CTA per 16x16 tile, 8 warps, each warp owns an 8x4 pixel block. The tile's sorted (tile, octant)
-// list is staged CHUNK entries at a time into shared memory (voxel geometry relative to the camera centre
-// in double-float form, 8 corner raws, per-view colour, pixel rectangle). Each warp first culls a batch of
-// 32 staged voxels against its own 8x4 block (one rectangle test per lane, ballot), then walks only the
-// survivors in list order; every lane slab-tests the survivor against its ray, integrates K midpoint
-// samples of the trilinear raw density, and composites (eqs. 2-4). w_max (eq. 5) is reduced
-// across the warp with one REDUX and one atomicMax per (warp, voxel). A ray stops once T < T_min; a warp
-// stops when all its rays have, the CTA when all warps have.
+// One CTA per 16x16 tile; each of its 8 warps owns an 8x4 pixel block and runs independently (no CTA
+// barrier anywhere): a barrier per staged chunk cost 37% of the issue slots in the first version
+// (profiles/r1a_*), because the 8 blocks of a tile see very different numbers of voxels.
 //
-// Precision: the ray is set up in fp64 per pixel and kept as hi+lo floats; voxel centres relative to the
-// camera are staged as hi+lo floats. The slab test runs in coordinates relative to the ray's closest
-// approach to the voxel centre, so the segment length (a difference of two O(1) ray parameters in the
-// naive form) keeps ~1e-7 relative accuracy even for 4e-3-wide voxels 2.5 units away.
+// Per warp, over the tile's sorted (tile, octant) list:
+//   1. cull: 32 entries at a time, lane i reads entry i's pixel rectangle (stored in list order by the
+//      range kernel, so the read is coalesced) and computes the 32-bit mask M of this warp's pixels it
+//      covers. M == 0 => the entry is skipped by this warp (76% of (warp, entry) pairs on C4).
+//   2. stage: surviving lanes gather their voxel (octree cell, 8 corner raws, per-view colour) and write
+//      it, in list order, into a warp-private shared-memory ring: centre relative to the camera as hi+lo
+//      floats (computed in fp64), half edge, raws, colour, M.
+//   3. walk: once >= 32 survivors are staged (or the list ends), the 32x32 bit matrix M[slot][pixel] is
+//      transposed across the warp with 5 shuffles, giving every lane the bitmask of slots that cover ITS
+//      pixel. Each lane then pops its own next candidate (ffs) and slab-tests / integrates / composites it:
+//      lanes work on different voxels in the same instruction, so the expensive hit path (K trilinear
+//      samples, exp) runs with most lanes active instead of the ~7 of 32 a 2-pixel voxel covers.
+//      Front-to-back order per pixel is kept because slots are in list order.
+// Forward: eqs. 2-4; w_max (eq. 5) by atomicMax guarded by a plain read (w_max only grows).
+// Backward: same walk with the stored final colour, S_k = image - prefix_k (no division by 1 - alpha),
+//   dL/dtau_k = G . (T_k c_k - S_k); each hit adds its 8 corner + 3 colour gradients with three 16-byte
+//   vector reductions (red.global.add.v4.f32) - measured 165 G vector ops/s on B200, independent of
+//   how many lanes share an address, so no shared-memory staging (float atomics in shared memory are CAS
+//   loops on sm_100a: ATOMS.CAST.SPIN).
 //
-// Backward re-walks the list in the same front-to-back order with the stored final colour: the suffix
-// colour S_k = image - prefix_k needs no division by (1 - alpha) (stable for tau >> 1), and
-// dL/dtau_k = G . (T_k c_k - S_k). Per (warp, voxel) the 8 corner gradients + 3 colour gradients are
-// reduced with a transposing butterfly (16 shuffles for all 11 values), accumulated per CTA in shared
-// memory, and flushed once per chunk with coalesced float atomics.
+// Density: the trilinear raw density is staged as polynomial coefficients (c0, cx, cy, cz, cxy, cxz, cyz,
+// cxyz), pre-multiplied by log2(e), so a sample costs 7 FMA + one EX2 instead of 7 lerps (14 ops) + MUL + EX2.
+// Backward accumulates the gradient w.r.t. those coefficients (monomials 1, qx, qy, qz, qxqy, ...) into a
+// per-voxel scratch; the per-voxel finalize kernel (preprocess.cu) maps it back to the 8 corners.
+//
+// Precision: the ray is set up in fp64 per pixel and kept as hi+lo floats; the slab test runs in
+// coordinates relative to the ray's closest approach to the voxel centre, so the segment length keeps
+// ~1e-7 relative accuracy even for 4e-3-wide voxels 2.5 units away (a plain fp32 t_out - t_in loses 1e-4).
 #include "svr_internal.cuh"
 
 namespace {
 
-constexpr int CHUNK = 256;
 constexpr unsigned FULL = 0xffffffffu;
+constexpr int RING = 64;          // staging slots per warp
+constexpr int WARPS = 8;
 
-struct Staged {
-    float4 g0[CHUNK];   // gh.xyz, h (half edge)
-    float4 g1[CHUNK];   // gl.xyz, voxel id bits
-    float4 r0[CHUNK];   // raw corners 0..3
-    float4 r1[CHUNK];   // raw corners 4..7
-    float4 col[CHUNK];  // r, g, b, clamp mask
-    uint2 rect[CHUNK];  // x0 | y0 << 16, x1 | y1 << 16
+struct WarpStage {
+    float4 g0[RING];    // gh.xyz, h (half edge)
+    float4 g1[RING];    // gl.xyz, voxel id bits
+    float4 r0[RING];    // log2(e) * (c0, cx, cy, cz)
+    float4 r1[RING];    // log2(e) * (cxy, cxz, cyz, cxyz)
+    float4 col[RING];   // r, g, b, clamp mask
+    unsigned int M[RING];   // pixels of this warp's 8x4 block covered by the voxel's rectangle
 };
 
 struct RayF {
@@ -60,13 +74,11 @@ __device__ __forceinline__ void setup_ray(const CamDev& c, int px, int py, RayF&
     }
 }
 
-__device__ __forceinline__ void stage_entry(Staged& S, int j, bool valid, uint32_t vid, const SceneDev& s, const CamDev& c,
-                                            const ushort4* __restrict__ rects, const float4* __restrict__ rgbm) {
-    if (!valid) {
-        S.rect[j] = make_uint2(0xFFFFFFFFu, 0u);
-        return;
-    }
+__device__ __forceinline__ void stage_voxel(WarpStage& S, int slot, uint32_t vid, unsigned int M, const SceneDev& s,
+                                            const CamDev& c, const float4* __restrict__ rgbm) {
     uint2 q = __ldg(reinterpret_cast<const uint2*>(s.ijkl) + vid);
+    const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
+    float4 ra = __ldg(rp), rb = __ldg(rp + 1), col = __ldg(rgbm + vid);
     int L = q.y >> 16;
     float ef = s.root_edge * __int_as_float((127 - L) << 23);
     double e = (double)ef;
@@ -74,20 +86,45 @@ __device__ __forceinline__ void stage_entry(Staged& S, int j, bool valid, uint32
     double gy = (double)s.root_lo[1] + ((double)(q.x >> 16) + 0.5) * e - c.o[1];
     double gz = (double)s.root_lo[2] + ((double)(q.y & 0xFFFF) + 0.5) * e - c.o[2];
     float hx = (float)gx, hy = (float)gy, hz = (float)gz;
-    S.g0[j] = make_float4(hx, hy, hz, 0.5f * ef);
-    S.g1[j] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
-    const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
-    S.r0[j] = __ldg(rp);
-    S.r1[j] = __ldg(rp + 1);
-    S.col[j] = __ldg(rgbm + vid);
-    ushort4 r = __ldg(rects + vid);
-    S.rect[j] = make_uint2((unsigned)r.x | ((unsigned)r.y << 16), (unsigned)r.z | ((unsigned)r.w << 16));
+    S.g0[slot] = make_float4(hx, hy, hz, 0.5f * ef);
+    S.g1[slot] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
+    // trilinear -> polynomial coefficients, scaled by log2(e) (corner c = bx + 2 by + 4 bz)
+    const float L2E = 1.4426950408889634f;
+    float c0 = ra.x, cx = ra.y - ra.x, cy = ra.z - ra.x, cz = rb.x - ra.x;
+    float cxy = (ra.w - ra.y) - cy, cxz = (rb.y - ra.y) - cz, cyz = (rb.z - ra.z) - cz;
+    float cxyz = ((rb.w - rb.z) - (rb.y - rb.x)) - ((ra.w - ra.z) - (ra.y - ra.x));
+    S.r0[slot] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
+    S.r1[slot] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
+    S.col[slot] = col;
+    S.M[slot] = M;
+}
+
+// 32-bit mask of the lanes (pixel = (wbx0 + (lane & 7), wby0 + (lane >> 3))) inside the rectangle.
+__device__ __forceinline__ unsigned int block_cover_mask(uint2 rc, int wbx0, int wby0) {
+    int cx0 = max((int)(rc.x & 0xFFFF) - wbx0, 0), cx1 = min((int)(rc.y & 0xFFFF) - wbx0, 7);
+    int cy0 = max((int)(rc.x >> 16) - wby0, 0), cy1 = min((int)(rc.y >> 16) - wby0, 3);
+    if (cx0 > cx1 || cy0 > cy1) return 0u;
+    unsigned int colm = ((2u << cx1) - (1u << cx0)) & 0xFFu;
+    unsigned int rowb = ((2u << cy1) - (1u << cy0)) & 0xFu;
+    unsigned int rows = (rowb & 1u) | ((rowb & 2u) << 7) | ((rowb & 4u) << 14) | ((rowb & 8u) << 21);
+    return colm * rows;
+}
+
+// Transpose a 32x32 bit matrix held one row per lane (row i in lane i): returns column `lane`.
+__device__ __forceinline__ unsigned int transpose32(unsigned int x, int lane) {
+#pragma unroll
+    for (int j = 16; j >= 1; j >>= 1) {
+        const unsigned int m = (j == 16) ? 0x0000FFFFu : (j == 8) ? 0x00FF00FFu : (j == 4) ? 0x0F0F0F0Fu
+                             : (j == 2) ? 0x33333333u : 0x55555555u;
+        unsigned int t = __shfl_xor_sync(FULL, x, j);
+        x = (lane & j) ? (((t >> j) & m) | (x & ~m)) : ((x & m) | ((t & m) << j));
+    }
+    return x;
 }
 
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
 
 // Ray/voxel segment in coordinates relative to t_ref (the ray parameter closest to the voxel centre).
-// Returns hit; outputs s0, s1 (segment in relative parameter), t_ref, D[3] (centre offset from the ray).
 __device__ __forceinline__ bool slab(const RayF& r, const float4& a, const float4& b, float& s0, float& s1, float& t_ref,
                                      float* D) {
     t_ref = fmaf(a.z, r.dh[2], fmaf(a.y, r.dh[1], a.x * r.dh[0]));
@@ -102,15 +139,23 @@ __device__ __forceinline__ bool slab(const RayF& r, const float4& a, const float
     return s1 > s0;
 }
 
+__device__ __forceinline__ float ex2f(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// K midpoint samples (R5). ca/cb = polynomial coefficients * log2(e). Returns tau; BWD also returns
+// dtau[m] = d tau / d coef_m (natural-scale coefficients), m over monomials 1, qx, qy, qz, qxqy, qxqz, qyqz, qxqyqz.
 template <int K, bool BWD>
-__device__ __forceinline__ float integrate(const RayF& r, const float* D, float h, float s0, float s1, const float4& ra,
-                                           const float4& rb, float* dtau) {
+__device__ __forceinline__ float integrate(const RayF& r, const float* D, float h, float s0, float s1, const float4& ca,
+                                           const float4& cb, float* dtau) {
     float inv_e = __int_as_float(0x7E800000 - __float_as_int(h));   // 0.5 / h for h a power of two
     float dt = (s1 - s0) * (1.0f / (float)K);
     float sum = 0.f;
     if (BWD) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) dtau[c] = 0.f;
+        for (int c = 1; c < 8; ++c) dtau[c] = 0.f;
     }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
@@ -118,72 +163,44 @@ __device__ __forceinline__ float integrate(const RayF& r, const float* D, float 
         float qx = __saturatef(fmaf(fmaf(s, r.dh[0], -D[0]), inv_e, 0.5f));
         float qy = __saturatef(fmaf(fmaf(s, r.dh[1], -D[1]), inv_e, 0.5f));
         float qz = __saturatef(fmaf(fmaf(s, r.dh[2], -D[2]), inv_e, 0.5f));
-        float r00 = lerpf(ra.x, ra.y, qx), r10 = lerpf(ra.z, ra.w, qx);
-        float r01 = lerpf(rb.x, rb.y, qx), r11 = lerpf(rb.z, rb.w, qx);
-        float rr = lerpf(lerpf(r00, r10, qy), lerpf(r01, r11, qy), qz);
-        float sig = __expf(rr);
+        float hi = fmaf(fmaf(cb.w, qz, cb.x), qy, fmaf(cb.y, qz, ca.y));     // (cxyz qz + cxy) qy + (cxz qz + cx)
+        float lo = fmaf(fmaf(cb.z, qz, ca.z), qy, fmaf(ca.w, qz, ca.x));     // (cyz qz + cy) qy + (cz qz + c0)
+        float sig = ex2f(fmaf(hi, qx, lo));
         sum += sig;
         if (BWD) {
-            float sy0 = sig * (1.f - qy), sy1 = sig * qy;
-            float a00 = sy0 * (1.f - qx), a10 = sy0 * qx, a01 = sy1 * (1.f - qx), a11 = sy1 * qx;
-            float z0 = 1.f - qz;
-            dtau[0] = fmaf(a00, z0, dtau[0]); dtau[1] = fmaf(a10, z0, dtau[1]);
-            dtau[2] = fmaf(a01, z0, dtau[2]); dtau[3] = fmaf(a11, z0, dtau[3]);
-            dtau[4] = fmaf(a00, qz, dtau[4]); dtau[5] = fmaf(a10, qz, dtau[5]);
-            dtau[6] = fmaf(a01, qz, dtau[6]); dtau[7] = fmaf(a11, qz, dtau[7]);
+            float sx = sig * qx, sy = sig * qy, sz = sig * qz;
+            dtau[1] += sx; dtau[2] += sy; dtau[3] += sz;
+            float sxy = sx * qy;
+            dtau[4] += sxy;
+            dtau[5] = fmaf(sx, qz, dtau[5]);
+            dtau[6] = fmaf(sy, qz, dtau[6]);
+            dtau[7] = fmaf(sxy, qz, dtau[7]);
         }
     }
     if (BWD) {
+        dtau[0] = sum * dt;
 #pragma unroll
-        for (int c = 0; c < 8; ++c) dtau[c] *= dt;
+        for (int c = 1; c < 8; ++c) dtau[c] *= dt;
     }
     return dt * sum;
 }
 
-// Sum 11 per-lane values across the warp; after the call lane l (even) holds the total of value
-// idx(l) = 8*b4 + 4*b3 + 2*b2 + b1 (bits of l). 16 shuffles instead of 55.
-__device__ __forceinline__ float transpose_reduce11(float* v, int lane) {
-    bool up = lane & 16;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        float hi = (i + 8 < 11) ? v[i + 8] : 0.f;
-        float send = up ? v[i] : hi, keep = up ? hi : v[i];
-        v[i] = keep + __shfl_xor_sync(FULL, send, 16);
-    }
-    up = lane & 8;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        float send = up ? v[i] : v[i + 4], keep = up ? v[i + 4] : v[i];
-        v[i] = keep + __shfl_xor_sync(FULL, send, 8);
-    }
-    up = lane & 4;
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        float send = up ? v[i] : v[i + 2], keep = up ? v[i + 2] : v[i];
-        v[i] = keep + __shfl_xor_sync(FULL, send, 4);
-    }
-    up = lane & 2;
-    {
-        float send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
-        v[0] = keep + __shfl_xor_sync(FULL, send, 2);
-    }
-    return v[0] + __shfl_xor_sync(FULL, v[0], 1);
+__device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, float d) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
-
 template <int K, bool BWD, bool STATS>
 __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ vals,
-                                                        const uint32_t* __restrict__ ranges, const ushort4* __restrict__ rects,
+                                                        const uint2* __restrict__ rects_sorted,
+                                                        const uint32_t* __restrict__ ranges,
                                                         const float4* __restrict__ rgbm, float T_min,
                                                         float* __restrict__ image, float* __restrict__ depth,
                                                         float* __restrict__ T_final, unsigned int* __restrict__ w_max,
                                                         const float* __restrict__ dL, const float* __restrict__ image_in,
-                                                        float* __restrict__ grad_raw, float* __restrict__ grad_rgb,
-                                                        unsigned long long* __restrict__ stats) {
+                                                        float* __restrict__ grad_coef, float* __restrict__ grad_rgb,
+                                                        unsigned long long* __restrict__ stats, int dbg) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    Staged& S = *reinterpret_cast<Staged*>(smem_raw);
-    float* acc = reinterpret_cast<float*>(smem_raw + sizeof(Staged));   // [CHUNK*12], BWD only
-
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    WarpStage& S = reinterpret_cast<WarpStage*>(smem_raw)[warp];
     const int tile = blockIdx.x;
     const int tile_x = tile % c.tiles_x, tile_y = tile / c.tiles_x;
     const int wbx0 = tile_x * SVR_TILE + (warp & 1) * 8, wby0 = tile_y * SVR_TILE + (warp >> 1) * 4;
@@ -201,105 +218,96 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
         for (int a = 0; a < 3; ++a) { ray.dh[a] = 0.f; ray.dl[a] = 0.f; ray.inv[a] = 0.f; ray.ainv[a] = 0.f; }
     }
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dep = 0.f;
-    unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_staged = 0;   // STATS only
     float G0 = 0.f, G1 = 0.f, G2 = 0.f, F0 = 0.f, F1 = 0.f, F2 = 0.f;
-    if (BWD) {
-        if (inimg) {
-            G0 = dL[pix * 3]; G1 = dL[pix * 3 + 1]; G2 = dL[pix * 3 + 2];
-            F0 = image_in[pix * 3]; F1 = image_in[pix * 3 + 1]; F2 = image_in[pix * 3 + 2];
-        }
-        for (int i = tid; i < CHUNK * 12; i += 256) acc[i] = 0.f;
+    unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_read = 0;   // STATS only
+    if (BWD && inimg) {
+        G0 = dL[pix * 3]; G1 = dL[pix * 3 + 1]; G2 = dL[pix * 3 + 2];
+        F0 = image_in[pix * 3]; F1 = image_in[pix * 3 + 1]; F2 = image_in[pix * 3 + 2];
     }
 
     for (int so = 0; so < 8; ++so) {
         const uint32_t start = ranges[(tile * 8 + so) * 2], end = ranges[(tile * 8 + so) * 2 + 1];
-        if (start == end) continue;                                   // CTA-uniform
+        if (start == end) continue;
         bool alive = inimg && (oct == so) && (T >= T_min);
-        for (uint32_t base = start; base < end; base += CHUNK) {
-            __syncthreads();                                          // previous chunk fully consumed / flushed
-            {
-                uint32_t idx = base + tid;
-                bool valid = idx < end;
-                uint32_t vid = valid ? __ldg(vals + idx) : 0u;
-                stage_entry(S, tid, valid, vid, s, c, rects, rgbm);
-                if (STATS && valid) ++n_staged;
+        unsigned int alive_mask = __ballot_sync(FULL, alive);
+        if (alive_mask == 0u) continue;                               // no pixel of this warp uses this list
+        int head = 0, count = 0;                                      // ring state (warp-uniform)
+        uint32_t base = start;
+        while (true) {
+            // ---- cull + stage until 32 survivors are waiting or the list is exhausted ----
+            while (count < 32 && base < end) {
+                uint32_t idx = base + lane;
+                unsigned int M = 0u;
+                uint32_t vid = 0u;
+                if (idx < end) {
+                    M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
+                    if (M) vid = __ldg(vals + idx);
+                }
+                unsigned int m = __ballot_sync(FULL, M != 0u);
+                if (M) stage_voxel(S, (head + count + __popc(m & ((1u << lane) - 1u))) & (RING - 1), vid, M, s, c, rgbm);
+                if (BWD && M) {
+                    // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the
+                    // DRAM fill (3.4 ms -> 5.2 ms without this on C4)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
+                }
+                count += __popc(m);
+                base += 32;
+                if (STATS) { n_read += (idx < end); n_surv += (M != 0u); }
             }
-            __syncthreads();
-            const int nchunk = min((uint32_t)CHUNK, end - base);
-            for (int b = 0; b < nchunk; b += 32) {
-                if (!__any_sync(FULL, alive)) break;                  // whole warp terminated
-                uint2 rc = S.rect[b + lane];
-                bool ov = (int)(rc.x & 0xFFFF) <= wbx0 + 7 && (int)(rc.y & 0xFFFF) >= wbx0 &&
-                          (int)(rc.x >> 16) <= wby0 + 3 && (int)(rc.y >> 16) >= wby0;
-                unsigned m = __ballot_sync(FULL, ov);
-                while (m) {
-                    const int jj = __ffs(m) - 1;
-                    m &= m - 1;
-                    const int j = b + jj;
-                    const unsigned rx = __shfl_sync(FULL, rc.x, jj), ry = __shfl_sync(FULL, rc.y, jj);
-                    const bool inside = alive && px >= (int)(rx & 0xFFFF) && px <= (int)(ry & 0xFFFF) &&
-                                        py >= (int)(rx >> 16) && py <= (int)(ry >> 16);
-                    float w = 0.f;
-                    float gv[11];
-                    if (STATS) { n_surv += (lane == 0); n_test += inside; }
-                    if (BWD) {
-#pragma unroll
-                        for (int i = 0; i < 11; ++i) gv[i] = 0.f;
-                    }
-                    if (inside) {
-                        const float4 a = S.g0[j], bq = S.g1[j];
-                        float s0, s1, t_ref, D[3];
-                        if (slab(ray, a, bq, s0, s1, t_ref, D)) {
-                            const float4 ra = S.r0[j], rb = S.r1[j], col = S.col[j];
-                            float dtau[8];
-                            float tau = integrate<K, BWD>(ray, D, a.w, s0, s1, ra, rb, dtau);
-                            float E = __expf(-tau);
-                            if (STATS) ++n_hit;
-                            w = T * (1.f - E);
-                            T *= E;
-                            C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
-                            if (!BWD) Dep = fmaf(w, t_ref + 0.5f * (s0 + s1), Dep);
-                            if (BWD) {
-                                // suffix colour S_k = final - prefix_k; dL/dtau = G . (T_k c_k - S_k)
-                                float dLdtau = G0 * (fmaf(T, col.x, C0) - F0) + G1 * (fmaf(T, col.y, C1) - F1) +
-                                               G2 * (fmaf(T, col.z, C2) - F2);
-#pragma unroll
-                                for (int cc = 0; cc < 8; ++cc) gv[cc] = dLdtau * dtau[cc];
-                                gv[8] = w * G0; gv[9] = w * G1; gv[10] = w * G2;
-                            }
-                            if (T < T_min) alive = false;             // R8: stop after the voxel that crosses T_min
-                        }
-                    }
-                    const unsigned wu = __reduce_max_sync(FULL, __float_as_uint(w));
-                    if (wu != 0u) {
-                        if (w_max != nullptr && lane == 0) atomicMax(w_max + __float_as_uint(S.g1[j].w), wu);
+            if (count == 0) break;
+            __syncwarp();
+            // ---- walk up to 32 staged voxels, every lane through its own candidates ----
+            const int n = min(count, 32);
+            unsigned int cand = transpose32(lane < n ? S.M[(head + lane) & (RING - 1)] : 0u, lane);
+            if (!alive) cand = 0u;
+            while (__any_sync(FULL, cand != 0u)) {
+                if (cand) {
+                    const int slot = (head + __ffs(cand) - 1) & (RING - 1);
+                    cand &= cand - 1;
+                    const float4 a = S.g0[slot], bq = S.g1[slot];
+                    float s0, s1, t_ref, D[3];
+                    if (STATS) ++n_test;
+                    if (slab(ray, a, bq, s0, s1, t_ref, D)) {
+                        const uint32_t vid = __float_as_uint(bq.w);
+                        // w_max only grows, so a stale (cached) read is safe; issued first so that its latency
+                        // hides behind the integration instead of queueing behind this hit's reductions
+                        unsigned int wm_old = 0u;
+                        if (w_max != nullptr) wm_old = w_max[vid];
+                        const float4 ra = S.r0[slot], rb = S.r1[slot], col = S.col[slot];
+                        float dtau[8];
+                        float tau = integrate<K, BWD>(ray, D, a.w, s0, s1, ra, rb, dtau);
+                        float E = ex2f(-1.4426950408889634f * tau);
+                        float w = T * (1.f - E);
+                        T *= E;
+                        C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
+                        if (STATS) ++n_hit;
+                        if (!BWD) Dep = fmaf(w, t_ref + 0.5f * (s0 + s1), Dep);
                         if (BWD) {
-                            float tot = transpose_reduce11(gv, lane);
-                            int idx = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
-                            if (!(lane & 1) && idx < 11 && tot != 0.f) atomicAdd(&acc[j * 12 + idx], tot);
+                            // suffix colour S_k = final - prefix_k; dL/dtau = G . (T_k c_k - S_k)
+                            float dLdtau = G0 * (fmaf(T, col.x, C0) - F0) + G1 * (fmaf(T, col.y, C1) - F1) +
+                                           G2 * (fmaf(T, col.z, C2) - F2);
+                            float* gc = grad_coef + (size_t)vid * 8;
+                            if (!(dbg & 1)) {
+                                red_add_v4(gc, dLdtau * dtau[0], dLdtau * dtau[1], dLdtau * dtau[2], dLdtau * dtau[3]);
+                                red_add_v4(gc + 4, dLdtau * dtau[4], dLdtau * dtau[5], dLdtau * dtau[6], dLdtau * dtau[7]);
+                                red_add_v4(grad_rgb + (size_t)vid * 4, w * G0, w * G1, w * G2, 0.f);
+                            } else if (dLdtau * dtau[0] + dLdtau * dtau[5] + w * G0 == 123.456f) gc[0] = 1.f;
                         }
+                        if (w_max != nullptr && __float_as_uint(w) > wm_old) atomicMax(w_max + vid, __float_as_uint(w));
+                        if (T < T_min) { alive = false; cand = 0u; }          // R8: stop after the voxel that crosses T_min
                     }
                 }
             }
-            const int any_alive = __syncthreads_or(alive ? 1 : 0);
-            if (BWD) {
-                // flush the chunk's accumulators: consecutive threads -> consecutive floats of one voxel
-                for (int i = tid; i < nchunk * 12; i += 256) {
-                    float val = acc[i];
-                    if (val != 0.f) {
-                        acc[i] = 0.f;
-                        int j = i / 12, k = i - j * 12;
-                        uint32_t vid = __float_as_uint(S.g1[j].w);
-                        if (k < 8) atomicAdd(grad_raw + (size_t)vid * 8 + k, val);
-                        else atomicAdd(grad_rgb + (size_t)vid * 4 + (k - 8), val);
-                    }
-                }
-            }
-            if (!any_alive) break;
+            __syncwarp();
+            head = (head + n) & (RING - 1);
+            count -= n;
+            alive_mask = __ballot_sync(FULL, alive);
+            if (alive_mask == 0u) break;                              // whole warp terminated
         }
     }
     if (STATS) {
-        unsigned int v4[4] = {n_hit, n_test, n_surv, n_staged};
+        unsigned int v4[4] = {n_hit, n_test, n_surv, n_read};
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             unsigned int t = __reduce_add_sync(FULL, v4[i]);
@@ -317,19 +325,28 @@ __global__ void __launch_bounds__(256) composite_kernel(SceneDev s, CamDev c, co
 
 template <bool BWD>
 SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
-                           float* w_max, const float* dL, const float* image_in, float* grad_raw, float* grad_rgb,
+                           float* w_max, const float* dL, const float* image_in, float* grad_coef, float* grad_rgb,
                            unsigned long long* stats) {
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, BWD ? ST_BACKWARD : ST_FORWARD);
-    size_t smem = sizeof(Staged) + (BWD ? CHUNK * 12 * sizeof(float) : 0);
-    const ushort4* rects = reinterpret_cast<const ushort4*>(f->rects);
+    const size_t smem = sizeof(WarpStage) * WARPS;
     const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
+    const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
-#define SVR_ARGS f->scene, f->cam, f->vals, f->ranges, rects, rgbm, T_min, image, depth, T_final, wm, dL, image_in, grad_raw, grad_rgb, stats
-#define SVR_LAUNCH(KK)                                                                             \
-    do {                                                                                           \
-        if (!BWD && stats) composite_kernel<KK, false, true><<<f->n_tiles, 256, smem, ctx->stream>>>(SVR_ARGS); \
-        else composite_kernel<KK, BWD, false><<<f->n_tiles, 256, smem, ctx->stream>>>(SVR_ARGS);   \
+#define SVR_ARGS f->scene, f->cam, f->vals, rs, f->ranges, rgbm, T_min, image, depth, T_final, wm, dL, image_in, grad_coef, grad_rgb, stats, ctx->debug_flags
+#define SVR_GO(KERNEL)                                                                                     \
+    do {                                                                                                   \
+        static bool attr_set = false;                                                                      \
+        if (!attr_set) {                                                                                   \
+            SVR_CUDA(ctx, cudaFuncSetAttribute(KERNEL, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+            attr_set = true;                                                                               \
+        }                                                                                                  \
+        KERNEL<<<f->n_tiles, 256, smem, ctx->stream>>>(SVR_ARGS);                                          \
+    } while (0)
+#define SVR_LAUNCH(KK)                                                                \
+    do {                                                                              \
+        if (!BWD && stats) SVR_GO((composite_kernel<KK, false, true>));               \
+        else SVR_GO((composite_kernel<KK, BWD, false>));                              \
     } while (0)
     switch (K) {
         case 1: SVR_LAUNCH(1); break;
@@ -339,6 +356,7 @@ SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_mi
         default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     }
 #undef SVR_LAUNCH
+#undef SVR_GO
 #undef SVR_ARGS
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
@@ -353,6 +371,6 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
 }
 
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
-                          float* grad_raw, float* grad_rgb, float* w_max) {
-    return launch_composite<true>(ctx, f, K, T_min, nullptr, nullptr, nullptr, w_max, dL, image, grad_raw, grad_rgb, nullptr);
+                          float* grad_coef, float* grad_rgb, float* w_max) {
+    return launch_composite<true>(ctx, f, K, T_min, nullptr, nullptr, nullptr, w_max, dL, image, grad_coef, grad_rgb, nullptr);
 }

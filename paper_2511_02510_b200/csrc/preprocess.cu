@@ -197,9 +197,11 @@ __global__ void __launch_bounds__(256) emit_big_kernel(SceneDev s, CamDev c, con
 
 // ---- B4: ranges -------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ranges_kernel(const uint64_t* __restrict__ keys, int64_t n, int shift,
-                                                     uint32_t* __restrict__ ranges) {
+                                                     uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals,
+                                                     const uint2* __restrict__ rects, uint2* __restrict__ rects_sorted) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    rects_sorted[i] = __ldg(rects + vals[i]);     // rectangle in list order: the compositing cull reads it coalesced
     uint64_t p = keys[i] >> shift;
     if (i == 0 || (keys[i - 1] >> shift) != p) ranges[2 * p] = (uint32_t)i;
     if (i + 1 == n || (keys[i + 1] >> shift) != p) ranges[2 * p + 1] = (uint32_t)(i + 1);
@@ -240,16 +242,37 @@ __global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, 
     rgbm[v] = make_float4(fmaxf(acc[0], 0.f), fmaxf(acc[1], 0.f), fmaxf(acc[2], 0.f), __uint_as_float(mask));
 }
 
-// ---- a10: SH backward ----------------------------------------------------------------------------------
-// grad_sh[v,i,ch] += Y_i(dir_v) * grad_rgb[v,ch] * [c_v,ch > 0]; consumed grad_rgb entries are re-zeroed.
+// ---- a10: per-voxel backward finalize ---------------------------------------------------------------
+// (i) corner gradients from the polynomial-coefficient gradients the compositing kernel accumulated:
+//     coef = A raw (see composite.cu) => grad_raw += A^T grad_coef;
+// (ii) grad_sh[v,i,ch] += Y_i(dir_v) * grad_rgb[v,ch] * [c_v,ch > 0] (zero sub-gradient at the clamp).
+// Consumed scratch entries are re-zeroed, so the scratch buffers stay all-zero between calls.
 template <int DEG>
-__global__ void __launch_bounds__(256) sh_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
-                                                          const float4* __restrict__ rgbm, float4* __restrict__ grad_rgb,
-                                                          float* __restrict__ grad_sh) {
+__global__ void __launch_bounds__(256) voxel_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                             const float4* __restrict__ rgbm, float4* __restrict__ grad_coef,
+                                                             float4* __restrict__ grad_rgb, float4* __restrict__ grad_raw,
+                                                             float* __restrict__ grad_sh) {
     int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= s.n) return;
     ushort4 r = rects[v];
     if (r.x > r.z) return;
+    float4 ga = grad_coef[2 * v], gb = grad_coef[2 * v + 1];
+    if (ga.x != 0.f || ga.y != 0.f || ga.z != 0.f || ga.w != 0.f || gb.x != 0.f || gb.y != 0.f || gb.z != 0.f || gb.w != 0.f) {
+        grad_coef[2 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        grad_coef[2 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float g0 = ga.x, gx = ga.y, gy = ga.z, gz = ga.w, gxy = gb.x, gxz = gb.y, gyz = gb.z, gxyz = gb.w;
+        float4 ra = grad_raw[2 * v], rb = grad_raw[2 * v + 1];
+        ra.x += ((g0 - gx) - (gy + gz)) + ((gxy + gxz) + (gyz - gxyz));
+        ra.y += (gx - gxy) - (gxz - gxyz);
+        ra.z += (gy - gxy) - (gyz - gxyz);
+        ra.w += gxy - gxyz;
+        rb.x += (gz - gxz) - (gyz - gxyz);
+        rb.y += gxz - gxyz;
+        rb.z += gyz - gxyz;
+        rb.w += gxyz;
+        grad_raw[2 * v] = ra;
+        grad_raw[2 * v + 1] = rb;
+    }
     float4 g = grad_rgb[v];
     if (g.x == 0.f && g.y == 0.f && g.z == 0.f) return;
     grad_rgb[v] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -319,8 +342,9 @@ SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
     StageScope scope__(ctx, ST_RANGES);
     SVR_CUDA(ctx, cudaMemsetAsync(f->ranges, 0, sizeof(uint32_t) * 16 * (size_t)f->n_tiles, ctx->stream));
     if (f->n_entries > 0) {
-        ranges_kernel<<<blocks_for(f->n_entries, 256), 256, 0, ctx->stream>>>(f->keys, f->n_entries, 3 * f->scene.max_level,
-                                                                              f->ranges);
+        ranges_kernel<<<blocks_for(f->n_entries, 256), 256, 0, ctx->stream>>>(
+            f->keys, f->n_entries, 3 * f->scene.max_level, f->ranges, f->vals, reinterpret_cast<const uint2*>(f->rects),
+            reinterpret_cast<uint2*>(f->rects_sorted));
         ctx->launches += 1;
     }
     SVR_CUDA(ctx, cudaGetLastError());
@@ -344,18 +368,20 @@ SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
     return SVR_OK;
 }
 
-SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_rgb, float* grad_sh) {
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw, float* grad_sh) {
     StageScope scope__(ctx, ST_SH_BACKWARD);
     if (f->scene.n == 0) return SVR_OK;
     unsigned int g = blocks_for(f->scene.n, 256);
     const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
     const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
+    float4* gc = reinterpret_cast<float4*>(grad_coef);
     float4* gr = reinterpret_cast<float4*>(grad_rgb);
+    float4* graw = reinterpret_cast<float4*>(grad_raw);
     switch (f->scene.sh_degree) {
-        case 0: sh_backward_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
-        case 1: sh_backward_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
-        case 2: sh_backward_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
-        default: sh_backward_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gr, grad_sh); break;
+        case 0: voxel_backward_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        case 1: voxel_backward_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        case 2: voxel_backward_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        default: voxel_backward_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
     }
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());

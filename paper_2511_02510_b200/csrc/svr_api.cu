@@ -71,7 +71,7 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
     // sizes are tracked in aggregate: free pointers, then give the bytes back in one go
-    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges};
+    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted};
     for (void* p : ptrs)
         if (p) cudaFreeAsync(p, ctx->stream);
     ctx->in_use -= f->bytes;
@@ -116,6 +116,7 @@ void svr_destroy(SvrContext* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     if (ctx->grad_rgb) cudaFreeAsync(ctx->grad_rgb, ctx->stream);
+    if (ctx->grad_coef) cudaFreeAsync(ctx->grad_coef, ctx->stream);
     if (ctx->loss_ws) cudaFreeAsync(ctx->loss_ws, ctx->stream);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     cudaStreamSynchronize(ctx->stream);
@@ -231,6 +232,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         svr_free(ctx, big_list, big_bytes);
         big_list = nullptr;
         f->keys = ks; f->vals = vs;
+        TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
         f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
         keys_a = keys_b = nullptr;
         vals_a = vals_b = nullptr;
@@ -279,14 +281,17 @@ SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOp
     if (n == 0) return SVR_OK;
     if (ctx->grad_rgb_cap < n) {
         if (ctx->grad_rgb) svr_free(ctx, ctx->grad_rgb, sizeof(float) * 4 * (size_t)ctx->grad_rgb_cap);
-        ctx->grad_rgb = nullptr;
+        if (ctx->grad_coef) svr_free(ctx, ctx->grad_coef, sizeof(float) * 8 * (size_t)ctx->grad_rgb_cap);
+        ctx->grad_rgb = ctx->grad_coef = nullptr;
         ctx->grad_rgb_cap = 0;
         SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_rgb, sizeof(float) * 4 * (size_t)n));
+        SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_coef, sizeof(float) * 8 * (size_t)n));
         ctx->grad_rgb_cap = n;
         SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_rgb, 0, sizeof(float) * 4 * (size_t)n, ctx->stream));
+        SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_coef, 0, sizeof(float) * 8 * (size_t)n, ctx->stream));
     }
-    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, grad_raw_density, ctx->grad_rgb, w_max));
-    return launch_sh_backward(ctx, frame, ctx->grad_rgb, grad_sh);
+    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_coef, ctx->grad_rgb, w_max));
+    return launch_sh_backward(ctx, frame, ctx->grad_coef, ctx->grad_rgb, grad_raw_density, grad_sh);
 }
 
 SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam_host, const SvrRenderOpts* ropts,
@@ -359,6 +364,10 @@ void svr_set_stage_timing(SvrContext* ctx, int enabled) {
 }
 
 int svr_num_stages(void) { return ST_COUNT; }
+
+void svr_set_debug_flags(SvrContext* ctx, int flags) {
+    if (ctx) ctx->debug_flags = flags;
+}
 
 const char* svr_stage_name(int stage) {
     static const char* names[ST_COUNT] = {"tile_masks", "rects_counts", "scan", "emit_keys", "sort", "ranges", "voxel_colors",

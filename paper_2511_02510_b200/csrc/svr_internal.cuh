@@ -19,6 +19,7 @@ struct StagePending { int stage; cudaEvent_t e0, e1; };
 
 struct SvrContext {
     bool timing = false;
+    int debug_flags = 0;          // measurement experiments only (svr_set_debug_flags)
     std::vector<StagePending> pending;
     std::vector<cudaEvent_t> event_pool;
     double stage_ms[ST_COUNT] = {0};
@@ -31,6 +32,7 @@ struct SvrContext {
     std::string err;
     // persistent scratch
     float* grad_rgb = nullptr;    // [n_cap,4] per-voxel colour-gradient scratch, kept all-zero between calls
+    float* grad_coef = nullptr;   // [n_cap,8] per-voxel density-coefficient-gradient scratch, same
     int64_t grad_rgb_cap = 0;
     void* loss_ws = nullptr;      // loss workspace (see loss.cu)
     size_t loss_ws_bytes = 0;
@@ -71,6 +73,7 @@ struct SvrFrame {
     float* rgbm = nullptr;           // [n,4]
     uint64_t* keys = nullptr;        // [E] sorted
     uint32_t* vals = nullptr;        // [E] sorted
+    uint16_t* rects_sorted = nullptr;// [E,4] pixel rectangle of vals[i] (coalesced reads in the compositing cull)
     uint32_t* ranges = nullptr;      // [n_tiles*8*2]
     size_t bytes = 0;
 };
@@ -122,8 +125,9 @@ SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
                          float* T_final, float* w_max, unsigned long long* stats);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
-                          float* grad_raw, float* grad_rgb, float* w_max);
-SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_rgb, float* grad_sh);
+                          float* grad_coef, float* grad_rgb, float* w_max);
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw,
+                             float* grad_sh);
 SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma,
                            float eps, float q, int sobel_source, float* dL, float* loss);
 
