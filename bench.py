@@ -135,6 +135,27 @@ def run_reference(args):
     return 0
 
 
+def camera_index(step: int, rank: int, n_cams: int) -> int:
+    """Replica `rank` walks the config's cameras round-robin starting at camera `rank` (no data-path exchange)."""
+    return (step + rank) % n_cams
+
+
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Device-timed milliseconds -> max over ranks (the whole job is as slow as its slowest replica)."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(rays_per_step: int, steps: int, world: int, ms: float) -> float:
+    """Whole-job Mrays/s: every rank processed `steps` views in the max-over-ranks time."""
+    return rays_per_step * steps * world / (ms * 1e-3) / 1e6
+
+
 def workload_config(cfg, args):
     cam = cfg.cameras[0]
     return {"workload": f"{cfg.name}: {cfg.scene.n} voxels, {cam.W}x{cam.H}, {len(cfg.cameras)} cameras round-robin, K={cfg.K}, "
@@ -207,7 +228,7 @@ def main():
         targets.append(t_host.to(dev))
 
     def step(i):
-        k = (i + rank) % len(ccams)
+        k = camera_index(i, rank, len(ccams))
         fr = ctx.svr_preprocess(vox, ccams[k])
         ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, depth=depth, T_final=Tf)
         ctx.svr_loss_grad(image, targets[k], cfg.gamma, dL=dL, loss=loss)
@@ -215,13 +236,13 @@ def main():
         fr.release()
 
     def render_step(i):
-        k = (i + rank) % len(ccams)
+        k = camera_index(i, rank, len(ccams))
         fr = ctx.svr_preprocess(vox, ccams[k])
         ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False)
         fr.release()
 
     def e2e_step(i):
-        k = (i + rank) % len(ccams)
+        k = camera_index(i, rank, len(ccams))
         return ctx.svr_train_view_host(vox, ccams[k], cfg.K, cfg.gamma, targets_host[k], g_raw, g_sh,
                                        w_max=w_max if cfg.emit_wmax_in_backward else None, T_min=cfg.T_min)
 
@@ -243,11 +264,7 @@ def main():
         barrier()
         ms = e0.elapsed_time(e1)
         clocks = sampler.stop() if sampler else None
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms, clocks
+        return max_over_ranks(ms, world, dev), clocks
 
     for i in range(args.warmup):
         step(i)
@@ -262,7 +279,7 @@ def main():
     stage = ctx.svr_get_stage_times(reset=True)
     ctx.svr_set_stage_timing(False)
     launches = ctx.kernel_launches - launches0
-    value = rays * args.steps * world / (ms_total * 1e-3) / 1e6
+    value = aggregate_value(rays, args.steps, world, ms_total)
 
     # ---- render-only FPS (preprocess + forward, w_max off) ----
     for i in range(3):
@@ -274,13 +291,13 @@ def main():
     for i in range(3):
         e2e_step(i)
     ms_e2e, _ = timed(e2e_step, args.steps)
-    e2e_value = rays * args.steps * world / (ms_e2e * 1e-3) / 1e6
+    e2e_value = aggregate_value(rays, args.steps, world, ms_e2e)
 
     peak_vram = int(torch.cuda.max_memory_allocated(dev)) + int(ctx.workspace_peak_bytes)
 
     # ---- work counters (outside the timed region): hits / tests per view ----
     stats = []
-    for k in sorted({(i + rank) % len(ccams) for i in range(args.steps)}):
+    for k in sorted({camera_index(i, rank, len(ccams)) for i in range(args.steps)}):
         fr = ctx.svr_preprocess(vox, ccams[k])
         st = ctx.svr_forward_stats(fr, cfg.K, cfg.T_min)
         st["entries"] = fr.n_entries
