@@ -248,57 +248,83 @@ __global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, 
 // (ii) grad_sh[v,i,ch] += Y_i(dir_v) * grad_rgb[v,ch] * [c_v,ch > 0] (zero sub-gradient at the clamp).
 // Consumed scratch entries are re-zeroed, so the scratch buffers stay all-zero between calls.
 template <int DEG>
-__global__ void __launch_bounds__(256) voxel_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+__global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
                                                              const float4* __restrict__ rgbm, float4* __restrict__ grad_coef,
                                                              float4* __restrict__ grad_rgb, float4* __restrict__ grad_raw,
                                                              float* __restrict__ grad_sh) {
-    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= s.n) return;
-    ushort4 r = rects[v];
-    if (r.x > r.z) return;
-    float4 ga = grad_coef[2 * v], gb = grad_coef[2 * v + 1];
-    if (ga.x != 0.f || ga.y != 0.f || ga.z != 0.f || ga.w != 0.f || gb.x != 0.f || gb.y != 0.f || gb.z != 0.f || gb.w != 0.f) {
-        grad_coef[2 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
-        grad_coef[2 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
-        const float g0 = ga.x, gx = ga.y, gy = ga.z, gz = ga.w, gxy = gb.x, gxz = gb.y, gyz = gb.z, gxyz = gb.w;
-        float4 ra = grad_raw[2 * v], rb = grad_raw[2 * v + 1];
-        ra.x += ((g0 - gx) - (gy + gz)) + ((gxy + gxz) + (gyz - gxyz));
-        ra.y += (gx - gxy) - (gxz - gxyz);
-        ra.z += (gy - gxy) - (gyz - gxyz);
-        ra.w += gxy - gxyz;
-        rb.x += (gz - gxz) - (gyz - gxyz);
-        rb.y += gxz - gxyz;
-        rb.z += gyz - gxyz;
-        rb.w += gxyz;
-        grad_raw[2 * v] = ra;
-        grad_raw[2 * v + 1] = rb;
-    }
-    float4 g = grad_rgb[v];
-    if (g.x == 0.f && g.y == 0.f && g.z == 0.f) return;
-    grad_rgb[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-    unsigned mask = __float_as_uint(rgbm[v].w);
-    float gv[3] = {(mask & 1u) ? g.x : 0.f, (mask & 2u) ? g.y : 0.f, (mask & 4u) ? g.z : 0.f};
     constexpr int NB = (DEG + 1) * (DEG + 1);
-    float dx, dy, dz, Y[NB];
-    voxel_dir_dev(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v], dx, dy, dz);
-    sh_basis_dev(DEG, dx, dy, dz, Y);
-    float* p = grad_sh + v * (NB * 3);
-    if (NB * 3 % 4 == 0) {
-        float4* p4 = reinterpret_cast<float4*>(p);
+    constexpr int ROW = NB * 3;
+    __shared__ float Ysm[4][32][NB + 1];
+    __shared__ float gsm[4][32][3];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t v0 = ((int64_t)blockIdx.x * 4 + warp) * 32;
+    if (v0 >= s.n) return;
+    const int64_t v = v0 + lane;
+    bool vis = false;
+    if (v < s.n) { ushort4 r = rects[v]; vis = r.x <= r.z; }
+    bool sh_active = false;
+    if (vis) {
+        float4 ga = grad_coef[2 * v], gb = grad_coef[2 * v + 1];
+        if (ga.x != 0.f || ga.y != 0.f || ga.z != 0.f || ga.w != 0.f || gb.x != 0.f || gb.y != 0.f || gb.z != 0.f || gb.w != 0.f) {
+            grad_coef[2 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
+            grad_coef[2 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float g0 = ga.x, gx = ga.y, gy = ga.z, gz = ga.w, gxy = gb.x, gxz = gb.y, gyz = gb.z, gxyz = gb.w;
+            float4 ra = grad_raw[2 * v], rb = grad_raw[2 * v + 1];
+            ra.x += ((g0 - gx) - (gy + gz)) + ((gxy + gxz) + (gyz - gxyz));
+            ra.y += (gx - gxy) - (gxz - gxyz);
+            ra.z += (gy - gxy) - (gyz - gxyz);
+            ra.w += gxy - gxyz;
+            rb.x += (gz - gxz) - (gyz - gxyz);
+            rb.y += gxz - gxyz;
+            rb.z += gyz - gxyz;
+            rb.w += gxyz;
+            grad_raw[2 * v] = ra;
+            grad_raw[2 * v + 1] = rb;
+        }
+        float4 g = grad_rgb[v];
+        if (g.x != 0.f || g.y != 0.f || g.z != 0.f) {
+            grad_rgb[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+            unsigned mask = __float_as_uint(rgbm[v].w);
+            float gv0 = (mask & 1u) ? g.x : 0.f, gv1 = (mask & 2u) ? g.y : 0.f, gv2 = (mask & 4u) ? g.z : 0.f;
+            sh_active = (gv0 != 0.f || gv1 != 0.f || gv2 != 0.f);
+            if (sh_active) {
+                float dx, dy, dz, Y[NB];
+                voxel_dir_dev(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v], dx, dy, dz);
+                sh_basis_dev(DEG, dx, dy, dz, Y);
 #pragma unroll
-        for (int k = 0; k < NB * 3 / 4; ++k) {
-            float4 t = p4[k];
+                for (int i = 0; i < NB; ++i) Ysm[warp][lane][i] = Y[i];
+                gsm[warp][lane][0] = gv0; gsm[warp][lane][1] = gv1; gsm[warp][lane][2] = gv2;
+            }
+        }
+    }
+    const unsigned amask = __ballot_sync(0xffffffffu, sh_active);
+    if (amask == 0u) return;
+    __syncwarp();
+    // cooperative read-modify-write of the warp's contiguous grad_sh block, skipping untouched voxels
+    const int nvox = (int)min((int64_t)32, s.n - v0);
+    if (ROW % 4 == 0) {
+        float4* p4 = reinterpret_cast<float4*>(grad_sh + v0 * ROW);
+        for (int e = lane; e < nvox * (ROW / 4); e += 32) {
+            int vv = e / (ROW / 4);
+            if (!((amask >> vv) & 1u)) continue;
+            int f0 = (e - vv * (ROW / 4)) * 4;
+            float4 t = p4[e];
             float tv[4] = {t.x, t.y, t.z, t.w};
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                int idx = 4 * k + e;
-                tv[e] = fmaf(Y[idx / 3], gv[idx % 3], tv[e]);
+            for (int k = 0; k < 4; ++k) {
+                int idx = f0 + k;
+                tv[k] = fmaf(Ysm[warp][vv][idx / 3], gsm[warp][vv][idx % 3], tv[k]);
             }
-            p4[k] = make_float4(tv[0], tv[1], tv[2], tv[3]);
+            p4[e] = make_float4(tv[0], tv[1], tv[2], tv[3]);
         }
     } else {
-#pragma unroll
-        for (int idx = 0; idx < NB * 3; ++idx) p[idx] = fmaf(Y[idx / 3], gv[idx % 3], p[idx]);
+        float* p = grad_sh + v0 * ROW;
+        for (int e = lane; e < nvox * ROW; e += 32) {
+            int vv = e / ROW;
+            if (!((amask >> vv) & 1u)) continue;
+            int idx = e - vv * ROW;
+            p[e] = fmaf(Ysm[warp][vv][idx / 3], gsm[warp][vv][idx % 3], p[e]);
+        }
     }
 }
 
@@ -371,17 +397,17 @@ SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
 SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw, float* grad_sh) {
     StageScope scope__(ctx, ST_SH_BACKWARD);
     if (f->scene.n == 0) return SVR_OK;
-    unsigned int g = blocks_for(f->scene.n, 256);
+    unsigned int g = blocks_for(f->scene.n, 128);
     const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
     const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
     float4* gc = reinterpret_cast<float4*>(grad_coef);
     float4* gr = reinterpret_cast<float4*>(grad_rgb);
     float4* graw = reinterpret_cast<float4*>(grad_raw);
     switch (f->scene.sh_degree) {
-        case 0: voxel_backward_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
-        case 1: voxel_backward_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
-        case 2: voxel_backward_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
-        default: voxel_backward_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        case 0: voxel_backward_kernel<0><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        case 1: voxel_backward_kernel<1><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        case 2: voxel_backward_kernel<2><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        default: voxel_backward_kernel<3><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
     }
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
