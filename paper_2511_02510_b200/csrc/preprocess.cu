@@ -207,6 +207,38 @@ __global__ void __launch_bounds__(256) ranges_kernel(const uint64_t* __restrict_
     if (i + 1 == n || (keys[i + 1] >> shift) != p) ranges[2 * p + 1] = (uint32_t)(i + 1);
 }
 
+// ---- tile launch order: longest lists first -----------------------------------------------------------
+// List lengths are heavy-tailed (C4: mean 1.3k, max 12k entries per tile). CTAs are dispatched in blockIdx
+// order, so handing out the longest tiles first (LPT) keeps a few giants from forming the kernel's tail.
+// Rank by counting: every thread compares its tile against all others (n_tiles <= ~7000).
+__global__ void __launch_bounds__(256) tile_len_kernel(const uint32_t* __restrict__ ranges, int n_tiles, uint32_t* __restrict__ tile_len) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_tiles) return;
+    uint32_t len = 0;
+#pragma unroll
+    for (int o = 0; o < 8; ++o) len += ranges[(t * 8 + o) * 2 + 1] - ranges[(t * 8 + o) * 2];
+    tile_len[t] = len;
+}
+
+__global__ void __launch_bounds__(256) tile_order_kernel(const uint32_t* __restrict__ tile_len, int n_tiles,
+                                                         uint32_t* __restrict__ tile_order) {
+    __shared__ uint32_t chunk[256];
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t mine = (t < n_tiles) ? tile_len[t] : 0u;
+    int rank = 0;
+    for (int base = 0; base < n_tiles; base += 256) {
+        __syncthreads();
+        chunk[threadIdx.x] = (base + threadIdx.x < n_tiles) ? tile_len[base + threadIdx.x] : 0u;
+        __syncthreads();
+        const int m = min(256, n_tiles - base);
+        for (int u = 0; u < m; ++u) {
+            const uint32_t other = chunk[u];
+            rank += (other > mine) || (other == mine && base + u < t);
+        }
+    }
+    if (t < n_tiles) tile_order[rank] = (uint32_t)t;
+}
+
 // ---- a3: per-view voxel colour (R6) -------------------------------------------------------------------
 // c_v = max(0, 0.5 + sum_i Y_i(dir_v) sh[v,i,:]); rgbm[v] = (r, g, b, clamp-mask bits).
 template <int DEG>
@@ -373,6 +405,9 @@ SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
             reinterpret_cast<uint2*>(f->rects_sorted));
         ctx->launches += 1;
     }
+    tile_len_kernel<<<blocks_for(f->n_tiles, 256), 256, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles);
+    tile_order_kernel<<<blocks_for(f->n_tiles, 256), 256, 0, ctx->stream>>>(f->tile_order + f->n_tiles, f->n_tiles, f->tile_order);
+    ctx->launches += 2;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

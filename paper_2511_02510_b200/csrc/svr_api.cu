@@ -71,7 +71,7 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
     // sizes are tracked in aggregate: free pointers, then give the bytes back in one go
-    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted};
+    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order};
     for (void* p : ptrs)
         if (p) cudaFreeAsync(p, ctx->stream);
     ctx->in_use -= f->bytes;
@@ -192,6 +192,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     TRYF(A.get((void**)&f->offsets, sizeof(uint32_t) * (size_t)(n + 1)));
     TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->ranges, sizeof(uint32_t) * 16 * (size_t)f->n_tiles));
+    TRYF(A.get((void**)&f->tile_order, sizeof(uint32_t) * 2 * (size_t)f->n_tiles));
     TRYF(svr_alloc(ctx, (void**)&counts, counts_bytes));
     TRYF(svr_alloc(ctx, (void**)&totals, 64));
     CUDAF(cudaMemsetAsync(totals, 0, 64, ctx->stream));

@@ -75,6 +75,7 @@ struct SvrFrame {
     uint32_t* vals = nullptr;        // [E] sorted
     uint16_t* rects_sorted = nullptr;// [E,4] pixel rectangle of vals[i] (coalesced reads in the compositing cull)
     uint32_t* ranges = nullptr;      // [n_tiles*8*2]
+    uint32_t* tile_order = nullptr;  // [2*n_tiles]: tile ids by descending list length, then the lengths
     size_t bytes = 0;
 };
 
