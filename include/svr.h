@@ -84,9 +84,10 @@ int64_t svr_kernel_launches(const SvrContext* ctx);
 
 /* (1)+(2) of the path: per-voxel projection to pixel rectangles and tile-overlap counts (B1), per-view SH
  * colour c_v (R6), key build (tile | direction octant | direction-flipped Morton code, B3), device radix
- * sort, per-(tile,octant) ranges (B4). The frame borrows `vox` pointers: keep them alive and the topology
- * (ijkl) unchanged until svr_frame_release; raw_density / sh VALUES are re-read by forward/backward.
- * svr_frame_refresh_colors recomputes c_v after sh changed without redoing the lists. */
+ * sort, per-(tile,octant) ranges (B4), and a per-entry record of the voxel (geometry relative to the camera,
+ * density coefficients, colour) in list order. The frame borrows `vox` pointers: keep them alive and the
+ * topology (ijkl) unchanged until svr_frame_release. raw_density / sh VALUES are captured by svr_preprocess;
+ * svr_frame_refresh_colors re-captures them (colours + records) after they changed, without redoing the lists. */
 SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam, SvrFrame** out);
 SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame);
 void svr_frame_release(SvrContext* ctx, SvrFrame* frame);

@@ -74,8 +74,14 @@ __device__ __forceinline__ void setup_ray(const CamDev& c, int px, int py, RayF&
     }
 }
 
-__device__ __forceinline__ void stage_voxel(WarpStage& S, int slot, uint32_t vid, unsigned int M, const SceneDev& s,
-                                            const CamDev& c, const float4* __restrict__ rgbm) {
+// Per list entry, once per view: everything the compositing warps need about the voxel, in list order
+// (5 x 16 B): centre relative to the camera as hi+lo floats (fp64 arithmetic), half edge, voxel id,
+// the trilinear raw density as polynomial coefficients * log2(e), and the per-view colour.
+__global__ void __launch_bounds__(256) pack_entries_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ vals, int64_t n,
+                                                           const float4* __restrict__ rgbm, float4* __restrict__ packed) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t vid = __ldg(vals + i);
     uint2 q = __ldg(reinterpret_cast<const uint2*>(s.ijkl) + vid);
     const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
     float4 ra = __ldg(rp), rb = __ldg(rp + 1), col = __ldg(rgbm + vid);
@@ -86,17 +92,17 @@ __device__ __forceinline__ void stage_voxel(WarpStage& S, int slot, uint32_t vid
     double gy = (double)s.root_lo[1] + ((double)(q.x >> 16) + 0.5) * e - c.o[1];
     double gz = (double)s.root_lo[2] + ((double)(q.y & 0xFFFF) + 0.5) * e - c.o[2];
     float hx = (float)gx, hy = (float)gy, hz = (float)gz;
-    S.g0[slot] = make_float4(hx, hy, hz, 0.5f * ef);
-    S.g1[slot] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
     // trilinear -> polynomial coefficients, scaled by log2(e) (corner c = bx + 2 by + 4 bz)
     const float L2E = 1.4426950408889634f;
     float c0 = ra.x, cx = ra.y - ra.x, cy = ra.z - ra.x, cz = rb.x - ra.x;
     float cxy = (ra.w - ra.y) - cy, cxz = (rb.y - ra.y) - cz, cyz = (rb.z - ra.z) - cz;
     float cxyz = ((rb.w - rb.z) - (rb.y - rb.x)) - ((ra.w - ra.z) - (ra.y - ra.x));
-    S.r0[slot] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
-    S.r1[slot] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
-    S.col[slot] = col;
-    S.M[slot] = M;
+    float4* out = packed + 5 * i;
+    out[0] = make_float4(hx, hy, hz, 0.5f * ef);
+    out[1] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
+    out[2] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
+    out[3] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
+    out[4] = col;
 }
 
 // 32-bit mask of the lanes (pixel = (wbx0 + (lane & 7), wby0 + (lane >> 3))) inside the rectangle.
@@ -189,11 +195,11 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, 
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 template <int K, bool BWD, bool STATS>
-__global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ vals,
+__global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, const float4* __restrict__ packed,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
                                                         const uint32_t* __restrict__ tile_order,
-                                                        const float4* __restrict__ rgbm, float T_min,
+                                                        float T_min,
                                                         float* __restrict__ image, float* __restrict__ depth,
                                                         float* __restrict__ T_final, unsigned int* __restrict__ w_max,
                                                         const float* __restrict__ dL, const float* __restrict__ image_in,
@@ -239,18 +245,21 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(SceneDev s,
             while (count < 32 && base < end) {
                 uint32_t idx = base + lane;
                 unsigned int M = 0u;
-                uint32_t vid = 0u;
-                if (idx < end) {
-                    M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
-                    if (M) vid = __ldg(vals + idx);
-                }
+                if (idx < end) M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
                 unsigned int m = __ballot_sync(FULL, M != 0u);
-                if (M) stage_voxel(S, (head + count + __popc(m & ((1u << lane) - 1u))) & (RING - 1), vid, M, s, c, rgbm);
-                if (BWD && M) {
-                    // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the
-                    // DRAM fill (3.4 ms -> 5.2 ms without this on C4)
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
+                if (M) {
+                    const float4* rec = packed + 5 * (size_t)idx;
+                    const float4 t0 = __ldg(rec), t1 = __ldg(rec + 1), t2 = __ldg(rec + 2), t3 = __ldg(rec + 3), t4 = __ldg(rec + 4);
+                    const int slot = (head + count + __popc(m & ((1u << lane) - 1u))) & (RING - 1);
+                    S.g0[slot] = t0; S.g1[slot] = t1; S.r0[slot] = t2; S.r1[slot] = t3; S.col[slot] = t4;
+                    S.M[slot] = M;
+                    if (BWD) {
+                        // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the
+                        // DRAM fill (3.4 ms -> 5.2 ms without this on C4)
+                        const uint32_t vid = __float_as_uint(t1.w);
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
+                    }
                 }
                 count += __popc(m);
                 base += 32;
@@ -396,10 +405,9 @@ SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_mi
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, BWD ? ST_BACKWARD : ST_FORWARD);
     const size_t smem = sizeof(WarpStage) * WARPS;
-    const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
-#define SVR_ARGS f->scene, f->cam, f->vals, rs, f->ranges, f->tile_order, rgbm, T_min, image, depth, T_final, wm, dL, image_in, grad_coef, grad_rgb, stats, ctx->debug_flags
+#define SVR_ARGS f->cam, reinterpret_cast<const float4*>(f->packed), rs, f->ranges, f->tile_order, T_min, image, depth, T_final, wm, dL, image_in, grad_coef, grad_rgb, stats, ctx->debug_flags
 #define SVR_GO(KERNEL)                                                                                     \
     do {                                                                                                   \
         static bool attr_set = false;                                                                      \
@@ -439,4 +447,14 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
                           float* grad_coef, float* grad_rgb, float* w_max) {
     return launch_composite<true>(ctx, f, K, T_min, nullptr, nullptr, nullptr, w_max, dL, image, grad_coef, grad_rgb, nullptr);
+}
+
+SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f) {
+    if (f->n_entries == 0) return SVR_OK;
+    StageScope scope__(ctx, ST_PACK);
+    pack_entries_kernel<<<(unsigned int)((f->n_entries + 255) / 256), 256, 0, ctx->stream>>>(
+        f->scene, f->cam, f->vals, f->n_entries, reinterpret_cast<const float4*>(f->rgbm), reinterpret_cast<float4*>(f->packed));
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
 }

@@ -71,7 +71,7 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
     // sizes are tracked in aggregate: free pointers, then give the bytes back in one go
-    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order};
+    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed};
     for (void* p : ptrs)
         if (p) cudaFreeAsync(p, ctx->stream);
     ctx->in_use -= f->bytes;
@@ -234,6 +234,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         big_list = nullptr;
         f->keys = ks; f->vals = vs;
         TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
+        TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
         f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
         keys_a = keys_b = nullptr;
         vals_a = vals_b = nullptr;
@@ -241,6 +242,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     svr_free(ctx, totals, 64);
     totals = nullptr;
     TRYF(launch_ranges(ctx, f));
+    TRYF(launch_pack_entries(ctx, f));
 #undef TRYF
 #undef CUDAF
     *out = f;
@@ -249,7 +251,8 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 
 SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame) {
     if (!ctx || !frame) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
-    return launch_voxel_colors(ctx, frame);
+    SVR_TRY(launch_voxel_colors(ctx, frame));
+    return launch_pack_entries(ctx, frame);
 }
 
 void svr_frame_release(SvrContext* ctx, SvrFrame* frame) {
@@ -372,7 +375,7 @@ void svr_set_debug_flags(SvrContext* ctx, int flags) {
 
 const char* svr_stage_name(int stage) {
     static const char* names[ST_COUNT] = {"tile_masks", "rects_counts", "scan", "emit_keys", "sort", "ranges", "voxel_colors",
-                                          "forward_composite", "loss_grad", "backward_composite", "sh_backward"};
+                                          "forward_composite", "loss_grad", "backward_composite", "sh_backward", "pack_entries"};
     return (stage >= 0 && stage < ST_COUNT) ? names[stage] : "";
 }
 

@@ -12,7 +12,7 @@
 
 enum SvrStage {
     ST_TILE_MASKS = 0, ST_RECTS, ST_SCAN, ST_EMIT, ST_SORT, ST_RANGES, ST_COLORS, ST_FORWARD, ST_LOSS, ST_BACKWARD,
-    ST_SH_BACKWARD, ST_COUNT
+    ST_SH_BACKWARD, ST_PACK, ST_COUNT
 };
 
 struct StagePending { int stage; cudaEvent_t e0, e1; };
@@ -75,6 +75,7 @@ struct SvrFrame {
     uint32_t* vals = nullptr;        // [E] sorted
     uint16_t* rects_sorted = nullptr;// [E,4] pixel rectangle of vals[i] (coalesced reads in the compositing cull)
     uint32_t* ranges = nullptr;      // [n_tiles*8*2]
+    float* packed = nullptr;         // [E,20] per-entry voxel record in list order (composite.cu pack_entries_kernel)
     uint32_t* tile_order = nullptr;  // [2*n_tiles]: tile ids by descending list length, then the lengths
     size_t bytes = 0;
 };
@@ -123,6 +124,7 @@ SvrStatus launch_sort_pairs(SvrContext* ctx, uint64_t* keys, uint64_t* keys_alt,
                             int64_t n, int bits, uint64_t** keys_sorted, uint32_t** vals_sorted);
 SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
                          float* T_final, float* w_max, unsigned long long* stats);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
