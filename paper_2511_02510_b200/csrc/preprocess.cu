@@ -210,33 +210,51 @@ __global__ void __launch_bounds__(256) ranges_kernel(const uint64_t* __restrict_
 // ---- tile launch order: longest lists first -----------------------------------------------------------
 // List lengths are heavy-tailed (C4: mean 1.3k, max 12k entries per tile). CTAs are dispatched in blockIdx
 // order, so handing out the longest tiles first (LPT) keeps a few giants from forming the kernel's tail.
-// Rank by counting: every thread compares its tile against all others (n_tiles <= ~7000).
-__global__ void __launch_bounds__(256) tile_len_kernel(const uint32_t* __restrict__ ranges, int n_tiles, uint32_t* __restrict__ tile_len) {
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n_tiles) return;
-    uint32_t len = 0;
+// One block: counting sort of the tiles on their quantised length (1024 bins, longest first). The order
+// inside a bin is arbitrary; it only decides which CTA starts first.
+__global__ void __launch_bounds__(1024) tile_order_kernel(const uint32_t* __restrict__ ranges, int n_tiles,
+                                                          uint32_t* __restrict__ tile_len, uint32_t* __restrict__ tile_order) {
+    __shared__ uint32_t hist[1024];
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t max_len;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    hist[tid] = 0;
+    if (tid == 0) max_len = 0;
+    __syncthreads();
+    for (int t = tid; t < n_tiles; t += 1024) {
+        uint32_t len = 0;
 #pragma unroll
-    for (int o = 0; o < 8; ++o) len += ranges[(t * 8 + o) * 2 + 1] - ranges[(t * 8 + o) * 2];
-    tile_len[t] = len;
-}
-
-__global__ void __launch_bounds__(256) tile_order_kernel(const uint32_t* __restrict__ tile_len, int n_tiles,
-                                                         uint32_t* __restrict__ tile_order) {
-    __shared__ uint32_t chunk[256];
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    const uint32_t mine = (t < n_tiles) ? tile_len[t] : 0u;
-    int rank = 0;
-    for (int base = 0; base < n_tiles; base += 256) {
-        __syncthreads();
-        chunk[threadIdx.x] = (base + threadIdx.x < n_tiles) ? tile_len[base + threadIdx.x] : 0u;
-        __syncthreads();
-        const int m = min(256, n_tiles - base);
-        for (int u = 0; u < m; ++u) {
-            const uint32_t other = chunk[u];
-            rank += (other > mine) || (other == mine && base + u < t);
-        }
+        for (int o = 0; o < 8; ++o) len += ranges[(t * 8 + o) * 2 + 1] - ranges[(t * 8 + o) * 2];
+        tile_len[t] = len;
+        atomicMax(&max_len, len);
     }
-    if (t < n_tiles) tile_order[rank] = (uint32_t)t;
+    __syncthreads();
+    int shift = 0;
+    while ((max_len >> shift) >= 1024u) ++shift;
+    for (int t = tid; t < n_tiles; t += 1024) atomicAdd(&hist[1023u - (tile_len[t] >> shift)], 1u);   // bin 0 = longest
+    __syncthreads();
+    // exclusive scan of the 1024 bins
+    uint32_t v = hist[tid], inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = wsum[lane], winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        wsum[lane] = winc - w;
+    }
+    __syncthreads();
+    hist[tid] = wsum[warp] + inc - v;
+    __syncthreads();
+    for (int t = tid; t < n_tiles; t += 1024) tile_order[atomicAdd(&hist[1023u - (tile_len[t] >> shift)], 1u)] = (uint32_t)t;
 }
 
 // ---- a3: per-view voxel colour (R6) -------------------------------------------------------------------
@@ -405,9 +423,8 @@ SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
             reinterpret_cast<uint2*>(f->rects_sorted));
         ctx->launches += 1;
     }
-    tile_len_kernel<<<blocks_for(f->n_tiles, 256), 256, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles);
-    tile_order_kernel<<<blocks_for(f->n_tiles, 256), 256, 0, ctx->stream>>>(f->tile_order + f->n_tiles, f->n_tiles, f->tile_order);
-    ctx->launches += 2;
+    tile_order_kernel<<<1, 1024, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
+    ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

@@ -115,17 +115,27 @@ __global__ void __launch_bounds__(SORT_THREADS) radix_upsweep_kernel(const uint6
     tile_hist[(size_t)threadIdx.x * n_tiles + blockIdx.x] = h[threadIdx.x];   // bin-major: [bin][tile]
 }
 
-// one warp per bin: exclusive scan across tiles in place; bin_total[bin] = number of keys with that digit
+// one warp per bin: exclusive scan across tiles in place; bin_total[bin] = number of keys with that digit.
+// 128 counts per iteration (four coalesced loads in flight) so the row's L2 latency is paid n_tiles/128 times.
 __global__ void __launch_bounds__(256) radix_scan_kernel(uint32_t* __restrict__ tile_hist, int n_tiles, uint32_t* __restrict__ bin_total) {
     const int lane = threadIdx.x & 31, bin = blockIdx.x * 8 + (threadIdx.x >> 5);
     uint32_t* row = tile_hist + (size_t)bin * n_tiles;
     uint32_t carry = 0;
-    for (int base = 0; base < n_tiles; base += 32) {
-        int i = base + lane;
-        uint32_t v = (i < n_tiles) ? row[i] : 0u;
-        uint32_t inc = warp_incl_scan(v, lane);
-        if (i < n_tiles) row[i] = carry + inc - v;
-        carry += __shfl_sync(FULL, inc, 31);
+    for (int base = 0; base < n_tiles; base += 128) {
+        uint32_t v[4], inc[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            int i = base + k * 32 + lane;
+            v[k] = (i < n_tiles) ? row[i] : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) inc[k] = warp_incl_scan(v[k], lane);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            int i = base + k * 32 + lane;
+            if (i < n_tiles) row[i] = carry + inc[k] - v[k];
+            carry += __shfl_sync(FULL, inc[k], 31);
+        }
     }
     if (lane == 0) bin_total[bin] = carry;
 }
