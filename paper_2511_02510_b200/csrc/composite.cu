@@ -398,29 +398,311 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, c
     }
 }
 
+
+// ================================================================================================
+// Hit-packed backward compositing (row a9). The lane-centric walk above keeps only ~12 of 32 lanes busy
+// in the expensive part of the backward pass (K samples + exp + the monomial sums) and needs a quad
+// exchange before every reduction. Here only the cheap part stays pixel-centric; the expensive part runs
+// on a compacted hit queue:
+//   1. cull + stage as above (32 voxel records in list order, warp-private);
+//   2. test: every lane pops its own pixel's candidates among the staged voxels and slab-tests them
+//      against a slightly dilated box (centre hi parts only, ray in registers), recording a hit bitmask;
+//   3. queue: the 32x32 hit matrix is transposed so that lane k knows which pixels hit slot k; a warp scan
+//      gives every slot its queue offset; every pixel lane then writes its own hits to their slot-major
+//      positions (slot offset + its rank among the slot's pixels);
+//   4. hit rounds: 32 hits per round, one per lane, all lanes busy in the precise slab test and the K
+//      samples. The sequential per-pixel state (T, P = G . C) lives in shared memory; hits of the same
+//      pixel inside a round (match_any) are chained in slot order by a short loop of shuffles, so every
+//      pixel composites front to back in exactly the list order:
+//          dL/dtau_k = G . (T_k c_k + C_k - C_final) = T_k (G . c_k) + P_k - G . C_final.
+//   5. reduce: hits of one voxel are contiguous lanes, so two steps of a segmented shuffle sum give every
+//      fragment of up to 4 consecutive hits of a voxel one set of three red.global.add.v4.f32: a voxel that
+//      covers 7 of the warp's pixels leaves as 2 reduction sets instead of 7.
+// Pixel tables are indexed by a swizzled pixel id (row y rotated by 3y) so that the pixels of a small
+// rectangle fall into different shared-memory bank groups.
+constexpr int QCAP = 512;          // queue entries per warp (a batch is cut so that its hits fit)
+constexpr int RED_STEPS = 2;       // fragments of up to 4 consecutive hits of one voxel share a reduction set
+constexpr int NSLOT = 32;          // staged voxels per batch
+#ifndef BWD_CTAS
+#define BWD_CTAS 4
+#endif
+
+struct WarpWork {
+    float4 g0[NSLOT];   // gh.xyz, h
+    float4 g1[NSLOT];   // gl.xyz, voxel id bits
+    float4 r0[NSLOT];   // log2(e) * (c0, cx, cy, cz)
+    float4 r1[NSLOT];   // log2(e) * (cxy, cxz, cyz, cxyz)
+    float4 col[NSLOT];  // r, g, b, cover mask M of this warp's 8x4 block
+    float4 P0[32];      // per pixel (swizzled index): dh.xyz
+    float4 P1[32];      //   dl.xyz
+    float4 PI[32];      //   1/dh.xyz
+    float4 PG[32];      //   G = dL/dC, and G . C_final
+    float2 ST[32];      //   T, P = G . C
+    uint2 Hs[32];       // per slot of the batch: pixels that hit it, queue offset
+    unsigned short q[QCAP];
+};
+
+__device__ __forceinline__ int warp_incl_scan_i(int v, int lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(FULL, v, o);
+        if (lane >= o) v += t;
+    }
+    return v;
+}
+
+template <int K>
+__global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed,
+                                                               const uint2* __restrict__ rects_sorted,
+                                                               const uint32_t* __restrict__ ranges,
+                                                               const uint32_t* __restrict__ tile_order, float T_min,
+                                                               unsigned int* __restrict__ w_max, const float* __restrict__ dL,
+                                                               const float* __restrict__ image_in, float* __restrict__ grad_coef,
+                                                               float* __restrict__ grad_rgb) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    WarpWork& S = reinterpret_cast<WarpWork*>(smem_raw)[warp];
+    const int tile = (int)tile_order[blockIdx.x];
+    const int tile_x = tile % c.tiles_x, tile_y = tile / c.tiles_x;
+    const int wbx0 = tile_x * SVR_TILE + (warp & 1) * 8, wby0 = tile_y * SVR_TILE + (warp >> 1) * 4;
+    const int px = wbx0 + (lane & 7), py = wby0 + (lane >> 3);
+    const bool inimg = px < c.W && py < c.H;
+    const size_t pix = (size_t)py * c.W + px;
+    const unsigned int lt = (1u << lane) - 1u;
+    const int swl = (lane & 24) | ((lane + 3 * (lane >> 3)) & 7);     // this pixel's row in the tables
+
+    int oct = -1;
+    float dh[3], inv[3], ainv[3];
+    {
+        RayF ray;
+        float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (inimg) {
+            setup_ray(c, px, py, ray);
+            oct = pixel_octant_dev(c, px, py);
+            g = make_float4(dL[pix * 3], dL[pix * 3 + 1], dL[pix * 3 + 2], 0.f);
+            g.w = g.x * image_in[pix * 3] + g.y * image_in[pix * 3 + 1] + g.z * image_in[pix * 3 + 2];
+        } else {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { ray.dh[a] = 0.f; ray.dl[a] = 0.f; ray.inv[a] = 0.f; ray.ainv[a] = 0.f; }
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { dh[a] = ray.dh[a]; inv[a] = ray.inv[a]; ainv[a] = ray.ainv[a]; }
+        S.P0[swl] = make_float4(ray.dh[0], ray.dh[1], ray.dh[2], 0.f);
+        S.P1[swl] = make_float4(ray.dl[0], ray.dl[1], ray.dl[2], 0.f);
+        S.PI[swl] = make_float4(ray.inv[0], ray.inv[1], ray.inv[2], 0.f);
+        S.PG[swl] = g;
+        S.ST[swl] = make_float2(1.f, 0.f);
+    }
+    __syncwarp();
+    float Tpix = 1.f;
+
+    for (int so = 0; so < 8; ++so) {
+        const uint32_t start = ranges[(tile * 8 + so) * 2], end = ranges[(tile * 8 + so) * 2 + 1];
+        if (start == end) continue;
+        bool alive = inimg && (oct == so) && (Tpix >= T_min);
+        unsigned int alive_mask = __ballot_sync(FULL, alive);
+        if (alive_mask == 0u) continue;                               // no pixel of this warp uses this list
+        int head = 0, count = 0;                                      // ring state (warp-uniform)
+        uint32_t base = start;
+        while (true) {
+            // ---- 1. cull + stage until 32 survivors are waiting or the list is exhausted ----
+            while (count < NSLOT && base < end) {
+                const uint32_t idx = base + lane;
+                unsigned int M = 0u;
+                if (idx < end) M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
+                unsigned int m = __ballot_sync(FULL, M != 0u);
+                const int rank = __popc(m & lt);
+                int adv = 32;
+                if (__popc(m) > NSLOT - count) {                       // more survivors than free slots: take the first ones
+                    if (rank >= NSLOT - count) M = 0u;
+                    m = __ballot_sync(FULL, M != 0u);
+                    adv = 32 - __clz(m);                               // resume after the last survivor taken
+                }
+                if (M) {
+                    const float4* rec = packed + 5 * (size_t)idx;
+                    const float4 t0 = __ldg(rec), t1 = __ldg(rec + 1), t2 = __ldg(rec + 2), t3 = __ldg(rec + 3);
+                    float4 t4 = __ldg(rec + 4);
+                    t4.w = __uint_as_float(M);
+                    const int slot = (head + count + rank) & (NSLOT - 1);
+                    const uint32_t vid = __float_as_uint(t1.w);
+                    // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the DRAM fill
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
+                    S.g0[slot] = t0; S.g1[slot] = t1; S.r0[slot] = t2; S.r1[slot] = t3; S.col[slot] = t4;
+                }
+                count += __popc(m);
+                base += adv;
+            }
+            if (count == 0) break;
+            __syncwarp();
+            // ---- 2. test: every lane walks its own pixel's candidates (conservative slab test) ----
+            int n = count;
+            unsigned int hits = 0u;
+            {
+                unsigned int cand = transpose32(lane < n ? __float_as_uint(S.col[(head + lane) & (NSLOT - 1)].w) : 0u, lane);
+                if (!alive) cand = 0u;
+                while (__any_sync(FULL, cand != 0u)) {
+                    if (cand) {
+                        const int k = __ffs(cand) - 1;
+                        cand &= cand - 1;
+                        const float4 a = S.g0[(head + k) & (NSLOT - 1)];
+                        // box dilated by a bound on what the lo parts and the rounding can move: never loses a true hit
+                        const float hd = fmaf(fabsf(a.x) + fabsf(a.y) + fabsf(a.z), 4.8e-7f, a.w * 1.000002f);
+                        const float cx = a.x * inv[0], cy = a.y * inv[1], cz = a.z * inv[2];
+                        const float wx = hd * ainv[0], wy = hd * ainv[1], wz = hd * ainv[2];
+                        const float s0 = fmaxf(fmaxf(cx - wx, cy - wy), fmaxf(cz - wz, 0.f));
+                        const float s1 = fminf(fminf(cx + wx, cy + wy), cz + wz);
+                        if (s1 > s0) hits |= 1u << k;
+                    }
+                }
+            }
+            // ---- 3. queue: slot-major positions from the transposed hit matrix ----
+            int nh;
+            {
+                const unsigned int H = transpose32(hits, lane);         // lane k: pixels that hit slot k
+                const int cnt = __popc(H);
+                const int inc = warp_incl_scan_i(cnt, lane);
+                n = min(n, __popc(__ballot_sync(FULL, inc <= QCAP)));  // cut the batch where the queue is full
+                nh = __shfl_sync(FULL, inc, n - 1);
+                S.Hs[lane] = make_uint2(H, (unsigned int)(inc - cnt));
+                __syncwarp();
+                unsigned int m = (n < 32) ? (hits & ((1u << n) - 1u)) : hits;
+                while (__any_sync(FULL, m != 0u)) {
+                    if (m) {
+                        const int k = __ffs(m) - 1;
+                        m &= m - 1;
+                        const uint2 hk = S.Hs[k];
+                        S.q[hk.y + __popc(hk.x & lt)] = (unsigned short)((k << 5) | swl);
+                    }
+                }
+            }
+            __syncwarp();
+            // ---- 4. hit rounds: one hit per lane ----
+            for (int r = 0; r < nh; r += 32) {
+                const bool valid = r + lane < nh;
+                const unsigned int e = valid ? (unsigned int)S.q[r + lane] : 0xFFFFu;
+                const int k = (int)(e >> 5);                         // slot inside the batch (2047 = no entry)
+                const int i = (int)(e & 31u);                        // swizzled pixel id
+                const int slot = (head + k) & (NSLOT - 1);
+                // hits of the same pixel inside this round are chained in slot (= lane) order; issued first so that
+                // the match latency hides behind the samples
+                const unsigned int peers = __match_any_sync(FULL, valid ? (unsigned int)i : 32u + (unsigned int)lane);
+                // hits of one voxel are contiguous lanes (a run): RED_STEPS steps of a segmented sum towards lower lanes,
+                // then every lane that starts a fragment of 2^RED_STEPS lanes of its run sends the fragment's sums
+                const int kprev = __shfl_up_sync(FULL, k, 1);
+                const unsigned int heads = __ballot_sync(FULL, lane == 0 || kprev != k);
+                const unsigned int above = (heads >> lane) >> 1;
+                const int rem = above ? __ffs(above) - 1 : 31 - lane;     // lanes after this one in its run
+                const int run_pos = lane - (31 - __clz(heads & (lt | (1u << lane))));
+                const bool frag_head = valid && (run_pos & ((1 << RED_STEPS) - 1)) == 0;
+                const uint32_t vid = valid ? __float_as_uint(S.g1[slot].w) : 0u;
+                // w_max only grows, so a stale guard read is safe; issued here so that its latency hides behind the samples
+                unsigned int wm_old = 0xFFFFFFFFu;
+                if (frag_head && w_max != nullptr) wm_old = w_max[vid];
+                float tau = 0.f, dtau[8], gc = 0.f;
+                float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int m = 0; m < 8; ++m) dtau[m] = 0.f;
+                if (valid) {
+                    const float4 a = S.g0[slot], bq = S.g1[slot];
+                    const float4 d = S.P0[i], dl = S.P1[i], iv = S.PI[i];
+                    RayF rr;
+                    rr.dh[0] = d.x; rr.dh[1] = d.y; rr.dh[2] = d.z;
+                    rr.dl[0] = dl.x; rr.dl[1] = dl.y; rr.dl[2] = dl.z;
+                    rr.inv[0] = iv.x; rr.inv[1] = iv.y; rr.inv[2] = iv.z;
+                    rr.ainv[0] = fabsf(iv.x); rr.ainv[1] = fabsf(iv.y); rr.ainv[2] = fabsf(iv.z);
+                    const float4 col = S.col[slot];
+                    G = S.PG[i];
+                    gc = G.x * col.x + G.y * col.y + G.z * col.z;
+                    float s0, s1, t_ref, D[3];
+                    if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
+                        const float4 ra = S.r0[slot], rb = S.r1[slot];
+                        tau = integrate<K, true>(rr, D, a.w, s0, s1, ra, rb, dtau);
+                    }
+                }
+                const float E = ex2f(-1.4426950408889634f * tau);
+                const unsigned int lower = peers & lt;
+                const int level = __popc(lower);
+                const int pred = lower ? 31 - __clz(lower) : lane;
+                const int maxL = (int)__reduce_max_sync(FULL, (unsigned int)level);
+                float2 st = make_float2(0.f, 0.f);
+                if (valid && level == 0) st = S.ST[i];
+                float w = 0.f;
+                bool live = false;
+                for (int L = 0; L <= maxL; ++L) {
+                    if (L > 0) {
+                        const float t0 = __shfl_sync(FULL, st.x, pred), t1 = __shfl_sync(FULL, st.y, pred);
+                        if (level == L) st = make_float2(t0, t1);
+                    }
+                    if (level == L) {
+                        live = valid && st.x >= T_min;                // R8: a ray stops after the voxel that crosses T_min
+                        w = live ? st.x * (1.f - E) : 0.f;
+                        st.x = live ? st.x * E : st.x;
+                        st.y = fmaf(w, gc, st.y);
+                    }
+                }
+                if (valid && (peers >> lane) == 1u) S.ST[i] = st;     // last hit of its pixel in this round
+                // ---- 5. reduce ----
+                float v[11];
+                {
+                    const float dLdtau = live ? fmaf(st.x, gc, st.y) - G.w : 0.f;
+#pragma unroll
+                    for (int m = 0; m < 8; ++m) v[m] = dLdtau * dtau[m];
+                    v[8] = w * G.x; v[9] = w * G.y; v[10] = w * G.z;
+                }
+                float wq = w;
+#pragma unroll
+                for (int s = 0; s < RED_STEPS; ++s) {
+                    const int step = 1 << s;
+                    const float take = (step <= rem) ? 1.f : 0.f;
+#pragma unroll
+                    for (int m = 0; m < 11; ++m) v[m] = fmaf(take, __shfl_down_sync(FULL, v[m], step), v[m]);
+                    wq = fmaxf(wq, take * __shfl_down_sync(FULL, wq, step));
+                }
+                if (frag_head && wq > 0.f) {
+                    red_add_v4(grad_coef + (size_t)vid * 8, v[0], v[1], v[2], v[3]);
+                    red_add_v4(grad_coef + (size_t)vid * 8 + 4, v[4], v[5], v[6], v[7]);
+                    red_add_v4(grad_rgb + (size_t)vid * 4, v[8], v[9], v[10], 0.f);
+                    if (__float_as_uint(wq) > wm_old) atomicMax(w_max + vid, __float_as_uint(wq));
+                }
+                __syncwarp();                                          // pixel state is reused by the next round
+            }
+            head = (head + n) & (NSLOT - 1);
+            count -= n;
+            Tpix = S.ST[swl].x;
+            alive = inimg && (oct == so) && (Tpix >= T_min);
+            alive_mask = __ballot_sync(FULL, alive);
+            if (alive_mask == 0u) break;                              // whole warp terminated
+        }
+    }
+}
+
 template <bool BWD>
 SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
                            float* w_max, const float* dL, const float* image_in, float* grad_coef, float* grad_rgb,
                            unsigned long long* stats) {
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, BWD ? ST_BACKWARD : ST_FORWARD);
-    const size_t smem = sizeof(WarpStage) * WARPS;
+    const bool packed = BWD && (ctx->debug_flags & 2) == 0;      // debug flag 2: lane-centric backward (first design, for A/B)
+    const size_t smem = packed ? sizeof(WarpWork) * WARPS : sizeof(WarpStage) * WARPS;
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
-#define SVR_ARGS f->cam, reinterpret_cast<const float4*>(f->packed), rs, f->ranges, f->tile_order, T_min, image, depth, T_final, wm, dL, image_in, grad_coef, grad_rgb, stats, ctx->debug_flags
-#define SVR_GO(KERNEL)                                                                                     \
+    const float4* pk = reinterpret_cast<const float4*>(f->packed);
+#define SVR_ARGS f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, T_final, wm, dL, image_in, grad_coef, grad_rgb, stats, ctx->debug_flags
+#define SVR_GO(KERNEL, ...)                                                                                \
     do {                                                                                                   \
         static bool attr_set = false;                                                                      \
         if (!attr_set) {                                                                                   \
             SVR_CUDA(ctx, cudaFuncSetAttribute(KERNEL, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
             attr_set = true;                                                                               \
         }                                                                                                  \
-        KERNEL<<<f->n_tiles, 256, smem, ctx->stream>>>(SVR_ARGS);                                          \
+        KERNEL<<<f->n_tiles, 256, smem, ctx->stream>>>(__VA_ARGS__);                                       \
     } while (0)
-#define SVR_LAUNCH(KK)                                                                \
-    do {                                                                              \
-        if (!BWD && stats) SVR_GO((composite_kernel<KK, false, true>));               \
-        else SVR_GO((composite_kernel<KK, BWD, false>));                              \
+#define SVR_LAUNCH(KK)                                                                          \
+    do {                                                                                        \
+        if (packed) SVR_GO((backward_packed_kernel<KK>), f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, image_in, grad_coef, grad_rgb); \
+        else if (!BWD && stats) SVR_GO((composite_kernel<KK, false, true>), SVR_ARGS);          \
+        else SVR_GO((composite_kernel<KK, BWD, false>), SVR_ARGS);                              \
     } while (0)
     switch (K) {
         case 1: SVR_LAUNCH(1); break;
