@@ -78,10 +78,12 @@ __device__ __forceinline__ void setup_ray(const CamDev& c, int px, int py, RayF&
 // (5 x 16 B): centre relative to the camera as hi+lo floats (fp64 arithmetic), half edge, voxel id,
 // the trilinear raw density as polynomial coefficients * log2(e), and the per-view colour.
 __global__ void __launch_bounds__(256) pack_entries_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ vals, int64_t n,
-                                                           const float4* __restrict__ rgbm, float4* __restrict__ packed) {
+                                                           const float4* __restrict__ rgbm, float4* __restrict__ packed,
+                                                           const uint2* __restrict__ rects, uint2* __restrict__ rects_sorted) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const uint32_t vid = __ldg(vals + i);
+    rects_sorted[i] = __ldg(rects + vid);         // rectangle in list order: the compositing cull reads it coalesced
     uint2 q = __ldg(reinterpret_cast<const uint2*>(s.ijkl) + vid);
     const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
     float4 ra = __ldg(rp), rb = __ldg(rp + 1), col = __ldg(rgbm + vid);
@@ -735,7 +737,8 @@ SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f) {
     if (f->n_entries == 0) return SVR_OK;
     StageScope scope__(ctx, ST_PACK);
     pack_entries_kernel<<<(unsigned int)((f->n_entries + 255) / 256), 256, 0, ctx->stream>>>(
-        f->scene, f->cam, f->vals, f->n_entries, reinterpret_cast<const float4*>(f->rgbm), reinterpret_cast<float4*>(f->packed));
+        f->scene, f->cam, f->vals, f->n_entries, reinterpret_cast<const float4*>(f->rgbm), reinterpret_cast<float4*>(f->packed),
+        reinterpret_cast<const uint2*>(f->rects), reinterpret_cast<uint2*>(f->rects_sorted));
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;

@@ -197,11 +197,9 @@ __global__ void __launch_bounds__(256) emit_big_kernel(SceneDev s, CamDev c, con
 
 // ---- B4: ranges -------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ranges_kernel(const uint64_t* __restrict__ keys, int64_t n, int shift,
-                                                     uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals,
-                                                     const uint2* __restrict__ rects, uint2* __restrict__ rects_sorted) {
+                                                     uint32_t* __restrict__ ranges) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    rects_sorted[i] = __ldg(rects + vals[i]);     // rectangle in list order: the compositing cull reads it coalesced
     uint64_t p = keys[i] >> shift;
     if (i == 0 || (keys[i - 1] >> shift) != p) ranges[2 * p] = (uint32_t)i;
     if (i + 1 == n || (keys[i + 1] >> shift) != p) ranges[2 * p + 1] = (uint32_t)(i + 1);
@@ -378,6 +376,423 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
     }
 }
 
+// ================================================================================================
+// Bucketed list build (rows a4-a6, second design). The first design gave every voxel a contiguous block of
+// entries (per-voxel counts -> scan over N voxels -> emit) and sorted all E (key, id) pairs on the full
+// 51-bit key with 7 radix passes over global memory (21 launches, ~225 B of traffic per entry). The lists are
+// (tile, octant) buckets, so here the top key bits are never sorted at all:
+//   count    per voxel: atomic count into its (tile, octant) buckets; voxels that cover more than BIG_TILES
+//            tiles add a +1/-1 corner pattern to a 2-D difference array instead (4 atomics);
+//   scan     one block: 2-D prefix of the difference array -> per-tile cover of big voxels, added to the
+//            buckets; exclusive scan of the bucket counts = the ranges (B4) and the write cursors;
+//   scatter  per voxel: position = atomicAdd(cursor[bucket]); entry = (flipped Morton code << vb) | voxel id
+//            in one 64-bit word (any order inside a bucket);
+//   sort     one block per non-empty bucket (dynamic work fetch): radix passes over the code bits only, in shared
+//            memory (buckets larger than SORT_CAP: through L2); tiny buckets use a bitonic network.
+// Codes are unique within a bucket, so the result is the one sequence the oracle's full sort gives (bit-exact).
+// Traffic per entry: 8 B written + 8 B read + 12 B written. Needs 3*Lmax + ceil(log2 N) <= 64 (else: first design).
+constexpr int BIG_TILES = 16;
+constexpr int SORT_CAP = 6144;        // largest bucket whose radix passes stay in shared memory (two buffers)
+constexpr int SORT_CAP_BIG = 12288;   // same with one 1024-thread block per SM; beyond: passes through L2
+constexpr int SMALL_CAP = 256;        // buckets up to this size: bitonic network
+constexpr int SORT_THREADS2 = 512;
+
+__global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamDev c, const uint8_t* __restrict__ masks,
+                                                                ushort4* __restrict__ rects, uint32_t* __restrict__ bcount,
+                                                                int* __restrict__ bigdiff, unsigned long long* __restrict__ totals) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    ushort4 r = voxel_rect(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v]);
+    rects[v] = r;
+    if (r.x > r.z) return;
+    const int i0 = r.x >> 4, i1 = r.z >> 4, j0 = r.y >> 4, j1 = r.w >> 4;
+    if ((i1 - i0 + 1) * (j1 - j0 + 1) > BIG_TILES) {
+        const int sx = c.tiles_x + 1;
+        atomicAdd(&totals[1], 1ULL);
+        atomicAdd(&bigdiff[j0 * sx + i0], 1);
+        atomicAdd(&bigdiff[j0 * sx + i1 + 1], -1);
+        atomicAdd(&bigdiff[(j1 + 1) * sx + i0], -1);
+        atomicAdd(&bigdiff[(j1 + 1) * sx + i1 + 1], 1);
+        return;
+    }
+    for (int j = j0; j <= j1; ++j)
+        for (int i = i0; i <= i1; ++i) {
+            const int tile = j * c.tiles_x + i;
+            unsigned m = masks[tile];
+            while (m) {
+                const int o = __ffs(m) - 1;
+                m &= m - 1;
+                atomicAdd(&bcount[tile * 8 + o], 1u);
+            }
+        }
+}
+
+// One block of 1024 threads. bcount[b] becomes the write cursor (= first entry) of bucket b; ranges[b] = [start, end)
+// ((0,0) when empty, B4); nonempty = ids of the non-empty buckets; totals[0] = E, totals[3] = number of non-empty buckets.
+// Dynamic shared memory: the (ty+1) x (tx+1) difference array.
+__global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __restrict__ masks, const int* __restrict__ bigdiff, int tx, int ty,
+                                                           uint32_t* __restrict__ bcount, uint32_t* __restrict__ ranges,
+                                                           uint32_t* __restrict__ nonempty, unsigned long long* __restrict__ totals) {
+    extern __shared__ int sd[];
+    __shared__ uint32_t wsum[32], wsum2[32], wsum3[32], n_big_buckets;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int sx = tx + 1, nd = sx * (ty + 1);
+    for (int i = tid; i < nd; i += 1024) sd[i] = bigdiff[i];
+    __syncthreads();
+    for (int j = warp; j <= ty; j += 32) {            // row prefix sums, one warp per row
+        int carry = 0;
+        for (int i0 = 0; i0 <= tx; i0 += 32) {
+            const int i = i0 + lane;
+            int v = (i <= tx) ? sd[j * sx + i] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, v, o);
+                if (lane >= o) v += t;
+            }
+            if (i <= tx) sd[j * sx + i] = v + carry;
+            carry += __shfl_sync(0xffffffffu, v, 31);
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i <= tx; i += 1024) {           // column prefix sums: sd[j][i] = big voxels covering tile (i, j)
+        int run = 0;
+        for (int j = 0; j <= ty; ++j) { run += sd[j * sx + i]; sd[j * sx + i] = run; }
+    }
+    __syncthreads();
+    const int n_tiles = tx * ty;
+    const int tpt = (n_tiles + 1023) / 1024;          // whole tiles per thread: 8 buckets = two 16-byte words each
+    const int t0 = tid * tpt, t1 = min(n_tiles, t0 + tpt);
+    uint32_t local = 0, local_ne = 0, local_big = 0;
+    for (int t = t0; t < t1; ++t) {
+        const uint4 a = reinterpret_cast<const uint4*>(bcount)[2 * t], b = reinterpret_cast<const uint4*>(bcount)[2 * t + 1];
+        const uint32_t c[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+        const uint32_t m = masks[t], cover = (uint32_t)sd[(t / tx) * sx + (t % tx)];
+#pragma unroll
+        for (int o = 0; o < 8; ++o) {
+            const uint32_t cnt = c[o] + (((m >> o) & 1u) ? cover : 0u);
+            local += cnt;
+            local_big += (cnt > (uint32_t)SORT_CAP);
+            local_ne += (cnt != 0u && cnt <= (uint32_t)SORT_CAP);
+        }
+    }
+    // block-wide exclusive scans of (local, local_ne, local_big)
+    uint32_t inc = local, inc2 = local_ne, inc3 = local_big;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o), t2 = __shfl_up_sync(0xffffffffu, inc2, o), t3 = __shfl_up_sync(0xffffffffu, inc3, o);
+        if (lane >= o) { inc += t; inc2 += t2; inc3 += t3; }
+    }
+    if (lane == 31) { wsum[warp] = inc; wsum2[warp] = inc2; wsum3[warp] = inc3; }
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = wsum[lane], w2 = wsum2[lane], w3 = wsum3[lane], a = w, a2 = w2, a3 = w3;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, a, o), t2 = __shfl_up_sync(0xffffffffu, a2, o), t3 = __shfl_up_sync(0xffffffffu, a3, o);
+            if (lane >= o) { a += t; a2 += t2; a3 += t3; }
+        }
+        wsum[lane] = a - w; wsum2[lane] = a2 - w2; wsum3[lane] = a3 - w3;
+        if (lane == 31) { totals[0] = a; totals[3] = a2 + a3; totals[5] = a3; n_big_buckets = a3; }
+    }
+    __syncthreads();
+    // the largest buckets go to the front of the work list: they take longest to sort
+    uint32_t run = wsum[warp] + inc - local, run_ne = n_big_buckets + wsum2[warp] + inc2 - local_ne, run_big = wsum3[warp] + inc3 - local_big;
+    for (int t = t0; t < t1; ++t) {
+        const uint4 a = reinterpret_cast<const uint4*>(bcount)[2 * t], b = reinterpret_cast<const uint4*>(bcount)[2 * t + 1];
+        const uint32_t c[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+        const uint32_t m = masks[t], cover = (uint32_t)sd[(t / tx) * sx + (t % tx)];
+        uint32_t cur[8], rg[16];
+#pragma unroll
+        for (int o = 0; o < 8; ++o) {
+            const uint32_t cnt = c[o] + (((m >> o) & 1u) ? cover : 0u);
+            cur[o] = run;
+            rg[2 * o] = cnt ? run : 0u;
+            rg[2 * o + 1] = cnt ? run + cnt : 0u;
+            if (cnt > (uint32_t)SORT_CAP) nonempty[run_big++] = (uint32_t)(t * 8 + o);
+            else if (cnt) nonempty[run_ne++] = (uint32_t)(t * 8 + o);
+            run += cnt;
+        }
+        reinterpret_cast<uint4*>(bcount)[2 * t] = make_uint4(cur[0], cur[1], cur[2], cur[3]);
+        reinterpret_cast<uint4*>(bcount)[2 * t + 1] = make_uint4(cur[4], cur[5], cur[6], cur[7]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            reinterpret_cast<uint4*>(ranges)[4 * t + q] = make_uint4(rg[4 * q], rg[4 * q + 1], rg[4 * q + 2], rg[4 * q + 3]);
+    }
+}
+
+__device__ __forceinline__ void scatter_tile(uint64_t* __restrict__ ent, uint32_t* __restrict__ cursor, int tile, unsigned m,
+                                             uint64_t code, int Lm, int vb, uint32_t v) {
+    while (m) {
+        const int o = __ffs(m) - 1;
+        m &= m - 1;
+        const uint32_t pos = atomicAdd(&cursor[tile * 8 + o], 1u);
+        ent[pos] = ((code ^ flip_mask(o, Lm)) << vb) | (uint64_t)v;
+    }
+}
+
+__global__ void __launch_bounds__(256) scatter_small_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                            const uint8_t* __restrict__ masks, uint32_t* __restrict__ cursor,
+                                                            uint64_t* __restrict__ ent, int vb, uint32_t* __restrict__ big_list,
+                                                            unsigned int* __restrict__ big_count) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    const ushort4 r = rects[v];
+    if (r.x > r.z) return;
+    const int i0 = r.x >> 4, i1 = r.z >> 4, j0 = r.y >> 4, j1 = r.w >> 4;
+    if ((i1 - i0 + 1) * (j1 - j0 + 1) > BIG_TILES) { big_list[atomicAdd(big_count, 1u)] = (uint32_t)v; return; }
+    const uint64_t code = voxel_code(reinterpret_cast<const uint2*>(s.ijkl)[v], s.max_level);
+    for (int j = j0; j <= j1; ++j)
+        for (int i = i0; i <= i1; ++i) {
+            const int tile = j * c.tiles_x + i;
+            scatter_tile(ent, cursor, tile, masks[tile], code, s.max_level, vb, (uint32_t)v);
+        }
+}
+
+__global__ void __launch_bounds__(256) scatter_big_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                          const uint8_t* __restrict__ masks, uint32_t* __restrict__ cursor,
+                                                          uint64_t* __restrict__ ent, int vb, const uint32_t* __restrict__ big_list,
+                                                          const unsigned int* __restrict__ big_count) {
+    const unsigned int nb = *big_count;
+    for (unsigned int b = blockIdx.x; b < nb; b += gridDim.x) {
+        const uint32_t v = big_list[b];
+        const ushort4 r = rects[v];
+        const uint64_t code = voxel_code(reinterpret_cast<const uint2*>(s.ijkl)[v], s.max_level);
+        const int i0 = r.x >> 4, j0 = r.y >> 4, w = (r.z >> 4) - i0 + 1, h = (r.w >> 4) - j0 + 1;
+        for (int k = threadIdx.x; k < w * h; k += blockDim.x) {
+            const int j = k / w, i = k - j * w;
+            const int tile = (j0 + j) * c.tiles_x + i0 + i;
+            scatter_tile(ent, cursor, tile, masks[tile], code, s.max_level, vb, v);
+        }
+    }
+}
+
+// ---- per-bucket sort ----
+// Buckets of up to SMALL_CAP words: bitonic network in shared memory (all compare-exchanges ascending, so virtual
+// +inf padding never moves). Larger buckets: least-significant-digit radix sort, 8 bits per pass over the code bits
+// only, ping-pong between two buffers that live in shared memory (<= CAP words) or in global memory (the
+// bucket's own segment and its slice of the key output array, L2-resident). A pass = per-warp digit counts over
+// warp-contiguous segments (match_any, no atomics), a scan over (digit, warp), and a stable scatter that repeats
+// the walk with the scanned counters. A pass whose digit is the same for the whole bucket is skipped.
+template <int THREADS>
+__device__ __forceinline__ void smem_merge_steps(uint64_t* sk, int P, int j_first) {
+    for (int j = j_first; j > 0; j >>= 1) {
+        for (int t = threadIdx.x; t < (P >> 1); t += THREADS) {
+            const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+            uint64_t a = sk[i], b = sk[i + j];
+            if (b < a) { sk[i] = b; sk[i + j] = a; }
+        }
+        __syncthreads();
+    }
+}
+
+template <int THREADS>
+__device__ __forceinline__ void smem_sort(uint64_t* sk, int P) {
+    for (int k = 2; k <= P; k <<= 1) {
+        const int hk = k >> 1;
+        for (int t = threadIdx.x; t < (P >> 1); t += THREADS) {      // flip step: (i, i ^ (k - 1))
+            const int blk = t / hk, off = t - blk * hk;
+            const int i = blk * k + off, l = blk * k + (k - 1 - off);
+            uint64_t a = sk[i], b = sk[l];
+            if (b < a) { sk[i] = b; sk[l] = a; }
+        }
+        __syncthreads();
+        smem_merge_steps<THREADS>(sk, P, k >> 2);
+    }
+}
+
+// One radix pass over src[0, m) -> dst[0, m) on digit (word >> shift) & mask. wh = [(THREADS / 32)][256] counters, tot = [256].
+// Returns false (and writes nothing) when all words share the digit.
+template <int THREADS>
+__device__ __forceinline__ bool radix_pass(const uint64_t* src, uint64_t* dst, uint32_t m, int shift, uint32_t mask,
+                                           uint32_t* wh, uint32_t* tot, uint32_t* sh8) {
+    constexpr unsigned FULLM = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+    for (int i = tid; i < (THREADS / 32) * 256; i += THREADS) wh[i] = 0;
+    __syncthreads();
+    const uint32_t rounds = (m + 31) >> 5, rpw = (rounds + (THREADS / 32) - 1) / (THREADS / 32);
+    const uint32_t r0 = warp * rpw, r1 = min(rounds, r0 + rpw);
+    uint32_t* my = wh + warp * 256;
+    for (uint32_t r = r0; r < r1; ++r) {
+        const uint32_t i = (r << 5) + lane;
+        const uint32_t d = (i < m) ? ((uint32_t)(src[i] >> shift) & mask) : 256u;
+        const unsigned peers = __match_any_sync(FULLM, d);
+        if ((peers & lt) == 0u && d < 256u) my[d] += __popc(peers);
+        __syncwarp();
+    }
+    __syncthreads();
+    uint32_t run = 0;
+    if (tid < 256) {
+#pragma unroll
+        for (int w = 0; w < (THREADS / 32); ++w) { const uint32_t c = wh[w * 256 + tid]; wh[w * 256 + tid] = run; run += c; }
+    }
+    const int uniform = __syncthreads_or(tid < 256 && run == m);
+    if (uniform) return false;
+    {   // exclusive scan of the 256 digit totals (threads 0..255 = 8 warps)
+        uint32_t inc = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(FULLM, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (tid < 256 && lane == 31) sh8[warp] = inc;
+        __syncthreads();
+        if (tid < 256) {
+            uint32_t basev = 0;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) if (w < warp) basev += sh8[w];
+            tot[tid] = basev + inc - run;
+        }
+        __syncthreads();
+    }
+    for (uint32_t r = r0; r < r1; ++r) {
+        const uint32_t i = (r << 5) + lane;
+        const bool valid = i < m;
+        const uint64_t e = valid ? src[i] : 0ull;
+        const uint32_t d = valid ? ((uint32_t)(e >> shift) & mask) : 256u;
+        const unsigned peers = __match_any_sync(FULLM, d);
+        const int leader = __ffs(peers) - 1;
+        uint32_t old = 0;
+        if (lane == leader && valid) { old = my[d]; my[d] = old + __popc(peers); }
+        old = __shfl_sync(FULLM, old, leader);
+        if (valid) dst[tot[d] + old + __popc(peers & lt)] = e;
+        __syncwarp();
+    }
+    __syncthreads();
+    return true;
+}
+
+// Same pass for buckets of up to CAP words (shared-memory buffers): every warp keeps its (CAP / THREADS) rounds of
+// words in registers, ranks them once (match_any + a running per-warp counter) and scatters after the scan without
+// walking the data again.
+template <int THREADS, int CAP>
+__device__ __forceinline__ bool radix_pass_reg(const uint64_t* src, uint64_t* dst, uint32_t m, int shift, uint32_t mask,
+                                               uint16_t* wh, uint32_t* tot, uint32_t* sh8) {
+    constexpr unsigned FULLM = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+    const uint32_t rounds = (m + 31) >> 5, rpw = (rounds + (THREADS / 32) - 1) / (THREADS / 32);     // <= (CAP / THREADS)
+    const uint32_t i0 = (warp * rpw << 5) + lane;
+    uint64_t e[(CAP / THREADS)];
+    uint32_t pre[(CAP / THREADS)];
+#pragma unroll
+    for (int k = 0; k < (CAP / THREADS); ++k) {
+        const uint32_t i = i0 + (k << 5);
+        e[k] = ((uint32_t)k < rpw && i < m) ? src[i] : ~0ull;
+    }
+    for (int i = tid; i < (THREADS / 32) * 256; i += THREADS) wh[i] = 0;
+    __syncthreads();
+    uint16_t* my = wh + warp * 256;
+#pragma unroll
+    for (int k = 0; k < (CAP / THREADS); ++k) {
+        if ((uint32_t)k < rpw) {
+            const uint32_t i = i0 + (k << 5);
+            const uint32_t d = (i < m) ? ((uint32_t)(e[k] >> shift) & mask) : 256u;
+            const unsigned peers = __match_any_sync(FULLM, d);
+            const int leader = __ffs(peers) - 1;
+            uint32_t old = 0;
+            if (lane == leader && d < 256u) { old = my[d]; my[d] = (uint16_t)(old + __popc(peers)); }
+            pre[k] = __shfl_sync(FULLM, old, leader) + __popc(peers & lt);
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    uint32_t run = 0;
+    if (tid < 256) {
+#pragma unroll
+        for (int w = 0; w < (THREADS / 32); ++w) { const uint32_t c = wh[w * 256 + tid]; wh[w * 256 + tid] = (uint16_t)run; run += c; }
+    }
+    const int uniform = __syncthreads_or(tid < 256 && run == m);
+    if (uniform) return false;
+    {   // exclusive scan of the 256 digit totals (threads 0..255 = 8 warps)
+        uint32_t inc = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(FULLM, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (tid < 256 && lane == 31) sh8[warp] = inc;
+        __syncthreads();
+        if (tid < 256) {
+            uint32_t basev = 0;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) if (w < warp) basev += sh8[w];
+            tot[tid] = basev + inc - run;
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int k = 0; k < (CAP / THREADS); ++k) {
+        const uint32_t i = i0 + (k << 5);
+        if ((uint32_t)k < rpw && i < m) {
+            const uint32_t d = (uint32_t)(e[k] >> shift) & mask;
+            dst[tot[d] + my[d] + pre[k]] = e[k];
+        }
+    }
+    __syncthreads();
+    return true;
+}
+
+template <int THREADS, int CAP>
+__global__ void __launch_bounds__(THREADS) bucket_sort_kernel(uint64_t* __restrict__ ent, const uint32_t* __restrict__ ranges,
+                                                                    const uint32_t* __restrict__ nonempty, const unsigned long long* __restrict__ totals,
+                                                                    unsigned int* __restrict__ work, int big_part, int code_bits, int vb,
+                                                                    uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint64_t* bufA = reinterpret_cast<uint64_t*>(smem_raw);
+    uint64_t* bufB = bufA + CAP;
+    uint16_t* wh = reinterpret_cast<uint16_t*>(bufB + CAP);
+    __shared__ uint32_t tot[256];
+    __shared__ uint32_t sh8[8];
+    __shared__ unsigned int next;
+    // work list: the buckets larger than SORT_CAP first (totals[5] of them), then the rest (totals[3] in all)
+    const unsigned int w_first = big_part ? 0u : (unsigned int)totals[5];
+    const unsigned int n_ne = big_part ? (unsigned int)totals[5] : (unsigned int)totals[3];
+    const uint64_t vmask = (1ull << vb) - 1ull;
+    while (true) {
+        __syncthreads();
+        if (threadIdx.x == 0) next = atomicAdd(work, 1u);
+        __syncthreads();
+        const unsigned int w = w_first + next;
+        if (w >= n_ne) break;
+        const uint32_t b = nonempty[w];
+        const uint32_t start = ranges[2 * b], m = ranges[2 * b + 1] - start;
+        uint64_t* seg = ent + start;
+        const uint64_t prefix = (uint64_t)b << code_bits;
+        const uint64_t* res;
+        if (m <= SMALL_CAP) {
+            int P = 2;
+            while ((uint32_t)P < m) P <<= 1;
+            for (int i = threadIdx.x; i < P; i += THREADS) bufA[i] = ((uint32_t)i < m) ? seg[i] : ~0ull;
+            __syncthreads();
+            smem_sort<THREADS>(bufA, P);
+            res = bufA;
+        } else {
+            uint64_t *src, *dst;
+            if (m <= CAP) {
+                for (uint32_t i = threadIdx.x; i < m; i += THREADS) bufA[i] = seg[i];
+                src = bufA; dst = bufB;
+            } else {
+                src = seg; dst = keys_out + start;                     // global ping-pong (both L2-resident)
+            }
+            __syncthreads();
+            for (int shift = 0; shift < code_bits; shift += 8) {
+                const uint32_t mask = (code_bits - shift < 8) ? ((1u << (code_bits - shift)) - 1u) : 255u;
+                const bool moved = (m <= CAP) ? radix_pass_reg<THREADS, CAP>(src, dst, m, vb + shift, mask, wh, tot, sh8)
+                                                   : radix_pass<THREADS>(src, dst, m, vb + shift, mask, reinterpret_cast<uint32_t*>(bufA), tot, sh8);
+                if (moved) { uint64_t* t = src; src = dst; dst = t; }
+            }
+            res = src;
+        }
+        // res may alias keys_out + start: every thread reads its word before it writes the same index
+        for (uint32_t i = threadIdx.x; i < m; i += THREADS) {
+            const uint64_t e = res[i];
+            keys_out[start + i] = prefix | (e >> vb);
+            vals_out[start + i] = (uint32_t)(e & vmask);
+        }
+    }
+}
+
 inline unsigned int blocks_for(int64_t n, int bs) { return (unsigned int)((n + bs - 1) / bs); }
 
 }  // namespace
@@ -419,8 +834,7 @@ SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
     SVR_CUDA(ctx, cudaMemsetAsync(f->ranges, 0, sizeof(uint32_t) * 16 * (size_t)f->n_tiles, ctx->stream));
     if (f->n_entries > 0) {
         ranges_kernel<<<blocks_for(f->n_entries, 256), 256, 0, ctx->stream>>>(
-            f->keys, f->n_entries, 3 * f->scene.max_level, f->ranges, f->vals, reinterpret_cast<const uint2*>(f->rects),
-            reinterpret_cast<uint2*>(f->rects_sorted));
+            f->keys, f->n_entries, 3 * f->scene.max_level, f->ranges);
         ctx->launches += 1;
     }
     tile_order_kernel<<<1, 1024, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
@@ -461,6 +875,67 @@ SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coe
         case 2: voxel_backward_kernel<2><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
         default: voxel_backward_kernel<3><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
     }
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+// ---- launchers of the bucketed list build ----
+SvrStatus launch_bucket_count(SvrContext* ctx, SvrFrame* f, uint32_t* bcount, int* bigdiff, uint32_t* nonempty,
+                              unsigned long long* totals) {
+    if (f->scene.n > 0) {
+        StageScope scope__(ctx, ST_RECTS);
+        rect_bucket_count_kernel<<<blocks_for(f->scene.n, 256), 256, 0, ctx->stream>>>(
+            f->scene, f->cam, f->tile_masks, reinterpret_cast<ushort4*>(f->rects), bcount, bigdiff, totals);
+        ctx->launches += 1;
+    }
+    {
+        StageScope scope__(ctx, ST_SCAN);
+        bucket_scan_kernel<<<1, 1024, sizeof(int) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1), ctx->stream>>>(f->tile_masks, bigdiff, f->cam.tiles_x, f->cam.tiles_y, bcount, f->ranges,
+                                                        nonempty, totals);
+        ctx->launches += 1;
+    }
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_bucket_scatter(SvrContext* ctx, SvrFrame* f, uint32_t* cursor, uint64_t* ent, int vb, uint32_t* big_list,
+                                unsigned int* big_count) {
+    StageScope scope__(ctx, ST_EMIT);
+    const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
+    scatter_small_kernel<<<blocks_for(f->scene.n, 256), 256, 0, ctx->stream>>>(f->scene, f->cam, r, f->tile_masks, cursor, ent, vb,
+                                                                              big_list, big_count);
+    scatter_big_kernel<<<148 * 4, 256, 0, ctx->stream>>>(f->scene, f->cam, r, f->tile_masks, cursor, ent, vb, big_list, big_count);
+    ctx->launches += 2;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const uint32_t* nonempty, const unsigned long long* totals,
+                             unsigned int* work, int vb) {
+    StageScope scope__(ctx, ST_SORT);
+    static bool attr_set = false;
+    const int smem_small = 2 * SORT_CAP * (int)sizeof(uint64_t) + (SORT_THREADS2 / 32) * 256 * (int)sizeof(uint16_t);
+    const int smem_big = 2 * SORT_CAP_BIG * (int)sizeof(uint64_t) + (1024 / 32) * 256 * (int)sizeof(uint16_t);
+    if (!attr_set) {
+        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<SORT_THREADS2, SORT_CAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_small));
+        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<1024, SORT_CAP_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_big));
+        attr_set = true;
+    }
+    // the few buckets above SORT_CAP: one 1024-thread block per SM with both buffers still in shared memory
+    bucket_sort_kernel<1024, SORT_CAP_BIG><<<148, 1024, smem_big, ctx->stream>>>(ent, f->ranges, nonempty, totals, work + 1, 1,
+                                                                                3 * f->scene.max_level, vb, f->keys, f->vals);
+    bucket_sort_kernel<SORT_THREADS2, SORT_CAP><<<148 * 2, SORT_THREADS2, smem_small, ctx->stream>>>(
+        ent, f->ranges, nonempty, totals, work, 0, 3 * f->scene.max_level, vb, f->keys, f->vals);
+    ctx->launches += 2;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+// rectangles in list order + longest-list-first tile order (the ranges themselves come from the bucket scan)
+SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f) {
+    StageScope scope__(ctx, ST_RANGES);
+    tile_order_kernel<<<1, 1024, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;

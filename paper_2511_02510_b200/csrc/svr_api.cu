@@ -163,12 +163,20 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 
     FrameAlloc A{ctx, f};
     const int64_t n = vox->n;
+    const int vb = bits_for(n > 1 ? n : 2);
+    // second design of the list build (preprocess.cu "Bucketed list build") whenever code and voxel id fit one word
+    const bool bucketed = (3 * vox->max_level + vb <= 64) && (ctx->debug_flags & 8) == 0;
+    const size_t n_buckets = (size_t)f->n_tiles * 8;
     uint32_t* counts = nullptr;
     unsigned long long* totals = nullptr;
     uint32_t* big_list = nullptr;
     uint64_t *keys_a = nullptr, *keys_b = nullptr;
     uint32_t *vals_a = nullptr, *vals_b = nullptr;
-    size_t counts_bytes = sizeof(uint32_t) * (size_t)(n + 1), big_bytes = 0, ka = 0, va = 0;
+    uint32_t *bcount = nullptr, *nonempty = nullptr;
+    int* bigdiff = nullptr;
+    const size_t counts_bytes = sizeof(uint32_t) * (size_t)(n + 1), bucket_bytes = sizeof(uint32_t) * n_buckets;
+    const size_t diff_bytes = sizeof(int) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1);
+    size_t big_bytes = 0, ka = 0, va = 0;
     SvrStatus st = SVR_OK;
     auto fail = [&](SvrStatus s) {
         if (counts) svr_free(ctx, counts, counts_bytes);
@@ -178,6 +186,9 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         if (keys_b) svr_free(ctx, keys_b, ka);
         if (vals_a) svr_free(ctx, vals_a, va);
         if (vals_b) svr_free(ctx, vals_b, va);
+        if (bcount) svr_free(ctx, bcount, bucket_bytes);
+        if (nonempty) svr_free(ctx, nonempty, bucket_bytes);
+        if (bigdiff) svr_free(ctx, bigdiff, diff_bytes);
         f->keys = nullptr; f->vals = nullptr;
         release_frame_buffers(ctx, f);
         delete f;
@@ -189,60 +200,106 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     TRYF(A.get((void**)&f->rects, sizeof(uint16_t) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->tile_masks, (size_t)f->n_tiles));
     TRYF(A.get((void**)&f->sat, sizeof(uint32_t) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1)));
-    TRYF(A.get((void**)&f->offsets, sizeof(uint32_t) * (size_t)(n + 1)));
     TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->ranges, sizeof(uint32_t) * 16 * (size_t)f->n_tiles));
     TRYF(A.get((void**)&f->tile_order, sizeof(uint32_t) * 2 * (size_t)f->n_tiles));
-    TRYF(svr_alloc(ctx, (void**)&counts, counts_bytes));
     TRYF(svr_alloc(ctx, (void**)&totals, 64));
     CUDAF(cudaMemsetAsync(totals, 0, 64, ctx->stream));
-
     TRYF(launch_tile_masks(ctx, f));
-    TRYF(launch_rects_counts(ctx, f, counts, totals));
-    TRYF(launch_exclusive_scan(ctx, counts, f->offsets, n + 1));
-    // E = offsets[n]; number of big voxels = totals[1]: one small readback sizes the sort buffers
-    CUDAF(cudaMemcpyAsync(totals, f->offsets + n, sizeof(uint32_t), cudaMemcpyDeviceToDevice, ctx->stream));
-    CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 16, cudaMemcpyDeviceToHost, ctx->stream));
-    // per-view colours do not depend on E: enqueue before the sync so they overlap the readback
-    TRYF(launch_voxel_colors(ctx, f));
-    CUDAF(cudaStreamSynchronize(ctx->stream));
-    const int64_t E = (int64_t)(ctx->host_pinned[0] & 0xFFFFFFFFull);
-    const int64_t n_big = (int64_t)ctx->host_pinned[1];
-    svr_free(ctx, counts, counts_bytes);
-    counts = nullptr;
-    if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));
-    f->n_entries = E;
 
-    if (E > 0) {
-        ka = sizeof(uint64_t) * (size_t)E;
-        va = sizeof(uint32_t) * (size_t)E;
-        big_bytes = sizeof(uint32_t) * (size_t)(n_big + 1);
-        TRYF(svr_alloc(ctx, (void**)&keys_a, ka));
-        TRYF(svr_alloc(ctx, (void**)&keys_b, ka));
-        TRYF(svr_alloc(ctx, (void**)&vals_a, va));
-        TRYF(svr_alloc(ctx, (void**)&vals_b, va));
-        TRYF(svr_alloc(ctx, (void**)&big_list, big_bytes));
-        unsigned int* big_count = reinterpret_cast<unsigned int*>(totals + 2);
-        TRYF(launch_emit_keys(ctx, f, keys_a, vals_a, big_list, big_count));
-        uint64_t* ks = nullptr;
-        uint32_t* vs = nullptr;
-        TRYF(launch_sort_pairs(ctx, keys_a, keys_b, vals_a, vals_b, E, f->key_bits, &ks, &vs));
-        // keep the buffers holding the sorted result, return the others to the pool
-        svr_free(ctx, ks == keys_a ? keys_b : keys_a, ka);
-        svr_free(ctx, vs == vals_a ? vals_b : vals_a, va);
-        svr_free(ctx, big_list, big_bytes);
-        big_list = nullptr;
-        f->keys = ks; f->vals = vs;
-        TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
-        TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
-        f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
-        keys_a = keys_b = nullptr;
-        vals_a = vals_b = nullptr;
+    if (bucketed) {
+        TRYF(svr_alloc(ctx, (void**)&bcount, bucket_bytes));
+        TRYF(svr_alloc(ctx, (void**)&nonempty, bucket_bytes));
+        TRYF(svr_alloc(ctx, (void**)&bigdiff, diff_bytes));
+        CUDAF(cudaMemsetAsync(bcount, 0, bucket_bytes, ctx->stream));
+        CUDAF(cudaMemsetAsync(bigdiff, 0, diff_bytes, ctx->stream));
+        TRYF(launch_bucket_count(ctx, f, bcount, bigdiff, nonempty, totals));
+        // E, the number of many-tile voxels and the number of non-empty buckets: one small readback sizes the lists
+        CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 32, cudaMemcpyDeviceToHost, ctx->stream));
+        TRYF(launch_voxel_colors(ctx, f));     // independent of E: overlaps the readback
+        CUDAF(cudaStreamSynchronize(ctx->stream));
+        const int64_t E = (int64_t)ctx->host_pinned[0];
+        const int64_t n_big = (int64_t)ctx->host_pinned[1];
+        if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));
+        f->n_entries = E;
+        if (E > 0) {
+            ka = sizeof(uint64_t) * (size_t)E;
+            va = sizeof(uint32_t) * (size_t)E;
+            big_bytes = sizeof(uint32_t) * (size_t)(n_big + 1);
+            // frame-lifetime buffers first, largest first (the pool then reuses the previous frame's blocks one for one),
+            // scratch last
+            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
+            TRYF(svr_alloc(ctx, (void**)&keys_b, ka));   // canonical keys
+            TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
+            TRYF(svr_alloc(ctx, (void**)&vals_a, va));
+            TRYF(svr_alloc(ctx, (void**)&keys_a, ka));   // packed (code << vb | id) words, scratch
+            TRYF(svr_alloc(ctx, (void**)&big_list, big_bytes));
+            f->keys = keys_b; f->vals = vals_a;
+            TRYF(launch_bucket_scatter(ctx, f, bcount, keys_a, vb, big_list, reinterpret_cast<unsigned int*>(totals + 2)));
+            TRYF(launch_bucket_sort(ctx, f, keys_a, nonempty, totals, reinterpret_cast<unsigned int*>(totals + 4), vb));
+            svr_free(ctx, keys_a, ka);
+            svr_free(ctx, big_list, big_bytes);
+            keys_a = nullptr; big_list = nullptr;
+            f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
+            keys_b = nullptr; vals_a = nullptr;
+        }
+        svr_free(ctx, bcount, bucket_bytes);
+        svr_free(ctx, nonempty, bucket_bytes);
+        svr_free(ctx, bigdiff, diff_bytes);
+        bcount = nonempty = nullptr; bigdiff = nullptr;
+        svr_free(ctx, totals, 64);
+        totals = nullptr;
+        TRYF(launch_lists_finish(ctx, f));
+        TRYF(launch_pack_entries(ctx, f));
+    } else {
+        TRYF(A.get((void**)&f->offsets, sizeof(uint32_t) * (size_t)(n + 1)));
+        TRYF(svr_alloc(ctx, (void**)&counts, counts_bytes));
+        TRYF(launch_rects_counts(ctx, f, counts, totals));
+        TRYF(launch_exclusive_scan(ctx, counts, f->offsets, n + 1));
+        // E = offsets[n]; number of big voxels = totals[1]: one small readback sizes the sort buffers
+        CUDAF(cudaMemcpyAsync(totals, f->offsets + n, sizeof(uint32_t), cudaMemcpyDeviceToDevice, ctx->stream));
+        CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 16, cudaMemcpyDeviceToHost, ctx->stream));
+        // per-view colours do not depend on E: enqueue before the sync so they overlap the readback
+        TRYF(launch_voxel_colors(ctx, f));
+        CUDAF(cudaStreamSynchronize(ctx->stream));
+        const int64_t E = (int64_t)(ctx->host_pinned[0] & 0xFFFFFFFFull);
+        const int64_t n_big = (int64_t)ctx->host_pinned[1];
+        svr_free(ctx, counts, counts_bytes);
+        counts = nullptr;
+        if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));
+        f->n_entries = E;
+
+        if (E > 0) {
+            ka = sizeof(uint64_t) * (size_t)E;
+            va = sizeof(uint32_t) * (size_t)E;
+            big_bytes = sizeof(uint32_t) * (size_t)(n_big + 1);
+            TRYF(svr_alloc(ctx, (void**)&keys_a, ka));
+            TRYF(svr_alloc(ctx, (void**)&keys_b, ka));
+            TRYF(svr_alloc(ctx, (void**)&vals_a, va));
+            TRYF(svr_alloc(ctx, (void**)&vals_b, va));
+            TRYF(svr_alloc(ctx, (void**)&big_list, big_bytes));
+            unsigned int* big_count = reinterpret_cast<unsigned int*>(totals + 2);
+            TRYF(launch_emit_keys(ctx, f, keys_a, vals_a, big_list, big_count));
+            uint64_t* ks = nullptr;
+            uint32_t* vs = nullptr;
+            TRYF(launch_sort_pairs(ctx, keys_a, keys_b, vals_a, vals_b, E, f->key_bits, &ks, &vs));
+            // keep the buffers holding the sorted result, return the others to the pool
+            svr_free(ctx, ks == keys_a ? keys_b : keys_a, ka);
+            svr_free(ctx, vs == vals_a ? vals_b : vals_a, va);
+            svr_free(ctx, big_list, big_bytes);
+            big_list = nullptr;
+            f->keys = ks; f->vals = vs;
+            TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
+            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
+            f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
+            keys_a = keys_b = nullptr;
+            vals_a = vals_b = nullptr;
+        }
+        svr_free(ctx, totals, 64);
+        totals = nullptr;
+        TRYF(launch_ranges(ctx, f));
+        TRYF(launch_pack_entries(ctx, f));
     }
-    svr_free(ctx, totals, 64);
-    totals = nullptr;
-    TRYF(launch_ranges(ctx, f));
-    TRYF(launch_pack_entries(ctx, f));
 #undef TRYF
 #undef CUDAF
     *out = f;
@@ -382,6 +439,18 @@ const char* svr_stage_name(int stage) {
 SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset) {
     if (!ctx) return SVR_ERR_INVALID_ARG;
     SVR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (ctx->debug_flags & 1024) {   // measurement experiment: idle time on the stream before each stage
+        static double gap_ms[ST_COUNT] = {0};
+        static long gap_n = 0;
+        for (size_t i = 1; i < ctx->pending.size(); ++i) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, ctx->pending[i - 1].e1, ctx->pending[i].e0) == cudaSuccess) gap_ms[ctx->pending[i].stage] += t;
+        }
+        gap_n += 1;
+        fprintf(stderr, "gaps before stage (ms, cumulative):");
+        for (int i = 0; i < ST_COUNT; ++i) fprintf(stderr, " %s=%.3f", svr_stage_name(i), gap_ms[i]);
+        fprintf(stderr, "\n");
+    }
     for (const StagePending& p : ctx->pending) {
         float t = 0.f;
         if (cudaEventElapsedTime(&t, p.e0, p.e1) == cudaSuccess) {

@@ -123,6 +123,13 @@ SvrStatus launch_emit_keys(SvrContext* ctx, SvrFrame* f, uint64_t* keys, uint32_
 SvrStatus launch_sort_pairs(SvrContext* ctx, uint64_t* keys, uint64_t* keys_alt, uint32_t* vals, uint32_t* vals_alt,
                             int64_t n, int bits, uint64_t** keys_sorted, uint32_t** vals_sorted);
 SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_bucket_count(SvrContext* ctx, SvrFrame* f, uint32_t* bcount, int* bigdiff, uint32_t* nonempty,
+                              unsigned long long* totals);
+SvrStatus launch_bucket_scatter(SvrContext* ctx, SvrFrame* f, uint32_t* cursor, uint64_t* ent, int vb, uint32_t* big_list,
+                                unsigned int* big_count);
+SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const uint32_t* nonempty, const unsigned long long* totals,
+                             unsigned int* work, int vb);
+SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
