@@ -393,6 +393,7 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
 // Traffic per entry: 8 B written + 8 B read + 12 B written. Needs 3*Lmax + ceil(log2 N) <= 64 (else: first design).
 constexpr int BIG_TILES = 16;
 constexpr int SORT_CAP = 6144;        // largest bucket whose radix passes stay in shared memory (two buffers)
+constexpr int SORT_CAP_SMALL = 1536;   // size classes: <= 1536 words: 128-thread blocks, <= 6144: 512, <= 12288: 1024
 constexpr int SORT_CAP_BIG = 12288;   // same with one 1024-thread block per SM; beyond: passes through L2
 constexpr int SMALL_CAP = 256;        // buckets up to this size: bitonic network
 constexpr int SORT_THREADS2 = 512;
@@ -434,7 +435,7 @@ __global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __rest
                                                            uint32_t* __restrict__ bcount, uint32_t* __restrict__ ranges,
                                                            uint32_t* __restrict__ nonempty, unsigned long long* __restrict__ totals) {
     extern __shared__ int sd[];
-    __shared__ uint32_t wsum[32], wsum2[32], wsum3[32], n_big_buckets;
+    __shared__ uint32_t wsum[32], wsum2[32], wsum3[32], wsum4[32], n_big_buckets, n_mid_buckets;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int sx = tx + 1, nd = sx * (ty + 1);
     for (int i = tid; i < nd; i += 1024) sd[i] = bigdiff[i];
@@ -462,7 +463,7 @@ __global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __rest
     const int n_tiles = tx * ty;
     const int tpt = (n_tiles + 1023) / 1024;          // whole tiles per thread: 8 buckets = two 16-byte words each
     const int t0 = tid * tpt, t1 = min(n_tiles, t0 + tpt);
-    uint32_t local = 0, local_ne = 0, local_big = 0;
+    uint32_t local = 0, local_ne = 0, local_big = 0, local_mid = 0;
     for (int t = t0; t < t1; ++t) {
         const uint4 a = reinterpret_cast<const uint4*>(bcount)[2 * t], b = reinterpret_cast<const uint4*>(bcount)[2 * t + 1];
         const uint32_t c[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
@@ -472,31 +473,36 @@ __global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __rest
             const uint32_t cnt = c[o] + (((m >> o) & 1u) ? cover : 0u);
             local += cnt;
             local_big += (cnt > (uint32_t)SORT_CAP);
-            local_ne += (cnt != 0u && cnt <= (uint32_t)SORT_CAP);
+            local_mid += (cnt > (uint32_t)SORT_CAP_SMALL && cnt <= (uint32_t)SORT_CAP);
+            local_ne += (cnt != 0u && cnt <= (uint32_t)SORT_CAP_SMALL);
         }
     }
-    // block-wide exclusive scans of (local, local_ne, local_big)
-    uint32_t inc = local, inc2 = local_ne, inc3 = local_big;
+    // block-wide exclusive scans of (local, local_ne, local_big, local_mid)
+    uint32_t inc = local, inc2 = local_ne, inc3 = local_big, inc4 = local_mid;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o), t2 = __shfl_up_sync(0xffffffffu, inc2, o), t3 = __shfl_up_sync(0xffffffffu, inc3, o);
-        if (lane >= o) { inc += t; inc2 += t2; inc3 += t3; }
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o), t2 = __shfl_up_sync(0xffffffffu, inc2, o), t3 = __shfl_up_sync(0xffffffffu, inc3, o),
+                 t4 = __shfl_up_sync(0xffffffffu, inc4, o);
+        if (lane >= o) { inc += t; inc2 += t2; inc3 += t3; inc4 += t4; }
     }
-    if (lane == 31) { wsum[warp] = inc; wsum2[warp] = inc2; wsum3[warp] = inc3; }
+    if (lane == 31) { wsum[warp] = inc; wsum2[warp] = inc2; wsum3[warp] = inc3; wsum4[warp] = inc4; }
     __syncthreads();
     if (warp == 0) {
-        uint32_t w = wsum[lane], w2 = wsum2[lane], w3 = wsum3[lane], a = w, a2 = w2, a3 = w3;
+        uint32_t w = wsum[lane], w2 = wsum2[lane], w3 = wsum3[lane], w4 = wsum4[lane], a = w, a2 = w2, a3 = w3, a4 = w4;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, a, o), t2 = __shfl_up_sync(0xffffffffu, a2, o), t3 = __shfl_up_sync(0xffffffffu, a3, o);
-            if (lane >= o) { a += t; a2 += t2; a3 += t3; }
+            uint32_t t = __shfl_up_sync(0xffffffffu, a, o), t2 = __shfl_up_sync(0xffffffffu, a2, o), t3 = __shfl_up_sync(0xffffffffu, a3, o),
+                     t4 = __shfl_up_sync(0xffffffffu, a4, o);
+            if (lane >= o) { a += t; a2 += t2; a3 += t3; a4 += t4; }
         }
-        wsum[lane] = a - w; wsum2[lane] = a2 - w2; wsum3[lane] = a3 - w3;
-        if (lane == 31) { totals[0] = a; totals[3] = a2 + a3; totals[5] = a3; n_big_buckets = a3; }
+        wsum[lane] = a - w; wsum2[lane] = a2 - w2; wsum3[lane] = a3 - w3; wsum4[lane] = a4 - w4;
+        if (lane == 31) { totals[0] = a; totals[3] = a2 + a3 + a4; totals[5] = a3; totals[6] = a3 + a4; n_big_buckets = a3; n_mid_buckets = a4; }
     }
     __syncthreads();
-    // the largest buckets go to the front of the work list: they take longest to sort
-    uint32_t run = wsum[warp] + inc - local, run_ne = n_big_buckets + wsum2[warp] + inc2 - local_ne, run_big = wsum3[warp] + inc3 - local_big;
+    // work list by size class, largest first: [ > SORT_CAP | > SORT_CAP_SMALL | rest ]
+    uint32_t run = wsum[warp] + inc - local, run_big = wsum3[warp] + inc3 - local_big;
+    uint32_t run_mid = n_big_buckets + wsum4[warp] + inc4 - local_mid;
+    uint32_t run_ne = n_big_buckets + n_mid_buckets + wsum2[warp] + inc2 - local_ne;
     for (int t = t0; t < t1; ++t) {
         const uint4 a = reinterpret_cast<const uint4*>(bcount)[2 * t], b = reinterpret_cast<const uint4*>(bcount)[2 * t + 1];
         const uint32_t c[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
@@ -509,6 +515,7 @@ __global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __rest
             rg[2 * o] = cnt ? run : 0u;
             rg[2 * o + 1] = cnt ? run + cnt : 0u;
             if (cnt > (uint32_t)SORT_CAP) nonempty[run_big++] = (uint32_t)(t * 8 + o);
+            else if (cnt > (uint32_t)SORT_CAP_SMALL) nonempty[run_mid++] = (uint32_t)(t * 8 + o);
             else if (cnt) nonempty[run_ne++] = (uint32_t)(t * 8 + o);
             run += cnt;
         }
@@ -600,6 +607,47 @@ __device__ __forceinline__ void smem_sort(uint64_t* sk, int P) {
     }
 }
 
+// wh[w][d] (per-warp counts of digit d) -> exclusive offsets over the warps; tot[d] = first position of digit d.
+// Returns true (block-uniform) when one digit holds all m words. DPT digits per thread when the block has < 256 threads.
+template <int THREADS, typename CT>
+__device__ __forceinline__ bool digit_scan(CT* wh, uint32_t* tot, uint32_t* sh8, uint32_t m) {
+    constexpr int DPT = (THREADS >= 256) ? 1 : 256 / THREADS;
+    constexpr int ACTIVE = 256 / DPT;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t sum[DPT], total = 0;
+    bool all = false;
+    if (tid < ACTIVE) {
+#pragma unroll
+        for (int j = 0; j < DPT; ++j) {
+            const int d = tid * DPT + j;
+            uint32_t run = 0;
+#pragma unroll
+            for (int w = 0; w < (THREADS / 32); ++w) { const uint32_t c = wh[w * 256 + d]; wh[w * 256 + d] = (CT)run; run += c; }
+            sum[j] = run;
+            total += run;
+            all = all || (run == m);
+        }
+    }
+    if (__syncthreads_or(all)) return true;
+    uint32_t inc = total;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (tid < ACTIVE && lane == 31) sh8[warp] = inc;
+    __syncthreads();
+    if (tid < ACTIVE) {
+        uint32_t basev = inc - total;
+#pragma unroll
+        for (int w = 0; w < ACTIVE / 32; ++w) if (w < warp) basev += sh8[w];
+#pragma unroll
+        for (int j = 0; j < DPT; ++j) { tot[tid * DPT + j] = basev; basev += sum[j]; }
+    }
+    __syncthreads();
+    return false;
+}
+
 // One radix pass over src[0, m) -> dst[0, m) on digit (word >> shift) & mask. wh = [(THREADS / 32)][256] counters, tot = [256].
 // Returns false (and writes nothing) when all words share the digit.
 template <int THREADS>
@@ -621,30 +669,7 @@ __device__ __forceinline__ bool radix_pass(const uint64_t* src, uint64_t* dst, u
         __syncwarp();
     }
     __syncthreads();
-    uint32_t run = 0;
-    if (tid < 256) {
-#pragma unroll
-        for (int w = 0; w < (THREADS / 32); ++w) { const uint32_t c = wh[w * 256 + tid]; wh[w * 256 + tid] = run; run += c; }
-    }
-    const int uniform = __syncthreads_or(tid < 256 && run == m);
-    if (uniform) return false;
-    {   // exclusive scan of the 256 digit totals (threads 0..255 = 8 warps)
-        uint32_t inc = run;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(FULLM, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (tid < 256 && lane == 31) sh8[warp] = inc;
-        __syncthreads();
-        if (tid < 256) {
-            uint32_t basev = 0;
-#pragma unroll
-            for (int w = 0; w < 8; ++w) if (w < warp) basev += sh8[w];
-            tot[tid] = basev + inc - run;
-        }
-        __syncthreads();
-    }
+    if (digit_scan<THREADS>(wh, tot, sh8, m)) return false;
     for (uint32_t r = r0; r < r1; ++r) {
         const uint32_t i = (r << 5) + lane;
         const bool valid = i < m;
@@ -697,30 +722,7 @@ __device__ __forceinline__ bool radix_pass_reg(const uint64_t* src, uint64_t* ds
         }
     }
     __syncthreads();
-    uint32_t run = 0;
-    if (tid < 256) {
-#pragma unroll
-        for (int w = 0; w < (THREADS / 32); ++w) { const uint32_t c = wh[w * 256 + tid]; wh[w * 256 + tid] = (uint16_t)run; run += c; }
-    }
-    const int uniform = __syncthreads_or(tid < 256 && run == m);
-    if (uniform) return false;
-    {   // exclusive scan of the 256 digit totals (threads 0..255 = 8 warps)
-        uint32_t inc = run;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(FULLM, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (tid < 256 && lane == 31) sh8[warp] = inc;
-        __syncthreads();
-        if (tid < 256) {
-            uint32_t basev = 0;
-#pragma unroll
-            for (int w = 0; w < 8; ++w) if (w < warp) basev += sh8[w];
-            tot[tid] = basev + inc - run;
-        }
-        __syncthreads();
-    }
+    if (digit_scan<THREADS>(wh, tot, sh8, m)) return false;
 #pragma unroll
     for (int k = 0; k < (CAP / THREADS); ++k) {
         const uint32_t i = i0 + (k << 5);
@@ -745,9 +747,9 @@ __global__ void __launch_bounds__(THREADS) bucket_sort_kernel(uint64_t* __restri
     __shared__ uint32_t tot[256];
     __shared__ uint32_t sh8[8];
     __shared__ unsigned int next;
-    // work list: the buckets larger than SORT_CAP first (totals[5] of them), then the rest (totals[3] in all)
-    const unsigned int w_first = big_part ? 0u : (unsigned int)totals[5];
-    const unsigned int n_ne = big_part ? (unsigned int)totals[5] : (unsigned int)totals[3];
+    // work list by size class: [0, totals[5]) > SORT_CAP, [totals[5], totals[6]) > SORT_CAP_SMALL, [totals[6], totals[3]) the rest
+    const unsigned int w_first = big_part == 0 ? 0u : (unsigned int)totals[big_part == 1 ? 5 : 6];
+    const unsigned int n_ne = (unsigned int)totals[big_part == 0 ? 5 : (big_part == 1 ? 6 : 3)];
     const uint64_t vmask = (1ull << vb) - 1ull;
     while (true) {
         __syncthreads();
@@ -915,19 +917,23 @@ SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const 
                              unsigned int* work, int vb) {
     StageScope scope__(ctx, ST_SORT);
     static bool attr_set = false;
-    const int smem_small = 2 * SORT_CAP * (int)sizeof(uint64_t) + (SORT_THREADS2 / 32) * 256 * (int)sizeof(uint16_t);
+    const int smem_small = 2 * SORT_CAP_SMALL * (int)sizeof(uint64_t) + (128 / 32) * 256 * (int)sizeof(uint16_t);
+    const int smem_mid = 2 * SORT_CAP * (int)sizeof(uint64_t) + (SORT_THREADS2 / 32) * 256 * (int)sizeof(uint16_t);
     const int smem_big = 2 * SORT_CAP_BIG * (int)sizeof(uint64_t) + (1024 / 32) * 256 * (int)sizeof(uint16_t);
     if (!attr_set) {
-        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<SORT_THREADS2, SORT_CAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_small));
+        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<128, SORT_CAP_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_small));
+        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<SORT_THREADS2, SORT_CAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_mid));
         SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<1024, SORT_CAP_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_big));
         attr_set = true;
     }
-    // the few buckets above SORT_CAP: one 1024-thread block per SM with both buffers still in shared memory
-    bucket_sort_kernel<1024, SORT_CAP_BIG><<<148, 1024, smem_big, ctx->stream>>>(ent, f->ranges, nonempty, totals, work + 1, 1,
-                                                                                3 * f->scene.max_level, vb, f->keys, f->vals);
-    bucket_sort_kernel<SORT_THREADS2, SORT_CAP><<<148 * 2, SORT_THREADS2, smem_small, ctx->stream>>>(
-        ent, f->ranges, nonempty, totals, work, 0, 3 * f->scene.max_level, vb, f->keys, f->vals);
-    ctx->launches += 2;
+    // three block shapes so that the fixed cost of a pass (counter reset, scan) scales with the bucket; work[0..2] = fetch counters
+    const int cb = 3 * f->scene.max_level;
+    bucket_sort_kernel<1024, SORT_CAP_BIG><<<148, 1024, smem_big, ctx->stream>>>(ent, f->ranges, nonempty, totals, work, 0, cb, vb, f->keys, f->vals);
+    bucket_sort_kernel<SORT_THREADS2, SORT_CAP><<<148 * 2, SORT_THREADS2, smem_mid, ctx->stream>>>(ent, f->ranges, nonempty, totals, work + 1, 1, cb, vb,
+                                                                                                    f->keys, f->vals);
+    bucket_sort_kernel<128, SORT_CAP_SMALL><<<148 * 8, 128, smem_small, ctx->stream>>>(ent, f->ranges, nonempty, totals, work + 2, 2, cb, vb, f->keys,
+                                                                                      f->vals);
+    ctx->launches += 3;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

@@ -180,7 +180,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     SvrStatus st = SVR_OK;
     auto fail = [&](SvrStatus s) {
         if (counts) svr_free(ctx, counts, counts_bytes);
-        if (totals) svr_free(ctx, totals, 64);
+        if (totals) svr_free(ctx, totals, 128);
         if (big_list) svr_free(ctx, big_list, big_bytes);
         if (keys_a) svr_free(ctx, keys_a, ka);
         if (keys_b) svr_free(ctx, keys_b, ka);
@@ -203,8 +203,8 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->ranges, sizeof(uint32_t) * 16 * (size_t)f->n_tiles));
     TRYF(A.get((void**)&f->tile_order, sizeof(uint32_t) * 2 * (size_t)f->n_tiles));
-    TRYF(svr_alloc(ctx, (void**)&totals, 64));
-    CUDAF(cudaMemsetAsync(totals, 0, 64, ctx->stream));
+    TRYF(svr_alloc(ctx, (void**)&totals, 128));
+    CUDAF(cudaMemsetAsync(totals, 0, 128, ctx->stream));
     TRYF(launch_tile_masks(ctx, f));
 
     if (bucketed) {
@@ -236,7 +236,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             TRYF(svr_alloc(ctx, (void**)&big_list, big_bytes));
             f->keys = keys_b; f->vals = vals_a;
             TRYF(launch_bucket_scatter(ctx, f, bcount, keys_a, vb, big_list, reinterpret_cast<unsigned int*>(totals + 2)));
-            TRYF(launch_bucket_sort(ctx, f, keys_a, nonempty, totals, reinterpret_cast<unsigned int*>(totals + 4), vb));
+            TRYF(launch_bucket_sort(ctx, f, keys_a, nonempty, totals, reinterpret_cast<unsigned int*>(totals + 8), vb));   // totals[8..9]: the three work-fetch counters
             svr_free(ctx, keys_a, ka);
             svr_free(ctx, big_list, big_bytes);
             keys_a = nullptr; big_list = nullptr;
@@ -247,7 +247,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         svr_free(ctx, nonempty, bucket_bytes);
         svr_free(ctx, bigdiff, diff_bytes);
         bcount = nonempty = nullptr; bigdiff = nullptr;
-        svr_free(ctx, totals, 64);
+        svr_free(ctx, totals, 128);
         totals = nullptr;
         TRYF(launch_lists_finish(ctx, f));
         TRYF(launch_pack_entries(ctx, f));
@@ -295,7 +295,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             keys_a = keys_b = nullptr;
             vals_a = vals_b = nullptr;
         }
-        svr_free(ctx, totals, 64);
+        svr_free(ctx, totals, 128);
         totals = nullptr;
         TRYF(launch_ranges(ctx, f));
         TRYF(launch_pack_entries(ctx, f));
