@@ -250,6 +250,10 @@ class Context:
         self._check(_lib.svr_forward_stats(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(image), C.cast(out, C.c_void_p)))
         return dict(hits=int(out[0]), slab_tests=int(out[1]), warp_voxel_pairs=int(out[2]), entries_staged=int(out[3]))
 
+    def svr_set_debug_flags(self, flags: int):
+        """Measurement / test hook: bit 3 (8) selects the first list-build design (per-voxel scan + global radix sort)."""
+        _lib.svr_set_debug_flags(self.handle, int(flags))
+
     def svr_set_stage_timing(self, enabled: bool):
         _lib.svr_set_stage_timing(self.handle, 1 if enabled else 0)
 

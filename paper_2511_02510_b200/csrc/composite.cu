@@ -4,30 +4,29 @@
 // barrier anywhere): a barrier per staged chunk cost 37% of the issue slots in the first version
 // (profiles/r1a_*), because the 8 blocks of a tile see very different numbers of voxels.
 //
-// Per warp, over the tile's sorted (tile, octant) list:
-//   1. cull: 32 entries at a time, lane i reads entry i's pixel rectangle (stored in list order by the
-//      range kernel, so the read is coalesced) and computes the 32-bit mask M of this warp's pixels it
-//      covers. M == 0 => the entry is skipped by this warp (76% of (warp, entry) pairs on C4).
-//   2. stage: surviving lanes gather their voxel (octree cell, 8 corner raws, per-view colour) and write
-//      it, in list order, into a warp-private shared-memory ring: centre relative to the camera as hi+lo
-//      floats (computed in fp64), half edge, raws, colour, M.
-//   3. walk: once >= 32 survivors are staged (or the list ends), the 32x32 bit matrix M[slot][pixel] is
+// Forward (composite_kernel), per warp, over the tile's sorted (tile, octant) list:
+//   1. cull: 32 entries at a time, lane i reads entry i's pixel rectangle (in list order, so the read is
+//      coalesced) and computes the 32-bit mask M of this warp's pixels it covers. M == 0 => the entry is
+//      skipped by this warp (76% of (warp, entry) pairs on C4).
+//   2. stage: surviving lanes copy their packed voxel record (pack_entries_kernel: centre relative to the
+//      camera as hi+lo floats, half edge, density coefficients, per-view colour), in list order, into a
+//      warp-private shared-memory ring.
+//   3. test: once >= 32 survivors are staged (or the list ends), the 32x32 bit matrix M[slot][pixel] is
 //      transposed across the warp with 5 shuffles, giving every lane the bitmask of slots that cover ITS
-//      pixel. Each lane then pops its own next candidate (ffs) and slab-tests / integrates / composites it:
-//      lanes work on different voxels in the same instruction, so the expensive hit path (K trilinear
-//      samples, exp) runs with most lanes active instead of the ~7 of 32 a 2-pixel voxel covers.
-//      Front-to-back order per pixel is kept because slots are in list order.
-// Forward: eqs. 2-4; w_max (eq. 5) by atomicMax guarded by a plain read (w_max only grows).
-// Backward: same walk with the stored final colour, S_k = image - prefix_k (no division by 1 - alpha),
-//   dL/dtau_k = G . (T_k c_k - S_k); each hit adds its 8 corner + 3 colour gradients with three 16-byte
-//   vector reductions (red.global.add.v4.f32) - measured 165 G vector ops/s on B200, independent of
-//   how many lanes share an address, so no shared-memory staging (float atomics in shared memory are CAS
-//   loops on sm_100a: ATOMS.CAST.SPIN).
+//      pixel. Each lane pops its own candidates (ffs) and slab-tests them against a slightly dilated box:
+//      lanes work on different voxels in the same instruction.
+//   4. hits: each lane pops its own hits: precise slab test, K samples, eqs. 2-4; w_max (eq. 5,
+//      P:95) by atomicMax guarded by a plain read (w_max only grows). Front-to-back order per pixel is kept
+//      because slots are in list order.
+// Backward (backward_packed_kernel): same cull / stage / test, then the hits are compacted into a queue and
+// processed 32 at a time with all lanes busy; see the comment above that kernel.
 //
 // Density: the trilinear raw density is staged as polynomial coefficients (c0, cx, cy, cz, cxy, cxz, cyz,
 // cxyz), pre-multiplied by log2(e), so a sample costs 7 FMA + one EX2 instead of 7 lerps (14 ops) + MUL + EX2.
 // Backward accumulates the gradient w.r.t. those coefficients (monomials 1, qx, qy, qz, qxqy, ...) into a
-// per-voxel scratch; the per-voxel finalize kernel (preprocess.cu) maps it back to the 8 corners.
+// per-voxel scratch with 16-byte vector reductions (red.global.add.v4.f32; float atomics in shared memory are
+// CAS loops on sm_100a, so nothing is accumulated there); the per-voxel finalize kernel (preprocess.cu) maps
+// it back to the 8 corners.
 //
 // Precision: the ray is set up in fp64 per pixel and kept as hi+lo floats; the slab test runs in
 // coordinates relative to the ray's closest approach to the voxel centre, so the segment length keeps
@@ -130,8 +129,6 @@ __device__ __forceinline__ unsigned int transpose32(unsigned int x, int lane) {
     return x;
 }
 
-__device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
-
 // Ray/voxel segment in coordinates relative to t_ref (the ray parameter closest to the voxel centre).
 __device__ __forceinline__ bool slab(const RayF& r, const float4& a, const float4& b, float& s0, float& s1, float& t_ref,
                                      float* D) {
@@ -196,17 +193,15 @@ __device__ __forceinline__ float integrate(const RayF& r, const float* D, float 
 __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
-template <int K, bool BWD, bool STATS>
-__global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, const float4* __restrict__ packed,
+template <int K, bool STATS>
+__global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float4* __restrict__ packed,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
                                                         const uint32_t* __restrict__ tile_order,
                                                         float T_min,
                                                         float* __restrict__ image, float* __restrict__ depth,
                                                         float* __restrict__ T_final, unsigned int* __restrict__ w_max,
-                                                        const float* __restrict__ dL, const float* __restrict__ image_in,
-                                                        float* __restrict__ grad_coef, float* __restrict__ grad_rgb,
-                                                        unsigned long long* __restrict__ stats, int dbg) {
+                                                        unsigned long long* __restrict__ stats) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     WarpStage& S = reinterpret_cast<WarpStage*>(smem_raw)[warp];
@@ -227,12 +222,7 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, c
         for (int a = 0; a < 3; ++a) { ray.dh[a] = 0.f; ray.dl[a] = 0.f; ray.inv[a] = 0.f; ray.ainv[a] = 0.f; }
     }
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dep = 0.f;
-    float G0 = 0.f, G1 = 0.f, G2 = 0.f, F0 = 0.f, F1 = 0.f, F2 = 0.f;
     unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_read = 0;   // STATS only
-    if (BWD && inimg) {
-        G0 = dL[pix * 3]; G1 = dL[pix * 3 + 1]; G2 = dL[pix * 3 + 2];
-        F0 = image_in[pix * 3]; F1 = image_in[pix * 3 + 1]; F2 = image_in[pix * 3 + 2];
-    }
 
     for (int so = 0; so < 8; ++so) {
         const uint32_t start = ranges[(tile * 8 + so) * 2], end = ranges[(tile * 8 + so) * 2 + 1];
@@ -255,13 +245,6 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, c
                     const int slot = (head + count + __popc(m & ((1u << lane) - 1u))) & (RING - 1);
                     S.g0[slot] = t0; S.g1[slot] = t1; S.r0[slot] = t2; S.r1[slot] = t3; S.col[slot] = t4;
                     S.M[slot] = M;
-                    if (BWD) {
-                        // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the
-                        // DRAM fill (3.4 ms -> 5.2 ms without this on C4)
-                        const uint32_t vid = __float_as_uint(t1.w);
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
-                    }
                 }
                 count += __popc(m);
                 base += 32;
@@ -273,20 +256,37 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, c
             const int n = min(count, 32);
             unsigned int cand = transpose32(lane < n ? S.M[(head + lane) & (RING - 1)] : 0u, lane);
             if (!alive) cand = 0u;
-            if (!BWD) {
+            {
+                // two loops: (1) every lane slab-tests its own candidates against a slightly dilated box (centre hi
+                // parts only) and records the hits; (2) every lane integrates and composites its own hits. A lane that
+                // misses no longer sits idle through another lane's K samples, and the hit loop is as long as the
+                // pixel with the most HITS, not the most candidates.
+                unsigned int hits = 0u;
+                if (STATS) n_test += __popc(cand);
                 while (__any_sync(FULL, cand != 0u)) {
                     if (cand) {
-                        const int slot = (head + __ffs(cand) - 1) & (RING - 1);
+                        const int k = __ffs(cand) - 1;
                         cand &= cand - 1;
+                        const float4 a = S.g0[(head + k) & (RING - 1)];
+                        // dilation: a bound on what the lo parts and the rounding can move, so no true hit is lost
+                        const float hd = fmaf(fabsf(a.x) + fabsf(a.y) + fabsf(a.z), 4.8e-7f, a.w * 1.000002f);
+                        const float cx = a.x * ray.inv[0], cy = a.y * ray.inv[1], cz = a.z * ray.inv[2];
+                        const float wx = hd * ray.ainv[0], wy = hd * ray.ainv[1], wz = hd * ray.ainv[2];
+                        const float s0 = fmaxf(fmaxf(cx - wx, cy - wy), fmaxf(cz - wz, 0.f));
+                        const float s1 = fminf(fminf(cx + wx, cy + wy), cz + wz);
+                        if (s1 > s0) hits |= 1u << k;
+                    }
+                }
+                while (__any_sync(FULL, hits != 0u)) {
+                    if (hits) {
+                        const int slot = (head + __ffs(hits) - 1) & (RING - 1);
+                        hits &= hits - 1;
                         const float4 a = S.g0[slot], bq = S.g1[slot];
                         float s0, s1, t_ref, D[3];
-                        if (STATS) ++n_test;
-                        if (slab(ray, a, bq, s0, s1, t_ref, D)) {
+                        if (slab(ray, a, bq, s0, s1, t_ref, D)) {               // the precise test decides
                             const uint32_t vid = __float_as_uint(bq.w);
-                            // w_max only grows, so a stale (cached) read is safe; issued first so that its latency
-                            // hides behind the integration instead of queueing behind this hit's reductions
                             unsigned int wm_old = 0u;
-                            if (w_max != nullptr) wm_old = w_max[vid];
+                            if (w_max != nullptr) wm_old = w_max[vid];            // stale read is safe: w_max only grows
                             const float4 ra = S.r0[slot], rb = S.r1[slot], col = S.col[slot];
                             float dtau[8];
                             float tau = integrate<K, false>(ray, D, a.w, s0, s1, ra, rb, dtau);
@@ -297,81 +297,7 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, c
                             if (STATS) ++n_hit;
                             Dep = fmaf(w, t_ref + 0.5f * (s0 + s1), Dep);
                             if (w_max != nullptr && __float_as_uint(w) > wm_old) atomicMax(w_max + vid, __float_as_uint(w));
-                            if (T < T_min) { alive = false; cand = 0u; }          // R8: stop after the voxel that crosses T_min
-                        }
-                    }
-                }
-            } else {
-                // Backward: the four lanes of a 2x2 pixel quad (lane ^ 1 = x neighbour, lane ^ 8 = y neighbour) walk the
-                // union of their candidates in lock-step, so that their gradient contributions to one voxel can be
-                // summed with 12 shuffles and leave as ONE set of three vector reductions per (quad, voxel)
-                // instead of one set per (pixel, voxel): 2.5x fewer reductions on C4.
-                unsigned int cq = cand | __shfl_xor_sync(FULL, cand, 1);
-                cq |= __shfl_xor_sync(FULL, cq, 8);
-                const bool bx = (lane & 1) != 0, by = (lane & 8) != 0;
-                while (true) {
-                    const unsigned int run = __ballot_sync(FULL, cq != 0u);
-                    if (run == 0u) break;
-                    if (cq) {
-                        const int k = __ffs(cq) - 1;
-                        cq &= cq - 1;
-                        const int slot = (head + k) & (RING - 1);
-                        const float4 bq = S.g1[slot];
-                        const uint32_t vid = __float_as_uint(bq.w);
-                        float v[12];
-    #pragma unroll
-                        for (int i = 0; i < 12; ++i) v[i] = 0.f;
-                        float w = 0.f;
-                        if ((cand >> k) & 1u) {
-                            const float4 a = S.g0[slot];
-                            float s0, s1, t_ref, D[3];
-                            if (slab(ray, a, bq, s0, s1, t_ref, D)) {
-                                const float4 ra = S.r0[slot], rb = S.r1[slot], col = S.col[slot];
-                                float dtau[8];
-                                float tau = integrate<K, true>(ray, D, a.w, s0, s1, ra, rb, dtau);
-                                float E = ex2f(-1.4426950408889634f * tau);
-                                w = T * (1.f - E);
-                                T *= E;
-                                C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
-                                // suffix colour S_k = final - prefix_k; dL/dtau = G . (T_k c_k - S_k)
-                                float dLdtau = G0 * (fmaf(T, col.x, C0) - F0) + G1 * (fmaf(T, col.y, C1) - F1) +
-                                               G2 * (fmaf(T, col.z, C2) - F2);
-    #pragma unroll
-                                for (int i = 0; i < 8; ++i) v[i] = dLdtau * dtau[i];
-                                v[8] = w * G0; v[9] = w * G1; v[10] = w * G2;
-                                if (T < T_min) { alive = false; cand = 0u; }      // R8
-                            }
-                        }
-                        // quad maximum of w: zero means no lane of the quad hit this voxel
-                        float wq = fmaxf(w, __shfl_xor_sync(run, w, 1));
-                        wq = fmaxf(wq, __shfl_xor_sync(run, wq, 8));
-                        const unsigned int act = __ballot_sync(run, wq > 0.f);   // whole quads: wq is quad-uniform
-                        if (wq > 0.f) {
-                            // the quad's otherwise idle lane keeps w_max; its guard read (possibly stale: w_max only
-                            // grows) is issued before the shuffles so that its latency is hidden
-                            unsigned int wm_old = 0xFFFFFFFFu;
-                            if (w_max != nullptr && bx && by) wm_old = w_max[vid];
-                            // x neighbours: even lanes collect the 8 coefficient gradients, odd lanes the colour gradients
-    #pragma unroll
-                            for (int i = 0; i < 8; ++i) {
-                                float send = bx ? v[i] : ((i < 4) ? v[8 + i] : 0.f);
-                                float recv = __shfl_xor_sync(act, send, 1);
-                                if (!bx) v[i] += recv;
-                                else if (i < 4) v[8 + i] += recv;
-                            }
-                            // y neighbours: (by=0,bx=0) ends with coef 0..3, (by=1,bx=0) with coef 4..7, (by=0,bx=1) with colour
-                            float o4[4];
-    #pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                float keep = bx ? v[8 + i] : (by ? v[4 + i] : v[i]);
-                                float send = bx ? v[8 + i] : (by ? v[i] : v[4 + i]);
-                                o4[i] = keep + __shfl_xor_sync(act, send, 8);
-                            }
-                            if (!(bx && by) && !(dbg & 1)) {
-                                float* dst = bx ? (grad_rgb + (size_t)vid * 4) : (grad_coef + (size_t)vid * 8 + (by ? 4 : 0));
-                                red_add_v4(dst, o4[0], o4[1], o4[2], o4[3]);
-                            }
-                            if (__float_as_uint(wq) > wm_old) atomicMax(w_max + vid, __float_as_uint(wq));
+                            if (T < T_min) { alive = false; hits = 0u; }          // R8: stop after the voxel that crosses T_min
                         }
                     }
                 }
@@ -391,7 +317,7 @@ __global__ void __launch_bounds__(256, BWD ? 3 : 4) composite_kernel(CamDev c, c
             if (lane == 0 && t) atomicAdd(stats + i, (unsigned long long)t);
         }
     }
-    if (!BWD && inimg) {
+    if (inimg) {
         image[pix * 3] = fmaf(T, c.bg[0], C0);
         image[pix * 3 + 1] = fmaf(T, c.bg[1], C1);
         image[pix * 3 + 2] = fmaf(T, c.bg[2], C2);
@@ -679,45 +605,12 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     }
 }
 
-template <bool BWD>
-SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
-                           float* w_max, const float* dL, const float* image_in, float* grad_coef, float* grad_rgb,
-                           unsigned long long* stats) {
-    if (f->n_tiles == 0) return SVR_OK;
-    StageScope scope__(ctx, BWD ? ST_BACKWARD : ST_FORWARD);
-    const bool packed = BWD && (ctx->debug_flags & 2) == 0;      // debug flag 2: lane-centric backward (first design, for A/B)
-    const size_t smem = packed ? sizeof(WarpWork) * WARPS : sizeof(WarpStage) * WARPS;
-    const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
-    unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
-    const float4* pk = reinterpret_cast<const float4*>(f->packed);
-#define SVR_ARGS f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, T_final, wm, dL, image_in, grad_coef, grad_rgb, stats, ctx->debug_flags
-#define SVR_GO(KERNEL, ...)                                                                                \
-    do {                                                                                                   \
-        static bool attr_set = false;                                                                      \
-        if (!attr_set) {                                                                                   \
-            SVR_CUDA(ctx, cudaFuncSetAttribute(KERNEL, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-            attr_set = true;                                                                               \
-        }                                                                                                  \
-        KERNEL<<<f->n_tiles, 256, smem, ctx->stream>>>(__VA_ARGS__);                                       \
-    } while (0)
-#define SVR_LAUNCH(KK)                                                                          \
-    do {                                                                                        \
-        if (packed) SVR_GO((backward_packed_kernel<KK>), f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, image_in, grad_coef, grad_rgb); \
-        else if (!BWD && stats) SVR_GO((composite_kernel<KK, false, true>), SVR_ARGS);          \
-        else SVR_GO((composite_kernel<KK, BWD, false>), SVR_ARGS);                              \
-    } while (0)
-    switch (K) {
-        case 1: SVR_LAUNCH(1); break;
-        case 2: SVR_LAUNCH(2); break;
-        case 3: SVR_LAUNCH(3); break;
-        case 4: SVR_LAUNCH(4); break;
-        default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
+template <typename KernelT>
+SvrStatus set_smem_once(SvrContext* ctx, KernelT kernel, size_t smem, bool* done) {
+    if (!*done) {
+        SVR_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        *done = true;
     }
-#undef SVR_LAUNCH
-#undef SVR_GO
-#undef SVR_ARGS
-    ctx->launches += 1;
-    SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }
 
@@ -725,12 +618,64 @@ SvrStatus launch_composite(SvrContext* ctx, const SvrFrame* f, int K, float T_mi
 
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
                          float* w_max, unsigned long long* stats) {
-    return launch_composite<false>(ctx, f, K, T_min, image, depth, T_final, w_max, nullptr, nullptr, nullptr, nullptr, stats);
+    if (f->n_tiles == 0) return SVR_OK;
+    StageScope scope__(ctx, ST_FORWARD);
+    const size_t smem = sizeof(WarpStage) * WARPS;
+    const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
+    const float4* pk = reinterpret_cast<const float4*>(f->packed);
+    unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
+#define SVR_FWD(KK)                                                                                                  \
+    do {                                                                                                             \
+        static bool done_a = false, done_b = false;                                                                  \
+        if (stats) {                                                                                                 \
+            SVR_TRY(set_smem_once(ctx, composite_kernel<KK, true>, smem, &done_a));                                  \
+            composite_kernel<KK, true><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, \
+                                                                               T_final, wm, stats);                  \
+        } else {                                                                                                     \
+            SVR_TRY(set_smem_once(ctx, composite_kernel<KK, false>, smem, &done_b));                                 \
+            composite_kernel<KK, false><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, \
+                                                                                T_final, wm, stats);                 \
+        }                                                                                                            \
+    } while (0)
+    switch (K) {
+        case 1: SVR_FWD(1); break;
+        case 2: SVR_FWD(2); break;
+        case 3: SVR_FWD(3); break;
+        case 4: SVR_FWD(4); break;
+        default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
+    }
+#undef SVR_FWD
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
 }
 
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
                           float* grad_coef, float* grad_rgb, float* w_max) {
-    return launch_composite<true>(ctx, f, K, T_min, nullptr, nullptr, nullptr, w_max, dL, image, grad_coef, grad_rgb, nullptr);
+    if (f->n_tiles == 0) return SVR_OK;
+    StageScope scope__(ctx, ST_BACKWARD);
+    const size_t smem = sizeof(WarpWork) * WARPS;
+    const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
+    const float4* pk = reinterpret_cast<const float4*>(f->packed);
+    unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
+#define SVR_BWD(KK)                                                                                                  \
+    do {                                                                                                             \
+        static bool done = false;                                                                                    \
+        SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK>, smem, &done));                                        \
+        backward_packed_kernel<KK><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, image, \
+                                                                           grad_coef, grad_rgb);                     \
+    } while (0)
+    switch (K) {
+        case 1: SVR_BWD(1); break;
+        case 2: SVR_BWD(2); break;
+        case 3: SVR_BWD(3); break;
+        case 4: SVR_BWD(4); break;
+        default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
+    }
+#undef SVR_BWD
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
 }
 
 SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f) {

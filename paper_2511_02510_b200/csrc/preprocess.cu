@@ -350,7 +350,7 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
     __syncwarp();
     // cooperative read-modify-write of the warp's contiguous grad_sh block, skipping untouched voxels
     const int nvox = (int)min((int64_t)32, s.n - v0);
-    if (ROW % 4 == 0) {
+    if constexpr (ROW % 4 == 0) {
         float4* p4 = reinterpret_cast<float4*>(grad_sh + v0 * ROW);
         for (int e = lane; e < nvox * (ROW / 4); e += 32) {
             int vv = e / (ROW / 4);

@@ -117,6 +117,35 @@ def test_lists_bit_exact_camera_inside_and_ragged(orc, svr):
         check_lists(orc, svr, cfg4.scene, cam)
 
 
+def test_lists_bit_exact_every_bucket_size_class(orc, svr):
+    """The per-bucket sort has four paths (bitonic <= 256, 128/512/1024-thread radix in shared memory, radix through L2
+    above 12288 entries): far cameras put most of a scene into a handful of (tile, octant) buckets."""
+    cfg = make_config("C2")                                     # 50 000 voxels
+    sizes = []
+    for radius, res in [(40.0, 48), (12.0, 64), (4.0, 128)]:
+        cam = look_at_camera((radius * 0.8, radius * 0.5, radius * 0.33), (0, 0, 0), res, res)
+        check_lists(orc, svr, cfg.scene, cam)
+        pkg, ctx, torch = svr
+        fr = ctx.svr_preprocess(pkg.Voxels.from_scene(cfg.scene), cam)
+        r = fr.lists()["ranges"].reshape(-1, 2).astype(np.int64)
+        sizes.append(int((r[:, 1] - r[:, 0]).max()))
+        fr.release()
+    assert max(sizes) > 12288, sizes        # the regular cameras of the other tests cover the small classes
+
+
+def test_lists_bit_exact_first_design(orc, svr):
+    """Debug flag 8 selects the first list-build design (per-voxel scan + global radix sort), which is also the
+    fallback when code + voxel id do not fit one 64-bit word: it must give the same lists."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    ctx.svr_set_debug_flags(8)
+    try:
+        for cam in cfg.cameras[:2]:
+            assert check_lists(orc, svr, cfg.scene, cam) > 1000
+    finally:
+        ctx.svr_set_debug_flags(0)
+
+
 # ---------------------------------------------------------------------------------------------
 # forward + backward + loss on C1, C2
 # ---------------------------------------------------------------------------------------------
