@@ -265,9 +265,10 @@ def test_reduced_configs_full_images(orc, svr, name, n, scale):
         frame.release()
 
 
-@pytest.mark.parametrize("name", ["C3", "C4"])
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
 def test_full_size_sampled_rays(orc, svr, name):
-    """Full-size scene in the launch configuration bench.py times; the oracle brute-forces 384 sampled rays."""
+    """Full-size scene in the launch configuration bench.py times: lists bit-exact; the oracle brute-forces 384 sampled
+    rays for the forward outputs, and for the backward pass fed a dL/dC that is non-zero only on those rays."""
     pkg, ctx, torch = svr
     cfg = make_config(name, n_cams=1)
     cam = cfg.cameras[0]
@@ -285,4 +286,21 @@ def test_full_size_sampled_rays(orc, svr, name):
     # w_max is a max over ALL rays: at least the sampled rays' weights
     assert np.all(wm + 1e-4 >= ref["w_max"])
     assert ref["n_hits"].max() > 3
+    # backward: only the sampled pixels carry a gradient, so the full-size kernel must reproduce the oracle's sum over them
+    G = rng.normal(0, 1.0, size=(xy.shape[0], 3))
+    dL_img = np.zeros((cam.H, cam.W, 3), dtype=np.float32)
+    _, first = np.unique(xy[:, 1].astype(np.int64) * cam.W + xy[:, 0], return_index=True)      # duplicates: keep one
+    keep = np.zeros(xy.shape[0], dtype=bool)
+    keep[first] = True
+    dL_img[xy[keep, 1], xy[keep, 0]] = G[keep].astype(np.float32)
+    sc = cfg.scene
+    g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+    g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+    ctx.svr_backward(frame, cfg.K, torch.from_numpy(dL_img).cuda(), image, g_raw, g_sh, cfg.T_min)
+    ctx.synchronize()
+    Gs = dL_img[xy[keep, 1], xy[keep, 0]].astype(np.float64)
+    r_raw, r_sh = orc.backward(sc, cam, cfg.K, Gs, mode="pure", xy=np.ascontiguousarray(xy[keep]))
+    assert rel_l2(g_raw.cpu().numpy(), r_raw) <= GRAD_TOL and rel_l2(g_sh.cpu().numpy(), r_sh) <= GRAD_TOL
     frame.release()
+    del g_raw, g_sh
+    check_lists(orc, svr, sc, cam)
