@@ -18,25 +18,60 @@ SvrStatus svr_fail(SvrContext* ctx, SvrStatus st, const char* fmt, ...) {
     return st;
 }
 
+// Workspace blocks are cached by the context: a freed block goes to a free list and the next request that fits it
+// (capacity within 2x of the need) takes it back without touching the driver. Large blocks are allocated with 12.5%
+// slack, so the per-view buffers, whose sizes follow the entry count E, are reused from view to view even though E
+// changes; the first time a size is seen costs a cudaMallocAsync (milliseconds when the pool has to grow). Everything
+// is ordered on the context's one stream, so reuse needs no extra synchronisation.
 SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes) {
     *p = nullptr;
     if (bytes == 0) bytes = 256;
-    bytes = (bytes + 255) & ~(size_t)255;
-    if (ctx->budget && ctx->in_use + bytes > ctx->budget)
-        return svr_fail(ctx, SVR_ERR_WORKSPACE, "workspace budget exceeded: in use %zu + request %zu > budget %zu", ctx->in_use,
-                        bytes, ctx->budget);
-    SVR_CUDA(ctx, cudaMallocAsync(p, bytes, ctx->stream));
-    ctx->in_use += bytes;
-    if (ctx->in_use > ctx->peak) ctx->peak = ctx->in_use;
+    const size_t need = (bytes + 255) & ~(size_t)255;
+    int best = -1;
+    for (int i = 0; i < (int)ctx->free_blocks.size(); ++i) {
+        const size_t cap = ctx->free_blocks[i].second;
+        if (cap >= need && cap <= 2 * need + ((size_t)1 << 20) && (best < 0 || cap < ctx->free_blocks[best].second)) best = i;
+    }
+    size_t cap = best >= 0 ? ctx->free_blocks[best].second : (need > ((size_t)1 << 20) ? ((need + need / 8 + 255) & ~(size_t)255) : need);
+    if (ctx->budget && ctx->in_use + cap > ctx->budget) {
+        if (best < 0 && ctx->in_use + need <= ctx->budget) cap = need;     // no slack when the budget is tight
+        else if (ctx->in_use + cap > ctx->budget)
+            return svr_fail(ctx, SVR_ERR_WORKSPACE, "workspace budget exceeded: in use %zu + request %zu > budget %zu", ctx->in_use,
+                            need, ctx->budget);
+    }
+    if (best >= 0) {
+        *p = ctx->free_blocks[best].first;
+        ctx->cached -= cap;
+        ctx->free_blocks.erase(ctx->free_blocks.begin() + best);
+    } else {
+        // make room under the budget by dropping cached blocks first
+        while (ctx->budget && ctx->in_use + ctx->cached + cap > ctx->budget && !ctx->free_blocks.empty()) {
+            cudaFreeAsync(ctx->free_blocks.back().first, ctx->stream);
+            ctx->cached -= ctx->free_blocks.back().second;
+            ctx->free_blocks.pop_back();
+        }
+        SVR_CUDA(ctx, cudaMallocAsync(p, cap, ctx->stream));
+    }
+    ctx->live[*p] = cap;
+    ctx->in_use += cap;
+    if (ctx->in_use + ctx->cached > ctx->peak) ctx->peak = ctx->in_use + ctx->cached;
     return SVR_OK;
 }
 
-void svr_free(SvrContext* ctx, void* p, size_t bytes) {
+void svr_free(SvrContext* ctx, void* p, size_t /*bytes*/) {
     if (!p) return;
-    if (bytes == 0) bytes = 256;
-    bytes = (bytes + 255) & ~(size_t)255;
-    cudaFreeAsync(p, ctx->stream);
-    ctx->in_use -= bytes;
+    auto it = ctx->live.find(p);
+    if (it == ctx->live.end()) return;
+    const size_t cap = it->second;
+    ctx->live.erase(it);
+    ctx->in_use -= cap;
+    if (ctx->free_blocks.size() >= 48) {         // bounded list: drop the oldest cached block
+        cudaFreeAsync(ctx->free_blocks.front().first, ctx->stream);
+        ctx->cached -= ctx->free_blocks.front().second;
+        ctx->free_blocks.erase(ctx->free_blocks.begin());
+    }
+    ctx->free_blocks.emplace_back(p, cap);
+    ctx->cached += cap;
 }
 
 namespace {
@@ -45,9 +80,7 @@ struct FrameAlloc {
     SvrContext* ctx;
     SvrFrame* f;
     SvrStatus get(void** p, size_t bytes) {
-        SvrStatus st = svr_alloc(ctx, p, bytes);
-        if (st == SVR_OK) f->bytes += (bytes == 0 ? 256 : (bytes + 255) & ~(size_t)255);
-        return st;
+        return svr_alloc(ctx, p, bytes);
     }
 };
 
@@ -70,12 +103,9 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 }
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
-    // sizes are tracked in aggregate: free pointers, then give the bytes back in one go
     void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed};
     for (void* p : ptrs)
-        if (p) cudaFreeAsync(p, ctx->stream);
-    ctx->in_use -= f->bytes;
-    f->bytes = 0;
+        if (p) svr_free(ctx, p, 0);
     return SVR_OK;
 }
 
@@ -115,9 +145,8 @@ void svr_destroy(SvrContext* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    if (ctx->grad_rgb) cudaFreeAsync(ctx->grad_rgb, ctx->stream);
-    if (ctx->grad_coef) cudaFreeAsync(ctx->grad_coef, ctx->stream);
-    if (ctx->loss_ws) cudaFreeAsync(ctx->loss_ws, ctx->stream);
+    for (auto& b : ctx->free_blocks) cudaFreeAsync(b.first, ctx->stream);
+    for (auto& b : ctx->live) cudaFreeAsync(b.first, ctx->stream);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
@@ -240,7 +269,6 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             svr_free(ctx, keys_a, ka);
             svr_free(ctx, big_list, big_bytes);
             keys_a = nullptr; big_list = nullptr;
-            f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
             keys_b = nullptr; vals_a = nullptr;
         }
         svr_free(ctx, bcount, bucket_bytes);
@@ -291,7 +319,6 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             f->keys = ks; f->vals = vs;
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
             TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
-            f->bytes += ((ka + 255) & ~(size_t)255) + ((va + 255) & ~(size_t)255);
             keys_a = keys_b = nullptr;
             vals_a = vals_b = nullptr;
         }

@@ -4,6 +4,8 @@
 #include <stdint.h>
 #include <stddef.h>
 #include <string>
+#include <unordered_map>
+#include <utility>
 #include <vector>
 #include "svr.h"
 
@@ -27,7 +29,9 @@ struct SvrContext {
     int device = 0;
     cudaStream_t stream = nullptr;
     size_t budget = 0;            // 0 = unlimited
-    size_t in_use = 0, peak = 0;
+    size_t in_use = 0, cached = 0, peak = 0;   // bytes in live blocks, in cached free blocks, and the peak of their sum
+    std::vector<std::pair<void*, size_t>> free_blocks;   // cached free workspace blocks (pointer, capacity)
+    std::unordered_map<void*, size_t> live;             // live workspace blocks -> capacity
     int64_t launches = 0;
     std::string err;
     // persistent scratch
