@@ -315,8 +315,13 @@ def main():
     flop = {"forward_composite": FLOP_PER_FWD_HIT, "backward_composite": FLOP_PER_BWD_HIT}
     if dom in flop:
         achieved = hits * flop[dom] / (stage_ms[dom] * 1e-3) / 1e12
+        traffic = None      # DRAM bytes of one launch of this kernel from the committed ncu capture (full-size C4 only)
+        tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
+        if os.path.exists(tpath) and args.workload == "C4" and args.n_voxels is None and args.res_scale == 1.0:
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(dom)
         roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                    "frac": achieved / fp32_peak, "traffic": None,
+                    "frac": achieved / fp32_peak, "traffic": traffic,
                     "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x sm_max_mhz, clocks {peak_src}",
                     "algorithmic": f"{hits:.4g} ray-voxel hits/view x {flop[dom]:.0f} flop",
                     "kernel_ms": stage_ms[dom], "slab_tests_per_hit": tests / max(hits, 1.0)}
