@@ -190,6 +190,10 @@ __device__ __forceinline__ float integrate(const RayF& r, const float* D, float 
     return dt * sum;
 }
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned int d = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
 __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
@@ -230,31 +234,46 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
         bool alive = inimg && (oct == so) && (T >= T_min);
         unsigned int alive_mask = __ballot_sync(FULL, alive);
         if (alive_mask == 0u) continue;                               // no pixel of this warp uses this list
-        int head = 0, count = 0;                                      // ring state (warp-uniform)
+        // Double-buffered staging: the ring is two halves of 32 slots. While one half is walked, the records of the
+        // next batch are already on their way into the other half (cp.async: no registers held, no stall on the load).
         uint32_t base = start;
-        while (true) {
-            // ---- cull + stage until 32 survivors are waiting or the list is exhausted ----
-            while (count < 32 && base < end) {
-                uint32_t idx = base + lane;
+        auto stage = [&](int half) -> int {
+            int cnt = 0;
+            while (cnt < 32 && base < end) {
+                const uint32_t idx = base + lane;
+                if (lane < 2) asm volatile("prefetch.global.L1 [%0];" ::"l"(rects_sorted + min(base + 64u + 16u * lane, end - 1u)));   // two chunks ahead
                 unsigned int M = 0u;
                 if (idx < end) M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
                 unsigned int m = __ballot_sync(FULL, M != 0u);
+                const int rank = __popc(m & ((1u << lane) - 1u));
+                int adv = 32;
+                if (__popc(m) > 32 - cnt) {                            // more survivors than free slots: take the first ones
+                    if (rank >= 32 - cnt) M = 0u;
+                    m = __ballot_sync(FULL, M != 0u);
+                    adv = 32 - __clz(m);                               // resume after the last survivor taken
+                }
                 if (M) {
                     const float4* rec = packed + 5 * (size_t)idx;
-                    const float4 t0 = __ldg(rec), t1 = __ldg(rec + 1), t2 = __ldg(rec + 2), t3 = __ldg(rec + 3), t4 = __ldg(rec + 4);
-                    const int slot = (head + count + __popc(m & ((1u << lane) - 1u))) & (RING - 1);
-                    S.g0[slot] = t0; S.g1[slot] = t1; S.r0[slot] = t2; S.r1[slot] = t3; S.col[slot] = t4;
+                    const int slot = half + cnt + rank;
+                    cp_async16(&S.g0[slot], rec); cp_async16(&S.g1[slot], rec + 1); cp_async16(&S.r0[slot], rec + 2);
+                    cp_async16(&S.r1[slot], rec + 3); cp_async16(&S.col[slot], rec + 4);
                     S.M[slot] = M;
                 }
-                count += __popc(m);
-                base += 32;
-                if (STATS) { n_read += (idx < end); n_surv += (M != 0u); }
+                if (STATS) { n_read += (idx < end && (int)lane < adv); n_surv += (M != 0u); }
+                cnt += __popc(m);
+                base += adv;
             }
-            if (count == 0) break;
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            return cnt;
+        };
+        int head = 0, count = stage(0);
+        while (count > 0) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
             __syncwarp();
+            const int count_next = stage(head ^ 32);                  // in flight during the walk below
             // ---- walk up to 32 staged voxels, every lane through its own candidates ----
-            const int n = min(count, 32);
-            unsigned int cand = transpose32(lane < n ? S.M[(head + lane) & (RING - 1)] : 0u, lane);
+            const int n = count;
+            unsigned int cand = transpose32(lane < n ? S.M[head + lane] : 0u, lane);
             if (!alive) cand = 0u;
             {
                 // two loops: (1) every lane slab-tests its own candidates against a slightly dilated box (centre hi
@@ -303,11 +322,13 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                 }
             }
             __syncwarp();
-            head = (head + n) & (RING - 1);
-            count -= n;
+            head ^= 32;
+            count = count_next;
             alive_mask = __ballot_sync(FULL, alive);
             if (alive_mask == 0u) break;                              // whole warp terminated
         }
+        asm volatile("cp.async.wait_all;" ::: "memory");            // nothing in flight when the ring is reused
+        __syncwarp();
     }
     if (STATS) {
         unsigned int v4[4] = {n_hit, n_test, n_surv, n_read};
