@@ -451,3 +451,99 @@ def test_sh_quadrature_golden_fixture():
     vals = [float(x) for x in open(os.path.join(GOLDEN, "sh_l1_axes.txt")).read().split("\n") if x and not x.startswith("#")]
     assert abs(vals[0] - math.sqrt(3 / (4 * math.pi))) < 1e-15
     assert abs(vals[1] - 0.5 / math.sqrt(math.pi)) < 1e-15
+
+
+# ---------------------------------------------------------------------------------------------
+# depth-aware quantile pruning (Sec. IV-C): pins of oracle/prune.py
+# ---------------------------------------------------------------------------------------------
+def _prune_case(n=6000, seed=5):
+    from svr_inputs import make_config
+    cfg = make_config("C2", n_voxels=n)
+    rng = np.random.default_rng(seed)
+    w = (rng.random(cfg.scene.n) ** 3).astype(np.float32)
+    w[rng.random(cfg.scene.n) < 0.25] = 0.0                     # never-seen voxels
+    return cfg, w
+
+
+def test_prune_quantile_is_eq11_eq12():
+    """tau_b = F_b^{-1}(q_b) (eq. 12) with F_b the empirical CDF of eq. 11: F_b(tau_b) >= q_b and no
+    smaller sample value reaches q_b. Checked against the CDF written out per sample, not against a sort."""
+    from oracle.prune import PruneOpts, bin_quantiles, depth_bins, depth_proxy
+    cfg, w = _prune_case()
+    opts = PruneOpts(n_bins=5, q_near=0.4, q_far=0.15)
+    z, _, _ = depth_proxy(cfg.scene, cfg.cameras)
+    bins, _, _ = depth_bins(z, opts.n_bins)
+    tau, q = bin_quantiles(w, bins, opts)
+    assert np.isclose(q[0], 0.4) and np.isclose(q[-1], 0.15) and np.all(np.diff(q) < 0)
+    for b in range(opts.n_bins):
+        v = w[bins == b]
+        assert v.size > 0
+        F = lambda t: np.count_nonzero(v <= t) / v.size          # eq. 11
+        assert F(tau[b]) >= q[b] - 1e-7
+        smaller = v[v < tau[b]]
+        if smaller.size:
+            assert F(smaller.max()) < q[b] + 1e-7
+
+
+def test_prune_depth_proxy_on_axis_and_bins_monotone():
+    from oracle.prune import depth_bins, depth_proxy
+    from svr_inputs import look_at_camera, tiny_scene
+    sc = tiny_scene(1, n=1, sh_degree=0)                         # one voxel
+    x = np.asarray(sc.root_lo, dtype=np.float64) + (sc.ijkl[0, :3] + 0.5) * sc.root_edge / 2.0 ** sc.ijkl[0, 3]
+    pos = x + np.array([0.0, -2.5, 0.0])
+    cam = look_at_camera(tuple(pos), tuple(x), 64, 48)
+    z, delta, half = depth_proxy(sc, [cam])
+    assert abs(z[0] - 2.5) < 1e-5 and abs(delta[0] - 2.5 / cam.fx) < 1e-7     # on the optical axis depth = distance
+    assert half[0] == np.float32(0.5 * sc.root_edge / 2.0 ** sc.ijkl[0, 3])
+    behind = look_at_camera(tuple(pos), tuple(2 * pos - x), 64, 48)           # looking away: no positive depth
+    assert np.isinf(depth_proxy(sc, [behind])[0][0])
+    zz = np.array([0.5, 0.7, 1.01, 1.9, 2.01, 3.9, 4.0, np.inf], dtype=np.float32)
+    b, lo, hi = depth_bins(zz, 3)
+    assert np.all(np.diff(b) >= 0) and b[0] == 0 and b[-1] == 2 and b[-2] == 2
+    assert list(b[:7]) == [0, 0, 1, 1, 2, 2, 2]                  # bit patterns are piecewise-linear in log2: octaves 0.5-1-2-4
+
+
+def test_prune_hysteresis_hand_sequence():
+    """Guard i on one voxel, alpha = 0.5, m_low = 0.3, m_high = 0.7, starting in with m = 1:
+    x = 0,0,1,0,0,1,1 -> m = .5,.25,.625,.3125,.15625,.578125,.7890625 -> in,out,out,out,out,out,in."""
+    from oracle.prune import PruneOpts, prune_step
+    from svr_inputs import look_at_camera, tiny_scene
+    sc = tiny_scene(2, n=2, sh_degree=0)
+    cam = look_at_camera((3.0, 1.0, 0.5), (0, 0, 0), 64, 48)
+    opts = PruneOpts(n_bins=1, q_near=0.5, q_far=0.5, ema_alpha=0.5, m_low=0.3, m_high=0.7, kappa=0.0, w_keep=2.0, cap_fraction=0.0)
+    m, s = np.ones(2, np.float32), np.ones(2, np.uint8)
+    got_m, got_s = [], []
+    for x in [0, 0, 1, 0, 0, 1, 1]:
+        # two voxels, q = 0.5 -> tau = the smaller w_max: voxel 0 is "inside" iff it holds the larger value
+        w = np.array([0.9, 0.1], np.float32) if x else np.array([0.1, 0.9], np.float32)
+        r = prune_step(sc, [cam], w, m, s, opts)
+        m, s = r["ema"], r["state"]
+        got_m.append(float(m[0])); got_s.append(int(s[0]))
+        assert r["n_removed"] == 0                               # cap_fraction = 0: guard iii removes nothing
+    assert np.allclose(got_m, [.5, .25, .625, .3125, .15625, .578125, .7890625], atol=0)
+    assert got_s == [1, 0, 0, 0, 0, 0, 1]
+
+
+def test_prune_guards_and_global_cut():
+    from oracle.prune import PruneOpts, prune_step
+    cfg, w = _prune_case()
+    n = cfg.scene.n
+    ones, ins = np.zeros(n, np.float32), np.zeros(n, np.uint8)   # m_{t-1} = 0, state out: every low voxel is a candidate
+    # one bin, no protection, no cap: exactly the global quantile cut w_max <= tau (P:163)
+    o = PruneOpts(n_bins=1, q_near=0.3, q_far=0.3, ema_alpha=1.0, m_low=0.5, m_high=0.5, kappa=0.0, w_keep=2.0, cap_fraction=1.0)
+    r = prune_step(cfg.scene, cfg.cameras, w, ones, ins, o)
+    tau = np.sort(w)[int(np.ceil(np.float32(0.3) * np.float32(n))) - 1]
+    assert r["tau"][0] == tau and np.array_equal(r["keep"], w > tau)
+    # cap: at most floor(f N) leave, and they are the smallest candidates; protected voxels never leave
+    o2 = PruneOpts(n_bins=4, q_near=0.5, q_far=0.3, ema_alpha=1.0, m_low=0.5, m_high=0.5, kappa=0.5, w_keep=0.6, cap_fraction=0.02)
+    r2 = prune_step(cfg.scene, cfg.cameras, w, ones, ins, o2)
+    removed = ~r2["keep"]
+    assert r2["n_removed"] == min(r2["cap"], int(r2["candidates"].sum())) == int(np.floor(np.float32(0.02) * np.float32(n)))
+    assert not np.any(removed & r2["protected"]) and np.all(r2["candidates"][removed])
+    assert w[removed].max() <= w[r2["candidates"] & ~removed].min()
+    assert np.all(w[r2["protected"] & (w < 0.6)] >= 0) and np.all(r2["protected"][w >= 0.6])
+    # q -> 0 with all-positive w_max: tau = min, only the minimum is "outside"
+    wp = np.maximum(w, 1e-3).astype(np.float32)
+    o3 = PruneOpts(n_bins=1, q_near=1e-9, q_far=1e-9, ema_alpha=1.0, m_low=0.5, m_high=0.5, kappa=0.0, w_keep=2.0, cap_fraction=1.0)
+    r3 = prune_step(cfg.scene, cfg.cameras, wp, ones, ins, o3)
+    assert np.array_equal(~r3["keep"], wp <= wp.min())
