@@ -347,6 +347,41 @@ def main():
                               "warp_voxel_pairs": float(np.mean([s["warp_voxel_pairs"] for s in stats]))},
             "peak_vram_bytes": peak_vram}
 
+    # ---- NEXT-1 (not part of `value`): one depth-quantile pruning step on the w_max the steps above gathered, and the
+    # compaction of the voxel arrays by its keep mask; HBM-bound streaming kernels, timed with CUDA events ----
+    if rank == 0:
+        po = pkg.SvrPruneOpts(8, 0.10, 0.05, 0.5, 0.3, 0.7, 1.0, 0.5, 0.05)
+        ema = torch.zeros(sc.n, dtype=torch.float32, device=dev)
+        st8 = torch.zeros(sc.n, dtype=torch.uint8, device=dev)
+        keep = None
+        for _ in range(2):
+            keep, tau, n_removed = ctx.svr_prune_step(vox, ccams, w_max, ema, st8, po)
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        reps = 5
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(reps):
+                keep, tau, n_removed = ctx.svr_prune_step(vox, ccams, w_max, ema, st8, po)
+            e1.record(stream)
+            for _ in range(reps):
+                for arr in (vox.ijkl, vox.raw, vox.sh):
+                    ctx.svr_compact_rows(keep, arr)
+            e2.record(stream)
+        torch.cuda.synchronize()
+        ms_prune, ms_compact = e0.elapsed_time(e1) / reps, e1.elapsed_time(e2) / reps
+        row_bytes = 8 + 32 + 12 * sc.n_basis
+        kept = int(keep.sum().item())
+        prune_bytes = sc.n * (8 + 4 + 4 + 4 + 1 + 1 + 1)             # ijkl, w_max, ema r/w, state r/w, keep
+        compact_bytes = sc.n * (1 + row_bytes) + kept * row_bytes     # keep + all rows read, kept rows written
+        line["next1_prune"] = {
+            "what": "svr_prune_step (P:143-172, 8 depth bins, all cameras) + svr_compact_rows(ijkl, raw, sh); outside `value`",
+            "prune_ms": ms_prune, "compact_ms": ms_compact, "removed": int(n_removed), "kept": kept,
+            "prune_roofline": {"bound": "hbm", "achieved": prune_bytes / (ms_prune * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                               "frac": prune_bytes / (ms_prune * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                               "algorithmic": "23 B per voxel (ijkl, w_max, ema r/w, state r/w, keep)"},
+            "compact_roofline": {"bound": "hbm", "achieved": compact_bytes / (ms_compact * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                 "unit": "GB/s", "frac": compact_bytes / (ms_compact * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()

@@ -82,8 +82,8 @@ size_t svr_workspace_peak_bytes(const SvrContext* ctx);
 /* Number of this library's kernels launched on the context so far (bench.py's gpu_launches). */
 int64_t svr_kernel_launches(const SvrContext* ctx);
 
-/* (1)+(2) of the path: per-voxel projection to pixel rectangles and tile-overlap counts (B1), per-view SH
- * colour c_v (R6), key build (tile | direction octant | direction-flipped Morton code, B3), device radix
+/* (1)+(2) of the path: per-voxel projection to pixel rectangles and (tile, octant) bucket counts (B1), per-view SH
+ * colour c_v (R6), key build (tile | direction octant | direction-flipped Morton code, B3), per-bucket device
  * sort, per-(tile,octant) ranges (B4), and a per-entry record of the voxel (geometry relative to the camera,
  * density coefficients, colour) in list order. The frame borrows `vox` pointers: keep them alive and the
  * topology (ijkl) unchanged until svr_frame_release. raw_density / sh VALUES are captured by svr_preprocess;
@@ -138,10 +138,42 @@ SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRen
                             uint64_t* stats_host);
 void svr_set_stage_timing(SvrContext* ctx, int enabled);
 int svr_num_stages(void);
-/* Experiments only: bit 0 makes svr_backward skip its gradient reductions (timing the arithmetic alone). */
+/* Experiments / tests only: bit 3 (8) selects the first list-build design (per-voxel scan + global radix sort, the
+ * fallback when Morton code + voxel id exceed 64 bits); bit 10 (1024) prints stream idle gaps per stage. */
 void svr_set_debug_flags(SvrContext* ctx, int flags);
 const char* svr_stage_name(int stage);
 SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset);
+
+/* ---- NEXT-1: depth-aware quantile pruning, the consumer of w_max (eqs. 11-12) ----
+ * One adaptation step over all voxels, statistics gathered over `n_cams` views (reading R11):
+ *  1. depth proxy z_v = min over cameras with positive depth of the camera-space depth of the voxel centre
+ *     (+inf if none), footprint delta_v = z_v / fx;
+ *  2. n_bins depth bins, piecewise-linear in log2 z between the smallest and largest finite depth (integer
+ *     arithmetic on the float bit patterns);
+ *  3. tau_b = F_b^{-1}(q_b), the nearest-rank q_b-quantile of w_max over the bin (eqs. 11-12),
+ *     q_b = q_near + (q_far - q_near) b / (n_bins - 1); inside score x = [w_max > tau_b];
+ *  4. guard i: ema = (1 - ema_alpha) ema + ema_alpha x; state = 0 (out) if ema < m_low, 1 (in) if
+ *     ema > m_high, else unchanged;
+ *  5. guard ii: protected if half-size < kappa * delta_v or w_max >= w_keep;
+ *  6. guard iii: at most floor(cap_fraction * n) voxels leave: the unprotected `out` voxels with the
+ *     smallest w_max, ties by lower index.
+ * w_max[n] in; ema[n] (float) and state[n] (uint8) in/out; keep[n] (uint8, 1 = stays) out. cams_host: HOST array
+ * (n_cams <= 64). tau_host[n_bins] (may be NULL) and n_removed_host are HOST outputs: the call synchronises. */
+typedef struct {
+    int32_t n_bins;           /* 1..64 */
+    float q_near, q_far;      /* per-bin quantile at the nearest / farthest bin (annealed by the caller) */
+    float ema_alpha, m_low, m_high;
+    float kappa, w_keep;
+    float cap_fraction;
+} SvrPruneOpts;
+SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cams_host, int32_t n_cams,
+                         const float* w_max, float* ema, uint8_t* state, const SvrPruneOpts* opts, uint8_t* keep,
+                         float* tau_host, int64_t* n_removed_host);
+/* Stable stream compaction of per-voxel rows: dst[j] = src[i] for the j-th i with keep[i] != 0 (row_bytes a
+ * multiple of 4 or 1, 2). Call once per array (ijkl 8 B, raw 32 B, sh 12(D+1)^2 B, ema, state, optimizer moments).
+ * src and dst must not overlap. *n_out_host (may be NULL) = number of rows kept (then the call synchronises). */
+SvrStatus svr_compact_rows(SvrContext* ctx, const uint8_t* keep, int64_t n, const void* src, void* dst,
+                           int64_t row_bytes, int64_t* n_out_host);
 
 /* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);

@@ -22,7 +22,8 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
            "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
-           "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags"]
+           "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
+           "svr_prune_step", "svr_compact_rows"]
 
 
 class SvrError(RuntimeError):
@@ -43,6 +44,11 @@ class SvrCamera(C.Structure):
 
 class SvrRenderOpts(C.Structure):
     _fields_ = [("K", C.c_int32), ("T_min", C.c_float)]
+
+
+class SvrPruneOpts(C.Structure):
+    _fields_ = [("n_bins", C.c_int32), ("q_near", C.c_float), ("q_far", C.c_float), ("ema_alpha", C.c_float), ("m_low", C.c_float),
+                ("m_high", C.c_float), ("kappa", C.c_float), ("w_keep", C.c_float), ("cap_fraction", C.c_float)]
 
 
 class SvrLossOpts(C.Structure):
@@ -77,6 +83,9 @@ def _load():
     lib.svr_frame_colors.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
     lib.svr_copy_to_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.svr_forward_stats.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts), C.c_void_p, C.c_void_p]
+    lib.svr_prune_step.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                   C.POINTER(SvrPruneOpts), C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+    lib.svr_compact_rows.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
     lib.svr_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.svr_set_stage_timing.restype = None
     lib.svr_num_stages.restype = C.c_int
@@ -318,6 +327,28 @@ class Context:
                                              _p(target_host), _p(grad_raw), _p(grad_sh), _p(w_max),
                                              C.cast(C.byref(loss), C.c_void_p), _p(image_host)))
         return float(loss.value)
+
+
+    # ---- NEXT-1: depth-aware quantile pruning -----------------------------------------
+    def svr_prune_step(self, vox: Voxels, cams, w_max: torch.Tensor, ema: torch.Tensor, state: torch.Tensor, opts: SvrPruneOpts):
+        """One adaptation step; ema / state are updated in place. Returns (keep uint8 [n], tau float32 [n_bins], n_removed)."""
+        arr = (SvrCamera * len(cams))(*[c if isinstance(c, SvrCamera) else make_camera(c) for c in cams])
+        keep = torch.empty(vox.n, dtype=torch.uint8, device=w_max.device)
+        tau = (C.c_float * opts.n_bins)()
+        n_removed = C.c_int64()
+        self._check(_lib.svr_prune_step(self.handle, C.byref(vox.c), C.cast(arr, C.c_void_p), len(cams), _p(w_max), _p(ema), _p(state),
+                                        C.byref(opts), _p(keep), C.cast(tau, C.c_void_p), C.byref(n_removed)))
+        return keep, np.array(list(tau), dtype=np.float32), int(n_removed.value)
+
+    def svr_compact_rows(self, keep: torch.Tensor, src: torch.Tensor) -> torch.Tensor:
+        """Stable compaction of the rows of `src` (first dimension) whose keep flag is set."""
+        assert src.is_contiguous() and keep.dtype == torch.uint8
+        n = src.shape[0]
+        row_bytes = src.element_size() * (src.numel() // max(n, 1)) if n else src.element_size()
+        dst = torch.empty_like(src)
+        n_out = C.c_int64()
+        self._check(_lib.svr_compact_rows(self.handle, _p(keep), n, _p(src), _p(dst), row_bytes, C.byref(n_out)))
+        return dst[: int(n_out.value)]
 
 
 def svr_gamma_schedule(t: float, T: float, t0_frac: float = 0.3, t1_frac: float = 0.6, gamma_max: float = 0.6) -> float:

@@ -304,3 +304,62 @@ def test_full_size_sampled_rays(orc, svr, name):
     frame.release()
     del g_raw, g_sh
     check_lists(orc, svr, sc, cam)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: depth-aware quantile pruning and row compaction against oracle/prune.py
+# ---------------------------------------------------------------------------------------------
+def _prune_inputs(name, n, seed):
+    cfg = make_config(name, n_voxels=n, n_cams=4) if name != "C1" else make_config("C1")
+    rng = np.random.default_rng(seed)
+    w = (rng.random(cfg.scene.n) ** 3).astype(np.float32)
+    w[rng.random(cfg.scene.n) < 0.25] = 0.0                     # never-seen voxels
+    w[rng.random(cfg.scene.n) < 0.05] = np.float32(0.125)       # ties at a non-zero value
+    return cfg, w
+
+
+@pytest.mark.parametrize("name,n", [("C1", 512), ("C2", 50_000), ("C4", 300_000)])
+def test_prune_step_bit_exact_over_steps(orc, svr, name, n):
+    """Keep mask, state and thresholds identical to the oracle, EMA bit-identical, over several adaptation steps with
+    changing w_max (so that the hysteresis takes every branch) and a cap that binds."""
+    from oracle.prune import PruneOpts, prune_step
+    pkg, ctx, torch = svr
+    cfg, w0 = _prune_inputs(name, n, 11)
+    sc = cfg.scene
+    vox = pkg.Voxels.from_scene(sc)
+    po = PruneOpts(n_bins=6, q_near=0.45, q_far=0.2, ema_alpha=0.4, m_low=0.35, m_high=0.65, kappa=0.4, w_keep=0.7, cap_fraction=0.03)
+    go = pkg.SvrPruneOpts(po.n_bins, po.q_near, po.q_far, po.ema_alpha, po.m_low, po.m_high, po.kappa, po.w_keep, po.cap_fraction)
+    ema_ref, st_ref = np.ones(sc.n, np.float32), np.ones(sc.n, np.uint8)
+    ema = torch.ones(sc.n, dtype=torch.float32, device="cuda")
+    state = torch.ones(sc.n, dtype=torch.uint8, device="cuda")
+    rng = np.random.default_rng(3)
+    removed_any = False
+    for step in range(4):
+        w = np.where(rng.random(sc.n) < 0.5, w0, np.float32(0.5) * w0).astype(np.float32)
+        ref = prune_step(sc, cfg.cameras, w, ema_ref, st_ref, po)
+        keep, tau, n_removed = ctx.svr_prune_step(vox, cfg.cameras, torch.from_numpy(w).cuda(), ema, state, go)
+        np.testing.assert_array_equal(tau, ref["tau"])
+        np.testing.assert_array_equal(ema.cpu().numpy(), ref["ema"])
+        np.testing.assert_array_equal(state.cpu().numpy(), ref["state"])
+        np.testing.assert_array_equal(keep.cpu().numpy().astype(bool), ref["keep"])
+        assert n_removed == ref["n_removed"]
+        removed_any |= n_removed > 0
+        ema_ref, st_ref = ref["ema"], ref["state"]
+    assert removed_any and ref["n_removed"] == ref["cap"]          # the cap was binding
+
+
+def test_compact_rows_and_rerender(orc, svr):
+    """Stable compaction of ijkl / raw / sh / state rows equals boolean indexing; the compacted scene renders."""
+    pkg, ctx, torch = svr
+    cfg, w = _prune_inputs("C2", 20_000, 5)
+    sc = cfg.scene
+    keep_np = np.random.default_rng(9).random(sc.n) < 0.7
+    keep = torch.from_numpy(keep_np.astype(np.uint8)).cuda()
+    for arr in [sc.ijkl, sc.raw, sc.sh, w, keep_np.astype(np.uint8)]:
+        got = ctx.svr_compact_rows(keep, torch.from_numpy(np.ascontiguousarray(arr)).cuda()).cpu().numpy()
+        np.testing.assert_array_equal(got, np.ascontiguousarray(arr)[keep_np])
+    none = ctx.svr_compact_rows(torch.zeros(sc.n, dtype=torch.uint8, device="cuda"), torch.from_numpy(sc.raw).cuda())
+    assert none.shape[0] == 0
+    from dataclasses import replace
+    small = replace(sc, ijkl=sc.ijkl[keep_np], raw=sc.raw[keep_np], sh=sc.sh[keep_np])
+    check_lists(orc, svr, small, cfg.cameras[0])
