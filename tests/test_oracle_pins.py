@@ -547,3 +547,81 @@ def test_prune_guards_and_global_cut():
     o3 = PruneOpts(n_bins=1, q_near=1e-9, q_far=1e-9, ema_alpha=1.0, m_low=0.5, m_high=0.5, kappa=0.0, w_keep=2.0, cap_fraction=1.0)
     r3 = prune_step(cfg.scene, cfg.cameras, wp, ones, ins, o3)
     assert np.array_equal(~r3["keep"], wp <= wp.min())
+
+
+# ---------------------------------------------------------------------------------------------
+# priority-driven subdivision (Sec. IV-D, eqs. 13-16): pins of oracle/subdivide.py
+# ---------------------------------------------------------------------------------------------
+def test_subdivide_eligibility_priority_budget():
+    from oracle.prune import depth_proxy
+    from oracle.subdivide import SubdivOpts, select_splits
+    from svr_inputs import make_config
+    cfg = make_config("C2", n_voxels=5000)
+    sc = cfg.scene
+    rng = np.random.default_rng(2)
+    P = rng.random(sc.n).astype(np.float32)
+    P[::7] = np.float32(0.5)                                     # ties
+    o = SubdivOpts(kappa=0.8, beta=0.25, max_level=8, max_splits=150)
+    r = select_splits(sc, cfg.cameras, P, o)
+    z, delta, half = depth_proxy(sc, cfg.cameras)
+    # eq. 13 typed out in float64 on the same inputs (strict inequality, not at the finest level)
+    elig = np.isfinite(z) & (sc.ijkl[:, 3] < 8) & (half.astype(np.float64) > 0.8 * delta.astype(np.float64) * (1 + 1e-6))
+    assert np.all(r["eligible"][elig]) and 0 < r["eligible"].sum() < sc.n
+    assert not np.any(r["eligible"] & (sc.ijkl[:, 3] >= 8))
+    # eqs. 14-16 with numbers
+    zf = np.sort(z[np.isfinite(z)].astype(np.float64))
+    p5, p95 = zf[int(np.ceil(0.05 * zf.size)) - 1], zf[int(np.ceil(0.95 * zf.size)) - 1]
+    assert abs(p5 - r["z_p5"]) < 1e-6 and abs(p95 - r["z_p95"]) < 1e-6
+    zt = np.clip((z.astype(np.float64) - p5) / (p95 - p5), 0, 1)
+    assert np.allclose(r["priority"], P * (1 + 0.25 * zt), rtol=1e-6)
+    assert np.all(r["priority"] >= P) and np.all(r["priority"] <= P * np.float32(1.25) * (1 + 1e-6))   # b in [1, 1 + beta]
+    # budget: exactly max_splits eligible voxels, none of lower priority than an unsplit eligible one
+    s = r["split"]
+    assert s.sum() == 150 and np.all(r["eligible"][s])
+    lo, hi = r["priority"][s].min(), r["priority"][r["eligible"] & ~s].max()
+    assert lo >= hi
+    tie = r["eligible"] & (r["priority"] == lo)
+    if (tie & s).any() and (tie & ~s).any():
+        assert np.flatnonzero(tie & s).max() < np.flatnonzero(tie & ~s).min()        # ties by lower index
+    # given (running) percentiles instead of this step's
+    r2 = select_splits(sc, cfg.cameras, P, SubdivOpts(kappa=0.8, beta=0.25, max_level=8, max_splits=150, use_current_percentiles=False,
+                                                      z_p5=2.0, z_p95=2.0))
+    assert np.array_equal(r2["priority"], P)                     # degenerate range: z~ = 0
+
+
+def test_subdivide_children_tile_parent_and_sample_its_field():
+    from oracle.subdivide import apply_splits, child_raws
+    from svr_inputs import tiny_scene
+    sc = tiny_scene(4, n=6, sh_degree=1)
+    split = np.array([True, False, True, False, False, True])
+    ijkl, raw, sh = apply_splits(sc, split)
+    assert ijkl.shape[0] == 3 + 24 and np.array_equal(ijkl[:3], sc.ijkl[~split])
+    def box(q, root_edge):
+        e = root_edge / 2.0 ** q[3]
+        return q[:3] * e, (q[:3] + 1) * e
+    for k, p in enumerate(np.flatnonzero(split)):
+        plo, phi = box(sc.ijkl[p].astype(np.float64), sc.root_edge)
+        vol = 0.0
+        for o in range(8):
+            c = ijkl[3 + 8 * k + o].astype(np.float64)
+            clo, chi = box(c, sc.root_edge)
+            assert np.all(clo >= plo) and np.all(chi <= phi) and c[3] == sc.ijkl[p, 3] + 1
+            off = (clo - plo) / (chi - clo)
+            assert tuple(off.astype(int)) == (o & 1, (o >> 1) & 1, o >> 2)          # child order bx + 2 by + 4 bz
+            vol += np.prod(chi - clo)
+        assert np.isclose(vol, np.prod(phi - plo))                                   # the 8 children tile the parent
+        assert np.array_equal(sh[3 + 8 * k: 3 + 8 * k + 8], np.repeat(sc.sh[p:p + 1], 8, axis=0))
+    # child raws = the parent's trilinear field (fp64 formula) at the child corners
+    r = sc.raw[split].astype(np.float64)
+    ch = child_raws(sc.raw[split])
+    def tri(rr, x, y, z):
+        w = [(1 - x) * (1 - y) * (1 - z), x * (1 - y) * (1 - z), (1 - x) * y * (1 - z), x * y * (1 - z),
+             (1 - x) * (1 - y) * z, x * (1 - y) * z, (1 - x) * y * z, x * y * z]
+        return sum(wi * rr[:, i] for i, wi in enumerate(w))
+    for o in range(8):
+        for c in range(8):
+            x, y, zc = ((o & 1) + (c & 1)) / 2, (((o >> 1) & 1) + ((c >> 1) & 1)) / 2, ((o >> 2) + (c >> 2)) / 2
+            assert np.allclose(ch[:, o, c], tri(r, x, y, zc), rtol=1e-6, atol=1e-6)
+    # splitting a child again still samples the ORIGINAL field (trilinear restricted to a sub-cube is trilinear)
+    gg = child_raws(ch[:, 5, :])                                  # child (1,0,1), then its children
+    assert np.allclose(gg[:, 2, 7], tri(r, (1 + 0.5) / 2, (0 + 1) / 2, (1 + 0.5) / 2), rtol=1e-5, atol=1e-6)
