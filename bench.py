@@ -168,7 +168,7 @@ def workload_config(cfg, args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=16)
+    ap.add_argument("--steps", type=int, default=64)
     ap.add_argument("--warmup", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4")
@@ -381,6 +381,27 @@ def main():
                                "algorithmic": "23 B per voxel (ijkl, w_max, ema r/w, state r/w, keep)"},
             "compact_roofline": {"bound": "hbm", "achieved": compact_bytes / (ms_compact * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                  "unit": "GB/s", "frac": compact_bytes / (ms_compact * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
+
+        # NEXT-2: priority-driven subdivision: selection (usefulness = w_max) and the 1 -> 8 split of 1% of the voxels
+        so = pkg.SvrSubdivOpts(1.0, 0.2, sc.max_level, sc.n // 100, 1, 0.0, 0.0)
+        split, _, _, n_split = ctx.svr_subdivide_select(vox, ccams, w_max, so)
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(reps):
+                split, _, _, n_split = ctx.svr_subdivide_select(vox, ccams, w_max, so)
+            e1.record(stream)
+            for _ in range(reps):
+                ctx.svr_subdivide_apply(vox, split, n_split)
+            e2.record(stream)
+        torch.cuda.synchronize()
+        ms_sel, ms_app = e0.elapsed_time(e1) / reps, e1.elapsed_time(e2) / reps
+        app_bytes = sc.n * (1 + row_bytes) + (sc.n + 7 * n_split) * row_bytes
+        line["next2_subdivide"] = {
+            "what": "svr_subdivide_select (eqs. 13-16, budget = 1% of the voxels) + svr_subdivide_apply (1 -> 8); outside `value`",
+            "select_ms": ms_sel, "apply_ms": ms_app, "n_split": int(n_split),
+            "apply_roofline": {"bound": "hbm", "achieved": app_bytes / (ms_app * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                               "frac": app_bytes / (ms_app * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle

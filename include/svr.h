@@ -175,6 +175,31 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 SvrStatus svr_compact_rows(SvrContext* ctx, const uint8_t* keep, int64_t n, const void* src, void* dst,
                            int64_t row_bytes, int64_t* n_out_host);
 
+/* ---- NEXT-2: priority-driven subdivision (eqs. 13-16; reading R12) ----
+ * svr_subdivide_select: depth z_v and footprint delta_v as in svr_prune_step; eligible (eq. 13) iff level <
+ * max_level, z_v finite and half-size > kappa * delta_v; z~ = clip((z - z_p5) / (z_p95 - z_p5), 0, 1) (eq. 14) with the
+ * 5th / 95th nearest-rank percentile of this step's finite depths (use_current_percentiles != 0) or the running values
+ * in the options; priority = usefulness * (1 + beta z~) (eqs. 15-16; usefulness[n] >= 0 is the caller's running score
+ * P_v); the max_splits eligible voxels of highest priority are selected, ties by lower index.
+ * split[n] (uint8) and priority[n] (may be NULL) are device outputs; z_percentiles_host[2] (may be NULL) and
+ * n_split_host are HOST outputs: the call synchronises.
+ * svr_subdivide_apply: the new voxel set = the unsplit voxels in their order, then 8 children per split voxel grouped
+ * by parent in parent order, child c = bx + 2 by + 4 bz at (2i + bx, 2j + by, 2k + bz, L + 1); child corner raws = the
+ * parent's trilinear field at the child's corners (x, then y, then z; a midpoint is 0.5 * (a + b)); SH copied.
+ * Output arrays must hold n + 7 * n_split rows; *n_out_host (may be NULL) = that number (then the call synchronises). */
+typedef struct {
+    float kappa, beta;
+    int32_t max_level;              /* voxels at this level or finer never split */
+    int64_t max_splits;             /* global growth cap per step */
+    int32_t use_current_percentiles;
+    float z_p5, z_p95;              /* running percentiles, used when use_current_percentiles == 0 */
+} SvrSubdivOpts;
+SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cams_host, int32_t n_cams,
+                               const float* usefulness, const SvrSubdivOpts* opts, uint8_t* split, float* priority,
+                               float* z_percentiles_host, int64_t* n_split_host);
+SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8_t* split, uint16_t* ijkl_out,
+                              float* raw_out, float* sh_out, int64_t* n_out_host);
+
 /* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);
 

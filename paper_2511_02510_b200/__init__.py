@@ -5,7 +5,7 @@ sm_100a, built in-tree by `_build.py`). The load is deferred to first use only s
 imported before the library exists; there is no fallback path: a missing library raises ImportError, a
 missing GPU raises at Context().
 """
-_NAMES = ["Context", "Frame", "Voxels", "SvrCamera", "SvrError", "SvrLossOpts", "SvrPruneOpts", "SvrRenderOpts", "SvrVoxels", "EXPORTS",
+_NAMES = ["Context", "Frame", "Voxels", "SvrCamera", "SvrError", "SvrLossOpts", "SvrPruneOpts", "SvrRenderOpts", "SvrSubdivOpts", "SvrVoxels", "EXPORTS",
           "make_camera", "svr_gamma_schedule", "lib"]
 __all__ = list(_NAMES)
 

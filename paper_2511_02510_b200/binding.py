@@ -23,7 +23,7 @@ EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_by
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
            "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
-           "svr_prune_step", "svr_compact_rows"]
+           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply"]
 
 
 class SvrError(RuntimeError):
@@ -49,6 +49,11 @@ class SvrRenderOpts(C.Structure):
 class SvrPruneOpts(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("q_near", C.c_float), ("q_far", C.c_float), ("ema_alpha", C.c_float), ("m_low", C.c_float),
                 ("m_high", C.c_float), ("kappa", C.c_float), ("w_keep", C.c_float), ("cap_fraction", C.c_float)]
+
+
+class SvrSubdivOpts(C.Structure):
+    _fields_ = [("kappa", C.c_float), ("beta", C.c_float), ("max_level", C.c_int32), ("max_splits", C.c_int64),
+                ("use_current_percentiles", C.c_int32), ("z_p5", C.c_float), ("z_p95", C.c_float)]
 
 
 class SvrLossOpts(C.Structure):
@@ -86,6 +91,9 @@ def _load():
     lib.svr_prune_step.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                    C.POINTER(SvrPruneOpts), C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
     lib.svr_compact_rows.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
+    lib.svr_subdivide_select.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(SvrSubdivOpts),
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+    lib.svr_subdivide_apply.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
     lib.svr_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.svr_set_stage_timing.restype = None
     lib.svr_num_stages.restype = C.c_int
@@ -349,6 +357,30 @@ class Context:
         n_out = C.c_int64()
         self._check(_lib.svr_compact_rows(self.handle, _p(keep), n, _p(src), _p(dst), row_bytes, C.byref(n_out)))
         return dst[: int(n_out.value)]
+
+
+    # ---- NEXT-2: priority-driven subdivision -------------------------------------------
+    def svr_subdivide_select(self, vox: Voxels, cams, usefulness: torch.Tensor, opts: SvrSubdivOpts):
+        """Returns (split uint8 [n], priority float32 [n], (z_p5, z_p95) of this step, n_split)."""
+        arr = (SvrCamera * len(cams))(*[c if isinstance(c, SvrCamera) else make_camera(c) for c in cams])
+        split = torch.empty(vox.n, dtype=torch.uint8, device=usefulness.device)
+        priority = torch.empty(vox.n, dtype=torch.float32, device=usefulness.device)
+        zp = (C.c_float * 2)()
+        n_split = C.c_int64()
+        self._check(_lib.svr_subdivide_select(self.handle, C.byref(vox.c), C.cast(arr, C.c_void_p), len(cams), _p(usefulness), C.byref(opts),
+                                              _p(split), _p(priority), C.cast(zp, C.c_void_p), C.byref(n_split)))
+        return split, priority, (float(zp[0]), float(zp[1])), int(n_split.value)
+
+    def svr_subdivide_apply(self, vox: Voxels, split: torch.Tensor, n_split: int):
+        """Returns (ijkl int16 [n', 4], raw [n', 8], sh [n', B, 3]) with n' = n + 7 n_split."""
+        n_new = vox.n + 7 * n_split
+        ijkl = torch.empty((n_new, 4), dtype=torch.int16, device=vox.raw.device)
+        raw = torch.empty((n_new, 8), dtype=torch.float32, device=vox.raw.device)
+        sh = torch.empty((n_new,) + tuple(vox.sh.shape[1:]), dtype=torch.float32, device=vox.raw.device)
+        n_out = C.c_int64()
+        self._check(_lib.svr_subdivide_apply(self.handle, C.byref(vox.c), _p(split), _p(ijkl), _p(raw), _p(sh), C.byref(n_out)))
+        assert int(n_out.value) == n_new, (int(n_out.value), n_new)
+        return ijkl, raw, sh
 
 
 def svr_gamma_schedule(t: float, T: float, t0_frac: float = 0.3, t1_frac: float = 0.6, gamma_max: float = 0.6) -> float:

@@ -248,6 +248,126 @@ __global__ void __launch_bounds__(256) compact_rows_kernel(int64_t n, const uint
     dst[(size_t)offs[v] * words + w] = src[(size_t)v * words + w];
 }
 
+// ---- priority-driven subdivision (Sec. IV-D, eqs. 13-16; R12) ----
+__global__ void __launch_bounds__(256) subdiv_finite_kernel(int64_t n, const float* __restrict__ z, uint8_t* __restrict__ finite) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v < n) finite[v] = (z[v] < __int_as_float(0x7f800000)) ? 1 : 0;
+}
+
+// eq. 13 eligibility, eq. 14 robust depth normalisation, eqs. 15-16 priority; key = ~bits(priority) so that the
+// "smallest keys first" selection of the cap machinery picks the HIGHEST priorities (priority >= 0 required).
+__global__ void __launch_bounds__(256) subdiv_priority_kernel(SceneDev s, const float* __restrict__ z, const float* __restrict__ delta,
+                                                              const float* __restrict__ P, const SelectState* __restrict__ st5,
+                                                              const SelectState* __restrict__ st95, int use_current, float z_p5, float z_p95,
+                                                              float kappa, float beta, int max_level, float* __restrict__ priority,
+                                                              float* __restrict__ key, uint8_t* __restrict__ cand) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    float a = z_p5, b = z_p95;
+    if (use_current) {
+        a = (st5->size[0] > 0u) ? __uint_as_float(st5->prefix[0]) : 0.0f;
+        b = (st95->size[0] > 0u) ? __uint_as_float(st95->prefix[0]) : 0.0f;
+    }
+    const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+    float x[3];
+    const float half = voxel_half_and_centre(s, q, x);
+    const float zv = z[v];
+    const bool finite = zv < __int_as_float(0x7f800000);
+    const bool elig = finite && ((int)(q.y >> 16) < max_level) && (half > __fmul_rn(kappa, delta[v]));
+    const float den = __fsub_rn(b, a);
+    float zt = 0.0f;
+    if (finite && den > 0.0f) zt = fminf(fmaxf(__fdiv_rn(__fsub_rn(zv, a), den), 0.0f), 1.0f);
+    const float pr = __fmul_rn(P[v], __fadd_rn(1.0f, __fmul_rn(beta, zt)));
+    if (priority) priority[v] = pr;
+    key[v] = __uint_as_float(~__float_as_uint(pr));
+    cand[v] = elig ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(256) subdiv_invert_kernel(int64_t n, const uint8_t* __restrict__ keep, uint8_t* __restrict__ split) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v < n) split[v] = keep[v] ? 0 : 1;
+}
+
+__global__ void __launch_bounds__(256) split_to_counts_kernel(int64_t n, const uint8_t* __restrict__ split, uint32_t* __restrict__ counts) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v <= n) counts[v] = (v < n && split[v]) ? 1u : 0u;
+}
+
+__device__ __forceinline__ float mix_half(float a, float b, int t2) {   // parent coordinate t = t2 / 2 in {0, 1/2, 1}
+    return t2 == 0 ? a : (t2 == 2 ? b : __fmul_rn(0.5f, __fadd_rn(a, b)));
+}
+
+// cells and corner raws: survivors keep their row (stable), a split voxel writes its 8 children after all survivors,
+// grouped by parent in parent order, child order c = bx + 2 by + 4 bz; child raws = the parent's trilinear field at the
+// child's corners, interpolated along x, then y, then z.
+__global__ void __launch_bounds__(256) subdiv_cells_kernel(int64_t n, const uint8_t* __restrict__ split, const uint32_t* __restrict__ offs,
+                                                           const uint2* __restrict__ ijkl, const float4* __restrict__ raw,
+                                                           uint2* __restrict__ ijkl_out, float4* __restrict__ raw_out) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= n) return;
+    const uint32_t r = offs[v], n_split = offs[n];
+    const uint2 q = ijkl[v];
+    const float4 ra = raw[2 * v], rb = raw[2 * v + 1];
+    if (!split[v]) {
+        const size_t d = (size_t)v - r;
+        ijkl_out[d] = q;
+        raw_out[2 * d] = ra;
+        raw_out[2 * d + 1] = rb;
+        return;
+    }
+    const float p[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+    const uint32_t ix = q.x & 0xFFFF, iy = q.x >> 16, iz = q.y & 0xFFFF, L = q.y >> 16;
+    const size_t base = (size_t)(n - n_split) + 8 * (size_t)r;
+#pragma unroll
+    for (int o = 0; o < 8; ++o) {
+        const int ox = o & 1, oy = (o >> 1) & 1, oz = o >> 2;
+        float c[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int tx = ox + (k & 1), ty = oy + ((k >> 1) & 1), tz = oz + (k >> 2);
+            const float x00 = mix_half(p[0], p[1], tx), x10 = mix_half(p[2], p[3], tx);
+            const float x01 = mix_half(p[4], p[5], tx), x11 = mix_half(p[6], p[7], tx);
+            c[k] = mix_half(mix_half(x00, x10, ty), mix_half(x01, x11, ty), tz);
+        }
+        ijkl_out[base + o] = make_uint2((2 * ix + ox) | ((2 * iy + oy) << 16), (2 * iz + oz) | ((L + 1) << 16));
+        raw_out[2 * (base + o)] = make_float4(c[0], c[1], c[2], c[3]);
+        raw_out[2 * (base + o) + 1] = make_float4(c[4], c[5], c[6], c[7]);
+    }
+}
+
+// SH rows: one thread per (voxel, 4-byte word); a split voxel's row is copied to its 8 children
+__global__ void __launch_bounds__(256) subdiv_sh_kernel(int64_t n, int words, const uint8_t* __restrict__ split, const uint32_t* __restrict__ offs,
+                                                        const uint32_t* __restrict__ sh, uint32_t* __restrict__ sh_out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t v = i / words;
+    if (v >= n) return;
+    const int w = (int)(i - v * words);
+    const uint32_t val = sh[i], r = offs[v];
+    if (!split[v]) { sh_out[((size_t)v - r) * words + w] = val; return; }
+    const size_t base = (size_t)(n - offs[n]) + 8 * (size_t)r;
+#pragma unroll
+    for (int o = 0; o < 8; ++o) sh_out[(base + o) * words + w] = val;
+}
+
+SceneDev scene_of(const SvrVoxels* vox) {
+    SceneDev s{};
+    s.n = vox->n; s.sh_degree = vox->sh_degree; s.n_basis = (vox->sh_degree + 1) * (vox->sh_degree + 1); s.max_level = vox->max_level;
+    for (int a = 0; a < 3; ++a) s.root_lo[a] = vox->root_lo[a];
+    s.root_edge = vox->root_edge; s.ijkl = vox->ijkl; s.raw = vox->raw_density; s.sh = vox->sh;
+    return s;
+}
+
+PruneCams cams_of(const SvrCamera* cams_host, int n_cams) {
+    PruneCams cams{};
+    cams.n = n_cams;
+    for (int c = 0; c < n_cams; ++c) {
+        for (int a = 0; a < 3; ++a) cams.r2[c][a] = cams_host[c].R[6 + a];
+        cams.t2[c] = cams_host[c].t[2];
+        cams.fx[c] = cams_host[c].fx;
+    }
+    return cams;
+}
+
 inline unsigned int nblocks(int64_t n, int bs) { return (unsigned int)((n + bs - 1) / bs); }
 
 }  // namespace
@@ -270,17 +390,8 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         return SVR_OK;
     }
     SVR_CUDA(ctx, cudaSetDevice(ctx->device));
-    SceneDev s{};
-    s.n = n; s.sh_degree = vox->sh_degree; s.n_basis = (vox->sh_degree + 1) * (vox->sh_degree + 1); s.max_level = vox->max_level;
-    for (int a = 0; a < 3; ++a) s.root_lo[a] = vox->root_lo[a];
-    s.root_edge = vox->root_edge; s.ijkl = vox->ijkl; s.raw = vox->raw_density; s.sh = vox->sh;
-    PruneCams cams{};
-    cams.n = n_cams;
-    for (int c = 0; c < n_cams; ++c) {
-        for (int a = 0; a < 3; ++a) cams.r2[c][a] = cams_host[c].R[6 + a];
-        cams.t2[c] = cams_host[c].t[2];
-        cams.fx[c] = cams_host[c].fx;
-    }
+    const SceneDev s = scene_of(vox);
+    const PruneCams cams = cams_of(cams_host, n_cams);
     const uint32_t cap = (uint32_t)floorf(opts->cap_fraction * (float)n);
 
     // workspace: z, delta [n] f32; bins, cand [n] u8; eq, eq_prefix [n+1] u32; hist [B][2048]; two selection states; a counter
@@ -383,6 +494,123 @@ SvrStatus svr_compact_rows(SvrContext* ctx, const uint8_t* keep, int64_t n, cons
             *n_out_host = (int64_t)total;
         }
         if (e != cudaSuccess) stt = svr_fail(ctx, SVR_ERR_CUDA, "compact: %s", cudaGetErrorString(e));
+    }
+    svr_free(ctx, counts, eb);
+    svr_free(ctx, offs, eb);
+    return stt;
+}
+
+SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cams_host, int32_t n_cams,
+                               const float* usefulness, const SvrSubdivOpts* opts, uint8_t* split, float* priority,
+                               float* z_percentiles_host, int64_t* n_split_host) {
+    if (!ctx || !vox || !cams_host || !usefulness || !opts || !split || !n_split_host)
+        return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (n_cams < 1 || n_cams > MAX_CAMS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_cams must be 1..%d", MAX_CAMS);
+    if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    if (opts->max_splits < 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "max_splits must be >= 0");
+    *n_split_host = 0;
+    if (z_percentiles_host) z_percentiles_host[0] = z_percentiles_host[1] = 0.0f;
+    const int64_t n = vox->n;
+    if (n == 0) return SVR_OK;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    const SceneDev s = scene_of(vox);
+    const PruneCams cams = cams_of(cams_host, n_cams);
+    const uint32_t cap = (uint32_t)(opts->max_splits < n ? opts->max_splits : n);
+
+    float *z = nullptr, *delta = nullptr, *key = nullptr;
+    uint8_t *finite = nullptr, *cand = nullptr, *keep = nullptr;
+    uint32_t *eq = nullptr, *eqp = nullptr, *hist = nullptr;
+    SelectState* st = nullptr;      // st[0]: 5th percentile, st[1]: 95th, st[2]: the budget
+    const size_t fb = sizeof(float) * (size_t)n, ub = (size_t)n, eb = sizeof(uint32_t) * (size_t)(n + 1);
+    const size_t hb = sizeof(uint32_t) * HBINS, sb = 3 * sizeof(SelectState) + 64;
+    SvrStatus stt = SVR_OK;
+    auto cleanup = [&]() {
+        svr_free(ctx, z, fb); svr_free(ctx, delta, fb); svr_free(ctx, key, fb); svr_free(ctx, finite, ub); svr_free(ctx, cand, ub);
+        svr_free(ctx, keep, ub); svr_free(ctx, eq, eb); svr_free(ctx, eqp, eb); svr_free(ctx, hist, hb); svr_free(ctx, st, sb);
+    };
+#define PTRY(call) do { stt = (call); if (stt != SVR_OK) { cleanup(); return stt; } } while (0)
+#define PCUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cleanup(); return svr_fail(ctx, SVR_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e__)); } } while (0)
+    PTRY(svr_alloc(ctx, (void**)&z, fb)); PTRY(svr_alloc(ctx, (void**)&delta, fb)); PTRY(svr_alloc(ctx, (void**)&key, fb));
+    PTRY(svr_alloc(ctx, (void**)&finite, ub)); PTRY(svr_alloc(ctx, (void**)&cand, ub)); PTRY(svr_alloc(ctx, (void**)&keep, ub));
+    PTRY(svr_alloc(ctx, (void**)&eq, eb)); PTRY(svr_alloc(ctx, (void**)&eqp, eb));
+    PTRY(svr_alloc(ctx, (void**)&hist, hb)); PTRY(svr_alloc(ctx, (void**)&st, sb));
+    SelectState* st_cap = st + 2;
+    uint32_t* n_sel_dev = reinterpret_cast<uint32_t*>(st + 3);
+    PCUDA(cudaMemsetAsync(st, 0, sb, ctx->stream));
+    PCUDA(cudaMemsetAsync(&st->zlo, 0xFF, sizeof(uint32_t), ctx->stream));
+    PCUDA(cudaMemsetAsync(hist, 0, hb, ctx->stream));
+    const unsigned int g = nblocks(n, 256);
+    const int shifts[3] = {21, 10, 0}, bits[3] = {11, 11, 10}, his[3] = {32, 21, 10};
+    prune_depth_kernel<<<g, 256, 0, ctx->stream>>>(s, cams, z, delta, st);
+    subdiv_finite_kernel<<<g, 256, 0, ctx->stream>>>(n, z, finite);
+    // eq. 14: this step's 5th / 95th percentile of the finite depths (nearest rank): two radix selects on the bits of z
+    const float qs[2] = {0.05f, 0.95f};
+    for (int k = 0; k < 2; ++k)
+        for (int p = 0; p < 3; ++p) {
+            select_hist_kernel<<<g, 256, 0, ctx->stream>>>(n, z, nullptr, finite, st + k, shifts[p], (1u << bits[p]) - 1u, his[p], hist);
+            select_digit_kernel<<<1, 1024, 0, ctx->stream>>>(st + k, hist, bits[p], p == 0, 1, qs[k], qs[k], 0u);
+        }
+    subdiv_priority_kernel<<<g, 256, 0, ctx->stream>>>(s, z, delta, usefulness, st, st + 1, opts->use_current_percentiles, opts->z_p5,
+                                                       opts->z_p95, opts->kappa, opts->beta, opts->max_level, priority, key, cand);
+    // budget: the max_splits eligible voxels of highest priority, ties by lower index
+    for (int p = 0; p < 3; ++p) {
+        select_hist_kernel<<<g, 256, 0, ctx->stream>>>(n, key, nullptr, cand, st_cap, shifts[p], (1u << bits[p]) - 1u, his[p], hist);
+        select_digit_kernel<<<1, 1024, 0, ctx->stream>>>(st_cap, hist, bits[p], p == 0, 1, -1.0f, -1.0f, cap);
+    }
+    prune_cap_flags_kernel<<<nblocks(n + 1, 256), 256, 0, ctx->stream>>>(n, key, cand, st_cap, eq);
+    ctx->launches += 22;
+    PCUDA(cudaGetLastError());
+    PTRY(launch_exclusive_scan(ctx, eq, eqp, n + 1));
+    prune_keep_kernel<<<g, 256, 0, ctx->stream>>>(n, key, cand, st_cap, eqp, cap, keep, n_sel_dev);
+    subdiv_invert_kernel<<<g, 256, 0, ctx->stream>>>(n, keep, split);
+    ctx->launches += 2;
+    PCUDA(cudaGetLastError());
+    SelectState h[2];
+    uint32_t n_sel = 0;
+    PCUDA(cudaMemcpyAsync(h, st, 2 * sizeof(SelectState), cudaMemcpyDeviceToHost, ctx->stream));
+    PCUDA(cudaMemcpyAsync(&n_sel, n_sel_dev, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+    PCUDA(cudaStreamSynchronize(ctx->stream));
+    *n_split_host = (int64_t)n_sel;
+    if (z_percentiles_host)
+        for (int k = 0; k < 2; ++k)
+            if (h[k].size[0] > 0) memcpy(&z_percentiles_host[k], &h[k].prefix[0], sizeof(float));
+#undef PTRY
+#undef PCUDA
+    cleanup();
+    return SVR_OK;
+}
+
+SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8_t* split, uint16_t* ijkl_out, float* raw_out,
+                              float* sh_out, int64_t* n_out_host) {
+    if (!ctx || !vox || !split || !ijkl_out || !raw_out || !sh_out) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (vox->n < 0 || vox->n >= ((int64_t)1 << 28)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    if (n_out_host) *n_out_host = 0;
+    const int64_t n = vox->n;
+    if (n == 0) return SVR_OK;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    uint32_t *counts = nullptr, *offs = nullptr;
+    const size_t eb = sizeof(uint32_t) * (size_t)(n + 1);
+    SVR_TRY(svr_alloc(ctx, (void**)&counts, eb));
+    SvrStatus stt = svr_alloc(ctx, (void**)&offs, eb);
+    if (stt != SVR_OK) { svr_free(ctx, counts, eb); return stt; }
+    split_to_counts_kernel<<<nblocks(n + 1, 256), 256, 0, ctx->stream>>>(n, split, counts);
+    stt = launch_exclusive_scan(ctx, counts, offs, n + 1);
+    if (stt == SVR_OK) {
+        const int words = 3 * (vox->sh_degree + 1) * (vox->sh_degree + 1);
+        subdiv_cells_kernel<<<nblocks(n, 256), 256, 0, ctx->stream>>>(n, split, offs, reinterpret_cast<const uint2*>(vox->ijkl),
+                                                                     reinterpret_cast<const float4*>(vox->raw_density),
+                                                                     reinterpret_cast<uint2*>(ijkl_out), reinterpret_cast<float4*>(raw_out));
+        subdiv_sh_kernel<<<nblocks(n * words, 256), 256, 0, ctx->stream>>>(n, words, split, offs, reinterpret_cast<const uint32_t*>(vox->sh),
+                                                                           reinterpret_cast<uint32_t*>(sh_out));
+        ctx->launches += 3;
+        cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess && n_out_host) {
+            uint32_t n_split = 0;
+            e = cudaMemcpyAsync(&n_split, offs + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+            *n_out_host = n + 7 * (int64_t)n_split;
+        }
+        if (e != cudaSuccess) stt = svr_fail(ctx, SVR_ERR_CUDA, "subdivide: %s", cudaGetErrorString(e));
     }
     svr_free(ctx, counts, eb);
     svr_free(ctx, offs, eb);
