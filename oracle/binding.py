@@ -153,8 +153,9 @@ def render(scene, cam, K: int, mode: str = "pure", xy: Optional[np.ndarray] = No
 
 
 def backward(scene, cam, K: int, G: np.ndarray, mode: str = "pure", xy: Optional[np.ndarray] = None,
-             act_mode: int = 0, grad_raw=None, grad_sh=None, raw=None, sh=None):
-    """Gradient of sum(G * image). Accumulates into (and returns) grad_raw [n,8], grad_sh [n,B,3]."""
+             act_mode: int = 0, grad_raw=None, grad_sh=None, raw=None, sh=None, G_depth=None, G_T=None):
+    """Gradient of sum(G * image) [+ sum(G_depth * depth) + sum(G_T * T_final)]. Accumulates into (and returns)
+    grad_raw [n,8], grad_sh [n,B,3]."""
     m = _Marshalled(scene, cam, raw, sh)
     n_rays, xy_a = _rays(cam, xy)
     G = np.ascontiguousarray(G, dtype=np.float64).reshape(n_rays, 3)
@@ -162,8 +163,14 @@ def backward(scene, cam, K: int, G: np.ndarray, mode: str = "pure", xy: Optional
         grad_raw = np.zeros((scene.n, 8))
     if grad_sh is None:
         grad_sh = np.zeros((scene.n, scene.n_basis, 3))
-    lib().orc_backward(C.byref(m.s), C.byref(m.c), C.c_int(K), C.c_int(act_mode), C.c_int(1 if mode == "bucketed" else 0),
-                       C.c_int64(n_rays), _ptr(xy_a), _ptr(G), _ptr(grad_raw), _ptr(grad_sh))
+    if G_depth is None and G_T is None:
+        lib().orc_backward(C.byref(m.s), C.byref(m.c), C.c_int(K), C.c_int(act_mode), C.c_int(1 if mode == "bucketed" else 0),
+                           C.c_int64(n_rays), _ptr(xy_a), _ptr(G), _ptr(grad_raw), _ptr(grad_sh))
+    else:
+        gd = None if G_depth is None else np.ascontiguousarray(G_depth, dtype=np.float64).reshape(n_rays)
+        gt = None if G_T is None else np.ascontiguousarray(G_T, dtype=np.float64).reshape(n_rays)
+        lib().orc_backward_heads(C.byref(m.s), C.byref(m.c), C.c_int(K), C.c_int(act_mode), C.c_int(1 if mode == "bucketed" else 0),
+                                 C.c_int64(n_rays), _ptr(xy_a), _ptr(G), _ptr(gd), _ptr(gt), _ptr(grad_raw), _ptr(grad_sh))
     return grad_raw, grad_sh
 
 

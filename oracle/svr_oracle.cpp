@@ -434,9 +434,12 @@ void orc_render(const OrcScene* sp, const OrcCamera* cp, int K, int act_mode, in
     }
 }
 
-// Backward of L = sum(G * image): grad_raw[n,8] and grad_sh[n,(D+1)^2,3] accumulate (+=).
-void orc_backward(const OrcScene* sp, const OrcCamera* cp, int K, int act_mode, int mode, int64_t n_rays,
-                  const int32_t* xy, const double* G, double* grad_raw, double* grad_sh) {
+// Backward of L = sum(G * image) + sum(GD * depth) + sum(GT * T_final): grad_raw[n,8] and grad_sh[n,(D+1)^2,3]
+// accumulate (+=). GD, GT (one value per ray) may be NULL. With D = sum_k w_k t_mid,k and T_K = prod_k exp(-tau_k)
+// (reading R7; geometry carries no gradient, so t_mid is a constant):
+//   dD/dtau_k = T_k t_mid,k - sum_{j>k} w_j t_mid,j,   dT_K/dtau_k = -T_K   (NEXT-3, heads for the depth / transmittance terms of eq. 17).
+void orc_backward_heads(const OrcScene* sp, const OrcCamera* cp, int K, int act_mode, int mode, int64_t n_rays,
+                        const int32_t* xy, const double* G, const double* GD, const double* GT, double* grad_raw, double* grad_sh) {
     const OrcScene& s = *sp; const OrcCamera& c = *cp;
     int nb = (s.sh_degree + 1) * (s.sh_degree + 1);
     std::vector<double> rgb((size_t)s.n * 3), pre((size_t)s.n * 3), grgb((size_t)s.n * 3, 0.0);
@@ -464,11 +467,16 @@ void orc_backward(const OrcScene* sp, const OrcCamera* cp, int K, int act_mode, 
                 Tk[k] = T;
             }
             const double* g = G + 3 * i;
+            const double gd = GD ? GD[i] : 0.0, gt = GT ? GT[i] : 0.0;
             double S[3];                                       // suffix colour S_k = sum_{j>k} w_j c_j + T_K bg
             for (int ch = 0; ch < 3; ++ch) S[ch] = T * (double)c.bg[ch];
+            double SD = 0.0;                                   // suffix depth sum_{j>k} w_j t_mid,j
+            const double TK = T;
             for (size_t kk = n; kk-- > 0;) {
                 int64_t v = hits[kk].v;
-                double dL_dtau = 0.0;                          // d alpha / d tau = 1 - alpha  =>  G.(T_k c_k - S_k)
+                const double tmid = hits[kk].tmid;
+                double dL_dtau = gd * (Tk[kk] * tmid - SD) - gt * TK;   // d alpha / d tau = 1 - alpha  =>  G.(T_k c_k - S_k)
+                SD += wk[kk] * tmid;
                 for (int ch = 0; ch < 3; ++ch) dL_dtau += g[ch] * (Tk[kk] * rgb[v * 3 + ch] - S[ch]);
                 for (int cc = 0; cc < 8; ++cc) {
                     double add = dL_dtau * dtau[8 * kk + cc];
@@ -497,6 +505,11 @@ void orc_backward(const OrcScene* sp, const OrcCamera* cp, int K, int act_mode, 
             for (int i = 0; i < nb; ++i) grad_sh[(v * nb + i) * 3 + ch] += Y[i] * grgb[v * 3 + ch];
         }
     }
+}
+
+void orc_backward(const OrcScene* sp, const OrcCamera* cp, int K, int act_mode, int mode, int64_t n_rays,
+                  const int32_t* xy, const double* G, double* grad_raw, double* grad_sh) {
+    orc_backward_heads(sp, cp, K, act_mode, mode, n_rays, xy, G, nullptr, nullptr, grad_raw, grad_sh);
 }
 
 // ---- part B ----
