@@ -111,6 +111,15 @@ SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOp
                        const float* dL_dimage, const float* image,
                        float* grad_raw_density, float* grad_sh, float* w_max);
 
+/* NEXT-3: the same with gradients arriving through the depth and transmittance heads too (for the depth /
+ * transmittance terms of eq. 17): L = sum(dL_dimage * image) + sum(dL_ddepth * depth) + sum(dL_dT * T_final).
+ * With D = sum_k w_k t_mid,k and T_K = prod_k exp(-tau_k) (R7; geometry carries no gradient):
+ * dD/dtau_k = T_k t_mid,k - sum_{j>k} w_j t_mid,j and dT_K/dtau_k = -T_K. dL_ddepth [H,W] and dL_dT [H,W] may each be NULL;
+ * depth / T_final are svr_forward's outputs for this frame (required with the matching gradient). */
+SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
+                             const float* dL_ddepth, const float* dL_dT, const float* image, const float* depth,
+                             const float* T_final, float* grad_raw_density, float* grad_sh, float* w_max);
+
 /* One whole training-view step with HOST inputs/outputs (bench.py's e2e leg): copies camera + target image
  * host->device, runs preprocess -> forward -> loss_grad -> backward on device-resident voxel parameters and
  * gradient buffers, copies the loss (and, if image_host != NULL, the render) device->host, and returns

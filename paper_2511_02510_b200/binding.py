@@ -21,7 +21,7 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
-           "svr_backward", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
+           "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply"]
 
@@ -82,6 +82,7 @@ def _load():
     lib.svr_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_float,
                                   C.POINTER(SvrLossOpts), C.c_void_p, C.c_void_p]
     lib.svr_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 5
+    lib.svr_backward_heads.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 9
     lib.svr_train_view_host.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.POINTER(SvrCamera), C.POINTER(SvrRenderOpts),
                                         C.POINTER(SvrLossOpts), C.c_float] + [C.c_void_p] * 6
     lib.svr_frame_lists.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 2 + [C.POINTER(C.c_int64)] + [C.POINTER(C.c_void_p)] * 3
@@ -323,6 +324,12 @@ class Context:
         o = SvrRenderOpts(K, T_min)
         self._check(_lib.svr_backward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(image), _p(grad_raw),
                                       _p(grad_sh), _p(w_max)))
+
+    def svr_backward_heads(self, frame: "Frame", K: int, dL, image, grad_raw, grad_sh, T_min: float = 1e-5, w_max=None,
+                           dL_ddepth=None, dL_dT=None, depth=None, T_final=None):
+        o = SvrRenderOpts(K, T_min)
+        self._check(_lib.svr_backward_heads(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(dL_ddepth), _p(dL_dT), _p(image),
+                                            _p(depth), _p(T_final), _p(grad_raw), _p(grad_sh), _p(w_max)))
 
     def svr_train_view_host(self, vox: Voxels, cam, K: int, gamma: float, target_host: torch.Tensor, grad_raw, grad_sh,
                             w_max=None, T_min: float = 1e-5, eps: float = 1e-3, percentile: float = 0.99,

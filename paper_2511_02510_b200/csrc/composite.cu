@@ -386,7 +386,8 @@ struct WarpWork {
     float4 P1[32];      //   dl.xyz
     float4 PI[32];      //   1/dh.xyz
     float4 PG[32];      //   G = dL/dC, and G . C_final
-    float2 ST[32];      //   T, P = G . C
+    float2 ST[32];      //   T, P = G . C (+ gD . D with the depth head)
+    float PD[32];       //   gD = dL/dDepth (kernels with HEADS only)
     uint2 Hs[32];       // per slot of the batch: pixels that hit it, queue offset
     unsigned short q[QCAP];
 };
@@ -400,14 +401,16 @@ __device__ __forceinline__ int warp_incl_scan_i(int v, int lane) {
     return v;
 }
 
-template <int K>
+template <int K, bool HEADS>
 __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed,
                                                                const uint2* __restrict__ rects_sorted,
                                                                const uint32_t* __restrict__ ranges,
                                                                const uint32_t* __restrict__ tile_order, float T_min,
                                                                unsigned int* __restrict__ w_max, const float* __restrict__ dL,
                                                                const float* __restrict__ image_in, float* __restrict__ grad_coef,
-                                                               float* __restrict__ grad_rgb) {
+                                                               float* __restrict__ grad_rgb, const float* __restrict__ dL_ddepth,
+                                                               const float* __restrict__ dL_dT, const float* __restrict__ depth_in,
+                                                               const float* __restrict__ T_in) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     WarpWork& S = reinterpret_cast<WarpWork*>(smem_raw)[warp];
@@ -425,11 +428,17 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     {
         RayF ray;
         float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
+        float gdep = 0.f;
         if (inimg) {
             setup_ray(c, px, py, ray);
             oct = pixel_octant_dev(c, px, py);
             g = make_float4(dL[pix * 3], dL[pix * 3 + 1], dL[pix * 3 + 2], 0.f);
             g.w = g.x * image_in[pix * 3] + g.y * image_in[pix * 3 + 1] + g.z * image_in[pix * 3 + 2];
+            if (HEADS) {
+                // dL/dtau_k = T_k (G . c_k + gD t_k) + P_k - (G . C_final + gD D_final + gT T_K): the heads only add constants
+                gdep = dL_ddepth ? dL_ddepth[pix] : 0.f;
+                g.w += gdep * (depth_in ? depth_in[pix] : 0.f) + (dL_dT ? dL_dT[pix] * T_in[pix] : 0.f);
+            }
         } else {
 #pragma unroll
             for (int a = 0; a < 3; ++a) { ray.dh[a] = 0.f; ray.dl[a] = 0.f; ray.inv[a] = 0.f; ray.ainv[a] = 0.f; }
@@ -440,6 +449,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
         S.P1[swl] = make_float4(ray.dl[0], ray.dl[1], ray.dl[2], 0.f);
         S.PI[swl] = make_float4(ray.inv[0], ray.inv[1], ray.inv[2], 0.f);
         S.PG[swl] = g;
+        if (HEADS) S.PD[swl] = gdep;
         S.ST[swl] = make_float2(1.f, 0.f);
     }
     __syncwarp();
@@ -567,6 +577,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
                         const float4 ra = S.r0[slot], rb = S.r1[slot];
                         tau = integrate<K, true>(rr, D, a.w, s0, s1, ra, rb, dtau);
+                        if (HEADS) gc = fmaf(S.PD[i], t_ref + 0.5f * (s0 + s1), gc);
                     }
                 }
                 const float E = ex2f(-1.4426950408889634f * tau);
@@ -672,7 +683,8 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
 }
 
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
-                          float* grad_coef, float* grad_rgb, float* w_max) {
+                          float* grad_coef, float* grad_rgb, float* w_max, const float* dL_ddepth, const float* dL_dT,
+                          const float* depth, const float* T_final) {
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, ST_BACKWARD);
     const size_t smem = sizeof(WarpWork) * WARPS;
@@ -681,10 +693,18 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
 #define SVR_BWD(KK)                                                                                                  \
     do {                                                                                                             \
-        static bool done = false;                                                                                    \
-        SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK>, smem, &done));                                        \
-        backward_packed_kernel<KK><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, image, \
-                                                                           grad_coef, grad_rgb);                     \
+        static bool done = false, done_h = false;                                                                   \
+        if (dL_ddepth || dL_dT) {                                                                                    \
+            SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, true>, smem, &done_h));                            \
+            backward_packed_kernel<KK, true><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, \
+                                                                                     image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth,   \
+                                                                                     T_final);                        \
+        } else {                                                                                                     \
+            SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, false>, smem, &done));                             \
+            backward_packed_kernel<KK, false><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, \
+                                                                                      image, grad_coef, grad_rgb, nullptr, nullptr, nullptr, \
+                                                                                      nullptr);                       \
+        }                                                                                                            \
     } while (0)
     switch (K) {
         case 1: SVR_BWD(1); break;

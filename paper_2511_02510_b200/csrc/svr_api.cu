@@ -360,10 +360,13 @@ SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* targe
     return launch_loss_grad(ctx, render, target, W, H, gamma, opts->eps, opts->percentile, opts->sobel_source, dL_dimage, loss);
 }
 
-SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
-                       const float* image, float* grad_raw_density, float* grad_sh, float* w_max) {
+SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
+                             const float* dL_ddepth, const float* dL_dT, const float* image, const float* depth, const float* T_final,
+                             float* grad_raw_density, float* grad_sh, float* w_max) {
     if (!ctx || !frame || !opts || !dL_dimage || !image || !grad_raw_density || !grad_sh)
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if ((dL_ddepth && !depth) || (dL_dT && !T_final))
+        return svr_fail(ctx, SVR_ERR_INVALID_ARG, "dL_ddepth needs depth and dL_dT needs T_final (svr_forward's outputs)");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     const int64_t n = frame->scene.n;
     if (n == 0) return SVR_OK;
@@ -378,8 +381,14 @@ SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOp
         SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_rgb, 0, sizeof(float) * 4 * (size_t)n, ctx->stream));
         SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_coef, 0, sizeof(float) * 8 * (size_t)n, ctx->stream));
     }
-    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_coef, ctx->grad_rgb, w_max));
+    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_coef, ctx->grad_rgb, w_max, dL_ddepth, dL_dT,
+                            depth, T_final));
     return launch_sh_backward(ctx, frame, ctx->grad_coef, ctx->grad_rgb, grad_raw_density, grad_sh);
+}
+
+SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
+                       const float* image, float* grad_raw_density, float* grad_sh, float* w_max) {
+    return svr_backward_heads(ctx, frame, opts, dL_dimage, nullptr, nullptr, image, nullptr, nullptr, grad_raw_density, grad_sh, w_max);
 }
 
 SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam_host, const SvrRenderOpts* ropts,

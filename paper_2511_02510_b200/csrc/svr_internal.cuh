@@ -139,7 +139,8 @@ SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
                          float* T_final, float* w_max, unsigned long long* stats);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
-                          float* grad_coef, float* grad_rgb, float* w_max);
+                          float* grad_coef, float* grad_rgb, float* w_max, const float* dL_ddepth, const float* dL_dT,
+                          const float* depth, const float* T_final);
 SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw,
                              float* grad_sh);
 SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma,

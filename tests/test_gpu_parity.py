@@ -405,3 +405,36 @@ def test_subdivide_bit_exact_and_rerender(orc, svr, name, n, use_cur):
         # same colours: the images agree closely but not exactly (K samples per child segment instead of per parent)
         assert float((img0 - img1).abs().max()) < 0.1 and float((img0 - img1).abs().mean()) < 5e-3
         f0.release(); f1.release()
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: backward through the depth and transmittance heads against the oracle
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,n,scale", [("C1", None, 1.0), ("C2", 20_000, 0.5), ("C4", 150_000, 0.25)])
+def test_backward_heads(orc, svr, name, n, scale):
+    pkg, ctx, torch = svr
+    cfg = make_config(name) if n is None else make_config(name, n_voxels=n, res_scale=scale, n_cams=1)
+    sc, cam = cfg.scene, cfg.cameras[0]
+    vox, frame, image, depth, Tf, _ = gpu_forward(svr, sc, cam, cfg.K, cfg.T_min)
+    rng = np.random.default_rng(17)
+    npx = cam.W * cam.H
+    G = rng.normal(0, 1.0 / npx, size=(cam.H, cam.W, 3)).astype(np.float32)
+    GD = rng.normal(0, 1.0 / npx, size=(cam.H, cam.W)).astype(np.float32)
+    GT = rng.normal(0, 1.0 / npx, size=(cam.H, cam.W)).astype(np.float32)
+    def run(gd, gt):
+        g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+        g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+        ctx.svr_backward_heads(frame, cfg.K, torch.from_numpy(G).cuda(), image, g_raw, g_sh, cfg.T_min,
+                               dL_ddepth=None if gd is None else torch.from_numpy(gd).cuda(),
+                               dL_dT=None if gt is None else torch.from_numpy(gt).cuda(), depth=depth, T_final=Tf)
+        ctx.synchronize()
+        return g_raw.cpu().numpy(), g_sh.cpu().numpy()
+    for gd, gt in [(GD, GT), (GD, None), (None, GT)]:
+        g_raw, g_sh = run(gd, gt)
+        r_raw, r_sh = orc.backward(sc, cam, cfg.K, G.astype(np.float64), mode="bucketed",
+                                   G_depth=None if gd is None else gd.astype(np.float64), G_T=None if gt is None else gt.astype(np.float64))
+        assert rel_l2(g_raw, r_raw) <= GRAD_TOL and rel_l2(g_sh, r_sh) <= GRAD_TOL, (rel_l2(g_raw, r_raw), rel_l2(g_sh, r_sh))
+    # the heads change the density gradient (they are not silently ignored) and leave the SH gradient alone
+    base_raw, base_sh = run(None, None)
+    assert rel_l2(g_raw, base_raw) > 1e-2 and rel_l2(g_sh, base_sh) < 1e-5
+    frame.release()
