@@ -799,12 +799,15 @@ inline unsigned int blocks_for(int64_t n, int bs) { return (unsigned int)((n + b
 
 }  // namespace
 
-SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f) {
+SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f, bool with_sat) {
     StageScope scope__(ctx, ST_TILE_MASKS);
     dim3 grid(f->cam.tiles_x, f->cam.tiles_y), block(SVR_TILE, SVR_TILE);
     tile_mask_kernel<<<grid, block, 0, ctx->stream>>>(f->cam, f->tile_masks);
-    sat_kernel<<<1, 256, 0, ctx->stream>>>(f->tile_masks, f->sat, f->cam.tiles_x, f->cam.tiles_y);
-    ctx->launches += 2;
+    ctx->launches += 1;
+    if (with_sat) {      // the summed-area table serves the per-voxel counts of the first list-build design only
+        sat_kernel<<<1, 256, 0, ctx->stream>>>(f->tile_masks, f->sat, f->cam.tiles_x, f->cam.tiles_y);
+        ctx->launches += 1;
+    }
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

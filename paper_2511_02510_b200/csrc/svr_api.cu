@@ -228,13 +228,13 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 
     TRYF(A.get((void**)&f->rects, sizeof(uint16_t) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->tile_masks, (size_t)f->n_tiles));
-    TRYF(A.get((void**)&f->sat, sizeof(uint32_t) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1)));
+    if (!bucketed) TRYF(A.get((void**)&f->sat, sizeof(uint32_t) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1)));
     TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->ranges, sizeof(uint32_t) * 16 * (size_t)f->n_tiles));
     TRYF(A.get((void**)&f->tile_order, sizeof(uint32_t) * 2 * (size_t)f->n_tiles));
     TRYF(svr_alloc(ctx, (void**)&totals, 128));
     CUDAF(cudaMemsetAsync(totals, 0, 128, ctx->stream));
-    TRYF(launch_tile_masks(ctx, f));
+    TRYF(launch_tile_masks(ctx, f, !bucketed));
 
     if (bucketed) {
         TRYF(svr_alloc(ctx, (void**)&bcount, bucket_bytes));

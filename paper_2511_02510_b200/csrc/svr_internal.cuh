@@ -119,7 +119,7 @@ SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes);
 void svr_free(SvrContext* ctx, void* p, size_t bytes);
 
 // ---- stage launchers (each counts its kernel launches into ctx->launches) --------------------
-SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f, bool with_sat);
 SvrStatus launch_rects_counts(SvrContext* ctx, SvrFrame* f, uint32_t* counts, unsigned long long* totals);
 SvrStatus launch_exclusive_scan(SvrContext* ctx, const uint32_t* in, uint32_t* out, int64_t n_plus_1);
 SvrStatus launch_emit_keys(SvrContext* ctx, SvrFrame* f, uint64_t* keys, uint32_t* vals, uint32_t* big_list,

@@ -668,3 +668,31 @@ def test_head_gradients_match_finite_differences(orc):
     gr, _ = orc.backward(one, cam, 3, np.zeros((cam.H, cam.W, 3)), G_T=gt1)
     tau = -np.log(np.maximum(r1["T_final"], 1e-300))
     assert np.isclose(gr.sum(), -(r1["T_final"] * tau).sum(), rtol=1e-10)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4 (part): Adam update, pins of oracle/adam.py
+# ---------------------------------------------------------------------------------------------
+def test_adam_first_step_and_fp64_rederivation():
+    from oracle.adam import adam_step
+    rng = np.random.default_rng(8)
+    th = rng.normal(0, 1, 4000).astype(np.float32)
+    g = rng.normal(0, 1e-3, 4000).astype(np.float32)
+    g[:5] = 0.0
+    lr, b1, b2, eps = 1e-2, 0.9, 0.999, 1e-15
+    t1, m1, v1 = adam_step(th, g, np.zeros_like(th), np.zeros_like(th), lr, b1, b2, eps, 1)
+    # step 1: m/c1 = g, v/c2 = g^2 => every parameter moves by lr sign(g) (textbook property of the bias correction)
+    np.testing.assert_allclose(th - t1, lr * np.sign(g), rtol=0, atol=2.5e-7)      # |theta| ~ 1: half an ulp of theta
+    assert np.all(t1[:5] == th[:5])
+    # ten steps against the same recurrences in fp64
+    T, M, V = th.astype(np.float64), np.zeros(4000), np.zeros(4000)
+    tt, mm, vv = th, np.zeros_like(th), np.zeros_like(th)
+    for t in range(1, 11):
+        gt = (g * np.float32(1 + 0.1 * t)).astype(np.float32)
+        tt, mm, vv = adam_step(tt, gt, mm, vv, lr, b1, b2, 1e-8, t)
+        M = b1 * M + (1 - b1) * gt
+        V = b2 * V + (1 - b2) * gt.astype(np.float64) ** 2
+        T = T - lr * (M / (1 - b1 ** t)) / (np.sqrt(V / (1 - b2 ** t)) + 1e-8)
+    np.testing.assert_allclose(tt, T, rtol=1e-5, atol=1e-6)
+    np.testing.assert_allclose(mm, M, rtol=1e-5, atol=1e-12)
+    np.testing.assert_allclose(vv, V, rtol=1e-5, atol=1e-15)
