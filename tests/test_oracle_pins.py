@@ -690,8 +690,10 @@ def test_adam_first_step_and_fp64_rederivation():
     for t in range(1, 11):
         gt = (g * np.float32(1 + 0.1 * t)).astype(np.float32)
         tt, mm, vv = adam_step(tt, gt, mm, vv, lr, b1, b2, 1e-8, t)
-        M = b1 * M + (1 - b1) * gt
-        V = b2 * V + (1 - b2) * gt.astype(np.float64) ** 2
+        # the float32-rounded coefficients (1 - b2 = 0.001 carries a 5e-5 relative rounding in float32), fp64 arithmetic
+        B1, B2 = float(np.float32(b1)), float(np.float32(b2))
+        M = B1 * M + float(np.float32(1) - np.float32(b1)) * gt
+        V = B2 * V + float(np.float32(1) - np.float32(b2)) * gt.astype(np.float64) ** 2
         T = T - lr * (M / (1 - b1 ** t)) / (np.sqrt(V / (1 - b2 ** t)) + 1e-8)
     np.testing.assert_allclose(tt, T, rtol=1e-5, atol=1e-6)
     np.testing.assert_allclose(mm, M, rtol=1e-5, atol=1e-12)
