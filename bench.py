@@ -403,6 +403,24 @@ def main():
             "apply_roofline": {"bound": "hbm", "achieved": app_bytes / (ms_app * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                "frac": app_bytes / (ms_app * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
 
+        # NEXT-4 (part): fused Adam over the SH coefficients (the largest parameter tensor), gradient cleared in the same pass
+        theta = vox.sh.view(-1)
+        gflat, m1, v1 = g_sh.view(-1), torch.zeros_like(theta), torch.zeros_like(theta)
+        ctx.svr_adam_step(theta, gflat, m1, v1, 0.0, 0.9, 0.999, 1e-8, 1, zero_grad=True)      # lr = 0: parameters unchanged
+        e0, e1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for k in range(reps):
+                ctx.svr_adam_step(theta, gflat, m1, v1, 0.0, 0.9, 0.999, 1e-8, 2 + k, zero_grad=True)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        ms_adam = e0.elapsed_time(e1) / reps
+        adam_bytes = theta.numel() * 32
+        line["next4_adam"] = {"what": "svr_adam_step over sh [n,16,3] with zero_grad (32 B per parameter); outside `value`",
+                              "ms": ms_adam, "params": int(theta.numel()),
+                              "roofline": {"bound": "hbm", "achieved": adam_bytes / (ms_adam * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                           "unit": "GB/s", "frac": adam_bytes / (ms_adam * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()

@@ -209,6 +209,14 @@ SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrC
 SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8_t* split, uint16_t* ijkl_out,
                               float* raw_out, float* sh_out, int64_t* n_out_host);
 
+/* ---- NEXT-4 (part): fused Adam over a flat float32 parameter array ("Adam state per voxel", ref. [14] P:334) ----
+ * m <- b1 m + (1-b1) g; v <- b2 v + (1-b2) g g; theta <- theta - (lr (m / c1)) / (sqrt(v / c2) + eps), c1 = 1 - b1^step,
+ * c2 = 1 - b2^step (fp64 on the host, rounded once); float32, each operation rounded in this order. One pass over
+ * theta, grad, m, v [n] (device, 16-byte aligned); zero_grad != 0 also clears grad (svr_backward accumulates into it).
+ * step >= 1. Asynchronous on the context's stream. */
+SvrStatus svr_adam_step(SvrContext* ctx, float* theta, float* grad, float* m, float* v, int64_t n, float lr, float beta1,
+                        float beta2, float eps, int32_t step, int32_t zero_grad);
+
 /* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);
 

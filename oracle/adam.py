@@ -4,7 +4,7 @@ float32, every operation rounded in the written order (the CUDA kernel uses the 
 bit-identical):
     m <- b1 m + (1 - b1) g
     v <- b2 v + (1 - b2) (g g)
-    theta <- theta - (lr (m / c1)) / (sqrt(v / c2) + eps),   c1 = 1 - b1^t, c2 = 1 - b2^t (computed in fp64, rounded once)
+    theta <- theta - (lr (m / c1)) / (sqrt(v / c2) + eps),   c1 = 1 - b1^t, c2 = 1 - b2^t (fp64 powers of the float32 b1, b2; rounded once)
 Pins (tests/test_oracle_pins.py): the first step moves every parameter by lr * sign(g) up to eps (textbook property of
 the bias correction); a constant gradient keeps |step| -> lr; against a fp64 re-derivation within rounding.
 """
@@ -17,7 +17,7 @@ def adam_step(theta, g, m, v, lr, b1, b2, eps, t):
     f = np.float32
     theta, g, m, v = (np.asarray(a, dtype=np.float32) for a in (theta, g, m, v))
     one_b1, one_b2 = f(1.0) - f(b1), f(1.0) - f(b2)
-    c1, c2 = f(1.0 - float(b1) ** t), f(1.0 - float(b2) ** t)
+    c1, c2 = f(1.0 - float(f(b1)) ** t), f(1.0 - float(f(b2)) ** t)      # b1, b2 are float32 values on both sides
     m2 = (f(b1) * m).astype(f) + (one_b1 * g).astype(f)
     v2 = (f(b2) * v).astype(f) + (one_b2 * (g * g).astype(f)).astype(f)
     mh = (m2 / c1).astype(f)

@@ -23,7 +23,7 @@ EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_by
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
            "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
-           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply"]
+           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step"]
 
 
 class SvrError(RuntimeError):
@@ -95,6 +95,7 @@ def _load():
     lib.svr_subdivide_select.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(SvrSubdivOpts),
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
     lib.svr_subdivide_apply.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+    lib.svr_adam_step.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, C.c_int32]
     lib.svr_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.svr_set_stage_timing.restype = None
     lib.svr_num_stages.restype = C.c_int
@@ -388,6 +389,12 @@ class Context:
         self._check(_lib.svr_subdivide_apply(self.handle, C.byref(vox.c), _p(split), _p(ijkl), _p(raw), _p(sh), C.byref(n_out)))
         assert int(n_out.value) == n_new, (int(n_out.value), n_new)
         return ijkl, raw, sh
+
+
+    def svr_adam_step(self, theta, grad, m, v, lr: float, beta1: float, beta2: float, eps: float, step: int, zero_grad: bool = True):
+        """Fused Adam over flat float32 tensors (in place)."""
+        self._check(_lib.svr_adam_step(self.handle, _p(theta), _p(grad), _p(m), _p(v), theta.numel(), lr, beta1, beta2, eps, step,
+                                       1 if zero_grad else 0))
 
 
 def svr_gamma_schedule(t: float, T: float, t0_frac: float = 0.3, t1_frac: float = 0.6, gamma_max: float = 0.6) -> float:

@@ -1,0 +1,62 @@
+// Fused Adam update over a flat float32 parameter array (NEXT-4: "fused Adam over voxel parameters";
+// PAPER.md P:62 "Adam state per voxel", ref. [14] P:334). One pass: reads theta, g, m, v, writes theta, m, v and
+// (optionally) zeroes g, because svr_backward ACCUMULATES into the gradient buffers: 28 or 32 bytes per parameter, HBM-bound.
+// Every operation is individually rounded in the order oracle/adam.py states, so the result is bit-identical to it.
+#include <cmath>
+
+#include "svr_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ void adam_one(float& th, float g, float& m, float& v, float lr, float b1, float b2, float one_b1,
+                                         float one_b2, float c1, float c2, float eps) {
+    m = __fadd_rn(__fmul_rn(b1, m), __fmul_rn(one_b1, g));
+    v = __fadd_rn(__fmul_rn(b2, v), __fmul_rn(one_b2, __fmul_rn(g, g)));
+    const float mh = __fdiv_rn(m, c1), vh = __fdiv_rn(v, c2);
+    th = __fsub_rn(th, __fdiv_rn(__fmul_rn(lr, mh), __fadd_rn(__fsqrt_rn(vh), eps)));
+}
+
+__global__ void __launch_bounds__(256) adam_kernel(float* __restrict__ theta, float* __restrict__ grad, float* __restrict__ m,
+                                                   float* __restrict__ v, int64_t n, float lr, float b1, float b2, float one_b1,
+                                                   float one_b2, float c1, float c2, float eps, int zero_grad) {
+    const int64_t i4 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i4 + 3 < n) {
+        float4 t = *reinterpret_cast<float4*>(theta + i4), g = *reinterpret_cast<float4*>(grad + i4);
+        float4 mm = *reinterpret_cast<float4*>(m + i4), vv = *reinterpret_cast<float4*>(v + i4);
+        adam_one(t.x, g.x, mm.x, vv.x, lr, b1, b2, one_b1, one_b2, c1, c2, eps);
+        adam_one(t.y, g.y, mm.y, vv.y, lr, b1, b2, one_b1, one_b2, c1, c2, eps);
+        adam_one(t.z, g.z, mm.z, vv.z, lr, b1, b2, one_b1, one_b2, c1, c2, eps);
+        adam_one(t.w, g.w, mm.w, vv.w, lr, b1, b2, one_b1, one_b2, c1, c2, eps);
+        *reinterpret_cast<float4*>(theta + i4) = t;
+        *reinterpret_cast<float4*>(m + i4) = mm;
+        *reinterpret_cast<float4*>(v + i4) = vv;
+        if (zero_grad) *reinterpret_cast<float4*>(grad + i4) = make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {
+        for (int64_t i = i4; i < n; ++i) {
+            float t = theta[i], mm = m[i], vv = v[i];
+            adam_one(t, grad[i], mm, vv, lr, b1, b2, one_b1, one_b2, c1, c2, eps);
+            theta[i] = t; m[i] = mm; v[i] = vv;
+            if (zero_grad) grad[i] = 0.f;
+        }
+    }
+}
+
+}  // namespace
+
+extern "C" SvrStatus svr_adam_step(SvrContext* ctx, float* theta, float* grad, float* m, float* v, int64_t n, float lr, float beta1,
+                                   float beta2, float eps, int32_t step, int32_t zero_grad) {
+    if (!ctx || !theta || !grad || !m || !v) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (n < 0 || step < 1) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n must be >= 0 and step >= 1");
+    if (((uintptr_t)theta | (uintptr_t)grad | (uintptr_t)m | (uintptr_t)v) & 15)
+        return svr_fail(ctx, SVR_ERR_INVALID_ARG, "arrays must be 16-byte aligned");
+    if (n == 0) return SVR_OK;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    const float c1 = (float)(1.0 - std::pow((double)beta1, (double)step)), c2 = (float)(1.0 - std::pow((double)beta2, (double)step));
+    const float one_b1 = 1.0f - beta1, one_b2 = 1.0f - beta2;
+    const int64_t n4 = (n + 3) / 4;
+    adam_kernel<<<(unsigned int)((n4 + 255) / 256), 256, 0, ctx->stream>>>(theta, grad, m, v, n, lr, beta1, beta2, one_b1, one_b2, c1, c2,
+                                                                          eps, zero_grad);
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}

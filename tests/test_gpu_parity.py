@@ -438,3 +438,26 @@ def test_backward_heads(orc, svr, name, n, scale):
     base_raw, base_sh = run(None, None)
     assert rel_l2(g_raw, base_raw) > 1e-2 and rel_l2(g_sh, base_sh) < 1e-5
     frame.release()
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4 (part): fused Adam against oracle/adam.py, bit-identical
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 7, 4096, 1_000_003])
+def test_adam_step_bit_exact(svr, n):
+    from oracle.adam import adam_step
+    pkg, ctx, torch = svr
+    rng = np.random.default_rng(n)
+    th = rng.normal(0, 1, n).astype(np.float32)
+    m, v = np.zeros(n, np.float32), np.zeros(n, np.float32)
+    d_th, d_m, d_v = (torch.from_numpy(a.copy()).cuda() for a in (th, m, v))
+    for step in range(1, 5):
+        g = (rng.normal(0, 1e-2, n) * (rng.random(n) < 0.8)).astype(np.float32)
+        d_g = torch.from_numpy(g.copy()).cuda()
+        ctx.svr_adam_step(d_th, d_g, d_m, d_v, 1e-2, 0.9, 0.999, 1e-8, step, zero_grad=(step % 2 == 0))
+        th, m, v = adam_step(th, g, m, v, 1e-2, 0.9, 0.999, 1e-8, step)
+        ctx.synchronize()
+        np.testing.assert_array_equal(d_th.cpu().numpy(), th)
+        np.testing.assert_array_equal(d_m.cpu().numpy(), m)
+        np.testing.assert_array_equal(d_v.cpu().numpy(), v)
+        assert float(d_g.abs().max()) == (0.0 if step % 2 == 0 else float(np.abs(g).max()))
