@@ -248,6 +248,35 @@ def test_workspace_budget_error(svr):
     small.close()
 
 
+def test_error_behaviour(svr):
+    """include/svr.h: calls return a status, svr_last_error has the detail, and a failed call leaves the context usable."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C1")
+    vox = pkg.Voxels.from_scene(cfg.scene)
+    frame = ctx.svr_preprocess(vox, cfg.cameras[0])
+    with pytest.raises(pkg.SvrError) as ei:                     # K out of range
+        ctx.svr_forward(frame, 5, cfg.T_min)
+    assert ei.value.status == 4 and "K" in str(ei.value)
+    import ctypes as C
+    lib = pkg.lib()
+    assert lib.svr_forward(ctx.handle, C.c_void_p(frame.handle), None, None, None, None, None) == 1      # null arguments
+    assert lib.svr_preprocess(ctx.handle, None, None, None) == 1
+    bad_cam = pkg.make_camera(cfg.cameras[0])
+    bad_cam.W = 70000                                           # image size must fit 16 bits
+    with pytest.raises(pkg.SvrError) as ei:
+        ctx.svr_preprocess(vox, bad_cam)
+    assert ei.value.status == 1
+    po = pkg.SvrPruneOpts(0, 0.1, 0.1, 0.5, 0.3, 0.7, 1.0, 0.5, 0.05)                                    # n_bins = 0
+    with pytest.raises(pkg.SvrError):
+        ctx.svr_prune_step(vox, cfg.cameras, torch.zeros(vox.n, device="cuda"), torch.zeros(vox.n, device="cuda"),
+                           torch.zeros(vox.n, dtype=torch.uint8, device="cuda"), po)
+    # the context still works after the failures
+    image, depth, Tf = ctx.svr_forward(frame, cfg.K, cfg.T_min)
+    ctx.synchronize()
+    assert np.isfinite(image.cpu().numpy()).all()
+    frame.release()
+
+
 # ---------------------------------------------------------------------------------------------
 # reduced copies of C3..C5 in full (all pixels), full-size C3/C4 on sampled rays
 # ---------------------------------------------------------------------------------------------
