@@ -490,3 +490,36 @@ def test_adam_step_bit_exact(svr, n):
         np.testing.assert_array_equal(d_m.cpu().numpy(), m)
         np.testing.assert_array_equal(d_v.cpu().numpy(), v)
         assert float(d_g.abs().max()) == (0.0 if step % 2 == 0 else float(np.abs(g).max()))
+
+
+# ---------------------------------------------------------------------------------------------
+# the pieces together: a short optimisation run (forward -> LF loss -> backward -> Adam) must reduce the loss
+# ---------------------------------------------------------------------------------------------
+def test_training_iterations_reduce_loss(orc, svr):
+    """Signs and scales of the whole chain: 30 Adam steps towards the render of a perturbed copy of C1 (the paper's loop,
+    P:112: project, rasterize, measure the photometric objective, back-propagate)."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C1")
+    sc, cam = cfg.scene, cfg.cameras[0]
+    rng = np.random.default_rng(4)
+    from dataclasses import replace
+    truth = replace(sc, raw=(sc.raw + rng.normal(0, 0.5, sc.raw.shape)).astype(np.float32),
+                    sh=(sc.sh + rng.normal(0, 0.3, sc.sh.shape)).astype(np.float32))
+    _, f_t, target, *_ = gpu_forward(svr, truth, cam, cfg.K, cfg.T_min)
+    target = target.clone()
+    f_t.release()
+    vox = pkg.Voxels.from_scene(sc)
+    g_raw, g_sh = torch.zeros_like(vox.raw), torch.zeros_like(vox.sh)
+    state = [torch.zeros_like(t.view(-1)) for t in (vox.raw, vox.raw, vox.sh, vox.sh)]
+    losses = []
+    for step in range(1, 31):
+        frame = ctx.svr_preprocess(vox, cam)
+        image, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min)
+        dL, loss = ctx.svr_loss_grad(image, target, 0.6)
+        ctx.svr_backward(frame, cfg.K, dL, image, g_raw, g_sh, cfg.T_min)
+        ctx.svr_adam_step(vox.raw.view(-1), g_raw.view(-1), state[0], state[1], 5e-2, 0.9, 0.999, 1e-15, step)
+        ctx.svr_adam_step(vox.sh.view(-1), g_sh.view(-1), state[2], state[3], 2e-2, 0.9, 0.999, 1e-15, step)
+        frame.release()
+        losses.append(float(loss.item()))
+    assert float(g_raw.abs().max()) == 0.0                       # zero_grad cleared the accumulators
+    assert losses[-1] < 0.5 * losses[0] and min(losses[-5:]) <= min(losses[:5]), losses
