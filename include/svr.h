@@ -217,6 +217,14 @@ SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8
 SvrStatus svr_adam_step(SvrContext* ctx, float* theta, float* grad, float* m, float* v, int64_t n, float lr, float beta1,
                         float beta2, float eps, int32_t step, int32_t zero_grad);
 
+/* NEXT-4 (part): shared grid-point densities. corner_index[n,8] (uint32, corner c = bx + 2 by + 4 bz) names the
+ * grid point of every voxel corner; svr_gather_corners fills raw_density[n,8] = grid[corner_index] before svr_preprocess,
+ * svr_scatter_add_corners adds grad_raw_density[n,8] into grad_grid[corner_index] (+=, float atomics) after svr_backward.
+ * All pointers are device pointers; asynchronous on the context's stream. */
+SvrStatus svr_gather_corners(SvrContext* ctx, const float* grid, const uint32_t* corner_index, int64_t n, float* raw_density);
+SvrStatus svr_scatter_add_corners(SvrContext* ctx, const float* grad_raw_density, const uint32_t* corner_index, int64_t n,
+                                  float* grad_grid);
+
 /* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);
 

@@ -23,7 +23,8 @@ EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_by
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
            "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
-           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step"]
+           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
+           "svr_gather_corners", "svr_scatter_add_corners"]
 
 
 class SvrError(RuntimeError):
@@ -96,6 +97,8 @@ def _load():
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
     lib.svr_subdivide_apply.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
     lib.svr_adam_step.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, C.c_int32]
+    lib.svr_gather_corners.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+    lib.svr_scatter_add_corners.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
     lib.svr_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.svr_set_stage_timing.restype = None
     lib.svr_num_stages.restype = C.c_int
@@ -395,6 +398,13 @@ class Context:
         """Fused Adam over flat float32 tensors (in place)."""
         self._check(_lib.svr_adam_step(self.handle, _p(theta), _p(grad), _p(m), _p(v), theta.numel(), lr, beta1, beta2, eps, step,
                                        1 if zero_grad else 0))
+
+
+    def svr_gather_corners(self, grid, corner_index, raw):
+        self._check(_lib.svr_gather_corners(self.handle, _p(grid), _p(corner_index), raw.shape[0], _p(raw)))
+
+    def svr_scatter_add_corners(self, grad_raw, corner_index, grad_grid):
+        self._check(_lib.svr_scatter_add_corners(self.handle, _p(grad_raw), _p(corner_index), grad_raw.shape[0], _p(grad_grid)))
 
 
 def svr_gamma_schedule(t: float, T: float, t0_frac: float = 0.3, t1_frac: float = 0.6, gamma_max: float = 0.6) -> float:

@@ -60,3 +60,46 @@ extern "C" SvrStatus svr_adam_step(SvrContext* ctx, float* theta, float* grad, f
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }
+
+// ---- shared grid-point densities (NEXT-4): voxels that share a corner share its raw density ----
+// gather: raw[v, c] = grid[idx[v, c]]; scatter: grad_grid[idx[v, c]] += grad_raw[v, c] (float atomics: order-dependent sums).
+namespace {
+
+__global__ void __launch_bounds__(256) gather_corners_kernel(const float* __restrict__ grid, const uint32_t* __restrict__ idx, int64_t n8,
+                                                             float* __restrict__ raw) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n8) raw[i] = __ldg(grid + idx[i]);
+}
+
+__global__ void __launch_bounds__(256) scatter_corners_kernel(const float* __restrict__ grad_raw, const uint32_t* __restrict__ idx, int64_t n8,
+                                                              float* __restrict__ grad_grid) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n8) return;
+    const float g = grad_raw[i];
+    if (g != 0.0f) atomicAdd(grad_grid + idx[i], g);
+}
+
+}  // namespace
+
+extern "C" SvrStatus svr_gather_corners(SvrContext* ctx, const float* grid, const uint32_t* corner_index, int64_t n, float* raw_density) {
+    if (!ctx || !grid || !corner_index || !raw_density) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (n < 0 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    if (n == 0) return SVR_OK;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    gather_corners_kernel<<<(unsigned int)((8 * n + 255) / 256), 256, 0, ctx->stream>>>(grid, corner_index, 8 * n, raw_density);
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+extern "C" SvrStatus svr_scatter_add_corners(SvrContext* ctx, const float* grad_raw_density, const uint32_t* corner_index, int64_t n,
+                                             float* grad_grid) {
+    if (!ctx || !grad_raw_density || !corner_index || !grad_grid) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (n < 0 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    if (n == 0) return SVR_OK;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    scatter_corners_kernel<<<(unsigned int)((8 * n + 255) / 256), 256, 0, ctx->stream>>>(grad_raw_density, corner_index, 8 * n, grad_grid);
+    ctx->launches += 1;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}

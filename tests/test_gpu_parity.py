@@ -523,3 +523,29 @@ def test_training_iterations_reduce_loss(orc, svr):
         losses.append(float(loss.item()))
     assert float(g_raw.abs().max()) == 0.0                       # zero_grad cleared the accumulators
     assert losses[-1] < 0.5 * losses[0] and min(losses[-5:]) <= min(losses[:5]), losses
+
+
+def test_shared_corner_gather_scatter(svr):
+    """NEXT-4 (part): raw = grid[idx] exactly; grad_grid += scatter of grad_raw equals np.add.at within float rounding.
+    The index is the real one of a uniform grid: neighbouring voxels of C1 share their corner points."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C1")                                     # 8^3 cells: 9^3 grid points
+    ijk = cfg.scene.ijkl[:, :3].astype(np.int64)
+    idx = np.empty((cfg.scene.n, 8), dtype=np.uint32)
+    for c in range(8):
+        p = ijk + np.array([c & 1, (c >> 1) & 1, c >> 2])
+        idx[:, c] = (p[:, 0] + 9 * (p[:, 1] + 9 * p[:, 2])).astype(np.uint32)
+    rng = np.random.default_rng(1)
+    grid = rng.normal(0, 1, 9 ** 3).astype(np.float32)
+    raw = torch.empty((cfg.scene.n, 8), dtype=torch.float32, device="cuda")
+    d_idx = torch.from_numpy(idx.view(np.int32)).cuda()
+    ctx.svr_gather_corners(torch.from_numpy(grid).cuda(), d_idx, raw)
+    np.testing.assert_array_equal(raw.cpu().numpy(), grid[idx])
+    g = rng.normal(0, 1, (cfg.scene.n, 8)).astype(np.float32)
+    g[::3] = 0.0
+    gg = torch.zeros(9 ** 3, dtype=torch.float32, device="cuda")
+    ctx.svr_scatter_add_corners(torch.from_numpy(g).cuda(), d_idx, gg)
+    want = np.zeros(9 ** 3, dtype=np.float64)
+    np.add.at(want, idx.reshape(-1), g.reshape(-1).astype(np.float64))
+    np.testing.assert_allclose(gg.cpu().numpy(), want, rtol=1e-5, atol=1e-5)
+    assert np.bincount(idx.reshape(-1)).max() == 8              # interior grid points are shared by 8 voxels
