@@ -352,18 +352,32 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
     const int nvox = (int)min((int64_t)32, s.n - v0);
     if constexpr (ROW % 4 == 0) {
         float4* p4 = reinterpret_cast<float4*>(grad_sh + v0 * ROW);
-        for (int e = lane; e < nvox * (ROW / 4); e += 32) {
-            int vv = e / (ROW / 4);
-            if (!((amask >> vv) & 1u)) continue;
-            int f0 = (e - vv * (ROW / 4)) * 4;
-            float4 t = p4[e];
-            float tv[4] = {t.x, t.y, t.z, t.w};
+        const int total = nvox * (ROW / 4);
+        // four independent 16-byte loads in flight per lane before the first use
+        for (int e0 = lane; e0 < total; e0 += 128) {
+            float4 t[4];
+            int vvs[4];
+            bool on[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                int idx = f0 + k;
-                tv[k] = fmaf(Ysm[warp][vv][idx / 3], gsm[warp][vv][idx % 3], tv[k]);
+            for (int u = 0; u < 4; ++u) {
+                const int e = e0 + 32 * u;
+                vvs[u] = e / (ROW / 4);
+                on[u] = e < total && ((amask >> vvs[u]) & 1u);
+                if (on[u]) t[u] = p4[e];
             }
-            p4[e] = make_float4(tv[0], tv[1], tv[2], tv[3]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (!on[u]) continue;
+                const int e = e0 + 32 * u, vv = vvs[u];
+                const int f0 = (e - vv * (ROW / 4)) * 4;
+                float tv[4] = {t[u].x, t[u].y, t[u].z, t[u].w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int idx = f0 + k;
+                    tv[k] = fmaf(Ysm[warp][vv][idx / 3], gsm[warp][vv][idx % 3], tv[k]);
+                }
+                p4[e] = make_float4(tv[0], tv[1], tv[2], tv[3]);
+            }
         }
     } else {
         float* p = grad_sh + v0 * ROW;
