@@ -116,7 +116,8 @@ def run_reference(args):
     from svr_inputs import make_config
     oracle.build()
     cfg = make_config(args.workload, n_voxels=args.n_voxels, res_scale=args.res_scale)
-    n_rays = args.ref_rays
+    # the oracle does ~23 k rays/s on 16 cores: 2.5 M rays in all keep K steps within about two minutes
+    n_rays = args.ref_rays if args.ref_rays else max(5_000, min(100_000, 2_500_000 // max(args.steps, 1)))
     for i in range(args.warmup if args.warmup < 2 else 1):
         oracle_sample_run(cfg, cfg.cameras[i % len(cfg.cameras)], min(n_rays, 2000), 900 + i)
     total = 0.0
@@ -174,7 +175,8 @@ def main():
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--n-voxels", type=int, default=None, help="reduced copy of the workload (debugging only)")
     ap.add_argument("--res-scale", type=float, default=1.0)
-    ap.add_argument("--ref-rays", type=int, default=100_000, help="rays per step of the CPU oracle sample")
+    ap.add_argument("--ref-rays", type=int, default=None,
+                    help="rays per step of the CPU oracle sample (default: sized so that the whole run takes about two minutes)")
     ap.add_argument("--cpu-baseline-rays", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
