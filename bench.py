@@ -318,10 +318,11 @@ def main():
     if dom in flop:
         achieved = hits * flop[dom] / (stage_ms[dom] * 1e-3) / 1e12
         traffic = None      # DRAM bytes of one launch of this kernel from the committed ncu capture (full-size C4 only)
-        tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "r1j_traffic.csv")
         if os.path.exists(tpath) and args.workload == "C4" and args.n_voxels is None and args.res_scale == 1.0:
             with open(tpath) as fh:
-                traffic = json.load(fh).get(dom)
+                rows = dict(line.strip().split(",") for line in fh.readlines()[1:] if "," in line)
+            traffic = float(rows[dom]) if dom in rows else None
         roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
                     "frac": achieved / fp32_peak, "traffic": traffic,
                     "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x sm_max_mhz, clocks {peak_src}",
