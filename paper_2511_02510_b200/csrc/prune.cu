@@ -94,9 +94,21 @@ __global__ void __launch_bounds__(256) select_hist_kernel(int64_t n, const float
         const int b = bins ? bins[v] : 0;
         if (hi_shift >= 32 || (key >> hi_shift) == st->prefix[b]) slot = (uint32_t)b * HBINS + ((key >> shift) & mask);
     }
-    // warp-aggregated: equal w_max values are common (never-seen voxels are all 0)
+    // Equal keys are common (never-seen voxels all have w_max = 0, so one histogram slot receives most of the voxels):
+    // aggregate per warp (match_any), then per block in a small tagged shared-memory table (slot mod 64; a warp whose
+    // slot loses the tag race goes to global memory directly), and flush the table once per block.
+    __shared__ uint32_t tag[64], cnt[64];
+    if (threadIdx.x < 64) { tag[threadIdx.x] = 0xFFFFFFFFu; cnt[threadIdx.x] = 0u; }
+    __syncthreads();
     const unsigned peers = __match_any_sync(FULL, slot);
-    if (slot != 0xFFFFFFFFu && (peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) atomicAdd(&hist[slot], (uint32_t)__popc(peers));
+    if (slot != 0xFFFFFFFFu && (peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) {
+        const uint32_t h = slot & 63u, c = (uint32_t)__popc(peers);
+        const uint32_t prev = atomicCAS(&tag[h], 0xFFFFFFFFu, slot);
+        if (prev == 0xFFFFFFFFu || prev == slot) atomicAdd(&cnt[h], c);
+        else atomicAdd(&hist[slot], c);
+    }
+    __syncthreads();
+    if (threadIdx.x < 64 && cnt[threadIdx.x]) atomicAdd(&hist[tag[threadIdx.x]], cnt[threadIdx.x]);
 }
 
 // One block per bin: find the digit that holds the bin's rank; refine prefix and rank; clear the histogram row.
