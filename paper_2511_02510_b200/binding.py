@@ -183,6 +183,10 @@ class Frame:
         except Exception:
             pass
 
+    def refresh_colors(self):
+        """svr_frame_refresh_colors: re-capture raw_density / sh values (colours + per-entry records); the lists stay."""
+        self.ctx._check(_lib.svr_frame_refresh_colors(self.ctx.handle, C.c_void_p(self.handle)))
+
     @property
     def n_entries(self) -> int:
         n = C.c_int64()

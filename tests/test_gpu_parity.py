@@ -549,3 +549,31 @@ def test_shared_corner_gather_scatter(svr):
     np.add.at(want, idx.reshape(-1), g.reshape(-1).astype(np.float64))
     np.testing.assert_allclose(gg.cpu().numpy(), want, rtol=1e-5, atol=1e-5)
     assert np.bincount(idx.reshape(-1)).max() == 8              # interior grid points are shared by 8 voxels
+
+
+def test_frame_refresh_colors(orc, svr):
+    """The topology is fixed between adaptation steps: after the parameters changed in place, svr_frame_refresh_colors
+    re-captures them without rebuilding the lists, and the render equals a fresh svr_preprocess of the new values."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    sc, cam = cfg.scene, cfg.cameras[1]
+    vox = pkg.Voxels.from_scene(sc)
+    frame = ctx.svr_preprocess(vox, cam)
+    img0, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min)
+    img0 = img0.clone()
+    rng = np.random.default_rng(12)
+    vox.raw.add_(torch.from_numpy(rng.normal(0, 0.4, sc.raw.shape).astype(np.float32)).cuda())
+    vox.sh.add_(torch.from_numpy(rng.normal(0, 0.1, sc.sh.shape).astype(np.float32)).cuda())
+    frame.refresh_colors()
+    img1, d1, t1 = ctx.svr_forward(frame, cfg.K, cfg.T_min)
+    fresh = ctx.svr_preprocess(vox, cam)
+    img2, d2, t2 = ctx.svr_forward(fresh, cfg.K, cfg.T_min)
+    ctx.synchronize()
+    assert float((img1 - img0).abs().max()) > 1e-3                          # the change is visible
+    np.testing.assert_array_equal(img1.cpu().numpy(), img2.cpu().numpy())    # and identical to a rebuilt frame
+    np.testing.assert_array_equal(d1.cpu().numpy(), d2.cpu().numpy())
+    from dataclasses import replace
+    new = replace(sc, raw=vox.raw.cpu().numpy(), sh=vox.sh.cpu().numpy())
+    ref = orc.render(new, cam, cfg.K, mode="bucketed")
+    assert max_rel(img1.cpu().numpy(), ref["image"]) <= IMG_TOL
+    frame.release(); fresh.release()
