@@ -220,7 +220,7 @@ def main():
     targets, targets_host = [], []
     for i, c in enumerate(ccams):
         fr = ctx.svr_preprocess(vox, c)
-        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False)
+        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False, record=False)
         ctx.synchronize()
         fr.release()
         rng = np.random.Generator(np.random.PCG64(cfg.seed * 100 + i))
@@ -240,7 +240,7 @@ def main():
     def render_step(i):
         k = camera_index(i, rank, len(ccams))
         fr = ctx.svr_preprocess(vox, ccams[k])
-        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False)
+        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, want_aux=False, record=False)      # render only: no backward follows
         fr.release()
 
     def e2e_step(i):

@@ -66,6 +66,10 @@ typedef struct {
 typedef struct {
     int32_t K;                /* 1..4 midpoint samples per ray segment (R5) */
     float T_min;              /* a ray stops after the first voxel that leaves T < T_min (R8); 0 = never */
+    int32_t record;           /* svr_forward: != 0 records the traversal (per warp and batch: staged list entries, slots
+                                 each pixel hit) in the frame; a following svr_backward with the same T_min replays it and
+                                 skips its own cull and test phases (training). 0: render only (about 4% faster).
+                                 Ignored by svr_backward: without a record it culls and tests itself. */
 } SvrRenderOpts;
 
 typedef struct {

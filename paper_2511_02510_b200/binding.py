@@ -44,7 +44,7 @@ class SvrCamera(C.Structure):
 
 
 class SvrRenderOpts(C.Structure):
-    _fields_ = [("K", C.c_int32), ("T_min", C.c_float)]
+    _fields_ = [("K", C.c_int32), ("T_min", C.c_float), ("record", C.c_int32)]
 
 
 class SvrPruneOpts(C.Structure):
@@ -272,7 +272,7 @@ class Context:
     def svr_forward_stats(self, frame: "Frame", K: int, T_min: float = 1e-5) -> dict:
         image = torch.empty((frame.H, frame.W, 3), dtype=torch.float32, device=frame.vox.raw.device)
         out = (C.c_uint64 * 4)()
-        o = SvrRenderOpts(K, T_min)
+        o = SvrRenderOpts(K, T_min, 1)
         self._check(_lib.svr_forward_stats(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(image), C.cast(out, C.c_void_p)))
         return dict(hits=int(out[0]), slab_tests=int(out[1]), warp_voxel_pairs=int(out[2]), entries_staged=int(out[3]))
 
@@ -297,7 +297,7 @@ class Context:
         return Frame(self, h.value, vox, c)
 
     def svr_forward(self, frame: Frame, K: int, T_min: float = 1e-5, w_max: Optional[torch.Tensor] = None,
-                    image=None, depth=None, T_final=None, want_aux: bool = True):
+                    image=None, depth=None, T_final=None, want_aux: bool = True, record: bool = True):
         dev = frame.vox.raw.device
         if image is None:
             image = torch.empty((frame.H, frame.W, 3), dtype=torch.float32, device=dev)
@@ -306,7 +306,7 @@ class Context:
                 depth = torch.empty((frame.H, frame.W), dtype=torch.float32, device=dev)
             if T_final is None:
                 T_final = torch.empty((frame.H, frame.W), dtype=torch.float32, device=dev)
-        o = SvrRenderOpts(K, T_min)
+        o = SvrRenderOpts(K, T_min, 1 if record else 0)
         self._check(_lib.svr_forward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(image), _p(depth), _p(T_final), _p(w_max)))
         return image, depth, T_final
 
@@ -329,13 +329,13 @@ class Context:
         _dev(image, torch.float32, "image")
         _dev(grad_raw, torch.float32, "grad_raw")
         _dev(grad_sh, torch.float32, "grad_sh")
-        o = SvrRenderOpts(K, T_min)
+        o = SvrRenderOpts(K, T_min, 1)
         self._check(_lib.svr_backward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(image), _p(grad_raw),
                                       _p(grad_sh), _p(w_max)))
 
     def svr_backward_heads(self, frame: "Frame", K: int, dL, image, grad_raw, grad_sh, T_min: float = 1e-5, w_max=None,
                            dL_ddepth=None, dL_dT=None, depth=None, T_final=None):
-        o = SvrRenderOpts(K, T_min)
+        o = SvrRenderOpts(K, T_min, 1)
         self._check(_lib.svr_backward_heads(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(dL_ddepth), _p(dL_dT), _p(image),
                                             _p(depth), _p(T_final), _p(grad_raw), _p(grad_sh), _p(w_max)))
 
@@ -344,7 +344,7 @@ class Context:
                             sobel_source: int = 0, image_host: Optional[torch.Tensor] = None) -> float:
         c = cam if isinstance(cam, SvrCamera) else make_camera(cam)
         assert not target_host.is_cuda and target_host.dtype == torch.float32 and target_host.is_contiguous()
-        ro, lo = SvrRenderOpts(K, T_min), SvrLossOpts(eps, percentile, sobel_source)
+        ro, lo = SvrRenderOpts(K, T_min, 1), SvrLossOpts(eps, percentile, sobel_source)
         loss = C.c_float()
         self._check(_lib.svr_train_view_host(self.handle, C.byref(vox.c), C.byref(c), C.byref(ro), C.byref(lo), gamma,
                                              _p(target_host), _p(grad_raw), _p(grad_sh), _p(w_max),

@@ -37,6 +37,7 @@ namespace {
 
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int RING = 64;          // staging slots per warp
+constexpr int TRAV_WORDS = SVR_TRAV_WORDS;   // words of one traversal record (forward -> backward), see composite_kernel
 constexpr int WARPS = 8;
 
 struct WarpStage {
@@ -197,7 +198,7 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
-template <int K, bool STATS>
+template <int K, bool STATS, bool REC>
 __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float4* __restrict__ packed,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
@@ -205,7 +206,8 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                                                         float T_min,
                                                         float* __restrict__ image, float* __restrict__ depth,
                                                         float* __restrict__ T_final, unsigned int* __restrict__ w_max,
-                                                        unsigned long long* __restrict__ stats) {
+                                                        unsigned long long* __restrict__ stats, uint32_t* __restrict__ trav,
+                                                        const uint32_t* __restrict__ trav_off, uint32_t* __restrict__ trav_count) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     WarpStage& S = reinterpret_cast<WarpStage*>(smem_raw)[warp];
@@ -227,6 +229,14 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
     }
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dep = 0.f;
     unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_read = 0;   // STATS only
+    // Traversal record for svr_backward (TRAV_WORDS words per batch: 32 hit masks, 32 list entries, the slot count): the
+    // backward pass replays the batches and skips its own cull and test phases. This warp's records are contiguous.
+    uint32_t* rec_out = nullptr;
+    uint32_t n_rec = 0;
+    if (REC) {
+        const uint32_t r0 = trav_off[tile], cap = (trav_off[tile + 1] - r0) >> 3;
+        rec_out = trav + ((size_t)r0 + (size_t)warp * cap) * TRAV_WORDS;
+    }
 
     for (int so = 0; so < 8; ++so) {
         const uint32_t start = ranges[(tile * 8 + so) * 2], end = ranges[(tile * 8 + so) * 2 + 1];
@@ -237,7 +247,7 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
         // Double-buffered staging: the ring is two halves of 32 slots. While one half is walked, the records of the
         // next batch are already on their way into the other half (cp.async: no registers held, no stall on the load).
         uint32_t base = start;
-        auto stage = [&](int half) -> int {
+        auto stage = [&](int half, uint32_t rec_i) -> int {
             int cnt = 0;
             while (cnt < 32 && base < end) {
                 const uint32_t idx = base + lane;
@@ -258,6 +268,7 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                     cp_async16(&S.g0[slot], rec); cp_async16(&S.g1[slot], rec + 1); cp_async16(&S.r0[slot], rec + 2);
                     cp_async16(&S.r1[slot], rec + 3); cp_async16(&S.col[slot], rec + 4);
                     S.M[slot] = M;
+                    if (REC) rec_out[(size_t)rec_i * TRAV_WORDS + 32 + cnt + rank] = idx;
                 }
                 if (STATS) { n_read += (idx < end && (int)lane < adv); n_surv += (M != 0u); }
                 cnt += __popc(m);
@@ -266,11 +277,11 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
             asm volatile("cp.async.commit_group;" ::: "memory");
             return cnt;
         };
-        int head = 0, count = stage(0);
+        int head = 0, count = stage(0, n_rec);
         while (count > 0) {
             asm volatile("cp.async.wait_all;" ::: "memory");
             __syncwarp();
-            const int count_next = stage(head ^ 32);                  // in flight during the walk below
+            const int count_next = stage(head ^ 32, n_rec + 1);       // in flight during the walk below
             // ---- walk up to 32 staged voxels, every lane through its own candidates ----
             const int n = count;
             unsigned int cand = transpose32(lane < n ? S.M[head + lane] : 0u, lane);
@@ -295,6 +306,12 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                         const float s1 = fminf(fminf(cx + wx, cy + wy), cz + wz);
                         if (s1 > s0) hits |= 1u << k;
                     }
+                }
+                if (REC) {
+                    uint32_t* r = rec_out + (size_t)n_rec * TRAV_WORDS;
+                    r[lane] = hits;                                    // the list entries were written when they were staged
+                    if (lane == 0) r[64] = (uint32_t)n;
+                    ++n_rec;
                 }
                 while (__any_sync(FULL, hits != 0u)) {
                     if (hits) {
@@ -338,6 +355,7 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
             if (lane == 0 && t) atomicAdd(stats + i, (unsigned long long)t);
         }
     }
+    if (REC && lane == 0) trav_count[tile * 8 + warp] = n_rec;
     if (inimg) {
         image[pix * 3] = fmaf(T, c.bg[0], C0);
         image[pix * 3 + 1] = fmaf(T, c.bg[1], C1);
@@ -405,7 +423,7 @@ __device__ __forceinline__ int warp_incl_scan_i(int v, int lane) {
     return v;
 }
 
-template <int K, bool HEADS>
+template <int K, bool HEADS, bool REPLAY>
 __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed,
                                                                const uint2* __restrict__ rects_sorted,
                                                                const uint32_t* __restrict__ ranges,
@@ -414,7 +432,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                                                                const float* __restrict__ image_in, float* __restrict__ grad_coef,
                                                                float* __restrict__ grad_rgb, const float* __restrict__ dL_ddepth,
                                                                const float* __restrict__ dL_dT, const float* __restrict__ depth_in,
-                                                               const float* __restrict__ T_in) {
+                                                               const float* __restrict__ T_in, const uint32_t* __restrict__ trav,
+                                                               const uint32_t* __restrict__ trav_off, const uint32_t* __restrict__ trav_count) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     WarpWork& S = reinterpret_cast<WarpWork*>(smem_raw)[warp];
@@ -458,6 +477,147 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     }
     __syncwarp();
     float Tpix = 1.f;
+    // steps 3-5 for the staged slots [head, head + n); returns the number of slots consumed (a batch is cut where the
+    // queue is full)
+    auto run_batch = [&](const unsigned int hits, int n, const int head) -> int {
+        // ---- 3. queue: slot-major positions from the transposed hit matrix ----
+        int nh;
+        {
+            const unsigned int H = transpose32(hits, lane);         // lane k: pixels that hit slot k
+            const int cnt = __popc(H);
+            const int inc = warp_incl_scan_i(cnt, lane);
+            n = min(n, __popc(__ballot_sync(FULL, inc <= QCAP)));  // cut the batch where the queue is full
+            nh = __shfl_sync(FULL, inc, n - 1);
+            S.Hs[lane] = make_uint2(H, (unsigned int)(inc - cnt));
+            __syncwarp();
+            unsigned int m = (n < 32) ? (hits & ((1u << n) - 1u)) : hits;
+            while (__any_sync(FULL, m != 0u)) {
+                if (m) {
+                    const int k = __ffs(m) - 1;
+                    m &= m - 1;
+                    const uint2 hk = S.Hs[k];
+                    S.q[hk.y + __popc(hk.x & lt)] = (unsigned short)((k << 5) | swl);
+                }
+            }
+        }
+        __syncwarp();
+        // ---- 4. hit rounds: one hit per lane ----
+        for (int r = 0; r < nh; r += 32) {
+            const bool valid = r + lane < nh;
+            const unsigned int e = valid ? (unsigned int)S.q[r + lane] : 0xFFFFu;
+            const int k = (int)(e >> 5);                         // slot inside the batch (2047 = no entry)
+            const int i = (int)(e & 31u);                        // swizzled pixel id
+            const int slot = (head + k) & (NSLOT - 1);
+            // hits of the same pixel inside this round are chained in slot (= lane) order; issued first so that
+            // the match latency hides behind the samples
+            const unsigned int peers = __match_any_sync(FULL, valid ? (unsigned int)i : 32u + (unsigned int)lane);
+            // hits of one voxel are contiguous lanes (a run): RED_STEPS steps of a segmented sum towards lower lanes,
+            // then every lane that starts a fragment of 2^RED_STEPS lanes of its run sends the fragment's sums
+            const int kprev = __shfl_up_sync(FULL, k, 1);
+            const unsigned int heads = __ballot_sync(FULL, lane == 0 || kprev != k);
+            const unsigned int above = (heads >> lane) >> 1;
+            const int rem = above ? __ffs(above) - 1 : 31 - lane;     // lanes after this one in its run
+            const int run_pos = lane - (31 - __clz(heads & (lt | (1u << lane))));
+            const bool frag_head = valid && (run_pos & ((1 << RED_STEPS) - 1)) == 0;
+            const uint32_t vid = valid ? __float_as_uint(S.g1[slot].w) : 0u;
+            // w_max only grows, so a stale guard read is safe; issued here so that its latency hides behind the samples
+            unsigned int wm_old = 0xFFFFFFFFu;
+            if (frag_head && w_max != nullptr) wm_old = w_max[vid];
+            float tau = 0.f, dtau[8], gc = 0.f;
+            float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) dtau[m] = 0.f;
+            if (valid) {
+                const float4 a = S.g0[slot], bq = S.g1[slot];
+                const float4 d = S.P0[i], dl = S.P1[i], iv = S.PI[i];
+                RayF rr;
+                rr.dh[0] = d.x; rr.dh[1] = d.y; rr.dh[2] = d.z;
+                rr.dl[0] = dl.x; rr.dl[1] = dl.y; rr.dl[2] = dl.z;
+                rr.inv[0] = iv.x; rr.inv[1] = iv.y; rr.inv[2] = iv.z;
+                rr.ainv[0] = fabsf(iv.x); rr.ainv[1] = fabsf(iv.y); rr.ainv[2] = fabsf(iv.z);
+                const float4 col = S.col[slot];
+                G = S.PG[i];
+                gc = G.x * col.x + G.y * col.y + G.z * col.z;
+                float s0, s1, t_ref, D[3];
+                if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
+                    const float4 ra = S.r0[slot], rb = S.r1[slot];
+                    tau = integrate<K, true>(rr, D, a.w, s0, s1, ra, rb, dtau);
+                    if (HEADS) gc = fmaf(S.PD[i], t_ref + 0.5f * (s0 + s1), gc);
+                }
+            }
+            const float E = ex2f(-1.4426950408889634f * tau);
+            const unsigned int lower = peers & lt;
+            const int level = __popc(lower);
+            const int pred = lower ? 31 - __clz(lower) : lane;
+            const int maxL = (int)__reduce_max_sync(FULL, (unsigned int)level);
+            float2 st = make_float2(0.f, 0.f);
+            if (valid && level == 0) st = S.ST[i];
+            float w = 0.f;
+            bool live = false;
+            for (int L = 0; L <= maxL; ++L) {
+                if (L > 0) {
+                    const float t0 = __shfl_sync(FULL, st.x, pred), t1 = __shfl_sync(FULL, st.y, pred);
+                    if (level == L) st = make_float2(t0, t1);
+                }
+                if (level == L) {
+                    live = valid && st.x >= T_min;                // R8: a ray stops after the voxel that crosses T_min
+                    w = live ? st.x * (1.f - E) : 0.f;
+                    st.x = live ? st.x * E : st.x;
+                    st.y = fmaf(w, gc, st.y);
+                }
+            }
+            if (valid && (peers >> lane) == 1u) S.ST[i] = st;     // last hit of its pixel in this round
+            // ---- 5. reduce ----
+            float v[11];
+            {
+                const float dLdtau = live ? fmaf(st.x, gc, st.y) - G.w : 0.f;
+#pragma unroll
+                for (int m = 0; m < 8; ++m) v[m] = dLdtau * dtau[m];
+                v[8] = w * G.x; v[9] = w * G.y; v[10] = w * G.z;
+            }
+            float wq = w;
+#pragma unroll
+            for (int s = 0; s < RED_STEPS; ++s) {
+                const int step = 1 << s;
+                const float take = (step <= rem) ? 1.f : 0.f;
+#pragma unroll
+                for (int m = 0; m < 11; ++m) v[m] = fmaf(take, __shfl_down_sync(FULL, v[m], step), v[m]);
+                wq = fmaxf(wq, take * __shfl_down_sync(FULL, wq, step));
+            }
+            if (frag_head && wq > 0.f) {
+                red_add_v4(grad_coef + (size_t)vid * 8, v[0], v[1], v[2], v[3]);
+                red_add_v4(grad_coef + (size_t)vid * 8 + 4, v[4], v[5], v[6], v[7]);
+                red_add_v4(grad_rgb + (size_t)vid * 4, v[8], v[9], v[10], 0.f);
+                if (__float_as_uint(wq) > wm_old) atomicMax(w_max + vid, __float_as_uint(wq));
+            }
+            __syncwarp();                                          // pixel state is reused by the next round
+        }
+        return n;
+    };
+
+    if (REPLAY) {
+        // The forward pass recorded, per batch, the list entries it staged and the slots every pixel hit: no cull, no test.
+        const uint32_t r0 = trav_off[tile], cap = (trav_off[tile + 1] - r0) >> 3;
+        const uint32_t* rec = trav + ((size_t)r0 + (size_t)warp * cap) * TRAV_WORDS;
+        const uint32_t n_rec = trav_count[tile * 8 + warp];
+        for (uint32_t rb = 0; rb < n_rec; ++rb, rec += TRAV_WORDS) {
+            const int n = (int)__ldg(rec + 64);
+            const unsigned int hits = __ldg(rec + lane);
+            if (__ballot_sync(FULL, hits != 0u) == 0u) continue;       // nothing hit in this batch
+            if (lane < n) {
+                const float4* pr = packed + 5 * (size_t)__ldg(rec + 32 + lane);
+                const float4 t0 = __ldg(pr), t1 = __ldg(pr + 1), t2 = __ldg(pr + 2), t3 = __ldg(pr + 3), t4 = __ldg(pr + 4);
+                const uint32_t vid = __float_as_uint(t1.w);
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
+                S.g0[lane] = t0; S.g1[lane] = t1; S.r0[lane] = t2; S.r1[lane] = t3; S.col[lane] = t4;
+            }
+            __syncwarp();
+            for (int k0 = 0; k0 < n;) k0 += run_batch(hits >> k0, n - k0, k0);
+            __syncwarp();
+        }
+        return;
+    }
 
     for (int so = 0; so < 8; ++so) {
         const uint32_t start = ranges[(tile * 8 + so) * 2], end = ranges[(tile * 8 + so) * 2 + 1];
@@ -519,118 +679,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     }
                 }
             }
-            // ---- 3. queue: slot-major positions from the transposed hit matrix ----
-            int nh;
-            {
-                const unsigned int H = transpose32(hits, lane);         // lane k: pixels that hit slot k
-                const int cnt = __popc(H);
-                const int inc = warp_incl_scan_i(cnt, lane);
-                n = min(n, __popc(__ballot_sync(FULL, inc <= QCAP)));  // cut the batch where the queue is full
-                nh = __shfl_sync(FULL, inc, n - 1);
-                S.Hs[lane] = make_uint2(H, (unsigned int)(inc - cnt));
-                __syncwarp();
-                unsigned int m = (n < 32) ? (hits & ((1u << n) - 1u)) : hits;
-                while (__any_sync(FULL, m != 0u)) {
-                    if (m) {
-                        const int k = __ffs(m) - 1;
-                        m &= m - 1;
-                        const uint2 hk = S.Hs[k];
-                        S.q[hk.y + __popc(hk.x & lt)] = (unsigned short)((k << 5) | swl);
-                    }
-                }
-            }
-            __syncwarp();
-            // ---- 4. hit rounds: one hit per lane ----
-            for (int r = 0; r < nh; r += 32) {
-                const bool valid = r + lane < nh;
-                const unsigned int e = valid ? (unsigned int)S.q[r + lane] : 0xFFFFu;
-                const int k = (int)(e >> 5);                         // slot inside the batch (2047 = no entry)
-                const int i = (int)(e & 31u);                        // swizzled pixel id
-                const int slot = (head + k) & (NSLOT - 1);
-                // hits of the same pixel inside this round are chained in slot (= lane) order; issued first so that
-                // the match latency hides behind the samples
-                const unsigned int peers = __match_any_sync(FULL, valid ? (unsigned int)i : 32u + (unsigned int)lane);
-                // hits of one voxel are contiguous lanes (a run): RED_STEPS steps of a segmented sum towards lower lanes,
-                // then every lane that starts a fragment of 2^RED_STEPS lanes of its run sends the fragment's sums
-                const int kprev = __shfl_up_sync(FULL, k, 1);
-                const unsigned int heads = __ballot_sync(FULL, lane == 0 || kprev != k);
-                const unsigned int above = (heads >> lane) >> 1;
-                const int rem = above ? __ffs(above) - 1 : 31 - lane;     // lanes after this one in its run
-                const int run_pos = lane - (31 - __clz(heads & (lt | (1u << lane))));
-                const bool frag_head = valid && (run_pos & ((1 << RED_STEPS) - 1)) == 0;
-                const uint32_t vid = valid ? __float_as_uint(S.g1[slot].w) : 0u;
-                // w_max only grows, so a stale guard read is safe; issued here so that its latency hides behind the samples
-                unsigned int wm_old = 0xFFFFFFFFu;
-                if (frag_head && w_max != nullptr) wm_old = w_max[vid];
-                float tau = 0.f, dtau[8], gc = 0.f;
-                float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                for (int m = 0; m < 8; ++m) dtau[m] = 0.f;
-                if (valid) {
-                    const float4 a = S.g0[slot], bq = S.g1[slot];
-                    const float4 d = S.P0[i], dl = S.P1[i], iv = S.PI[i];
-                    RayF rr;
-                    rr.dh[0] = d.x; rr.dh[1] = d.y; rr.dh[2] = d.z;
-                    rr.dl[0] = dl.x; rr.dl[1] = dl.y; rr.dl[2] = dl.z;
-                    rr.inv[0] = iv.x; rr.inv[1] = iv.y; rr.inv[2] = iv.z;
-                    rr.ainv[0] = fabsf(iv.x); rr.ainv[1] = fabsf(iv.y); rr.ainv[2] = fabsf(iv.z);
-                    const float4 col = S.col[slot];
-                    G = S.PG[i];
-                    gc = G.x * col.x + G.y * col.y + G.z * col.z;
-                    float s0, s1, t_ref, D[3];
-                    if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
-                        const float4 ra = S.r0[slot], rb = S.r1[slot];
-                        tau = integrate<K, true>(rr, D, a.w, s0, s1, ra, rb, dtau);
-                        if (HEADS) gc = fmaf(S.PD[i], t_ref + 0.5f * (s0 + s1), gc);
-                    }
-                }
-                const float E = ex2f(-1.4426950408889634f * tau);
-                const unsigned int lower = peers & lt;
-                const int level = __popc(lower);
-                const int pred = lower ? 31 - __clz(lower) : lane;
-                const int maxL = (int)__reduce_max_sync(FULL, (unsigned int)level);
-                float2 st = make_float2(0.f, 0.f);
-                if (valid && level == 0) st = S.ST[i];
-                float w = 0.f;
-                bool live = false;
-                for (int L = 0; L <= maxL; ++L) {
-                    if (L > 0) {
-                        const float t0 = __shfl_sync(FULL, st.x, pred), t1 = __shfl_sync(FULL, st.y, pred);
-                        if (level == L) st = make_float2(t0, t1);
-                    }
-                    if (level == L) {
-                        live = valid && st.x >= T_min;                // R8: a ray stops after the voxel that crosses T_min
-                        w = live ? st.x * (1.f - E) : 0.f;
-                        st.x = live ? st.x * E : st.x;
-                        st.y = fmaf(w, gc, st.y);
-                    }
-                }
-                if (valid && (peers >> lane) == 1u) S.ST[i] = st;     // last hit of its pixel in this round
-                // ---- 5. reduce ----
-                float v[11];
-                {
-                    const float dLdtau = live ? fmaf(st.x, gc, st.y) - G.w : 0.f;
-#pragma unroll
-                    for (int m = 0; m < 8; ++m) v[m] = dLdtau * dtau[m];
-                    v[8] = w * G.x; v[9] = w * G.y; v[10] = w * G.z;
-                }
-                float wq = w;
-#pragma unroll
-                for (int s = 0; s < RED_STEPS; ++s) {
-                    const int step = 1 << s;
-                    const float take = (step <= rem) ? 1.f : 0.f;
-#pragma unroll
-                    for (int m = 0; m < 11; ++m) v[m] = fmaf(take, __shfl_down_sync(FULL, v[m], step), v[m]);
-                    wq = fmaxf(wq, take * __shfl_down_sync(FULL, wq, step));
-                }
-                if (frag_head && wq > 0.f) {
-                    red_add_v4(grad_coef + (size_t)vid * 8, v[0], v[1], v[2], v[3]);
-                    red_add_v4(grad_coef + (size_t)vid * 8 + 4, v[4], v[5], v[6], v[7]);
-                    red_add_v4(grad_rgb + (size_t)vid * 4, v[8], v[9], v[10], 0.f);
-                    if (__float_as_uint(wq) > wm_old) atomicMax(w_max + vid, __float_as_uint(wq));
-                }
-                __syncwarp();                                          // pixel state is reused by the next round
-            }
+            n = run_batch(hits, n, head);
             head = (head + n) & (NSLOT - 1);
             count -= n;
             Tpix = S.ST[swl].x;
@@ -653,25 +702,26 @@ SvrStatus set_smem_once(SvrContext* ctx, KernelT kernel, size_t smem, bool* done
 }  // namespace
 
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
-                         float* w_max, unsigned long long* stats) {
+                         float* w_max, unsigned long long* stats, bool record) {
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, ST_FORWARD);
     const size_t smem = sizeof(WarpStage) * WARPS;
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
+    const bool rec = record && f->trav != nullptr;
+#define SVR_FWD_GO(KK, SS, RR)                                                                                       \
+    do {                                                                                                             \
+        static bool done = false;                                                                                    \
+        SVR_TRY(set_smem_once(ctx, composite_kernel<KK, SS, RR>, smem, &done));                                      \
+        composite_kernel<KK, SS, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, \
+                                                                             T_final, wm, stats, f->trav, f->trav_off, f->trav_count);       \
+    } while (0)
 #define SVR_FWD(KK)                                                                                                  \
     do {                                                                                                             \
-        static bool done_a = false, done_b = false;                                                                  \
-        if (stats) {                                                                                                 \
-            SVR_TRY(set_smem_once(ctx, composite_kernel<KK, true>, smem, &done_a));                                  \
-            composite_kernel<KK, true><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, \
-                                                                               T_final, wm, stats);                  \
-        } else {                                                                                                     \
-            SVR_TRY(set_smem_once(ctx, composite_kernel<KK, false>, smem, &done_b));                                 \
-            composite_kernel<KK, false><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, \
-                                                                                T_final, wm, stats);                 \
-        }                                                                                                            \
+        if (stats) SVR_FWD_GO(KK, true, false);                                                                      \
+        else if (rec) SVR_FWD_GO(KK, false, true);                                                                   \
+        else SVR_FWD_GO(KK, false, false);                                                                           \
     } while (0)
     switch (K) {
         case 1: SVR_FWD(1); break;
@@ -681,6 +731,7 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
         default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     }
 #undef SVR_FWD
+#undef SVR_FWD_GO
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
@@ -695,20 +746,23 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
+    // replay the forward pass's traversal record when there is one for this termination threshold
+    const bool replay = f->trav != nullptr && f->trav_valid && f->trav_T_min == T_min && (ctx->debug_flags & 16) == 0;
+    const bool heads = dL_ddepth != nullptr || dL_dT != nullptr;
+#define SVR_BWD_GO(KK, HH, RR)                                                                                       \
+    do {                                                                                                             \
+        static bool done = false;                                                                                    \
+        SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, HH, RR>, smem, &done));                                \
+        backward_packed_kernel<KK, HH, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(                                  \
+            f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth, T_final,         \
+            f->trav, f->trav_off, f->trav_count);                                                                    \
+    } while (0)
 #define SVR_BWD(KK)                                                                                                  \
     do {                                                                                                             \
-        static bool done = false, done_h = false;                                                                   \
-        if (dL_ddepth || dL_dT) {                                                                                    \
-            SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, true>, smem, &done_h));                            \
-            backward_packed_kernel<KK, true><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, \
-                                                                                     image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth,   \
-                                                                                     T_final);                        \
-        } else {                                                                                                     \
-            SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, false>, smem, &done));                             \
-            backward_packed_kernel<KK, false><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, \
-                                                                                      image, grad_coef, grad_rgb, nullptr, nullptr, nullptr, \
-                                                                                      nullptr);                       \
-        }                                                                                                            \
+        if (heads && replay) SVR_BWD_GO(KK, true, true);                                                             \
+        else if (heads) SVR_BWD_GO(KK, true, false);                                                                 \
+        else if (replay) SVR_BWD_GO(KK, false, true);                                                                \
+        else SVR_BWD_GO(KK, false, false);                                                                           \
     } while (0)
     switch (K) {
         case 1: SVR_BWD(1); break;
@@ -718,6 +772,7 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
         default: return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     }
 #undef SVR_BWD
+#undef SVR_BWD_GO
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;

@@ -255,6 +255,42 @@ __global__ void __launch_bounds__(1024) tile_order_kernel(const uint32_t* __rest
     for (int t = tid; t < n_tiles; t += 1024) tile_order[atomicAdd(&hist[1023u - (tile_len[t] >> shift)], 1u)] = (uint32_t)t;
 }
 
+// Record offsets of the traversal scratch (composite.cu: the forward pass records, per warp and batch, which list entries it
+// staged and which of them each pixel hit; the backward pass replays them). Tile t owns 8 * (ceil(len / 32) + 9) records,
+// one contiguous eighth per warp. One block of 1024 threads: exclusive scan in tile order.
+__global__ void __launch_bounds__(1024) trav_offsets_kernel(const uint32_t* __restrict__ tile_len, int n_tiles, uint32_t* __restrict__ trav_off) {
+    __shared__ uint32_t wsum[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int per = (n_tiles + 1023) / 1024, t0 = tid * per, t1 = min(n_tiles, t0 + per);
+    uint32_t local = 0;
+    for (int t = t0; t < t1; ++t) local += 8u * ((tile_len[t] + 31u) / 32u + 9u);
+    uint32_t inc = local;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = wsum[lane], a = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, a, o);
+            if (lane >= o) a += v;
+        }
+        wsum[lane] = a - w;
+    }
+    __syncthreads();
+    uint32_t run = wsum[warp] + inc - local;
+    for (int t = t0; t < t1; ++t) {
+        trav_off[t] = run;
+        run += 8u * ((tile_len[t] + 31u) / 32u + 9u);
+    }
+    if (t1 == n_tiles && t0 < n_tiles) trav_off[n_tiles] = run;
+    if (n_tiles == 0 && tid == 0) trav_off[0] = 0;
+}
+
 // ---- a3: per-view voxel colour (R6) -------------------------------------------------------------------
 // c_v = max(0, 0.5 + sum_i Y_i(dir_v) sh[v,i,:]); rgbm[v] = (r, g, b, clamp-mask bits).
 template <int DEG>
@@ -858,6 +894,10 @@ SvrStatus launch_ranges(SvrContext* ctx, SvrFrame* f) {
     }
     tile_order_kernel<<<1, 1024, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
     ctx->launches += 1;
+    if (f->trav_off) {
+        trav_offsets_kernel<<<1, 1024, 0, ctx->stream>>>(f->tile_order + f->n_tiles, f->n_tiles, f->trav_off);
+        ctx->launches += 1;
+    }
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }
@@ -960,6 +1000,10 @@ SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f) {
     StageScope scope__(ctx, ST_RANGES);
     tile_order_kernel<<<1, 1024, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
     ctx->launches += 1;
+    if (f->trav_off) {
+        trav_offsets_kernel<<<1, 1024, 0, ctx->stream>>>(f->tile_order + f->n_tiles, f->n_tiles, f->trav_off);
+        ctx->launches += 1;
+    }
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

@@ -103,9 +103,21 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 }
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
-    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed};
+    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed,
+                    f->trav, f->trav_off, f->trav_count};
     for (void* p : ptrs)
         if (p) svr_free(ctx, p, 0);
+    return SVR_OK;
+}
+
+// Traversal scratch (svr_forward records, svr_backward replays): at most E/4 + 80 n_tiles records of SVR_TRAV_WORDS words
+// (sum over tiles of 8 warps x (ceil(len / 32) + 9)). Debug flag 16 disables it (backward then culls and tests itself).
+SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
+    if (ctx->debug_flags & 16) return SVR_OK;
+    const size_t cap = (size_t)E / 4 + 80 * (size_t)f->n_tiles + 8;
+    SVR_TRY(svr_alloc(ctx, (void**)&f->trav, sizeof(uint32_t) * SVR_TRAV_WORDS * cap));
+    SVR_TRY(svr_alloc(ctx, (void**)&f->trav_off, sizeof(uint32_t) * (size_t)(f->n_tiles + 1)));
+    SVR_TRY(svr_alloc(ctx, (void**)&f->trav_count, sizeof(uint32_t) * 8 * (size_t)f->n_tiles));
     return SVR_OK;
 }
 
@@ -257,6 +269,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             big_bytes = sizeof(uint32_t) * (size_t)(n_big + 1);
             // frame-lifetime buffers first, largest first (the pool then reuses the previous frame's blocks one for one),
             // scratch last
+            TRYF(alloc_traversal(ctx, f, E));
             TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
             TRYF(svr_alloc(ctx, (void**)&keys_b, ka));   // canonical keys
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
@@ -317,6 +330,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             svr_free(ctx, big_list, big_bytes);
             big_list = nullptr;
             f->keys = ks; f->vals = vs;
+            TRYF(alloc_traversal(ctx, f, E));
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
             TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
             keys_a = keys_b = nullptr;
@@ -335,6 +349,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 
 SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame) {
     if (!ctx || !frame) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    frame->trav_valid = false;      // termination depends on the densities: the next forward pass records again
     SVR_TRY(launch_voxel_colors(ctx, frame));
     return launch_pack_entries(ctx, frame);
 }
@@ -349,7 +364,10 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
                       float* T_final, float* w_max) {
     if (!ctx || !frame || !opts || !image) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
-    return launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max, nullptr);
+    const bool record = opts->record != 0 && frame->trav != nullptr;
+    SvrStatus st = launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max, nullptr, record);
+    if (st == SVR_OK && record) { frame->trav_valid = true; frame->trav_T_min = opts->T_min; }
+    return st;
 }
 
 SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H, float gamma,
@@ -446,7 +464,7 @@ SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRen
     unsigned long long* d = nullptr;
     SVR_TRY(svr_alloc(ctx, (void**)&d, 64));
     cudaMemsetAsync(d, 0, 64, ctx->stream);
-    SvrStatus st = launch_forward(ctx, frame, opts->K, opts->T_min, image, nullptr, nullptr, nullptr, d);
+    SvrStatus st = launch_forward(ctx, frame, opts->K, opts->T_min, image, nullptr, nullptr, nullptr, d, false);
     if (st == SVR_OK) {
         cudaError_t e = cudaMemcpyAsync(stats_host, d, 32, cudaMemcpyDeviceToHost, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);

@@ -11,6 +11,7 @@
 
 #define SVR_TILE 16
 #define SVR_MAX_K 4
+#define SVR_TRAV_WORDS 68     // traversal record: 32 hit masks, 32 list entries, slot count (+ padding to 16 bytes)
 
 enum SvrStage {
     ST_TILE_MASKS = 0, ST_RECTS, ST_SCAN, ST_EMIT, ST_SORT, ST_RANGES, ST_COLORS, ST_FORWARD, ST_LOSS, ST_BACKWARD,
@@ -81,6 +82,12 @@ struct SvrFrame {
     uint32_t* ranges = nullptr;      // [n_tiles*8*2]
     float* packed = nullptr;         // [E,20] per-entry voxel record in list order (composite.cu pack_entries_kernel)
     uint32_t* tile_order = nullptr;  // [2*n_tiles]: tile ids by descending list length, then the lengths
+    // traversal scratch written by svr_forward, replayed by svr_backward (composite.cu)
+    uint32_t* trav = nullptr;        // [trav_cap, SVR_TRAV_WORDS] records
+    uint32_t* trav_off = nullptr;    // [n_tiles + 1] first record of each tile
+    uint32_t* trav_count = nullptr;  // [n_tiles * 8] records written per warp
+    mutable bool trav_valid = false; // a forward pass has recorded this frame's traversal ...
+    mutable float trav_T_min = 0.f;  // ... with this termination threshold
     size_t bytes = 0;
 };
 
@@ -137,7 +144,7 @@ SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
-                         float* T_final, float* w_max, unsigned long long* stats);
+                         float* T_final, float* w_max, unsigned long long* stats, bool record);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
                           float* grad_coef, float* grad_rgb, float* w_max, const float* dL_ddepth, const float* dL_dT,
                           const float* depth, const float* T_final);

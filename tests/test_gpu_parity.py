@@ -577,3 +577,27 @@ def test_frame_refresh_colors(orc, svr):
     ref = orc.render(new, cam, cfg.K, mode="bucketed")
     assert max_rel(img1.cpu().numpy(), ref["image"]) <= IMG_TOL
     frame.release(); fresh.release()
+
+
+def test_backward_with_and_without_traversal_record(orc, svr):
+    """svr_forward(record=1) lets svr_backward replay the traversal; without a record (render-only forward, or another
+    T_min) it culls and tests itself. Both must give the oracle's gradients, and the same w_max."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    sc, cam = cfg.scene, cfg.cameras[2]
+    vox = pkg.Voxels.from_scene(sc)
+    G = random_grad = np.random.default_rng(6).normal(0, 1.0 / (cam.W * cam.H), size=(cam.H, cam.W, 3)).astype(np.float32)
+    r_raw, r_sh = orc.backward(sc, cam, cfg.K, G.astype(np.float64), mode="bucketed")
+    outs = []
+    for record, T_min_bwd in [(True, cfg.T_min), (False, cfg.T_min), (True, 0.5 * cfg.T_min)]:
+        frame = ctx.svr_preprocess(vox, cam)
+        image, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min, record=record)
+        g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+        g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+        w_max = torch.zeros(sc.n, dtype=torch.float32, device="cuda")
+        ctx.svr_backward(frame, cfg.K, torch.from_numpy(G).cuda(), image, g_raw, g_sh, T_min_bwd, w_max=w_max)
+        ctx.synchronize()
+        assert rel_l2(g_raw.cpu().numpy(), r_raw) <= GRAD_TOL and rel_l2(g_sh.cpu().numpy(), r_sh) <= GRAD_TOL
+        outs.append(w_max.cpu().numpy())
+        frame.release()
+    np.testing.assert_array_equal(outs[0], outs[1])              # replayed and recomputed traversals are the same traversal
