@@ -385,8 +385,10 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
 //   5. reduce: hits of one voxel are contiguous lanes, so two steps of a segmented shuffle sum give every
 //      fragment of up to 4 consecutive hits of a voxel one set of three red.global.add.v4.f32: a voxel that
 //      covers 7 of the warp's pixels leaves as 2 reduction sets instead of 7.
-// Pixel tables are indexed by a swizzled pixel id (row y rotated by 3y) so that the pixels of a small
-// rectangle fall into different shared-memory bank groups.
+// With the traversal record the kernel is bound by the shared-memory pipe (loads of the per-pixel and per-slot data and
+// the shuffles): the per-pixel data are 8-byte columns indexed by a swizzled pixel id, so that the pixels of a small
+// rectangle read distinct banks (6 conflict-free 8-byte loads instead of 4 conflicting 16-byte loads per hit), and the
+// per-pixel constant of dL/dtau is folded into the chained scalar P.
 constexpr int QCAP = 512;          // queue entries per warp (a batch is cut so that its hits fit)
 #ifndef SVR_RED_STEPS
 #define SVR_RED_STEPS 3
@@ -404,11 +406,9 @@ struct WarpWork {
     float4 r0[NSLOT];   // log2(e) * (c0, cx, cy, cz)
     float4 r1[NSLOT];   // log2(e) * (cxy, cxz, cyz, cxyz)
     float4 col[NSLOT];  // r, g, b, cover mask M of this warp's 8x4 block
-    float4 P0[32];      // per pixel (swizzled index): dh.xyz
-    float4 P1[32];      //   dl.xyz
-    float4 PI[32];      //   1/dh.xyz
-    float4 PG[32];      //   G = dL/dC, and G . C_final
-    float2 ST[32];      //   T, P = G . C (+ gD . D with the depth head)
+    float2 A[6][32];    // per pixel (swizzled index), 8-byte columns so that distinct pixels fall into distinct banks:
+                        //   (dh.x, dh.y) (dh.z, dl.x) (dl.y, dl.z) (1/dh.x, 1/dh.y) (1/dh.z, G.x) (G.y, G.z), G = dL/dC
+    float2 ST[32];      //   T, P = G . C (+ gD . D with the depth head) - G . C_final (- the heads' constants)
     float PD[32];       //   gD = dL/dDepth (kernels with HEADS only)
     uint2 Hs[32];       // per slot of the batch: pixels that hit it, queue offset
     unsigned short q[QCAP];
@@ -444,7 +444,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     const bool inimg = px < c.W && py < c.H;
     const size_t pix = (size_t)py * c.W + px;
     const unsigned int lt = (1u << lane) - 1u;
-    const int swl = (lane & 24) | ((lane + 3 * (lane >> 3)) & 7);     // this pixel's row in the tables
+    const int swl = (lane & 16) | ((lane + 5 * (lane >> 4)) & 15);    // this pixel's row in the tables: pixels (x, y) and
+                                                                      // (x, y + 2) of one rectangle use different banks
 
     int oct = -1;
     float dh[3], inv[3], ainv[3];
@@ -468,12 +469,14 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
         }
 #pragma unroll
         for (int a = 0; a < 3; ++a) { dh[a] = ray.dh[a]; inv[a] = ray.inv[a]; ainv[a] = ray.ainv[a]; }
-        S.P0[swl] = make_float4(ray.dh[0], ray.dh[1], ray.dh[2], 0.f);
-        S.P1[swl] = make_float4(ray.dl[0], ray.dl[1], ray.dl[2], 0.f);
-        S.PI[swl] = make_float4(ray.inv[0], ray.inv[1], ray.inv[2], 0.f);
-        S.PG[swl] = g;
+        S.A[0][swl] = make_float2(ray.dh[0], ray.dh[1]);
+        S.A[1][swl] = make_float2(ray.dh[2], ray.dl[0]);
+        S.A[2][swl] = make_float2(ray.dl[1], ray.dl[2]);
+        S.A[3][swl] = make_float2(ray.inv[0], ray.inv[1]);
+        S.A[4][swl] = make_float2(ray.inv[2], g.x);
+        S.A[5][swl] = make_float2(g.y, g.z);
         if (HEADS) S.PD[swl] = gdep;
-        S.ST[swl] = make_float2(1.f, 0.f);
+        S.ST[swl] = make_float2(1.f, -g.w);      // the per-pixel constant of dL/dtau rides in P
     }
     __syncwarp();
     float Tpix = 1.f;
@@ -529,14 +532,14 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             for (int m = 0; m < 8; ++m) dtau[m] = 0.f;
             if (valid) {
                 const float4 a = S.g0[slot], bq = S.g1[slot];
-                const float4 d = S.P0[i], dl = S.P1[i], iv = S.PI[i];
+                const float2 a0 = S.A[0][i], a1 = S.A[1][i], a2 = S.A[2][i], a3 = S.A[3][i], a4 = S.A[4][i], a5 = S.A[5][i];
                 RayF rr;
-                rr.dh[0] = d.x; rr.dh[1] = d.y; rr.dh[2] = d.z;
-                rr.dl[0] = dl.x; rr.dl[1] = dl.y; rr.dl[2] = dl.z;
-                rr.inv[0] = iv.x; rr.inv[1] = iv.y; rr.inv[2] = iv.z;
-                rr.ainv[0] = fabsf(iv.x); rr.ainv[1] = fabsf(iv.y); rr.ainv[2] = fabsf(iv.z);
+                rr.dh[0] = a0.x; rr.dh[1] = a0.y; rr.dh[2] = a1.x;
+                rr.dl[0] = a1.y; rr.dl[1] = a2.x; rr.dl[2] = a2.y;
+                rr.inv[0] = a3.x; rr.inv[1] = a3.y; rr.inv[2] = a4.x;
+                rr.ainv[0] = fabsf(a3.x); rr.ainv[1] = fabsf(a3.y); rr.ainv[2] = fabsf(a4.x);
                 const float4 col = S.col[slot];
-                G = S.PG[i];
+                G = make_float4(a4.y, a5.x, a5.y, 0.f);
                 gc = G.x * col.x + G.y * col.y + G.z * col.z;
                 float s0, s1, t_ref, D[3];
                 if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
@@ -570,7 +573,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             // ---- 5. reduce ----
             float v[11];
             {
-                const float dLdtau = live ? fmaf(st.x, gc, st.y) - G.w : 0.f;
+                const float dLdtau = live ? fmaf(st.x, gc, st.y) : 0.f;
 #pragma unroll
                 for (int m = 0; m < 8; ++m) v[m] = dLdtau * dtau[m];
                 v[8] = w * G.x; v[9] = w * G.y; v[10] = w * G.z;
