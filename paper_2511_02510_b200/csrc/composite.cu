@@ -386,9 +386,9 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
 //      fragment of up to 4 consecutive hits of a voxel one set of three red.global.add.v4.f32: a voxel that
 //      covers 7 of the warp's pixels leaves as 2 reduction sets instead of 7.
 // With the traversal record the kernel is bound by the shared-memory pipe (loads of the per-pixel and per-slot data and
-// the shuffles): the per-pixel data are 8-byte columns indexed by a swizzled pixel id, so that the pixels of a small
-// rectangle read distinct banks (6 conflict-free 8-byte loads instead of 4 conflicting 16-byte loads per hit), and the
-// per-pixel constant of dL/dtau is folded into the chained scalar P.
+// the shuffles): the per-pixel data are 4-byte columns (32 pixels = 32 banks: any set of pixels loads in one
+// conflict-free wavefront, 12 per hit round instead of ~24 for four 16-byte rows), and the per-pixel constant of dL/dtau is
+// folded into the chained scalar P.
 constexpr int QCAP = 512;          // queue entries per warp (a batch is cut so that its hits fit)
 #ifndef SVR_RED_STEPS
 #define SVR_RED_STEPS 3
@@ -406,9 +406,10 @@ struct WarpWork {
     float4 r0[NSLOT];   // log2(e) * (c0, cx, cy, cz)
     float4 r1[NSLOT];   // log2(e) * (cxy, cxz, cyz, cxyz)
     float4 col[NSLOT];  // r, g, b, cover mask M of this warp's 8x4 block
-    float2 A[6][32];    // per pixel (swizzled index), 8-byte columns so that distinct pixels fall into distinct banks:
-                        //   (dh.x, dh.y) (dh.z, dl.x) (dl.y, dl.z) (1/dh.x, 1/dh.y) (1/dh.z, G.x) (G.y, G.z), G = dL/dC
-    float2 ST[32];      //   T, P = G . C (+ gD . D with the depth head) - G . C_final (- the heads' constants)
+    float A[12][32];    // per pixel, 4-byte columns: 32 pixels = 32 banks, so a load of any set of pixels is one
+                        // conflict-free wavefront: dh.xyz, dl.xyz, 1/dh.xyz, G.xyz (G = dL/dC)
+    float T[32];        //   transmittance
+    float Pp[32];       //   P = G . C (+ gD . D with the depth head) - G . C_final (- the heads' constants)
     float PD[32];       //   gD = dL/dDepth (kernels with HEADS only)
     uint2 Hs[32];       // per slot of the batch: pixels that hit it, queue offset
     unsigned short q[QCAP];
@@ -444,8 +445,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     const bool inimg = px < c.W && py < c.H;
     const size_t pix = (size_t)py * c.W + px;
     const unsigned int lt = (1u << lane) - 1u;
-    const int swl = (lane & 16) | ((lane + 5 * (lane >> 4)) & 15);    // this pixel's row in the tables: pixels (x, y) and
-                                                                      // (x, y + 2) of one rectangle use different banks
+    const int swl = lane;                                             // this pixel's row in the tables
 
     int oct = -1;
     float dh[3], inv[3], ainv[3];
@@ -469,14 +469,12 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
         }
 #pragma unroll
         for (int a = 0; a < 3; ++a) { dh[a] = ray.dh[a]; inv[a] = ray.inv[a]; ainv[a] = ray.ainv[a]; }
-        S.A[0][swl] = make_float2(ray.dh[0], ray.dh[1]);
-        S.A[1][swl] = make_float2(ray.dh[2], ray.dl[0]);
-        S.A[2][swl] = make_float2(ray.dl[1], ray.dl[2]);
-        S.A[3][swl] = make_float2(ray.inv[0], ray.inv[1]);
-        S.A[4][swl] = make_float2(ray.inv[2], g.x);
-        S.A[5][swl] = make_float2(g.y, g.z);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { S.A[a][swl] = ray.dh[a]; S.A[3 + a][swl] = ray.dl[a]; S.A[6 + a][swl] = ray.inv[a]; }
+        S.A[9][swl] = g.x; S.A[10][swl] = g.y; S.A[11][swl] = g.z;
         if (HEADS) S.PD[swl] = gdep;
-        S.ST[swl] = make_float2(1.f, -g.w);      // the per-pixel constant of dL/dtau rides in P
+        S.T[swl] = 1.f;
+        S.Pp[swl] = -g.w;                        // the per-pixel constant of dL/dtau rides in P
     }
     __syncwarp();
     float Tpix = 1.f;
@@ -532,14 +530,14 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             for (int m = 0; m < 8; ++m) dtau[m] = 0.f;
             if (valid) {
                 const float4 a = S.g0[slot], bq = S.g1[slot];
-                const float2 a0 = S.A[0][i], a1 = S.A[1][i], a2 = S.A[2][i], a3 = S.A[3][i], a4 = S.A[4][i], a5 = S.A[5][i];
                 RayF rr;
-                rr.dh[0] = a0.x; rr.dh[1] = a0.y; rr.dh[2] = a1.x;
-                rr.dl[0] = a1.y; rr.dl[1] = a2.x; rr.dl[2] = a2.y;
-                rr.inv[0] = a3.x; rr.inv[1] = a3.y; rr.inv[2] = a4.x;
-                rr.ainv[0] = fabsf(a3.x); rr.ainv[1] = fabsf(a3.y); rr.ainv[2] = fabsf(a4.x);
+#pragma unroll
+                for (int ax = 0; ax < 3; ++ax) {
+                    rr.dh[ax] = S.A[ax][i]; rr.dl[ax] = S.A[3 + ax][i]; rr.inv[ax] = S.A[6 + ax][i];
+                    rr.ainv[ax] = fabsf(rr.inv[ax]);
+                }
                 const float4 col = S.col[slot];
-                G = make_float4(a4.y, a5.x, a5.y, 0.f);
+                G = make_float4(S.A[9][i], S.A[10][i], S.A[11][i], 0.f);
                 gc = G.x * col.x + G.y * col.y + G.z * col.z;
                 float s0, s1, t_ref, D[3];
                 if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
@@ -554,7 +552,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             const int pred = lower ? 31 - __clz(lower) : lane;
             const int maxL = (int)__reduce_max_sync(FULL, (unsigned int)level);
             float2 st = make_float2(0.f, 0.f);
-            if (valid && level == 0) st = S.ST[i];
+            if (valid && level == 0) st = make_float2(S.T[i], S.Pp[i]);
             float w = 0.f;
             bool live = false;
             for (int L = 0; L <= maxL; ++L) {
@@ -569,7 +567,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     st.y = fmaf(w, gc, st.y);
                 }
             }
-            if (valid && (peers >> lane) == 1u) S.ST[i] = st;     // last hit of its pixel in this round
+            if (valid && (peers >> lane) == 1u) { S.T[i] = st.x; S.Pp[i] = st.y; }    // last hit of its pixel in this round
             // ---- 5. reduce ----
             float v[11];
             {
@@ -685,7 +683,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             n = run_batch(hits, n, head);
             head = (head + n) & (NSLOT - 1);
             count -= n;
-            Tpix = S.ST[swl].x;
+            Tpix = S.T[swl];
             alive = inimg && (oct == so) && (Tpix >= T_min);
             alive_mask = __ballot_sync(FULL, alive);
             if (alive_mask == 0u) break;                              // whole warp terminated
