@@ -294,15 +294,10 @@ __global__ void __launch_bounds__(1024) trav_offsets_kernel(const uint32_t* __re
 // ---- a3: per-view voxel colour (R6) -------------------------------------------------------------------
 // c_v = max(0, 0.5 + sum_i Y_i(dir_v) sh[v,i,:]); rgbm[v] = (r, g, b, clamp-mask bits).
 template <int DEG>
-__global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
-                                                          float4* __restrict__ rgbm) {
-    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= s.n) return;
-    ushort4 r = rects[v];
-    if (r.x > r.z) return;                                   // not visible in this view: never read
+__device__ __forceinline__ float4 voxel_color_dev(const SceneDev& s, const CamDev& c, uint2 q, int64_t v) {
     constexpr int NB = (DEG + 1) * (DEG + 1);
     float dx, dy, dz, Y[NB];
-    voxel_dir_dev(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v], dx, dy, dz);
+    voxel_dir_dev(s, c, q, dx, dy, dz);
     sh_basis_dev(DEG, dx, dy, dz, Y);
     const float* p = s.sh + v * (NB * 3);
     float acc[3] = {0.5f, 0.5f, 0.5f};
@@ -323,7 +318,17 @@ __global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, 
         for (int idx = 0; idx < NB * 3; ++idx) acc[idx % 3] = fmaf(Y[idx / 3], __ldg(p + idx), acc[idx % 3]);
     }
     unsigned mask = (acc[0] > 0.f ? 1u : 0u) | (acc[1] > 0.f ? 2u : 0u) | (acc[2] > 0.f ? 4u : 0u);
-    rgbm[v] = make_float4(fmaxf(acc[0], 0.f), fmaxf(acc[1], 0.f), fmaxf(acc[2], 0.f), __uint_as_float(mask));
+    return make_float4(fmaxf(acc[0], 0.f), fmaxf(acc[1], 0.f), fmaxf(acc[2], 0.f), __uint_as_float(mask));
+}
+
+template <int DEG>
+__global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                          float4* __restrict__ rgbm) {
+    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    ushort4 r = rects[v];
+    if (r.x > r.z) return;                                   // not visible in this view: never read
+    rgbm[v] = voxel_color_dev<DEG>(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v], v);
 }
 
 // ---- a10: per-voxel backward finalize ---------------------------------------------------------------
@@ -448,14 +453,20 @@ constexpr int SORT_CAP_BIG = 12288;   // same with one 1024-thread block per SM;
 constexpr int SMALL_CAP = 256;        // buckets up to this size: bitonic network
 constexpr int SORT_THREADS2 = 512;
 
+// The per-view colour (a3) of a visible voxel is computed here too: its 12 (D+1)^2-byte read overlaps the division-heavy
+// projection of other warps instead of taking a pass of its own.
+template <int DEG>
 __global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamDev c, const uint8_t* __restrict__ masks,
                                                                 ushort4* __restrict__ rects, uint32_t* __restrict__ bcount,
-                                                                int* __restrict__ bigdiff, unsigned long long* __restrict__ totals) {
+                                                                int* __restrict__ bigdiff, unsigned long long* __restrict__ totals,
+                                                                float4* __restrict__ rgbm) {
     int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= s.n) return;
-    ushort4 r = voxel_rect(s, c, reinterpret_cast<const uint2*>(s.ijkl)[v]);
+    const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+    ushort4 r = voxel_rect(s, c, q);
     rects[v] = r;
     if (r.x > r.z) return;
+    rgbm[v] = voxel_color_dev<DEG>(s, c, q, v);
     const int i0 = r.x >> 4, i1 = r.z >> 4, j0 = r.y >> 4, j1 = r.w >> 4;
     if ((i1 - i0 + 1) * (j1 - j0 + 1) > BIG_TILES) {
         const int sx = c.tiles_x + 1;
@@ -944,8 +955,15 @@ SvrStatus launch_bucket_count(SvrContext* ctx, SvrFrame* f, uint32_t* bcount, in
                               unsigned long long* totals) {
     if (f->scene.n > 0) {
         StageScope scope__(ctx, ST_RECTS);
-        rect_bucket_count_kernel<<<blocks_for(f->scene.n, 256), 256, 0, ctx->stream>>>(
-            f->scene, f->cam, f->tile_masks, reinterpret_cast<ushort4*>(f->rects), bcount, bigdiff, totals);
+        const unsigned int g = blocks_for(f->scene.n, 256);
+        ushort4* r = reinterpret_cast<ushort4*>(f->rects);
+        float4* col = reinterpret_cast<float4*>(f->rgbm);
+        switch (f->scene.sh_degree) {
+            case 0: rect_bucket_count_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
+            case 1: rect_bucket_count_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
+            case 2: rect_bucket_count_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
+            default: rect_bucket_count_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
+        }
         ctx->launches += 1;
     }
     {

@@ -257,7 +257,6 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         TRYF(launch_bucket_count(ctx, f, bcount, bigdiff, nonempty, totals));
         // E, the number of many-tile voxels and the number of non-empty buckets: one small readback sizes the lists
         CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 32, cudaMemcpyDeviceToHost, ctx->stream));
-        TRYF(launch_voxel_colors(ctx, f));     // independent of E: overlaps the readback
         CUDAF(cudaStreamSynchronize(ctx->stream));
         const int64_t E = (int64_t)ctx->host_pinned[0];
         const int64_t n_big = (int64_t)ctx->host_pinned[1];
