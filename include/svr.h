@@ -88,8 +88,8 @@ int64_t svr_kernel_launches(const SvrContext* ctx);
 
 /* (1)+(2) of the path: per-voxel projection to pixel rectangles and (tile, octant) bucket counts (B1), per-view SH
  * colour c_v (R6), key build (tile | direction octant | direction-flipped Morton code, B3), per-bucket device
- * sort, per-(tile,octant) ranges (B4), and a per-entry record of the voxel (geometry relative to the camera,
- * density coefficients, colour) in list order. The frame borrows `vox` pointers: keep them alive and the
+ * sort, per-(tile,octant) ranges (B4), and a per-voxel view record (geometry relative to the camera,
+ * density coefficients, colour) that the compositing kernels gather by voxel id. The frame borrows `vox` pointers: keep them alive and the
  * topology (ijkl) unchanged until svr_frame_release. raw_density / sh VALUES are captured by svr_preprocess;
  * svr_frame_refresh_colors re-captures them (colours + records) after they changed, without redoing the lists. */
 SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam, SvrFrame** out);

@@ -74,16 +74,16 @@ __device__ __forceinline__ void setup_ray(const CamDev& c, int px, int py, RayF&
     }
 }
 
-// Per list entry, once per view: everything the compositing warps need about the voxel, in list order
-// (5 x 16 B): centre relative to the camera as hi+lo floats (fp64 arithmetic), half edge, voxel id,
-// the trilinear raw density as polynomial coefficients * log2(e), and the per-view colour.
-__global__ void __launch_bounds__(256) pack_entries_kernel(SceneDev s, CamDev c, const uint32_t* __restrict__ vals, int64_t n,
-                                                           const float4* __restrict__ rgbm, float4* __restrict__ packed,
-                                                           const uint2* __restrict__ rects, uint2* __restrict__ rects_sorted) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const uint32_t vid = __ldg(vals + i);
-    rects_sorted[i] = __ldg(rects + vid);         // rectangle in list order: the compositing cull reads it coalesced
+// Per visible voxel, once per view: everything the compositing warps need about it (5 x 16 B): centre relative to the
+// camera as hi+lo floats (fp64 arithmetic), half edge, voxel id, the trilinear raw density as polynomial coefficients
+// * log2(e), and the per-view colour. The compositing warps gather these records by voxel id.
+__global__ void __launch_bounds__(256) voxel_record_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
+                                                           const float4* __restrict__ rgbm, float4* __restrict__ vrec) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    const ushort4 r = rects[v];
+    if (r.x > r.z) return;                                   // not visible in this view: never read
+    const uint32_t vid = (uint32_t)v;
     uint2 q = __ldg(reinterpret_cast<const uint2*>(s.ijkl) + vid);
     const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
     float4 ra = __ldg(rp), rb = __ldg(rp + 1), col = __ldg(rgbm + vid);
@@ -99,12 +99,19 @@ __global__ void __launch_bounds__(256) pack_entries_kernel(SceneDev s, CamDev c,
     float c0 = ra.x, cx = ra.y - ra.x, cy = ra.z - ra.x, cz = rb.x - ra.x;
     float cxy = (ra.w - ra.y) - cy, cxz = (rb.y - ra.y) - cz, cyz = (rb.z - ra.z) - cz;
     float cxyz = ((rb.w - rb.z) - (rb.y - rb.x)) - ((ra.w - ra.z) - (ra.y - ra.x));
-    float4* out = packed + 5 * i;
+    float4* out = vrec + 5 * (size_t)vid;
     out[0] = make_float4(hx, hy, hz, 0.5f * ef);
     out[1] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
     out[2] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
     out[3] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
     out[4] = col;
+}
+
+// rectangle in list order: the compositing cull reads it coalesced
+__global__ void __launch_bounds__(256) gather_rects_kernel(const uint32_t* __restrict__ vals, int64_t n, const uint2* __restrict__ rects,
+                                                           uint2* __restrict__ rects_sorted) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) rects_sorted[i] = __ldg(rects + __ldg(vals + i));
 }
 
 // 32-bit mask of the lanes (pixel = (wbx0 + (lane & 7), wby0 + (lane >> 3))) inside the rectangle.
@@ -199,7 +206,7 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, 
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 template <int K, bool STATS, bool REC>
-__global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float4* __restrict__ packed,
+__global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
                                                         const uint32_t* __restrict__ tile_order,
@@ -229,7 +236,7 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
     }
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dep = 0.f;
     unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_read = 0;   // STATS only
-    // Traversal record for svr_backward (TRAV_WORDS words per batch: 32 hit masks, 32 list entries, the slot count): the
+    // Traversal record for svr_backward (TRAV_WORDS words per batch: 32 hit masks, 32 voxel ids, the slot count): the
     // backward pass replays the batches and skips its own cull and test phases. This warp's records are contiguous.
     uint32_t* rec_out = nullptr;
     uint32_t n_rec = 0;
@@ -253,7 +260,8 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                 const uint32_t idx = base + lane;
                 if (lane < 2) asm volatile("prefetch.global.L1 [%0];" ::"l"(rects_sorted + min(base + 64u + 16u * lane, end - 1u)));   // two chunks ahead
                 unsigned int M = 0u;
-                if (idx < end) M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
+                uint32_t vid = 0u;
+                if (idx < end) { M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask; vid = __ldg(vals + idx); }
                 unsigned int m = __ballot_sync(FULL, M != 0u);
                 const int rank = __popc(m & ((1u << lane) - 1u));
                 int adv = 32;
@@ -263,12 +271,12 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                     adv = 32 - __clz(m);                               // resume after the last survivor taken
                 }
                 if (M) {
-                    const float4* rec = packed + 5 * (size_t)idx;
+                    const float4* rec = packed + 5 * (size_t)vid;
                     const int slot = half + cnt + rank;
                     cp_async16(&S.g0[slot], rec); cp_async16(&S.g1[slot], rec + 1); cp_async16(&S.r0[slot], rec + 2);
                     cp_async16(&S.r1[slot], rec + 3); cp_async16(&S.col[slot], rec + 4);
                     S.M[slot] = M;
-                    if (REC) rec_out[(size_t)rec_i * TRAV_WORDS + 32 + cnt + rank] = idx;
+                    if (REC) rec_out[(size_t)rec_i * TRAV_WORDS + 32 + cnt + rank] = vid;
                 }
                 if (STATS) { n_read += (idx < end && (int)lane < adv); n_surv += (M != 0u); }
                 cnt += __popc(m);
@@ -425,7 +433,7 @@ __device__ __forceinline__ int warp_incl_scan_i(int v, int lane) {
 }
 
 template <int K, bool HEADS, bool REPLAY>
-__global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed,
+__global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
                                                                const uint2* __restrict__ rects_sorted,
                                                                const uint32_t* __restrict__ ranges,
                                                                const uint32_t* __restrict__ tile_order, float T_min,
@@ -633,7 +641,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             while (count < NSLOT && base < end) {
                 const uint32_t idx = base + lane;
                 unsigned int M = 0u;
-                if (idx < end) M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask;
+                uint32_t vid_e = 0u;
+                if (idx < end) { M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask; vid_e = __ldg(vals + idx); }
                 unsigned int m = __ballot_sync(FULL, M != 0u);
                 const int rank = __popc(m & lt);
                 int adv = 32;
@@ -643,7 +652,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     adv = 32 - __clz(m);                               // resume after the last survivor taken
                 }
                 if (M) {
-                    const float4* rec = packed + 5 * (size_t)idx;
+                    const float4* rec = packed + 5 * (size_t)vid_e;
                     const float4 t0 = __ldg(rec), t1 = __ldg(rec + 1), t2 = __ldg(rec + 2), t3 = __ldg(rec + 3);
                     float4 t4 = __ldg(rec + 4);
                     t4.w = __uint_as_float(M);
@@ -715,7 +724,7 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
     do {                                                                                                             \
         static bool done = false;                                                                                    \
         SVR_TRY(set_smem_once(ctx, composite_kernel<KK, SS, RR>, smem, &done));                                      \
-        composite_kernel<KK, SS, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, rs, f->ranges, f->tile_order, T_min, image, depth, \
+        composite_kernel<KK, SS, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, image, depth, \
                                                                              T_final, wm, stats, f->trav, f->trav_off, f->trav_count);       \
     } while (0)
 #define SVR_FWD(KK)                                                                                                  \
@@ -755,7 +764,7 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
         static bool done = false;                                                                                    \
         SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, HH, RR>, smem, &done));                                \
         backward_packed_kernel<KK, HH, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(                                  \
-            f->cam, pk, rs, f->ranges, f->tile_order, T_min, wm, dL, image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth, T_final,         \
+            f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, wm, dL, image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth, T_final,         \
             f->trav, f->trav_off, f->trav_count);                                                                    \
     } while (0)
 #define SVR_BWD(KK)                                                                                                  \
@@ -780,12 +789,18 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
 }
 
 SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f) {
-    if (f->n_entries == 0) return SVR_OK;
     StageScope scope__(ctx, ST_PACK);
-    pack_entries_kernel<<<(unsigned int)((f->n_entries + 255) / 256), 256, 0, ctx->stream>>>(
-        f->scene, f->cam, f->vals, f->n_entries, reinterpret_cast<const float4*>(f->rgbm), reinterpret_cast<float4*>(f->packed),
-        reinterpret_cast<const uint2*>(f->rects), reinterpret_cast<uint2*>(f->rects_sorted));
-    ctx->launches += 1;
+    if (f->scene.n > 0) {
+        voxel_record_kernel<<<(unsigned int)((f->scene.n + 255) / 256), 256, 0, ctx->stream>>>(
+            f->scene, f->cam, reinterpret_cast<const ushort4*>(f->rects), reinterpret_cast<const float4*>(f->rgbm),
+            reinterpret_cast<float4*>(f->packed));
+        ctx->launches += 1;
+    }
+    if (f->n_entries > 0) {
+        gather_rects_kernel<<<(unsigned int)((f->n_entries + 255) / 256), 256, 0, ctx->stream>>>(
+            f->vals, f->n_entries, reinterpret_cast<const uint2*>(f->rects), reinterpret_cast<uint2*>(f->rects_sorted));
+        ctx->launches += 1;
+    }
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

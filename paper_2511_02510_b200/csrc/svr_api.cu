@@ -269,7 +269,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             // frame-lifetime buffers first, largest first (the pool then reuses the previous frame's blocks one for one),
             // scratch last
             TRYF(alloc_traversal(ctx, f, E));
-            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
+            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)n));
             TRYF(svr_alloc(ctx, (void**)&keys_b, ka));   // canonical keys
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
             TRYF(svr_alloc(ctx, (void**)&vals_a, va));
@@ -331,7 +331,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             f->keys = ks; f->vals = vs;
             TRYF(alloc_traversal(ctx, f, E));
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
-            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)E));
+            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)n));
             keys_a = keys_b = nullptr;
             vals_a = vals_b = nullptr;
         }

@@ -11,7 +11,7 @@
 
 #define SVR_TILE 16
 #define SVR_MAX_K 4
-#define SVR_TRAV_WORDS 68     // traversal record: 32 hit masks, 32 list entries, slot count (+ padding to 16 bytes)
+#define SVR_TRAV_WORDS 68     // traversal record: 32 hit masks, 32 voxel ids, slot count (+ padding to 16 bytes)
 
 enum SvrStage {
     ST_TILE_MASKS = 0, ST_RECTS, ST_SCAN, ST_EMIT, ST_SORT, ST_RANGES, ST_COLORS, ST_FORWARD, ST_LOSS, ST_BACKWARD,
@@ -80,7 +80,7 @@ struct SvrFrame {
     uint32_t* vals = nullptr;        // [E] sorted
     uint16_t* rects_sorted = nullptr;// [E,4] pixel rectangle of vals[i] (coalesced reads in the compositing cull)
     uint32_t* ranges = nullptr;      // [n_tiles*8*2]
-    float* packed = nullptr;         // [E,20] per-entry voxel record in list order (composite.cu pack_entries_kernel)
+    float* packed = nullptr;         // [n,20] per-voxel view record, visible voxels only (composite.cu voxel_record_kernel)
     uint32_t* tile_order = nullptr;  // [2*n_tiles]: tile ids by descending list length, then the lengths
     // traversal scratch written by svr_forward, replayed by svr_backward (composite.cu)
     uint32_t* trav = nullptr;        // [trav_cap, SVR_TRAV_WORDS] records
