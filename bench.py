@@ -312,7 +312,7 @@ def main():
     peaks, peak_src = measured_peaks()
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
     fp32_peak = n_sm * FP32_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12    # TFLOP/s
-    stage_ms = {k: v[0] / max(v[1], 1) for k, v in stage.items() if v[1] > 0}
+    stage_ms = {k: v[0] / args.steps for k, v in stage.items() if v[1] > 0}       # per step (a stage may launch twice)
     dom = max(stage_ms, key=stage_ms.get)
     flop = {"forward_composite": FLOP_PER_FWD_HIT, "backward_composite": FLOP_PER_BWD_HIT}
     if dom in flop:

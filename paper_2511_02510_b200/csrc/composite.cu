@@ -788,7 +788,8 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
     return SVR_OK;
 }
 
-SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f) {
+// per-voxel view records (needs rects + rgbm; independent of the lists)
+SvrStatus launch_voxel_records(SvrContext* ctx, SvrFrame* f) {
     StageScope scope__(ctx, ST_PACK);
     if (f->scene.n > 0) {
         voxel_record_kernel<<<(unsigned int)((f->scene.n + 255) / 256), 256, 0, ctx->stream>>>(
@@ -796,6 +797,13 @@ SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f) {
             reinterpret_cast<float4*>(f->packed));
         ctx->launches += 1;
     }
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+// rectangles in list order (a separate pass: gathering inside the per-bucket sort's output loop cost 0.12 ms, this 0.04)
+SvrStatus launch_gather_rects(SvrContext* ctx, SvrFrame* f) {
+    StageScope scope__(ctx, ST_PACK);
     if (f->n_entries > 0) {
         gather_rects_kernel<<<(unsigned int)((f->n_entries + 255) / 256), 256, 0, ctx->stream>>>(
             f->vals, f->n_entries, reinterpret_cast<const uint2*>(f->rects), reinterpret_cast<uint2*>(f->rects_sorted));

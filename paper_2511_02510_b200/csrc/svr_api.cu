@@ -143,6 +143,7 @@ SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t wor
         }
     }
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->host_pinned), 64);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->readback_ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         // no usable CUDA device: fail loudly, there is no other path
         fprintf(stderr, "svr_create: CUDA error: %s\n", cudaGetErrorString(e));
@@ -160,6 +161,7 @@ void svr_destroy(SvrContext* ctx) {
     for (auto& b : ctx->free_blocks) cudaFreeAsync(b.first, ctx->stream);
     for (auto& b : ctx->live) cudaFreeAsync(b.first, ctx->stream);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
+    if (ctx->readback_ev) cudaEventDestroy(ctx->readback_ev);
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
     for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
@@ -242,6 +244,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     TRYF(A.get((void**)&f->tile_masks, (size_t)f->n_tiles));
     if (!bucketed) TRYF(A.get((void**)&f->sat, sizeof(uint32_t) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1)));
     TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
+    TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)n));
     TRYF(A.get((void**)&f->ranges, sizeof(uint32_t) * 16 * (size_t)f->n_tiles));
     TRYF(A.get((void**)&f->tile_order, sizeof(uint32_t) * 2 * (size_t)f->n_tiles));
     TRYF(svr_alloc(ctx, (void**)&totals, 128));
@@ -257,7 +260,10 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         TRYF(launch_bucket_count(ctx, f, bcount, bigdiff, nonempty, totals));
         // E, the number of many-tile voxels and the number of non-empty buckets: one small readback sizes the lists
         CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 32, cudaMemcpyDeviceToHost, ctx->stream));
-        CUDAF(cudaStreamSynchronize(ctx->stream));
+        CUDAF(cudaEventRecord(ctx->readback_ev, ctx->stream));
+        // the per-voxel view records do not depend on E: they run while the host reads E and sizes the lists
+        TRYF(launch_voxel_records(ctx, f));
+        CUDAF(cudaEventSynchronize(ctx->readback_ev));
         const int64_t E = (int64_t)ctx->host_pinned[0];
         const int64_t n_big = (int64_t)ctx->host_pinned[1];
         if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));
@@ -269,7 +275,6 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             // frame-lifetime buffers first, largest first (the pool then reuses the previous frame's blocks one for one),
             // scratch last
             TRYF(alloc_traversal(ctx, f, E));
-            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)n));
             TRYF(svr_alloc(ctx, (void**)&keys_b, ka));   // canonical keys
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
             TRYF(svr_alloc(ctx, (void**)&vals_a, va));
@@ -290,7 +295,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         svr_free(ctx, totals, 128);
         totals = nullptr;
         TRYF(launch_lists_finish(ctx, f));
-        TRYF(launch_pack_entries(ctx, f));
+        TRYF(launch_gather_rects(ctx, f));
     } else {
         TRYF(A.get((void**)&f->offsets, sizeof(uint32_t) * (size_t)(n + 1)));
         TRYF(svr_alloc(ctx, (void**)&counts, counts_bytes));
@@ -300,8 +305,10 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         CUDAF(cudaMemcpyAsync(totals, f->offsets + n, sizeof(uint32_t), cudaMemcpyDeviceToDevice, ctx->stream));
         CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 16, cudaMemcpyDeviceToHost, ctx->stream));
         // per-view colours do not depend on E: enqueue before the sync so they overlap the readback
+        CUDAF(cudaEventRecord(ctx->readback_ev, ctx->stream));
         TRYF(launch_voxel_colors(ctx, f));
-        CUDAF(cudaStreamSynchronize(ctx->stream));
+        TRYF(launch_voxel_records(ctx, f));
+        CUDAF(cudaEventSynchronize(ctx->readback_ev));
         const int64_t E = (int64_t)(ctx->host_pinned[0] & 0xFFFFFFFFull);
         const int64_t n_big = (int64_t)ctx->host_pinned[1];
         svr_free(ctx, counts, counts_bytes);
@@ -331,14 +338,13 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             f->keys = ks; f->vals = vs;
             TRYF(alloc_traversal(ctx, f, E));
             TRYF(A.get((void**)&f->rects_sorted, sizeof(uint16_t) * 4 * (size_t)E));
-            TRYF(A.get((void**)&f->packed, sizeof(float) * 20 * (size_t)n));
             keys_a = keys_b = nullptr;
             vals_a = vals_b = nullptr;
         }
         svr_free(ctx, totals, 128);
         totals = nullptr;
         TRYF(launch_ranges(ctx, f));
-        TRYF(launch_pack_entries(ctx, f));
+        TRYF(launch_gather_rects(ctx, f));
     }
 #undef TRYF
 #undef CUDAF
@@ -350,7 +356,7 @@ SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame) {
     if (!ctx || !frame) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     frame->trav_valid = false;      // termination depends on the densities: the next forward pass records again
     SVR_TRY(launch_voxel_colors(ctx, frame));
-    return launch_pack_entries(ctx, frame);
+    return launch_voxel_records(ctx, frame);
 }
 
 void svr_frame_release(SvrContext* ctx, SvrFrame* frame) {

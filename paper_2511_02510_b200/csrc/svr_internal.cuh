@@ -42,6 +42,7 @@ struct SvrContext {
     void* loss_ws = nullptr;      // loss workspace (see loss.cu)
     size_t loss_ws_bytes = 0;
     uint64_t* host_pinned = nullptr;  // 64-byte pinned readback slot
+    cudaEvent_t readback_ev = nullptr; // marks the readback copy: the host waits for it, not for the work queued behind it
 };
 
 // Device-side copy of the camera with everything derived on the host in fp64.
@@ -142,7 +143,8 @@ SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const 
                              unsigned int* work, int vb);
 SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
-SvrStatus launch_pack_entries(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_voxel_records(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_gather_rects(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
                          float* T_final, float* w_max, unsigned long long* stats, bool record);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
