@@ -83,28 +83,7 @@ __global__ void __launch_bounds__(256) voxel_record_kernel(SceneDev s, CamDev c,
     if (v >= s.n) return;
     const ushort4 r = rects[v];
     if (r.x > r.z) return;                                   // not visible in this view: never read
-    const uint32_t vid = (uint32_t)v;
-    uint2 q = __ldg(reinterpret_cast<const uint2*>(s.ijkl) + vid);
-    const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
-    float4 ra = __ldg(rp), rb = __ldg(rp + 1), col = __ldg(rgbm + vid);
-    int L = q.y >> 16;
-    float ef = s.root_edge * __int_as_float((127 - L) << 23);
-    double e = (double)ef;
-    double gx = (double)s.root_lo[0] + ((double)(q.x & 0xFFFF) + 0.5) * e - c.o[0];
-    double gy = (double)s.root_lo[1] + ((double)(q.x >> 16) + 0.5) * e - c.o[1];
-    double gz = (double)s.root_lo[2] + ((double)(q.y & 0xFFFF) + 0.5) * e - c.o[2];
-    float hx = (float)gx, hy = (float)gy, hz = (float)gz;
-    // trilinear -> polynomial coefficients, scaled by log2(e) (corner c = bx + 2 by + 4 bz)
-    const float L2E = 1.4426950408889634f;
-    float c0 = ra.x, cx = ra.y - ra.x, cy = ra.z - ra.x, cz = rb.x - ra.x;
-    float cxy = (ra.w - ra.y) - cy, cxz = (rb.y - ra.y) - cz, cyz = (rb.z - ra.z) - cz;
-    float cxyz = ((rb.w - rb.z) - (rb.y - rb.x)) - ((ra.w - ra.z) - (ra.y - ra.x));
-    float4* out = vrec + 5 * (size_t)vid;
-    out[0] = make_float4(hx, hy, hz, 0.5f * ef);
-    out[1] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
-    out[2] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
-    out[3] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
-    out[4] = col;
+    voxel_record_dev(s, c, __ldg(reinterpret_cast<const uint2*>(s.ijkl) + v), (uint32_t)v, __ldg(rgbm + v), vrec);
 }
 
 // rectangle in list order: the compositing cull reads it coalesced

@@ -459,14 +459,18 @@ template <int DEG>
 __global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamDev c, const uint8_t* __restrict__ masks,
                                                                 ushort4* __restrict__ rects, uint32_t* __restrict__ bcount,
                                                                 int* __restrict__ bigdiff, unsigned long long* __restrict__ totals,
-                                                                float4* __restrict__ rgbm) {
+                                                                float4* __restrict__ rgbm, float4* __restrict__ vrec) {
     int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= s.n) return;
     const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
     ushort4 r = voxel_rect(s, c, q);
     rects[v] = r;
     if (r.x > r.z) return;
-    rgbm[v] = voxel_color_dev<DEG>(s, c, q, v);
+    {
+        const float4 col = voxel_color_dev<DEG>(s, c, q, v);
+        rgbm[v] = col;
+        voxel_record_dev(s, c, q, (uint32_t)v, col, vrec);
+    }
     const int i0 = r.x >> 4, i1 = r.z >> 4, j0 = r.y >> 4, j1 = r.w >> 4;
     if ((i1 - i0 + 1) * (j1 - j0 + 1) > BIG_TILES) {
         const int sx = c.tiles_x + 1;
@@ -959,10 +963,10 @@ SvrStatus launch_bucket_count(SvrContext* ctx, SvrFrame* f, uint32_t* bcount, in
         ushort4* r = reinterpret_cast<ushort4*>(f->rects);
         float4* col = reinterpret_cast<float4*>(f->rgbm);
         switch (f->scene.sh_degree) {
-            case 0: rect_bucket_count_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
-            case 1: rect_bucket_count_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
-            case 2: rect_bucket_count_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
-            default: rect_bucket_count_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col); break;
+            case 0: rect_bucket_count_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
+            case 1: rect_bucket_count_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
+            case 2: rect_bucket_count_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
+            default: rect_bucket_count_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
         }
         ctx->launches += 1;
     }

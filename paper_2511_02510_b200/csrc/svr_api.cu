@@ -260,10 +260,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         TRYF(launch_bucket_count(ctx, f, bcount, bigdiff, nonempty, totals));
         // E, the number of many-tile voxels and the number of non-empty buckets: one small readback sizes the lists
         CUDAF(cudaMemcpyAsync(ctx->host_pinned, totals, 32, cudaMemcpyDeviceToHost, ctx->stream));
-        CUDAF(cudaEventRecord(ctx->readback_ev, ctx->stream));
-        // the per-voxel view records do not depend on E: they run while the host reads E and sizes the lists
-        TRYF(launch_voxel_records(ctx, f));
-        CUDAF(cudaEventSynchronize(ctx->readback_ev));
+        CUDAF(cudaStreamSynchronize(ctx->stream));
         const int64_t E = (int64_t)ctx->host_pinned[0];
         const int64_t n_big = (int64_t)ctx->host_pinned[1];
         if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));

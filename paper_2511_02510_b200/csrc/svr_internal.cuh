@@ -65,6 +65,31 @@ struct SceneDev {
     const float* sh;
 };
 
+// The 80-byte view record of voxel `vid` (5 x 16 B at vrec + 5 vid): centre relative to the camera as hi+lo floats (fp64
+// arithmetic), half edge, voxel id, the trilinear raw density as polynomial coefficients * log2(e) (corner c = bx + 2 by +
+// 4 bz), the per-view colour. Written by the projection kernel (preprocess.cu) and by voxel_record_kernel (composite.cu).
+__device__ __forceinline__ void voxel_record_dev(const SceneDev& s, const CamDev& c, uint2 q, uint32_t vid, float4 col, float4* __restrict__ vrec) {
+    const float4* rp = reinterpret_cast<const float4*>(s.raw) + 2 * (size_t)vid;
+    const float4 ra = __ldg(rp), rb = __ldg(rp + 1);
+    const int L = q.y >> 16;
+    const float ef = s.root_edge * __int_as_float((127 - L) << 23);
+    const double e = (double)ef;
+    const double gx = (double)s.root_lo[0] + ((double)(q.x & 0xFFFF) + 0.5) * e - c.o[0];
+    const double gy = (double)s.root_lo[1] + ((double)(q.x >> 16) + 0.5) * e - c.o[1];
+    const double gz = (double)s.root_lo[2] + ((double)(q.y & 0xFFFF) + 0.5) * e - c.o[2];
+    const float hx = (float)gx, hy = (float)gy, hz = (float)gz;
+    const float L2E = 1.4426950408889634f;
+    const float c0 = ra.x, cx = ra.y - ra.x, cy = ra.z - ra.x, cz = rb.x - ra.x;
+    const float cxy = (ra.w - ra.y) - cy, cxz = (rb.y - ra.y) - cz, cyz = (rb.z - ra.z) - cz;
+    const float cxyz = ((rb.w - rb.z) - (rb.y - rb.x)) - ((ra.w - ra.z) - (ra.y - ra.x));
+    float4* out = vrec + 5 * (size_t)vid;
+    out[0] = make_float4(hx, hy, hz, 0.5f * ef);
+    out[1] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
+    out[2] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
+    out[3] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
+    out[4] = col;
+}
+
 struct SvrFrame {
     SceneDev scene;
     CamDev cam;
