@@ -231,6 +231,7 @@ def main():
 
     def step(i):
         k = camera_index(i, rank, len(ccams))
+        ctx.svr_loss_prepare(targets[k])        # target-only part of the loss: second stream, beside preprocess + forward
         fr = ctx.svr_preprocess(vox, ccams[k])
         ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, depth=depth, T_final=Tf)
         ctx.svr_loss_grad(image, targets[k], cfg.gamma, dL=dL, loss=loss)

@@ -107,6 +107,14 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
 SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H,
                         float gamma, const SvrLossOpts* opts, float* dL_dimage, float* loss);
 
+/* Optional, before svr_preprocess / svr_forward of the same view: queues the part of eq. 7 that reads only the
+ * target (Sobel magnitude and its quantile, R10) on the context's second stream, ordered after the work already
+ * queued on the context's stream, so that it runs beside the list build and the forward pass. The next
+ * svr_loss_grad with the same target, W, H and percentile (and sobel_source = 0) consumes it; any other
+ * svr_loss_grad waits for it and computes everything itself. `target` must stay unchanged in between.
+ * No-op when opts->sobel_source != 0. Results are identical with and without this call. */
+SvrStatus svr_loss_prepare(SvrContext* ctx, const float* target, int32_t W, int32_t H, const SvrLossOpts* opts);
+
 /* (4) backward compositing: gradients of sum(dL_dimage * image) w.r.t. corner raw densities and SH
  * coefficients. `image` is svr_forward's output for this frame (the suffix colour is image - prefix).
  * grad_raw_density[n,8] and grad_sh[n,(D+1)^2,3] ACCUMULATE (+=; caller zeroes) so several views sum

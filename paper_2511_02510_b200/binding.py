@@ -20,7 +20,7 @@ SVR_OK, SVR_ERR_INVALID_ARG, SVR_ERR_CUDA, SVR_ERR_WORKSPACE, SVR_ERR_UNSUPPORTE
 _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR_WORKSPACE", 4: "SVR_ERR_UNSUPPORTED"}
 
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
-           "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad",
+           "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare",
            "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
@@ -82,6 +82,7 @@ def _load():
     lib.svr_forward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 4
     lib.svr_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_float,
                                   C.POINTER(SvrLossOpts), C.c_void_p, C.c_void_p]
+    lib.svr_loss_prepare.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(SvrLossOpts)]
     lib.svr_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 5
     lib.svr_backward_heads.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 9
     lib.svr_train_view_host.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.POINTER(SvrCamera), C.POINTER(SvrRenderOpts),
@@ -309,6 +310,12 @@ class Context:
         o = SvrRenderOpts(K, T_min, 1 if record else 0)
         self._check(_lib.svr_forward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(image), _p(depth), _p(T_final), _p(w_max)))
         return image, depth, T_final
+
+    def svr_loss_prepare(self, target: torch.Tensor, eps: float = 1e-3, percentile: float = 0.99, sobel_source: int = 0):
+        H, W = int(target.shape[0]), int(target.shape[1])
+        _dev(target, torch.float32, "target")
+        o = SvrLossOpts(eps, percentile, sobel_source)
+        self._check(_lib.svr_loss_prepare(self.handle, _p(target), W, H, C.byref(o)))
 
     def svr_loss_grad(self, render: torch.Tensor, target: torch.Tensor, gamma: float, eps: float = 1e-3,
                       percentile: float = 0.99, sobel_source: int = 0, dL=None, loss=None):

@@ -153,10 +153,7 @@ __global__ void __launch_bounds__(256) grad_kernel(const float* __restrict__ mag
 
 }  // namespace
 
-SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma, float eps,
-                           float q, int sobel_source, float* dL, float* loss) {
-    StageScope scope__(ctx, ST_LOSS);
-    const int64_t n = (int64_t)W * H;
+static SvrStatus loss_workspace(SvrContext* ctx, int64_t n) {
     size_t need = sizeof(LossWs) + sizeof(float) * (size_t)n + 256;
     if (ctx->loss_ws_bytes < need) {
         if (ctx->loss_ws) svr_free(ctx, ctx->loss_ws, ctx->loss_ws_bytes);
@@ -165,25 +162,69 @@ SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* ta
         SVR_TRY(svr_alloc(ctx, &ctx->loss_ws, need));
         ctx->loss_ws_bytes = need;
     }
+    return SVR_OK;
+}
+
+// The part of eq. 7 that reads only the Sobel source: magnitude and its q-quantile (6 launches) on `stream`.
+static SvrStatus loss_source_phase(SvrContext* ctx, cudaStream_t stream, const float* src, int W, int H, float q) {
+    const int64_t n = (int64_t)W * H;
     LossWs* ws = reinterpret_cast<LossWs*>(ctx->loss_ws);
     float* mag = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(ctx->loss_ws) + ((sizeof(LossWs) + 255) & ~(size_t)255));
-    SVR_CUDA(ctx, cudaMemsetAsync(ws, 0, sizeof(LossWs), ctx->stream));
+    SVR_CUDA(ctx, cudaMemsetAsync(ws, 0, sizeof(LossWs), stream));
     // nearest-rank quantile: sorted[ceil(q n) - 1]
     double kq = ceil((double)q * (double)n) - 1.0;
     if (kq < 0) kq = 0;
     if (kq > (double)(n - 1)) kq = (double)(n - 1);
     unsigned int k0 = (unsigned int)kq;
     unsigned int g = (unsigned int)((n + 255) / 256);
-    const float* src = sobel_source == 0 ? target : render;
-    sobel_hist_kernel<<<g, 256, 0, ctx->stream>>>(src, W, H, mag, ws);
-    select_kernel<<<1, 256, 0, ctx->stream>>>(ws, 0, k0);
-    refine_hist_kernel<<<g, 256, 0, ctx->stream>>>(mag, n, ws, 1);
-    select_kernel<<<1, 256, 0, ctx->stream>>>(ws, 1, 0);
-    refine_hist_kernel<<<g, 256, 0, ctx->stream>>>(mag, n, ws, 2);
-    select_kernel<<<1, 256, 0, ctx->stream>>>(ws, 2, 0);
+    sobel_hist_kernel<<<g, 256, 0, stream>>>(src, W, H, mag, ws);
+    select_kernel<<<1, 256, 0, stream>>>(ws, 0, k0);
+    refine_hist_kernel<<<g, 256, 0, stream>>>(mag, n, ws, 1);
+    select_kernel<<<1, 256, 0, stream>>>(ws, 1, 0);
+    refine_hist_kernel<<<g, 256, 0, stream>>>(mag, n, ws, 2);
+    select_kernel<<<1, 256, 0, stream>>>(ws, 2, 0);
+    ctx->launches += 6;
+    SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+// svr_loss_prepare: the source phase on the context's second stream, ordered after everything already queued on the main
+// stream (the producer of `target`, the previous loss call that still reads the workspace) and after what is queued on the
+// second stream (the host path's upload).
+SvrStatus launch_loss_prepare(SvrContext* ctx, const float* target, int W, int H, float q) {
+    const int64_t n = (int64_t)W * H;
+    if (ctx->loss_prepared) SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->loss_ready_ev, 0));   // an unconsumed phase: replaced
+    SVR_TRY(loss_workspace(ctx, n));
+    SVR_CUDA(ctx, cudaEventRecord(ctx->fork_ev, ctx->stream));
+    SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->fork_ev, 0));
+    SVR_TRY(loss_source_phase(ctx, ctx->aux, target, W, H, q));
+    SVR_CUDA(ctx, cudaEventRecord(ctx->loss_ready_ev, ctx->aux));
+    ctx->loss_prepared = true;
+    ctx->loss_prep_target = target;
+    ctx->loss_prep_W = W; ctx->loss_prep_H = H; ctx->loss_prep_q = q;
+    return SVR_OK;
+}
+
+SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma, float eps,
+                           float q, int sobel_source, float* dL, float* loss) {
+    StageScope scope__(ctx, ST_LOSS);
+    const int64_t n = (int64_t)W * H;
+    const bool prepared = ctx->loss_prepared && sobel_source == 0 && ctx->loss_prep_target == target && ctx->loss_prep_W == W &&
+                          ctx->loss_prep_H == H && ctx->loss_prep_q == q;
+    if (ctx->loss_prepared) {        // a prepared phase is consumed (or discarded) by the next loss call; either way wait for it
+        SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->loss_ready_ev, 0));
+        ctx->loss_prepared = false;
+    }
+    if (!prepared) {
+        SVR_TRY(loss_workspace(ctx, n));
+        SVR_TRY(loss_source_phase(ctx, ctx->stream, sobel_source == 0 ? target : render, W, H, q));
+    }
+    LossWs* ws = reinterpret_cast<LossWs*>(ctx->loss_ws);
+    float* mag = reinterpret_cast<float*>(reinterpret_cast<unsigned char*>(ctx->loss_ws) + ((sizeof(LossWs) + 255) & ~(size_t)255));
+    unsigned int g = (unsigned int)((n + 255) / 256);
     weight_sum_kernel<<<g, 256, 0, ctx->stream>>>(mag, render, target, n, eps, gamma, ws);
     grad_kernel<<<g, 256, 0, ctx->stream>>>(mag, render, target, n, eps, gamma, ws, dL, loss);
-    ctx->launches += 8;
+    ctx->launches += 2;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }

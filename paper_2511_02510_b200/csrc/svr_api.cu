@@ -144,6 +144,10 @@ SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t wor
     }
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->host_pinned), 64);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->readback_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->aux, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->loss_ready_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->upload_ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         // no usable CUDA device: fail loudly, there is no other path
         fprintf(stderr, "svr_create: CUDA error: %s\n", cudaGetErrorString(e));
@@ -157,11 +161,16 @@ SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t wor
 void svr_destroy(SvrContext* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    if (ctx->aux) cudaStreamSynchronize(ctx->aux);
     cudaStreamSynchronize(ctx->stream);
     for (auto& b : ctx->free_blocks) cudaFreeAsync(b.first, ctx->stream);
     for (auto& b : ctx->live) cudaFreeAsync(b.first, ctx->stream);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     if (ctx->readback_ev) cudaEventDestroy(ctx->readback_ev);
+    if (ctx->fork_ev) cudaEventDestroy(ctx->fork_ev);
+    if (ctx->loss_ready_ev) cudaEventDestroy(ctx->loss_ready_ev);
+    if (ctx->upload_ev) cudaEventDestroy(ctx->upload_ev);
+    if (ctx->aux) cudaStreamDestroy(ctx->aux);
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
     for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
@@ -372,6 +381,14 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
     return st;
 }
 
+SvrStatus svr_loss_prepare(SvrContext* ctx, const float* target, int32_t W, int32_t H, const SvrLossOpts* opts) {
+    if (!ctx || !target || !opts) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (W <= 0 || H <= 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "empty image");
+    if (!(opts->percentile > 0.f && opts->percentile <= 1.f)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "percentile must be in (0,1]");
+    if (opts->sobel_source != 0) return SVR_OK;      // the weights read the render: nothing to do ahead of it
+    return launch_loss_prepare(ctx, target, W, H, opts->percentile);
+}
+
 SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H, float gamma,
                         const SvrLossOpts* opts, float* dL_dimage, float* loss) {
     if (!ctx || !render || !target || !opts || !dL_dimage || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
@@ -423,10 +440,16 @@ SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCa
     float *target = buf, *image = buf + npix * 3, *dL = buf + npix * 6, *loss = buf + npix * 9;
     SvrFrame* f = nullptr;
     SvrStatus st = SVR_OK;
-    cudaError_t e = cudaMemcpyAsync(target, target_host, sizeof(float) * npix * 3, cudaMemcpyHostToDevice, ctx->stream);
+    // the upload and the part of the loss that reads only the target run on the second stream, beside preprocess + forward
+    cudaError_t e = cudaEventRecord(ctx->fork_ev, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->aux, ctx->fork_ev, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(target, target_host, sizeof(float) * npix * 3, cudaMemcpyHostToDevice, ctx->aux);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->upload_ev, ctx->aux);
     if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "H2D copy: %s", cudaGetErrorString(e));
+    if (st == SVR_OK) st = svr_loss_prepare(ctx, target, cam_host->W, cam_host->H, lopts);
     if (st == SVR_OK) st = svr_preprocess(ctx, vox, cam_host, &f);
     if (st == SVR_OK) st = svr_forward(ctx, f, ropts, image, nullptr, nullptr, nullptr);
+    if (st == SVR_OK && cudaStreamWaitEvent(ctx->stream, ctx->upload_ev, 0) != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "stream wait");
     if (st == SVR_OK) st = svr_loss_grad(ctx, image, target, cam_host->W, cam_host->H, gamma, lopts, dL, loss);
     if (st == SVR_OK) st = svr_backward(ctx, f, ropts, dL, image, grad_raw_density, grad_sh, w_max);
     if (st == SVR_OK) {

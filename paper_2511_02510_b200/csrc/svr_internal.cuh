@@ -41,6 +41,13 @@ struct SvrContext {
     int64_t grad_rgb_cap = 0;
     void* loss_ws = nullptr;      // loss workspace (see loss.cu)
     size_t loss_ws_bytes = 0;
+    // second stream: work that does not depend on the render (the loss's source phase, the host path's upload)
+    cudaStream_t aux = nullptr;
+    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr;
+    bool loss_prepared = false;   // svr_loss_prepare queued a source phase that the next svr_loss_grad may consume
+    const float* loss_prep_target = nullptr;
+    int loss_prep_W = 0, loss_prep_H = 0;
+    float loss_prep_q = 0.f;
     uint64_t* host_pinned = nullptr;  // 64-byte pinned readback slot
     cudaEvent_t readback_ev = nullptr; // marks the readback copy: the host waits for it, not for the work queued behind it
 };
@@ -177,6 +184,7 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
                           const float* depth, const float* T_final);
 SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw,
                              float* grad_sh);
+SvrStatus launch_loss_prepare(SvrContext* ctx, const float* target, int W, int H, float q);
 SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma,
                            float eps, float q, int sobel_source, float* dL, float* loss);
 

@@ -207,6 +207,35 @@ def test_loss_grad_parity_and_gamma0(orc, svr):
     assert abs(pkg.svr_gamma_schedule(9000, 20000) - orc.gamma_schedule(9000, 20000)) < 1e-7
 
 
+def test_loss_prepare_same_result(orc, svr):
+    """svr_loss_prepare (the target-only phase on the second stream) changes the schedule, not the result: consumed by the
+    matching svr_loss_grad, discarded by a call with another target, replaced by a second prepare."""
+    pkg, ctx, torch = svr
+    rng = np.random.default_rng(6)
+    H, W = 61, 97
+    tgt = [np.clip(rng.uniform(0, 1, size=(H, W, 3)) * np.linspace(0.2, 1, W)[None, :, None], 0, 1).astype(np.float32) for _ in range(2)]
+    render = np.clip(tgt[0] + rng.normal(0, 0.05, size=tgt[0].shape), 0, 1).astype(np.float32)
+    t_dev = [torch.from_numpy(t).cuda() for t in tgt]
+    r_dev = torch.from_numpy(render).cuda()
+    ref = [orc.lf_loss_and_grad(render, t, 0.6) for t in tgt]
+
+    def check(dL, loss, k):
+        ctx.synchronize()
+        assert rel_l2(dL.cpu().numpy(), ref[k][1]) <= 1e-5
+        assert abs(float(loss.item()) - ref[k][0]) <= 1e-5 * abs(ref[k][0])
+
+    ctx.svr_loss_prepare(t_dev[0])
+    check(*ctx.svr_loss_grad(r_dev, t_dev[0], 0.6), 0)            # consumed
+    ctx.svr_loss_prepare(t_dev[0])
+    check(*ctx.svr_loss_grad(r_dev, t_dev[1], 0.6), 1)            # other target: discarded
+    check(*ctx.svr_loss_grad(r_dev, t_dev[0], 0.6), 0)            # nothing prepared any more
+    ctx.svr_loss_prepare(t_dev[0])
+    ctx.svr_loss_prepare(t_dev[1])                                # replaced
+    check(*ctx.svr_loss_grad(r_dev, t_dev[1], 0.6), 1)
+    ctx.svr_loss_prepare(t_dev[0], percentile=0.5)                # other percentile: discarded
+    check(*ctx.svr_loss_grad(r_dev, t_dev[0], 0.6), 0)
+
+
 # ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
