@@ -1018,14 +1018,28 @@ SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const 
 }
 
 // rectangles in list order + longest-list-first tile order (the ranges themselves come from the bucket scan)
-SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f) {
-    StageScope scope__(ctx, ST_RANGES);
-    tile_order_kernel<<<1, 1024, 0, ctx->stream>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
+SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f, bool fork) {
+    // Two one-block kernels that read only the ranges: with `fork` they are queued on the second stream (after the
+    // allocations queued so far) and run beside the scatter and the sort; launch_lists_join makes the main stream wait.
+    cudaStream_t st = ctx->stream;
+    if (fork) {
+        SVR_CUDA(ctx, cudaEventRecord(ctx->fork_ev, ctx->stream));
+        SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->fork_ev, 0));
+        st = ctx->aux;
+    }
+    tile_order_kernel<<<1, 1024, 0, st>>>(f->ranges, f->n_tiles, f->tile_order + f->n_tiles, f->tile_order);
     ctx->launches += 1;
     if (f->trav_off) {
-        trav_offsets_kernel<<<1, 1024, 0, ctx->stream>>>(f->tile_order + f->n_tiles, f->n_tiles, f->trav_off);
+        trav_offsets_kernel<<<1, 1024, 0, st>>>(f->tile_order + f->n_tiles, f->n_tiles, f->trav_off);
         ctx->launches += 1;
     }
+    if (fork) SVR_CUDA(ctx, cudaEventRecord(ctx->lists_ev, ctx->aux));
     SVR_CUDA(ctx, cudaGetLastError());
+    return SVR_OK;
+}
+
+SvrStatus launch_lists_join(SvrContext* ctx) {
+    StageScope scope__(ctx, ST_RANGES);
+    SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->lists_ev, 0));
     return SVR_OK;
 }

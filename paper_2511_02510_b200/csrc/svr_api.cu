@@ -148,6 +148,7 @@ SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t wor
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->loss_ready_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->upload_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->lists_ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         // no usable CUDA device: fail loudly, there is no other path
         fprintf(stderr, "svr_create: CUDA error: %s\n", cudaGetErrorString(e));
@@ -170,6 +171,7 @@ void svr_destroy(SvrContext* ctx) {
     if (ctx->fork_ev) cudaEventDestroy(ctx->fork_ev);
     if (ctx->loss_ready_ev) cudaEventDestroy(ctx->loss_ready_ev);
     if (ctx->upload_ev) cudaEventDestroy(ctx->upload_ev);
+    if (ctx->lists_ev) cudaEventDestroy(ctx->lists_ev);
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
@@ -231,6 +233,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     size_t big_bytes = 0, ka = 0, va = 0;
     SvrStatus st = SVR_OK;
     auto fail = [&](SvrStatus s) {
+        cudaStreamSynchronize(ctx->aux);     // forked list kernels may still read the frame's buffers
         if (counts) svr_free(ctx, counts, counts_bytes);
         if (totals) svr_free(ctx, totals, 128);
         if (big_list) svr_free(ctx, big_list, big_bytes);
@@ -274,6 +277,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         const int64_t n_big = (int64_t)ctx->host_pinned[1];
         if (E >= ((int64_t)1 << 31)) return fail(svr_fail(ctx, SVR_ERR_UNSUPPORTED, "%lld list entries (>= 2^31)", (long long)E));
         f->n_entries = E;
+        bool forked = false;
         if (E > 0) {
             ka = sizeof(uint64_t) * (size_t)E;
             va = sizeof(uint32_t) * (size_t)E;
@@ -287,6 +291,8 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
             TRYF(svr_alloc(ctx, (void**)&keys_a, ka));   // packed (code << vb | id) words, scratch
             TRYF(svr_alloc(ctx, (void**)&big_list, big_bytes));
             f->keys = keys_b; f->vals = vals_a;
+            TRYF(launch_lists_finish(ctx, f, true));
+            forked = true;
             TRYF(launch_bucket_scatter(ctx, f, bcount, keys_a, vb, big_list, reinterpret_cast<unsigned int*>(totals + 2)));
             TRYF(launch_bucket_sort(ctx, f, keys_a, nonempty, totals, reinterpret_cast<unsigned int*>(totals + 8), vb));   // totals[8..9]: the three work-fetch counters
             svr_free(ctx, keys_a, ka);
@@ -300,7 +306,8 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         bcount = nonempty = nullptr; bigdiff = nullptr;
         svr_free(ctx, totals, 128);
         totals = nullptr;
-        TRYF(launch_lists_finish(ctx, f));
+        if (forked) TRYF(launch_lists_join(ctx));
+        else TRYF(launch_lists_finish(ctx, f, false));
         TRYF(launch_gather_rects(ctx, f));
     } else {
         TRYF(A.get((void**)&f->offsets, sizeof(uint32_t) * (size_t)(n + 1)));

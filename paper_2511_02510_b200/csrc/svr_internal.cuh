@@ -43,7 +43,7 @@ struct SvrContext {
     size_t loss_ws_bytes = 0;
     // second stream: work that does not depend on the render (the loss's source phase, the host path's upload)
     cudaStream_t aux = nullptr;
-    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr;
+    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr, lists_ev = nullptr;
     bool loss_prepared = false;   // svr_loss_prepare queued a source phase that the next svr_loss_grad may consume
     const float* loss_prep_target = nullptr;
     int loss_prep_W = 0, loss_prep_H = 0;
@@ -173,7 +173,8 @@ SvrStatus launch_bucket_scatter(SvrContext* ctx, SvrFrame* f, uint32_t* cursor, 
                                 unsigned int* big_count);
 SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const uint32_t* nonempty, const unsigned long long* totals,
                              unsigned int* work, int vb);
-SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f);
+SvrStatus launch_lists_finish(SvrContext* ctx, SvrFrame* f, bool fork);
+SvrStatus launch_lists_join(SvrContext* ctx);
 SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_voxel_records(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_gather_rects(SvrContext* ctx, SvrFrame* f);
