@@ -1007,11 +1007,17 @@ SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const 
     }
     // three block shapes so that the fixed cost of a pass (counter reset, scan) scales with the bucket; work[0..2] = fetch counters
     const int cb = 3 * f->scene.max_level;
-    bucket_sort_kernel<1024, SORT_CAP_BIG><<<148, 1024, smem_big, ctx->stream>>>(ent, f->ranges, nonempty, totals, work, 0, cb, vb, f->keys, f->vals);
+    // The three classes are independent: the largest and the smallest run on the second stream beside the middle one
+    // (each alone leaves SMs idle in its tail).
+    SVR_CUDA(ctx, cudaEventRecord(ctx->fork_ev, ctx->stream));
+    SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->aux, ctx->fork_ev, 0));
+    bucket_sort_kernel<1024, SORT_CAP_BIG><<<148, 1024, smem_big, ctx->aux>>>(ent, f->ranges, nonempty, totals, work, 0, cb, vb, f->keys, f->vals);
     bucket_sort_kernel<SORT_THREADS2, SORT_CAP><<<148 * 2, SORT_THREADS2, smem_mid, ctx->stream>>>(ent, f->ranges, nonempty, totals, work + 1, 1, cb, vb,
                                                                                                     f->keys, f->vals);
-    bucket_sort_kernel<128, SORT_CAP_SMALL><<<148 * 8, 128, smem_small, ctx->stream>>>(ent, f->ranges, nonempty, totals, work + 2, 2, cb, vb, f->keys,
-                                                                                      f->vals);
+    bucket_sort_kernel<128, SORT_CAP_SMALL><<<148 * 8, 128, smem_small, ctx->aux>>>(ent, f->ranges, nonempty, totals, work + 2, 2, cb, vb, f->keys,
+                                                                                   f->vals);
+    SVR_CUDA(ctx, cudaEventRecord(ctx->sort_ev, ctx->aux));
+    SVR_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->sort_ev, 0));
     ctx->launches += 3;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;

@@ -149,6 +149,7 @@ SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t wor
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->loss_ready_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->upload_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->lists_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->sort_ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         // no usable CUDA device: fail loudly, there is no other path
         fprintf(stderr, "svr_create: CUDA error: %s\n", cudaGetErrorString(e));
@@ -172,6 +173,7 @@ void svr_destroy(SvrContext* ctx) {
     if (ctx->loss_ready_ev) cudaEventDestroy(ctx->loss_ready_ev);
     if (ctx->upload_ev) cudaEventDestroy(ctx->upload_ev);
     if (ctx->lists_ev) cudaEventDestroy(ctx->lists_ev);
+    if (ctx->sort_ev) cudaEventDestroy(ctx->sort_ev);
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }

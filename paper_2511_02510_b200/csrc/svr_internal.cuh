@@ -43,7 +43,7 @@ struct SvrContext {
     size_t loss_ws_bytes = 0;
     // second stream: work that does not depend on the render (the loss's source phase, the host path's upload)
     cudaStream_t aux = nullptr;
-    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr, lists_ev = nullptr;
+    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr, lists_ev = nullptr, sort_ev = nullptr;
     bool loss_prepared = false;   // svr_loss_prepare queued a source phase that the next svr_loss_grad may consume
     const float* loss_prep_target = nullptr;
     int loss_prep_W = 0, loss_prep_H = 0;
