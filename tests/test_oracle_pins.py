@@ -698,3 +698,65 @@ def test_adam_first_step_and_fp64_rederivation():
     np.testing.assert_allclose(tt, T, rtol=1e-5, atol=1e-6)
     np.testing.assert_allclose(mm, M, rtol=1e-5, atol=1e-12)
     np.testing.assert_allclose(vv, V, rtol=1e-5, atol=1e-15)
+
+
+# ---------------------------------------------------------------------------------------------
+# L_SSIM (eq. 17; R14: Wang et al. 2004, 11-tap Gaussian window, sigma 1.5)
+# ---------------------------------------------------------------------------------------------
+def test_ssim_window_identity_constants_symmetry():
+    from oracle import ssim
+    g = ssim.gaussian_window()
+    assert abs(g.sum() - 1.0) < 1e-15 and np.array_equal(g, g[::-1])
+    # by hand: sum_k exp(-k^2 / 4.5), k = -5..5, = 1 + 2 (0.800737 + 0.411112 + 0.135335 + 0.028566 + 0.003866) = 3.759232
+    assert abs(g[5] - 1.0 / 3.759232) < 2e-6 and abs(g[0] - 0.003866 / 3.759232) < 2e-6
+    rng = np.random.default_rng(3)
+    H, W = 23, 31
+    a = rng.uniform(0, 1, size=(H, W, 3))
+    b = np.clip(a + rng.normal(0, 0.1, size=a.shape), 0, 1)
+    # identical images: SSIM = 1 everywhere (borders included), L = 0, and L is at its minimum there: zero gradient
+    L, grad = ssim.ssim_loss_and_grad(a, a)
+    assert abs(L) < 1e-14 and np.abs(grad).max() < 1e-15
+    # two constant images, window inside the image: all (co)variances vanish and SSIM = (2ab + C1) / (a^2 + b^2 + C1)
+    ca, cb = 0.3, 0.7
+    S, _ = ssim.ssim_map(np.full((H, W, 1), ca), np.full((H, W, 1), cb))
+    want = (2 * ca * cb + 0.01 ** 2) / (ca * ca + cb * cb + 0.01 ** 2)
+    np.testing.assert_allclose(S[5:H - 5, 5:W - 5, 0], want, rtol=1e-12)
+    assert abs(S[0, 0, 0] - want) > 1e-3                 # zero padding: the border windows see the padding
+    # symmetric in its arguments, bounded by 1, and each channel is on its own
+    Sab, _ = ssim.ssim_map(a, b)
+    Sba, _ = ssim.ssim_map(b, a)
+    np.testing.assert_allclose(Sab, Sba, rtol=1e-12, atol=1e-15)
+    assert Sab.max() <= 1.0 + 1e-12 and Sab.mean() < 0.99
+    S0, _ = ssim.ssim_map(a[:, :, :1], b[:, :, :1])
+    np.testing.assert_allclose(S0[:, :, 0], Sab[:, :, 0], rtol=1e-13)
+
+
+def test_ssim_moments_brute_force_and_gradient_fd():
+    from oracle import ssim
+    rng = np.random.default_rng(4)
+    H, W = 17, 19
+    R = rng.uniform(0, 1, size=(H, W, 3))
+    I = np.clip(R + rng.normal(0, 0.15, size=R.shape), 0, 1)
+    # the index at a few pixels from explicit weighted sums over the 11 x 11 neighbourhood (zero outside the image)
+    g = ssim.gaussian_window()
+    S, _ = ssim.ssim_map(R, I)
+    for (y, x, ch) in [(0, 0, 0), (8, 9, 1), (16, 18, 2), (3, 17, 0)]:
+        m1 = m2 = e11 = e22 = e12 = 0.0
+        for dy in range(-5, 6):
+            for dx in range(-5, 6):
+                yy, xx = y + dy, x + dx
+                if 0 <= yy < H and 0 <= xx < W:
+                    wgt = g[dy + 5] * g[dx + 5]
+                    r, t = R[yy, xx, ch], I[yy, xx, ch]
+                    m1 += wgt * r; m2 += wgt * t; e11 += wgt * r * r; e22 += wgt * t * t; e12 += wgt * r * t
+        want = ((2 * m1 * m2 + 1e-4) * (2 * (e12 - m1 * m2) + 9e-4)) / ((m1 * m1 + m2 * m2 + 1e-4) * ((e11 - m1 * m1) + (e22 - m2 * m2) + 9e-4))
+        assert abs(S[y, x, ch] - want) < 1e-13
+    # analytic gradient against central differences of the loss
+    _, grad = ssim.ssim_loss_and_grad(R, I)
+    h = 1e-6
+    for (y, x, ch) in [(0, 0, 0), (8, 9, 1), (16, 18, 2), (5, 1, 1), (12, 12, 0)]:
+        Rp, Rm = R.copy(), R.copy()
+        Rp[y, x, ch] += h
+        Rm[y, x, ch] -= h
+        fd = (ssim.ssim_loss_and_grad(Rp, I)[0] - ssim.ssim_loss_and_grad(Rm, I)[0]) / (2 * h)
+        assert abs(fd - grad[y, x, ch]) <= 1e-6 * max(abs(fd), 1e-4), (y, x, ch, fd, grad[y, x, ch])
