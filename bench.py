@@ -425,6 +425,24 @@ def main():
                               "roofline": {"bound": "hbm", "achieved": adam_bytes / (ms_adam * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                            "unit": "GB/s", "frac": adam_bytes / (ms_adam * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
 
+        # NEXT-3 (part): L_SSIM and its gradient on the last render against its target, accumulated onto dL
+        ls = torch.empty(1, dtype=torch.float32, device=dev)
+        ctx.svr_ssim_loss_grad(image, targets[0], 0.2, dL=dL, loss=ls, accumulate=True)
+        e0, e1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(reps):
+                ctx.svr_ssim_loss_grad(image, targets[0], 0.2, dL=dL, loss=ls, accumulate=True)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        ms_ssim = e0.elapsed_time(e1) / reps
+        ssim_bytes = H * W * 48          # algorithmic: render, target, dL read + dL written, 12 B each per pixel (the kernels move 132 B)
+        line["next3_ssim"] = {"what": "svr_ssim_loss_grad (eq. 17 L_SSIM, 11-tap Gaussian window) accumulated onto dL; outside `value`",
+                              "ms": ms_ssim, "L_ssim": float(ls.item()),
+                              "roofline": {"bound": "hbm", "achieved": ssim_bytes / (ms_ssim * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                           "unit": "GB/s", "frac": ssim_bytes / (ms_ssim * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                           "algorithmic": "48 B per pixel"}}
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()

@@ -115,6 +115,15 @@ SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* targe
  * No-op when opts->sobel_source != 0. Results are identical with and without this call. */
 SvrStatus svr_loss_prepare(SvrContext* ctx, const float* target, int32_t W, int32_t H, const SvrLossOpts* opts);
 
+/* NEXT-3: the structure-aware penalty L_SSIM of eq. 17 and its gradient. The paper names the term
+ * only; reading R14: L_SSIM = 1 - mean over pixels and channels of the structural similarity index
+ * (Wang et al. 2004) with an 11-tap Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2.
+ * render, target, dL_dimage: device [H,W,3] floats. dL_dimage = lambda * dL_SSIM/d render, or += it when
+ * accumulate != 0 (so that it adds to svr_loss_grad's output); *loss (device float) = L_SSIM (not scaled by lambda).
+ * Errors: null pointers / empty image -> SVR_ERR_INVALID_ARG. */
+SvrStatus svr_ssim_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H,
+                             float lambda, int32_t accumulate, float* dL_dimage, float* loss);
+
 /* (4) backward compositing: gradients of sum(dL_dimage * image) w.r.t. corner raw densities and SH
  * coefficients. `image` is svr_forward's output for this frame (the suffix colour is image - prefix).
  * grad_raw_density[n,8] and grad_sh[n,(D+1)^2,3] ACCUMULATE (+=; caller zeroes) so several views sum

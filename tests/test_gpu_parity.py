@@ -236,6 +236,33 @@ def test_loss_prepare_same_result(orc, svr):
     check(*ctx.svr_loss_grad(r_dev, t_dev[0], 0.6), 0)
 
 
+def test_ssim_loss_grad_parity(svr):
+    """NEXT-3: L_SSIM and dL/dR against oracle/ssim.py on images that span several 16 x 16 tiles with a ragged edge, on
+    one smaller than the 11 x 11 window, and accumulating onto an existing gradient."""
+    from oracle import ssim
+    pkg, ctx, torch = svr
+    rng = np.random.default_rng(11)
+    for (H, W) in [(75, 133), (33, 17), (3, 5), (16, 16)]:
+        base = rng.uniform(0, 1, size=(H, W, 3)) * np.linspace(0.1, 1, W)[None, :, None]
+        base[H // 2:, :, :] = 0.4                                     # a flat region: the variances cancel against C2
+        target = np.clip(base, 0, 1).astype(np.float32)
+        render = np.clip(target + rng.normal(0, 0.05, size=target.shape), 0, 1).astype(np.float32)
+        render[H // 2:, : W // 2, :] = target[H // 2:, : W // 2, :]   # and a region where the render is exact
+        L_ref, g_ref = ssim.ssim_loss_and_grad(render, target)
+        dL, loss = ctx.svr_ssim_loss_grad(torch.from_numpy(render).cuda(), torch.from_numpy(target).cuda(), 1.0)
+        ctx.synchronize()
+        assert abs(float(loss.item()) - L_ref) <= 2e-6 * max(abs(L_ref), 1e-3), (H, W, float(loss.item()), L_ref)
+        assert rel_l2(dL.cpu().numpy(), g_ref) <= 1e-5, (H, W)
+        # accumulate: dL += lambda * grad
+        prior = rng.normal(0, 1e-4, size=target.shape).astype(np.float32)
+        acc = torch.from_numpy(prior.copy()).cuda()
+        ctx.svr_ssim_loss_grad(torch.from_numpy(render).cuda(), torch.from_numpy(target).cuda(), 0.2, dL=acc, accumulate=True)
+        ctx.synchronize()
+        assert rel_l2(acc.cpu().numpy(), prior.astype(np.float64) + 0.2 * g_ref) <= 1e-5, (H, W)
+    with pytest.raises(RuntimeError):
+        ctx.svr_ssim_loss_grad(torch.zeros((0, 4, 3), device="cuda"), torch.zeros((0, 4, 3), device="cuda"))
+
+
 # ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
