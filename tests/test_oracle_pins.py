@@ -760,3 +760,33 @@ def test_ssim_moments_brute_force_and_gradient_fd():
         Rm[y, x, ch] -= h
         fd = (ssim.ssim_loss_and_grad(Rp, I)[0] - ssim.ssim_loss_and_grad(Rm, I)[0]) / (2 * h)
         assert abs(fd - grad[y, x, ch]) <= 1e-6 * max(abs(fd), 1e-4), (y, x, ch, fd, grad[y, x, ch])
+
+
+# ---------------------------------------------------------------------------------------------
+# L_tv (eq. 17; R15: L1 total variation over the 12 edges of every cell)
+# ---------------------------------------------------------------------------------------------
+def test_tv_constant_linear_scaling_fd():
+    from oracle import tv
+    assert len(tv.EDGES) == 12 and all(bin(a ^ b).count("1") == 1 and a < b for a, b in tv.EDGES) and len(set(tv.EDGES)) == 12
+    L, g = tv.tv_loss_and_grad(np.full((5, 8), 0.7))
+    assert L == 0.0 and not g.any()
+    # corners of the unit cell sampled from alpha x + beta y + gamma z + d: four edges per axis, each |coefficient| long
+    al, be, ga = 0.3, -1.1, 0.45
+    corners = np.array([[al * (c & 1) + be * ((c >> 1) & 1) + ga * (c >> 2) + 2.0 for c in range(8)]])
+    L, g = tv.tv_loss_and_grad(np.repeat(corners, 3, axis=0))
+    assert abs(L - (abs(al) + abs(be) + abs(ga)) / 3.0) < 1e-15
+    np.testing.assert_allclose(g.sum(axis=1), 0.0, atol=1e-16)           # a constant offset does not change the loss
+    rng = np.random.default_rng(8)
+    raw = rng.normal(0, 1, size=(7, 8))
+    L0, g0 = tv.tv_loss_and_grad(raw)
+    assert abs(tv.tv_loss_and_grad(-2.5 * raw + 4.0)[0] - 2.5 * L0) < 1e-14
+    # brute force over all corner pairs at Hamming distance 1
+    want = sum(abs(raw[v, a] - raw[v, b]) for v in range(7) for a in range(8) for b in range(a + 1, 8) if bin(a ^ b).count("1") == 1)
+    assert abs(L0 - want / (12 * 7)) < 1e-15
+    h = 1e-7
+    for (v, c) in [(0, 0), (3, 5), (6, 7), (2, 2)]:
+        rp, rm = raw.copy(), raw.copy()
+        rp[v, c] += h
+        rm[v, c] -= h
+        fd = (tv.tv_loss_and_grad(rp)[0] - tv.tv_loss_and_grad(rm)[0]) / (2 * h)
+        assert abs(fd - g0[v, c]) < 1e-8
