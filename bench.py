@@ -425,6 +425,23 @@ def main():
                               "roofline": {"bound": "hbm", "achieved": adam_bytes / (ms_adam * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                            "unit": "GB/s", "frac": adam_bytes / (ms_adam * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
 
+        # NEXT-4 (part): L_tv over the raw corner densities, gradient accumulated into g_raw
+        lt = torch.empty(1, dtype=torch.float32, device=dev)
+        ctx.svr_tv_loss_grad(vox.raw, g_raw, 1e-3, loss=lt)
+        e0, e1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(reps):
+                ctx.svr_tv_loss_grad(vox.raw, g_raw, 1e-3, loss=lt)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        ms_tv = e0.elapsed_time(e1) / reps
+        tv_bytes = sc.n * 96
+        line["next4_tv"] = {"what": "svr_tv_loss_grad over raw [n,8] (32 B read + 64 B read-modify-write per voxel); outside `value`",
+                            "ms": ms_tv, "L_tv": float(lt.item()),
+                            "roofline": {"bound": "hbm", "achieved": tv_bytes / (ms_tv * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                         "unit": "GB/s", "frac": tv_bytes / (ms_tv * 1e-3) / 1e9 / peaks["hbm_gbs"]}}
+
         # NEXT-3 (part): L_SSIM and its gradient on the last render against its target, accumulated onto dL
         ls = torch.empty(1, dtype=torch.float32, device=dev)
         ctx.svr_ssim_loss_grad(image, targets[0], 0.2, dL=dL, loss=ls, accumulate=True)

@@ -246,6 +246,14 @@ SvrStatus svr_gather_corners(SvrContext* ctx, const float* grid, const uint32_t*
 SvrStatus svr_scatter_add_corners(SvrContext* ctx, const float* grad_raw_density, const uint32_t* corner_index, int64_t n,
                                   float* grad_grid);
 
+/* NEXT-4: the total-variation term L_tv of eq. 17 ("total-variation on the sparse density field"). The
+ * paper gives no formula; reading R15: L_tv = 1/(12 n) sum_v sum over the 12 edges (a,b) of the cell
+ * |raw[v,a] - raw[v,b]| on the raw corner densities. grad_raw_density[n,8] += lambda * dL_tv/draw (sign(0) = 0);
+ * *loss (device float) = L_tv (not scaled by lambda). Device pointers, 16-byte aligned; n >= 1. With shared grid points
+ * the gradient goes on through svr_scatter_add_corners. */
+SvrStatus svr_tv_loss_grad(SvrContext* ctx, const float* raw_density, int64_t n, float lambda, float* grad_raw_density,
+                           float* loss);
+
 /* Synchronous device->host copy of `bytes` from a pointer returned by the hooks above (tests). */
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes);
 

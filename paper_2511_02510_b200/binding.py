@@ -20,7 +20,7 @@ SVR_OK, SVR_ERR_INVALID_ARG, SVR_ERR_CUDA, SVR_ERR_WORKSPACE, SVR_ERR_UNSUPPORTE
 _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR_WORKSPACE", 4: "SVR_ERR_UNSUPPORTED"}
 
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
-           "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare", "svr_ssim_loss_grad",
+           "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare", "svr_ssim_loss_grad", "svr_tv_loss_grad",
            "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
@@ -84,6 +84,7 @@ def _load():
                                   C.POINTER(SvrLossOpts), C.c_void_p, C.c_void_p]
     lib.svr_ssim_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_int32,
                                        C.c_void_p, C.c_void_p]
+    lib.svr_tv_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_void_p, C.c_void_p]
     lib.svr_loss_prepare.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(SvrLossOpts)]
     lib.svr_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 5
     lib.svr_backward_heads.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 9
@@ -331,6 +332,15 @@ class Context:
             loss = torch.empty(1, dtype=torch.float32, device=render.device)
         self._check(_lib.svr_ssim_loss_grad(self.handle, _p(render), _p(target), W, H, lam, 1 if accumulate else 0, _p(dL), _p(loss)))
         return dL, loss
+
+    def svr_tv_loss_grad(self, raw: torch.Tensor, grad_raw: torch.Tensor, lam: float = 1.0, loss=None):
+        """grad_raw += lam * dL_tv/draw; returns the device scalar L_tv."""
+        _dev(raw, torch.float32, "raw")
+        _dev(grad_raw, torch.float32, "grad_raw")
+        if loss is None:
+            loss = torch.empty(1, dtype=torch.float32, device=raw.device)
+        self._check(_lib.svr_tv_loss_grad(self.handle, _p(raw), int(raw.shape[0]), lam, _p(grad_raw), _p(loss)))
+        return loss
 
     def svr_loss_grad(self, render: torch.Tensor, target: torch.Tensor, gamma: float, eps: float = 1e-3,
                       percentile: float = 0.99, sobel_source: int = 0, dL=None, loss=None):

@@ -103,3 +103,77 @@ extern "C" SvrStatus svr_scatter_add_corners(SvrContext* ctx, const float* grad_
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }
+
+// ---- L_tv (NEXT-4; eq. 17; R15) ----
+// L_tv = 1/(12 N) sum_v sum over the 12 cell edges |raw_a - raw_b|; grad_raw += lambda dL/draw. One thread per voxel, 64 B
+// read + 64 B read-modify-write; the loss is summed in fp64 (one atomic per block) and written by a second, one-thread kernel.
+namespace {
+
+__device__ __forceinline__ float sgnf(float x) { return (float)((x > 0.f) - (x < 0.f)); }
+
+__global__ void __launch_bounds__(256) tv_kernel(const float4* __restrict__ raw, int64_t n, float scale, float4* __restrict__ grad_raw,
+                                                 double* __restrict__ acc) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float local = 0.f;
+    if (v < n) {
+        const float4 a = raw[2 * v], b = raw[2 * v + 1];
+        const float r[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+        float g[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax)
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                if (!((c >> ax) & 1)) {
+                    const float d = r[c] - r[c | (1 << ax)];
+                    local += fabsf(d);
+                    const float sg = sgnf(d);
+                    g[c] += sg;
+                    g[c | (1 << ax)] -= sg;
+                }
+        float4 ga = grad_raw[2 * v], gb = grad_raw[2 * v + 1];
+        ga.x = fmaf(scale, g[0], ga.x); ga.y = fmaf(scale, g[1], ga.y); ga.z = fmaf(scale, g[2], ga.z); ga.w = fmaf(scale, g[3], ga.w);
+        gb.x = fmaf(scale, g[4], gb.x); gb.y = fmaf(scale, g[5], gb.y); gb.z = fmaf(scale, g[6], gb.z); gb.w = fmaf(scale, g[7], gb.w);
+        grad_raw[2 * v] = ga;
+        grad_raw[2 * v + 1] = gb;
+    }
+    __shared__ double wsum[8];
+    double s = (double)local;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += wsum[w];
+        if (t != 0.0) atomicAdd(acc, t);
+    }
+}
+
+__global__ void tv_finish_kernel(const double* __restrict__ acc, int64_t n, float* __restrict__ loss) {
+    *loss = (float)(*acc / (12.0 * (double)n));
+}
+
+}  // namespace
+
+extern "C" SvrStatus svr_tv_loss_grad(SvrContext* ctx, const float* raw_density, int64_t n, float lambda, float* grad_raw_density,
+                                      float* loss) {
+    if (!ctx || !raw_density || !grad_raw_density || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (n < 1 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    if (((uintptr_t)raw_density | (uintptr_t)grad_raw_density) & 15) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "arrays must be 16-byte aligned");
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    double* acc = nullptr;
+    SVR_TRY(svr_alloc(ctx, (void**)&acc, 64));
+    SvrStatus st = SVR_OK;
+    cudaError_t e = cudaMemsetAsync(acc, 0, sizeof(double), ctx->stream);
+    if (e == cudaSuccess) {
+        const float scale = (float)((double)lambda / (12.0 * (double)n));
+        tv_kernel<<<(unsigned int)((n + 255) / 256), 256, 0, ctx->stream>>>(reinterpret_cast<const float4*>(raw_density), n, scale,
+                                                                           reinterpret_cast<float4*>(grad_raw_density), acc);
+        tv_finish_kernel<<<1, 1, 0, ctx->stream>>>(acc, n, loss);
+        ctx->launches += 2;
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "tv: %s", cudaGetErrorString(e));
+    svr_free(ctx, acc, 64);
+    return st;
+}

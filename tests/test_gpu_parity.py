@@ -263,6 +263,25 @@ def test_ssim_loss_grad_parity(svr):
         ctx.svr_ssim_loss_grad(torch.zeros((0, 4, 3), device="cuda"), torch.zeros((0, 4, 3), device="cuda"))
 
 
+def test_tv_loss_grad_parity(svr):
+    """NEXT-4: L_tv and its gradient against oracle/tv.py; the gradient is a multiple of 1/(12 n) and accumulates."""
+    from oracle import tv
+    pkg, ctx, torch = svr
+    rng = np.random.default_rng(12)
+    for n in [1, 255, 1000, 70001]:
+        raw = rng.normal(0, 1, size=(n, 8)).astype(np.float32)
+        raw[n // 2:, :4] = raw[n // 2:, 4:]                           # ties: sign(0) = 0 on the z edges of half the voxels
+        prior = rng.normal(0, 1e-3, size=(n, 8)).astype(np.float32)
+        L_ref, g_ref = tv.tv_loss_and_grad(raw)
+        g = torch.from_numpy(prior.copy()).cuda()
+        loss = ctx.svr_tv_loss_grad(torch.from_numpy(raw).cuda(), g, 0.5)
+        ctx.synchronize()
+        assert abs(float(loss.item()) - L_ref) <= 1e-6 * L_ref
+        np.testing.assert_allclose(g.cpu().numpy(), prior.astype(np.float64) + 0.5 * g_ref, rtol=2e-6, atol=1e-9)
+    with pytest.raises(pkg.SvrError):
+        ctx.svr_tv_loss_grad(torch.zeros((0, 8), device="cuda"), torch.zeros((0, 8), device="cuda"))
+
+
 # ---------------------------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------------------------
