@@ -463,6 +463,14 @@ __global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamD
     int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= s.n) return;
     const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+    {
+        // the SH row and the corner densities are needed only after the division-heavy projection: start them now (90 % of
+        // the voxels are visible), so that their DRAM latency runs beside it
+        const char* psh = reinterpret_cast<const char*>(s.sh + v * ((DEG + 1) * (DEG + 1) * 3));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(psh));
+        if (DEG >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(psh + 12 * (DEG + 1) * (DEG + 1) - 4));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(s.raw + v * 8));
+    }
     ushort4 r = voxel_rect(s, c, q);
     rects[v] = r;
     if (r.x > r.z) return;
