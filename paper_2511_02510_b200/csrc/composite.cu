@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
         // Double-buffered staging: the ring is two halves of 32 slots. While one half is walked, the records of the
         // next batch are already on their way into the other half (cp.async: no registers held, no stall on the load).
         uint32_t base = start;
-        auto stage = [&](int half, uint32_t rec_i) -> int {
+        auto stage = [&](int half) -> int {
             int cnt = 0;
             while (cnt < 32 && base < end) {
                 const uint32_t idx = base + lane;
@@ -255,7 +255,6 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                     cp_async16(&S.g0[slot], rec); cp_async16(&S.g1[slot], rec + 1); cp_async16(&S.r0[slot], rec + 2);
                     cp_async16(&S.r1[slot], rec + 3); cp_async16(&S.col[slot], rec + 4);
                     S.M[slot] = M;
-                    if (REC) rec_out[(size_t)rec_i * TRAV_WORDS + 32 + cnt + rank] = vid;
                 }
                 if (STATS) { n_read += (idx < end && (int)lane < adv); n_surv += (M != 0u); }
                 cnt += __popc(m);
@@ -264,11 +263,11 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
             asm volatile("cp.async.commit_group;" ::: "memory");
             return cnt;
         };
-        int head = 0, count = stage(0, n_rec);
+        int head = 0, count = stage(0);
         while (count > 0) {
             asm volatile("cp.async.wait_all;" ::: "memory");
             __syncwarp();
-            const int count_next = stage(head ^ 32, n_rec + 1);       // in flight during the walk below
+            const int count_next = stage(head ^ 32);       // in flight during the walk below
             // ---- walk up to 32 staged voxels, every lane through its own candidates ----
             const int n = count;
             unsigned int cand = transpose32(lane < n ? S.M[head + lane] : 0u, lane);
@@ -296,7 +295,8 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                 }
                 if (REC) {
                     uint32_t* r = rec_out + (size_t)n_rec * TRAV_WORDS;
-                    r[lane] = hits;                                    // the list entries were written when they were staged
+                    r[lane] = hits;
+                    if (lane < n) r[32 + lane] = __float_as_uint(S.g1[(head + lane) & (RING - 1)].w);    // the staged voxel ids
                     if (lane == 0) r[64] = (uint32_t)n;
                     ++n_rec;
                 }
