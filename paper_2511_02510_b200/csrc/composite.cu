@@ -284,8 +284,9 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                         const int k = __ffs(cand) - 1;
                         cand &= cand - 1;
                         const float4 a = S.g0[(head + k) & (RING - 1)];
-                        // dilation: a bound on what the lo parts and the rounding can move, so no true hit is lost
-                        const float hd = fmaf(fabsf(a.x) + fabsf(a.y) + fabsf(a.z), 4.8e-7f, a.w * 1.000002f);
+                        // dilated half edge (voxel_record_dev): a bound on what the lo parts and the rounding can move, so no
+                        // true hit is lost
+                        const float hd = S.col[(head + k) & (RING - 1)].w;
                         const float cx = a.x * ray.inv[0], cy = a.y * ray.inv[1], cz = a.z * ray.inv[2];
                         const float wx = hd * ray.ainv[0], wy = hd * ray.ainv[1], wz = hd * ray.ainv[2];
                         const float s0 = fmaxf(fmaxf(cx - wx, cy - wy), fmaxf(cz - wz, 0.f));

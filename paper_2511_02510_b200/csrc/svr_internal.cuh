@@ -94,7 +94,9 @@ __device__ __forceinline__ void voxel_record_dev(const SceneDev& s, const CamDev
     out[1] = make_float4((float)(gx - (double)hx), (float)(gy - (double)hy), (float)(gz - (double)hz), __uint_as_float(vid));
     out[2] = make_float4(c0 * L2E, cx * L2E, cy * L2E, cz * L2E);
     out[3] = make_float4(cxy * L2E, cxz * L2E, cyz * L2E, cxyz * L2E);
-    out[4] = col;
+    // .w: the half edge dilated by a bound on what the lo parts and the rounding can move (the forward's conservative slab test);
+    // the clamp mask of the colour stays in rgbm
+    out[4] = make_float4(col.x, col.y, col.z, fmaf(fabsf(hx) + fabsf(hy) + fabsf(hz), 4.8e-7f, (0.5f * ef) * 1.000002f));
 }
 
 struct SvrFrame {
