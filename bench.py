@@ -319,7 +319,7 @@ def main():
     if dom in flop:
         achieved = hits * flop[dom] / (stage_ms[dom] * 1e-3) / 1e12
         traffic = None      # DRAM bytes of one launch of this kernel from the committed ncu capture (full-size C4 only)
-        tpath = os.path.join(ROOT, "profiles", "r1m_traffic.csv")
+        tpath = os.path.join(ROOT, "profiles", "r1q_traffic.csv")
         if os.path.exists(tpath) and args.workload == "C4" and args.n_voxels is None and args.res_scale == 1.0:
             with open(tpath) as fh:
                 rows = dict(line.strip().split(",") for line in fh.readlines()[1:] if "," in line)
