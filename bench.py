@@ -298,6 +298,22 @@ def main():
 
     peak_vram = int(torch.cuda.max_memory_allocated(dev)) + int(ctx.workspace_peak_bytes)
 
+    # ---- context (not part of `value`): a whole training iteration = the step + the fused Adam update of both parameter
+    # tensors, which also clears the gradients the next backward accumulates into. lr = 0: the parameters do not move. ----
+    adam_state = [torch.zeros_like(t.view(-1)) for t in (vox.raw, vox.raw, vox.sh, vox.sh)]
+    it_no = [0]
+
+    def train_iter(i):
+        step(i)
+        it_no[0] += 1
+        ctx.svr_adam_step(vox.raw.view(-1), g_raw.view(-1), adam_state[0], adam_state[1], 0.0, 0.9, 0.999, 1e-8, it_no[0], zero_grad=True)
+        ctx.svr_adam_step(vox.sh.view(-1), g_sh.view(-1), adam_state[2], adam_state[3], 0.0, 0.9, 0.999, 1e-8, it_no[0], zero_grad=True)
+
+    for i in range(3):
+        train_iter(i)
+    ms_iter, _ = timed(train_iter, args.steps)
+    del adam_state
+
     # ---- work counters (outside the timed region): hits / tests per view ----
     stats = []
     for k in sorted({camera_index(i, rank, len(ccams)) for i in range(args.steps)}):
@@ -349,7 +365,9 @@ def main():
             "work_per_view": {"hits": hits, "slab_tests": tests, "entries_staged": staged,
                               "list_entries": float(np.mean([s["entries"] for s in stats])),
                               "warp_voxel_pairs": float(np.mean([s["warp_voxel_pairs"] for s in stats]))},
-            "peak_vram_bytes": peak_vram}
+            "peak_vram_bytes": peak_vram,
+            "train_iteration": {"what": "step + svr_adam_step (zero_grad) over raw and sh; outside `value`",
+                                "ms": ms_iter / args.steps, "iterations_per_s": args.steps * world / (ms_iter * 1e-3)}}
 
     # ---- NEXT-1 (not part of `value`): one depth-quantile pruning step on the w_max the steps above gathered, and the
     # compaction of the voxel arrays by its keep mask; HBM-bound streaming kernels, timed with CUDA events ----
