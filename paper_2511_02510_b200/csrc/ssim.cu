@@ -150,16 +150,18 @@ extern "C" SvrStatus svr_ssim_loss_grad(SvrContext* ctx, const float* render, co
     if (!ctx || !render || !target || !dL_dimage || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (W <= 0 || H <= 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "empty image");
     SVR_CUDA(ctx, cudaSetDevice(ctx->device));
-    static bool init = false;
     const int smem_stats = 5 * TH * OUTF * (int)sizeof(double) + 2 * TH * ROWF * (int)sizeof(float);
-    if (!init) {
-        double g[11], sum = 0.0;
+    static double g[11];
+    static bool have_g = false;
+    if (!have_g) {
+        double sum = 0.0;
         for (int k = 0; k < 11; ++k) { g[k] = exp(-(double)((k - 5) * (k - 5)) / (2.0 * 1.5 * 1.5)); sum += g[k]; }
         for (int k = 0; k < 11; ++k) g[k] /= sum;
-        SVR_CUDA(ctx, cudaMemcpyToSymbol(c_g, g, sizeof(g)));
-        SVR_CUDA(ctx, cudaFuncSetAttribute(ssim_stats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_stats));
-        init = true;
+        have_g = true;
     }
+    // per call, on the context's stream: the constant and the attribute belong to the current device
+    SVR_CUDA(ctx, cudaMemcpyToSymbolAsync(c_g, g, sizeof(g), 0, cudaMemcpyHostToDevice, ctx->stream));
+    SVR_CUDA(ctx, cudaFuncSetAttribute(ssim_stats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_stats));
     const size_t nf = (size_t)W * H * 3, map_bytes = sizeof(float) * nf, bytes = 3 * map_bytes + 256;
     unsigned char* ws = nullptr;
     SVR_TRY(svr_alloc(ctx, (void**)&ws, bytes));
