@@ -188,7 +188,7 @@ class Frame:
             pass
 
     def refresh_colors(self):
-        """svr_frame_refresh_colors: re-capture raw_density / sh values (colours + per-entry records); the lists stay."""
+        """svr_frame_refresh_colors: re-capture raw_density / sh values (colours + per-voxel view records); the lists stay."""
         self.ctx._check(_lib.svr_frame_refresh_colors(self.ctx.handle, C.c_void_p(self.handle)))
 
     @property

@@ -8,9 +8,10 @@
 //   1. cull: 32 entries at a time, lane i reads entry i's pixel rectangle (in list order, so the read is
 //      coalesced) and computes the 32-bit mask M of this warp's pixels it covers. M == 0 => the entry is
 //      skipped by this warp (76% of (warp, entry) pairs on C4).
-//   2. stage: surviving lanes copy their packed voxel record (pack_entries_kernel: centre relative to the
-//      camera as hi+lo floats, half edge, density coefficients, per-view colour), in list order, into a
-//      warp-private shared-memory ring.
+//   2. stage: surviving lanes copy their voxel's 80-byte view record (voxel_record_dev, svr_internal.cuh: centre
+//      relative to the camera as hi+lo floats, half edge, density coefficients, per-view colour, dilated half edge),
+//      gathered by the voxel id read beside the rectangle, in list order, into a warp-private shared-memory ring
+//      (cp.async, double-buffered).
 //   3. test: once >= 32 survivors are staged (or the list ends), the 32x32 bit matrix M[slot][pixel] is
 //      transposed across the warp with 5 shuffles, giving every lane the bitmask of slots that cover ITS
 //      pixel. Each lane pops its own candidates (ffs) and slab-tests them against a slightly dilated box:
@@ -18,8 +19,9 @@
 //   4. hits: each lane pops its own hits: precise slab test, K samples, eqs. 2-4; w_max (eq. 5,
 //      P:95) by atomicMax guarded by a plain read (w_max only grows). Front-to-back order per pixel is kept
 //      because slots are in list order.
-// Backward (backward_packed_kernel): same cull / stage / test, then the hits are compacted into a queue and
-// processed 32 at a time with all lanes busy; see the comment above that kernel.
+// With REC the forward also writes, per batch, the staged voxel ids and every pixel's hit mask (the traversal record).
+// Backward (backward_packed_kernel): replays that record, or runs the same cull / stage / test itself; then the hits
+// are compacted into a queue and processed 32 at a time with all lanes busy; see the comment above that kernel.
 //
 // Density: the trilinear raw density is staged as polynomial coefficients (c0, cx, cy, cz, cxy, cxz, cyz,
 // cxyz), pre-multiplied by log2(e), so a sample costs 7 FMA + one EX2 instead of 7 lerps (14 ops) + MUL + EX2.
