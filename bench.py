@@ -157,9 +157,21 @@ def aggregate_value(rays_per_step: int, steps: int, world: int, ms: float) -> fl
     return rays_per_step * steps * world / (ms * 1e-3) / 1e6
 
 
+def morton_order(sc):
+    """Permutation that sorts the voxels by the Morton code of their cell at the finest level (z-order of the octree)."""
+    ij = sc.ijkl.astype(np.uint64)
+    shift = (np.uint64(sc.max_level) - ij[:, 3]).astype(np.uint64)
+    code = np.zeros(sc.n, dtype=np.uint64)
+    for b in range(sc.max_level):
+        for a in range(3):
+            code |= (((ij[:, a] << shift) >> np.uint64(b)) & np.uint64(1)) << np.uint64(3 * b + a)
+    return np.argsort(code, kind="stable")
+
+
 def workload_config(cfg, args):
     cam = cfg.cameras[0]
-    return {"workload": f"{cfg.name}: {cfg.scene.n} voxels, {cam.W}x{cam.H}, {len(cfg.cameras)} cameras round-robin, K={cfg.K}, "
+    name = cfg.name + (" (voxels stored in Morton order: NOT the metric's config)" if args.scene_order == "morton" else "")
+    return {"workload": f"{name}: {cfg.scene.n} voxels, {cam.W}x{cam.H}, {len(cfg.cameras)} cameras round-robin, K={cfg.K}, "
                         f"SH degree {cfg.scene.sh_degree}, T_min={cfg.T_min}, gamma={cfg.gamma}, backward emits w_max",
             "seed": cfg.seed, "rays_per_step": cam.W * cam.H,
             "l2": "inputs larger than L2 (scene parameters 928 MB at full size); no explicit flush",
@@ -179,6 +191,9 @@ def main():
                     help="rays per step of the CPU oracle sample (default: sized so that the whole run takes about two minutes)")
     ap.add_argument("--cpu-baseline-rays", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scene-order", default="config", choices=["config", "morton"],
+                    help="config: the storage order the workload recipe gives (random: BASELINE's configs); morton: the same voxels "
+                         "stored in octree (Morton) order, as a trainer that keeps its octree sorted would pass them (context only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -201,6 +216,9 @@ def main():
 
     cfg = make_config(args.workload, n_voxels=args.n_voxels, res_scale=args.res_scale)
     sc, cams = cfg.scene, cfg.cameras
+    if args.scene_order == "morton":
+        order = morton_order(sc)
+        sc.ijkl, sc.raw, sc.sh = sc.ijkl[order], sc.raw[order], sc.sh[order]
     W, H = cams[0].W, cams[0].H
     rays = W * H
     ctx = pkg.Context(local_rank, workspace_budget_bytes=cfg.workspace_budget_bytes)
