@@ -460,26 +460,46 @@ __global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamD
                                                                 ushort4* __restrict__ rects, uint32_t* __restrict__ bcount,
                                                                 int* __restrict__ bigdiff, unsigned long long* __restrict__ totals,
                                                                 float4* __restrict__ rgbm, float4* __restrict__ vrec) {
-    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= s.n) return;
-    const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
-    {
-        // the SH row and the corner densities are needed only after the division-heavy projection: start them now (90 % of
-        // the voxels are visible), so that their DRAM latency runs beside it
-        const char* psh = reinterpret_cast<const char*>(s.sh + v * ((DEG + 1) * (DEG + 1) * 3));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(psh));
-        if (DEG >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(psh + 12 * (DEG + 1) * (DEG + 1) - 4));
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(s.raw + v * 8));
-    }
-    ushort4 r = voxel_rect(s, c, q);
-    rects[v] = r;
-    if (r.x > r.z) return;
-    {
-        const float4 col = voxel_color_dev<DEG>(s, c, q, v);
-        rgbm[v] = col;
-        voxel_record_dev(s, c, q, (uint32_t)v, col, vrec);
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    ushort4 r = make_ushort4(1, 0, 0, 0);      // "not visible"
+    bool vis = false;
+    if (v < s.n) {
+        const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+        {
+            // the SH row and the corner densities are needed only after the division-heavy projection: start them now (90 % of
+            // the voxels are visible), so that their DRAM latency runs beside it
+            const char* psh = reinterpret_cast<const char*>(s.sh + v * ((DEG + 1) * (DEG + 1) * 3));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(psh));
+            if (DEG >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(psh + 12 * (DEG + 1) * (DEG + 1) - 4));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(s.raw + v * 8));
+        }
+        r = voxel_rect(s, c, q);
+        rects[v] = r;
+        vis = r.x <= r.z;
+        if (vis) {
+            const float4 col = voxel_color_dev<DEG>(s, c, q, v);
+            rgbm[v] = col;
+            voxel_record_dev(s, c, q, (uint32_t)v, col, vrec);
+        }
     }
     const int i0 = r.x >> 4, i1 = r.z >> 4, j0 = r.y >> 4, j1 = r.w >> 4;
+    // A voxel inside one tile that has one octant (69 % of the visible ones on C4) has one bucket: the lanes of a warp that
+    // share it send ONE atomic. In a scene stored in octree order neighbours share buckets and per-lane atomics serialise on
+    // the same address (0.38 instead of 0.28 ms); in a randomly ordered scene the match costs one instruction.
+    uint32_t key = 0xFFFFFFFFu - (uint32_t)lane;        // unique: no peers
+    bool single = false;
+    if (vis && i0 == i1 && j0 == j1) {
+        const int tile = j0 * c.tiles_x + i0;
+        const unsigned m = masks[tile];
+        if ((m & (m - 1u)) == 0u) { single = true; key = (uint32_t)(tile * 8 + __ffs(m) - 1); }
+    }
+    const unsigned peers = __match_any_sync(0xffffffffu, key);
+    if (single) {
+        if ((peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&bcount[key], (uint32_t)__popc(peers));
+        return;
+    }
+    if (!vis) return;
     if ((i1 - i0 + 1) * (j1 - j0 + 1) > BIG_TILES) {
         const int sx = c.tiles_x + 1;
         atomicAdd(&totals[1], 1ULL);
@@ -614,13 +634,34 @@ __global__ void __launch_bounds__(256) scatter_small_kernel(SceneDev s, CamDev c
                                                             const uint8_t* __restrict__ masks, uint32_t* __restrict__ cursor,
                                                             uint64_t* __restrict__ ent, int vb, uint32_t* __restrict__ big_list,
                                                             unsigned int* __restrict__ big_count) {
-    int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= s.n) return;
-    const ushort4 r = rects[v];
-    if (r.x > r.z) return;
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    ushort4 r = make_ushort4(1, 0, 0, 0);
+    if (v < s.n) r = rects[v];
+    const bool vis = r.x <= r.z;
     const int i0 = r.x >> 4, i1 = r.z >> 4, j0 = r.y >> 4, j1 = r.w >> 4;
+    uint64_t code = 0ull;
+    if (vis) code = voxel_code(reinterpret_cast<const uint2*>(s.ijkl)[v], s.max_level);
+    // one-bucket voxels: one cursor atomic per distinct bucket of the warp (see rect_bucket_count_kernel)
+    uint32_t key = 0xFFFFFFFFu - (uint32_t)lane;
+    bool single = false;
+    int o1 = 0;
+    if (vis && i0 == i1 && j0 == j1) {
+        const int tile = j0 * c.tiles_x + i0;
+        const unsigned m = masks[tile];
+        if ((m & (m - 1u)) == 0u) { single = true; o1 = __ffs(m) - 1; key = (uint32_t)(tile * 8 + o1); }
+    }
+    const unsigned peers = __match_any_sync(0xffffffffu, key);
+    const int leader = __ffs(peers) - 1;
+    uint32_t pos0 = 0u;
+    if (single && lane == leader) pos0 = atomicAdd(&cursor[key], (uint32_t)__popc(peers));
+    pos0 = __shfl_sync(0xffffffffu, pos0, leader);
+    if (single) {
+        ent[pos0 + __popc(peers & ((1u << lane) - 1u))] = ((code ^ flip_mask(o1, s.max_level)) << vb) | (uint64_t)v;
+        return;
+    }
+    if (!vis) return;
     if ((i1 - i0 + 1) * (j1 - j0 + 1) > BIG_TILES) { big_list[atomicAdd(big_count, 1u)] = (uint32_t)v; return; }
-    const uint64_t code = voxel_code(reinterpret_cast<const uint2*>(s.ijkl)[v], s.max_level);
     for (int j = j0; j <= j1; ++j)
         for (int i = i0; i <= i1; ++i) {
             const int tile = j * c.tiles_x + i;
