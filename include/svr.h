@@ -167,6 +167,11 @@ SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm);
 SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* image,
                             uint64_t* stats_host);
 void svr_set_stage_timing(SvrContext* ctx, int enabled);
+/* Microbenchmarks of the machine peaks the compositing kernels are set against, run on the context's device and
+ * stream, synchronising: out_host[0] = FP32 FMA rate in TFLOP/s (FFMA chains on every SM, FMA = 2 flop), out_host[1] = the
+ * same with packed FFMA2 (fma.rn.f32x2), out_host[2] = 1e9 red.global.add.v4.f32 per second into an L2-resident table (the
+ * backward pass's gradient reductions), out_host[3] = 1e9 warp instructions issued per second (integer ALU chains). */
+SvrStatus svr_measure_peaks(SvrContext* ctx, float* out_host /* [4] */);
 int svr_num_stages(void);
 /* Experiments / tests only: bit 3 (8) selects the first list-build design (per-voxel scan + global radix sort, the
  * fallback when Morton code + voxel id exceed 64 bits); bit 10 (1024) prints stream idle gaps per stage. */

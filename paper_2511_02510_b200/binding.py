@@ -22,7 +22,7 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare", "svr_ssim_loss_grad", "svr_tv_loss_grad",
            "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
-           "svr_forward_stats", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
+           "svr_forward_stats", "svr_measure_peaks", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
            "svr_gather_corners", "svr_scatter_add_corners"]
 
@@ -77,6 +77,7 @@ def _load():
     lib.svr_kernel_launches.restype = C.c_int64
     lib.svr_preprocess.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.POINTER(SvrCamera), C.POINTER(C.c_void_p)]
     lib.svr_frame_refresh_colors.argtypes = [C.c_void_p, C.c_void_p]
+    lib.svr_measure_peaks.argtypes = [C.c_void_p, C.c_void_p]
     lib.svr_frame_release.argtypes = [C.c_void_p, C.c_void_p]
     lib.svr_frame_release.restype = None
     lib.svr_forward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 4
@@ -286,6 +287,12 @@ class Context:
 
     def svr_set_stage_timing(self, enabled: bool):
         _lib.svr_set_stage_timing(self.handle, 1 if enabled else 0)
+
+    def svr_measure_peaks(self) -> dict:
+        out = (C.c_float * 4)()
+        self._check(_lib.svr_measure_peaks(self.handle, C.cast(out, C.c_void_p)))
+        return {"fp32_ffma_tflops": float(out[0]), "fp32_ffma2_tflops": float(out[1]), "l2_red_v4_gops": float(out[2]),
+                "issue_gwarp_inst_per_s": float(out[3])}
 
     def svr_get_stage_times(self, reset: bool = True) -> dict:
         n = _lib.svr_num_stages()

@@ -4,31 +4,37 @@
 // barrier anywhere): a barrier per staged chunk cost 37% of the issue slots in the first version
 // (profiles/r1a_*), because the 8 blocks of a tile see very different numbers of voxels.
 //
-// Forward (composite_kernel), per warp, over the tile's sorted (tile, octant) list:
+// Both kernels walk the tile's sorted (tile, octant) lists in BATCHES of up to 32 voxels that survive the
+// cull against the warp's pixel block, and split the work on a batch into a part that is parallel over
+// ray-voxel HITS (all 32 lanes busy whatever the shape of the voxels) and a part that is sequential per PIXEL
+// but cheap:
 //   1. cull: 32 entries at a time, lane i reads entry i's pixel rectangle (in list order, so the read is
-//      coalesced) and computes the 32-bit mask M of this warp's pixels it covers. M == 0 => the entry is
-//      skipped by this warp (76% of (warp, entry) pairs on C4).
-//   2. stage: surviving lanes copy their voxel's 80-byte view record (voxel_record_dev, svr_internal.cuh: centre
-//      relative to the camera as hi+lo floats, half edge, density coefficients, per-view colour, dilated half edge),
-//      gathered by the voxel id read beside the rectangle, in list order, into a warp-private shared-memory ring
-//      (cp.async, double-buffered).
-//   3. test: once >= 32 survivors are staged (or the list ends), the 32x32 bit matrix M[slot][pixel] is
-//      transposed across the warp with 5 shuffles, giving every lane the bitmask of slots that cover ITS
-//      pixel. Each lane pops its own candidates (ffs) and slab-tests them against a slightly dilated box:
-//      lanes work on different voxels in the same instruction.
-//   4. hits: each lane pops its own hits: precise slab test, K samples, eqs. 2-4; w_max (eq. 5,
-//      P:95) by atomicMax guarded by a plain read (w_max only grows). Front-to-back order per pixel is kept
-//      because slots are in list order.
-// With REC the forward also writes, per batch, the staged voxel ids and every pixel's hit mask (the traversal record).
-// Backward (backward_packed_kernel): replays that record, or runs the same cull / stage / test itself; then the hits
-// are compacted into a queue and processed 32 at a time with all lanes busy; see the comment above that kernel.
+//      coalesced) and computes the 32-bit mask M of this warp's pixels it covers. M == 0 => skipped.
+//   2. stage: surviving lanes copy their voxel's 80-byte view record (voxel_record_dev, svr_internal.cuh),
+//      gathered by the voxel id read beside the rectangle, in list order, into warp-private shared memory.
+//   3. test (pixel-major): the 32x32 bit matrix M[slot][pixel] is transposed with 5 shuffles, so every lane holds the
+//      slots that cover ITS pixel; it pops them and slab-tests them against a slightly dilated box -> hit bitmask.
+//   4. queue (layout): the hit matrix is transposed back (lane k: pixels that hit slot k), a warp scan gives every slot
+//      its offset: the hits of the batch form a slot-major queue of nh entries; entry e is worked on by lane e / C as its
+//      (e % C)-th item, C = ceil(nh / 32), and every per-entry array is indexed by st(e) = (e % C) * 32 + e / C: a lane's
+//      accesses are conflict-free and its C entries are CONSECUTIVE hits, i.e. mostly hits of one voxel.
+//   5. forward, hit-major (F1): precise slab test + K-sample integration per entry -> E = exp(-tau), t_mid into the queue.
+//      forward, pixel-major (F2): every lane pops its own hits front to back: eqs. 2-4, depth, w_max (eq. 5).
+//      With REC the forward writes the traversal record: per batch the staged voxel ids, every pixel's hit mask and the
+//      E of every queue entry.
+//   5'. backward, pixel-major: with E from the record (or recomputed by the same hit-major sweep), every lane chains its
+//      own hits: T_k, P_k = G . C_k and from them dL/dtau_k = T_k (G . c_k) + P_k - G . C_final and w_k, into the queue.
+//      backward, hit-major: precise slab + K samples per entry with dL/dtau_k already known, so the gradient of the 8
+//      density coefficients and the colour is accumulated IN REGISTERS over the lane's consecutive entries and leaves as
+//      one set of three red.global.add.v4.f32 per (lane, voxel) fragment: no cross-lane reduction at all. (Round 1 reduced
+//      11 values per hit with a segmented shuffle sum and chained the pixel state through shuffles: 45 % of its
+//      instructions, profiles/r1q_*.)
 //
 // Density: the trilinear raw density is staged as polynomial coefficients (c0, cx, cy, cz, cxy, cxz, cyz,
 // cxyz), pre-multiplied by log2(e), so a sample costs 7 FMA + one EX2 instead of 7 lerps (14 ops) + MUL + EX2.
 // Backward accumulates the gradient w.r.t. those coefficients (monomials 1, qx, qy, qz, qxqy, ...) into a
-// per-voxel scratch with 16-byte vector reductions (red.global.add.v4.f32; float atomics in shared memory are
-// CAS loops on sm_100a, so nothing is accumulated there); the per-voxel finalize kernel (preprocess.cu) maps
-// it back to the 8 corners.
+// per-voxel scratch with 16-byte vector reductions (float atomics in shared memory are CAS loops on sm_100a, so
+// nothing is accumulated there); the per-voxel finalize kernel (preprocess.cu) maps it back to the 8 corners.
 //
 // Precision: the ray is set up in fp64 per pixel and kept as hi+lo floats; the slab test runs in
 // coordinates relative to the ray's closest approach to the voxel centre, so the segment length keeps
@@ -38,18 +44,49 @@
 namespace {
 
 constexpr unsigned FULL = 0xffffffffu;
-constexpr int RING = 64;          // staging slots per warp
 constexpr int TRAV_WORDS = SVR_TRAV_WORDS;   // words of one traversal record (forward -> backward), see composite_kernel
 constexpr int WARPS = 8;
+constexpr int NSLOT = 32;          // staged voxels per batch
+#ifndef SVR_QCAP
+#define SVR_QCAP 256
+#endif
+constexpr int QCAP = SVR_QCAP;     // queue entries per warp (a batch is cut into sub-batches whose hits fit)
+constexpr int CMAX = QCAP / 32;
+static_assert(QCAP >= 256 && QCAP <= 512 && QCAP % 32 == 0, "a batch has at most 1024 hits: at most SVR_TRAV_SUB sub-batches");
+constexpr int RING = 64;           // forward staging slots per warp (two halves of 32)
+#ifndef FWD_CTAS
+#define FWD_CTAS 4
+#endif
+#ifndef SVR_BWD_DB
+#define SVR_BWD_DB 1              // replaying backward: 1 = gather of the next batch double-buffered (3 CTAs/SM), 0 = single buffer,
+#endif                            // next batch only prefetched into L2 (4 CTAs/SM)
+#ifndef BWD_CTAS
+#define BWD_CTAS (SVR_BWD_DB ? 3 : 4)
+#endif
+constexpr int BWD_BUFS = SVR_BWD_DB ? 2 : 1;
+constexpr int EROWS = 8;            // E rows a backward lane fetches into registers at the start of a sub-batch
+constexpr uint32_t ECHUNK = 16;    // the E record is handed out to warps in chunks of (at least) 16 rows of 32 floats
 
-struct WarpStage {
-    float4 g0[RING];    // gh.xyz, h (half edge)
-    float4 g1[RING];    // gl.xyz, voxel id bits
-    float4 r0[RING];    // log2(e) * (c0, cx, cy, cz)
-    float4 r1[RING];    // log2(e) * (cxy, cxz, cyz, cxyz)
-    float4 col[RING];   // r, g, b, clamp mask
-    unsigned int M[RING];   // pixels of this warp's 8x4 block covered by the voxel's rectangle
+// ceil(65536 / C): (pos * QINV[C]) >> 16 == pos / C for pos < 512, C <= 16
+__constant__ unsigned int QINV[17] = {0, 65536, 32768, 21846, 16384, 13108, 10923, 9363, 8192, 7282, 6554, 5958, 5462, 5042, 4682, 4370, 4096};
+
+struct WarpQ {              // hit queue of one sub-batch; per-entry arrays indexed by st(e)
+    uint2 Hs[32];           // per slot: pixels that hit it, queue offset
+    float E[QCAP];          // forward: exp(-tau); backward: exp(-tau), replaced by the blending weight w
+    float X[QCAP];          // forward: t_mid; backward: dL/dtau
+    unsigned short q[QCAP]; // (slot << 5) | pixel
 };
+
+struct QLayout { int n, nh, C; unsigned int inv; };
+
+// entry e = le * C + c lives at row c, column (le + c) mod 32: the C consecutive entries of a lane sit in different banks
+// (the pixel-major passes write runs of consecutive entries), and a row read by the 32 lanes is a permutation of the banks
+__device__ __forceinline__ int q_st(int pos, const QLayout& L) {
+    const int le = (int)(((unsigned int)pos * L.inv) >> 16);
+    const int c = pos - le * L.C;
+    return (c << 5) + ((le + c) & 31);
+}
+__device__ __forceinline__ int q_row(int c, int lane) { return (c << 5) + ((lane + c) & 31); }
 
 struct RayF {
     float dh[3], dl[3], inv[3], ainv[3];
@@ -118,6 +155,15 @@ __device__ __forceinline__ unsigned int transpose32(unsigned int x, int lane) {
     return x;
 }
 
+__device__ __forceinline__ int warp_incl_scan_i(int v, int lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(FULL, v, o);
+        if (lane >= o) v += t;
+    }
+    return v;
+}
+
 // Ray/voxel segment in coordinates relative to t_ref (the ray parameter closest to the voxel centre).
 __device__ __forceinline__ bool slab(const RayF& r, const float4& a, const float4& b, float& s0, float& s1, float& t_ref,
                                      float* D) {
@@ -139,18 +185,13 @@ __device__ __forceinline__ float ex2f(float x) {
     return y;
 }
 
-// K midpoint samples (R5). ca/cb = polynomial coefficients * log2(e). Returns tau; BWD also returns
-// dtau[m] = d tau / d coef_m (natural-scale coefficients), m over monomials 1, qx, qy, qz, qxqy, qxqz, qyqz, qxqyqz.
-template <int K, bool BWD>
+// K midpoint samples (R5). ca/cb = polynomial coefficients * log2(e). Returns tau.
+template <int K>
 __device__ __forceinline__ float integrate(const RayF& r, const float* D, float h, float s0, float s1, const float4& ca,
-                                           const float4& cb, float* dtau) {
+                                           const float4& cb) {
     float inv_e = __int_as_float(0x7E800000 - __float_as_int(h));   // 0.5 / h for h a power of two
     float dt = (s1 - s0) * (1.0f / (float)K);
     float sum = 0.f;
-    if (BWD) {
-#pragma unroll
-        for (int c = 1; c < 8; ++c) dtau[c] = 0.f;
-    }
 #pragma unroll
     for (int j = 0; j < K; ++j) {
         float s = fmaf((float)j + 0.5f, dt, s0);
@@ -159,24 +200,39 @@ __device__ __forceinline__ float integrate(const RayF& r, const float* D, float 
         float qz = __saturatef(fmaf(fmaf(s, r.dh[2], -D[2]), inv_e, 0.5f));
         float hi = fmaf(fmaf(cb.w, qz, cb.x), qy, fmaf(cb.y, qz, ca.y));     // (cxyz qz + cxy) qy + (cxz qz + cx)
         float lo = fmaf(fmaf(cb.z, qz, ca.z), qy, fmaf(ca.w, qz, ca.x));     // (cyz qz + cy) qy + (cz qz + c0)
-        float sig = ex2f(fmaf(hi, qx, lo));
-        sum += sig;
-        if (BWD) {
-            float sx = sig * qx, sy = sig * qy, sz = sig * qz;
-            dtau[1] += sx; dtau[2] += sy; dtau[3] += sz;
-            float sxy = sx * qy;
-            dtau[4] += sxy;
-            dtau[5] = fmaf(sx, qz, dtau[5]);
-            dtau[6] = fmaf(sy, qz, dtau[6]);
-            dtau[7] = fmaf(sxy, qz, dtau[7]);
-        }
-    }
-    if (BWD) {
-        dtau[0] = sum * dt;
-#pragma unroll
-        for (int c = 1; c < 8; ++c) dtau[c] *= dt;
+        sum += ex2f(fmaf(hi, qx, lo));
     }
     return dt * sum;
+}
+
+// Same samples with dL/dtau known: acc[m] += dL/dtau * d tau / d coef_m (natural-scale coefficients), m over the monomials
+// 1, qx, qy, qz, qxqy, qxqz, qyqz, qxqyqz.
+template <int K>
+__device__ __forceinline__ void integrate_bwd(const RayF& r, const float* D, float h, float s0, float s1, const float4& ca,
+                                              const float4& cb, float dLdtau, float* acc) {
+    float inv_e = __int_as_float(0x7E800000 - __float_as_int(h));
+    float dt = (s1 - s0) * (1.0f / (float)K);
+    const float sc = dLdtau * dt;
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+        float s = fmaf((float)j + 0.5f, dt, s0);
+        float qx = __saturatef(fmaf(fmaf(s, r.dh[0], -D[0]), inv_e, 0.5f));
+        float qy = __saturatef(fmaf(fmaf(s, r.dh[1], -D[1]), inv_e, 0.5f));
+        float qz = __saturatef(fmaf(fmaf(s, r.dh[2], -D[2]), inv_e, 0.5f));
+        float hi = fmaf(fmaf(cb.w, qz, cb.x), qy, fmaf(cb.y, qz, ca.y));
+        float lo = fmaf(fmaf(cb.z, qz, ca.z), qy, fmaf(ca.w, qz, ca.x));
+        const float sig = ex2f(fmaf(hi, qx, lo)) * sc;
+        const float sx = sig * qx, sy = sig * qy;
+        acc[0] += sig;
+        acc[1] += sx;
+        acc[2] += sy;
+        acc[3] = fmaf(sig, qz, acc[3]);
+        const float sxy = sx * qy;
+        acc[4] += sxy;
+        acc[5] = fmaf(sx, qz, acc[5]);
+        acc[6] = fmaf(sy, qz, acc[6]);
+        acc[7] = fmaf(sxy, qz, acc[7]);
+    }
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -186,8 +242,118 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
+
+// ---- step 4: queue layout of the sub-batch that starts at the first of `n` slots; hits = this pixel's hit bits over them ----
+__device__ __forceinline__ QLayout queue_layout(unsigned int hits, int n, WarpQ& Q, int lane) {
+    QLayout L;
+    const unsigned int H = transpose32(hits, lane);         // lane k: pixels that hit slot k
+    const int cnt = __popc(H);
+    const int inc = warp_incl_scan_i(cnt, lane);
+    L.n = min(n, __popc(__ballot_sync(FULL, inc <= QCAP)));  // cut where the queue is full (a slot has <= 32 hits: n >= 1)
+    L.nh = __shfl_sync(FULL, inc, L.n - 1);
+    L.C = (L.nh + 31) >> 5;
+    L.inv = QINV[L.C];
+    Q.Hs[lane] = make_uint2(H, (unsigned int)(inc - cnt));
+    return L;
+}
+
+// every pixel lane writes its own hits to their slot-major queue positions
+__device__ __forceinline__ void queue_fill(unsigned int m, WarpQ& Q, const QLayout& L, int lane) {
+    const unsigned int lt = (1u << lane) - 1u;
+    while (__any_sync(FULL, m != 0u)) {
+        if (m) {
+            const int k = __ffs(m) - 1;
+            m &= m - 1;
+            const uint2 hk = Q.Hs[k];
+            Q.q[q_st((int)hk.y + __popc(hk.x & lt), L)] = (unsigned short)((k << 5) | lane);
+        }
+    }
+}
+
+// ---- hit-major sweep: precise slab + K samples per queue entry -> Q.E = exp(-tau) (1 for a miss), tm_out = t_mid (0 for a miss).
+// g0..r1 point at the first slot of the sub-batch; A = per-pixel columns dh.xyz, dl.xyz, 1/dh.xyz. A lane's C entries are
+// consecutive hits, mostly of one voxel: its record stays in registers until the slot changes.
+template <int K, bool WANT_TM>
+__device__ __forceinline__ void sweep_E(const float4* g0, const float4* g1, const float4* r0, const float4* r1,
+                                        const float (*A)[32], WarpQ& Q, const QLayout& L, float* tm_out, int lane) {
+    int cur = -1;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), bq = a, ra = a, rb = a;
+    for (int c = 0; c < L.C; ++c) {
+        if (lane * L.C + c < L.nh) {
+            const int st = q_row(c, lane);
+            const unsigned int u = Q.q[st];
+            const int k = (int)(u >> 5), i = (int)(u & 31u);
+            if (k != cur) { a = g0[k]; bq = g1[k]; ra = r0[k]; rb = r1[k]; cur = k; }
+            RayF rr;
+#pragma unroll
+            for (int ax = 0; ax < 3; ++ax) {
+                rr.dh[ax] = A[ax][i]; rr.dl[ax] = A[3 + ax][i]; rr.inv[ax] = A[6 + ax][i];
+                rr.ainv[ax] = fabsf(rr.inv[ax]);
+            }
+            float s0, s1, t_ref, D[3], E = 1.f, tm = 0.f;
+            if (slab(rr, a, bq, s0, s1, t_ref, D)) {                 // the precise test decides
+                const float tau = integrate<K>(rr, D, a.w, s0, s1, ra, rb);
+                E = ex2f(-1.4426950408889634f * tau);
+                tm = t_ref + 0.5f * (s0 + s1);
+            }
+            Q.E[st] = E;
+            if (WANT_TM) tm_out[st] = tm;
+        }
+    }
+}
+
+// conservative slab test of this pixel's candidates among the staged slots (centre hi parts only, dilated half edge hd:
+// a bound on what the lo parts and the rounding can move, so no true hit is lost; the precise test decides later)
+template <bool HD_IN_COL>
+__device__ __forceinline__ unsigned int test_candidates(unsigned int cand, const float4* g0, const float4* col, const float* inv,
+                                                        unsigned int& n_test) {
+    unsigned int hits = 0u;
+    while (__any_sync(FULL, cand != 0u)) {
+        if (cand) {
+            const int k = __ffs(cand) - 1;
+            cand &= cand - 1;
+            const float4 a = g0[k];
+            const float hd = HD_IN_COL ? col[k].w : fmaf(fabsf(a.x) + fabsf(a.y) + fabsf(a.z), 4.8e-7f, a.w * 1.000002f);
+            const float cx = a.x * inv[0], cy = a.y * inv[1], cz = a.z * inv[2];
+            const float wx = hd * fabsf(inv[0]), wy = hd * fabsf(inv[1]), wz = hd * fabsf(inv[2]);
+            const float s0 = fmaxf(fmaxf(cx - wx, cy - wy), fmaxf(cz - wz, 0.f));
+            const float s1 = fminf(fminf(cx + wx, cy + wy), cz + wz);
+            if (s1 > s0) hits |= 1u << k;
+            ++n_test;
+        }
+    }
+    return hits;
+}
+
+// The list entries of one 32-entry chunk, one per lane (rectangle + voxel id); beyond the list: an empty rectangle.
+struct Chunk { uint2 rc; uint32_t vid; };
+__device__ __forceinline__ Chunk load_chunk(const uint2* __restrict__ rects_sorted, const uint32_t* __restrict__ vals, uint32_t b, uint32_t end,
+                                            int lane) {
+    Chunk c;
+    c.rc = make_uint2(0xFFFFFFFFu, 0u);
+    c.vid = 0u;
+    const uint32_t idx = b + (uint32_t)lane;
+    if (idx < end) { c.rc = __ldg(rects_sorted + idx); c.vid = __ldg(vals + idx); }
+    return c;
+}
+
+struct FwdWarp {
+    float4 g0[RING];    // gh.xyz, h (half edge)
+    float4 g1[RING];    // gl.xyz, voxel id bits
+    float4 r0[RING];    // log2(e) * (c0, cx, cy, cz)
+    float4 r1[RING];    // log2(e) * (cxy, cxz, cyz, cxyz)
+    float4 col[RING];   // r, g, b, dilated half edge
+    unsigned int M[RING];   // pixels of this warp's 8x4 block covered by the voxel's rectangle
+};
+
+// Forward (a7). After the test every lane pops its own HITS front to back: precise slab, K samples, eqs. 2-4, depth,
+// w_max (eq. 5) by atomicMax guarded by a plain read. (The hit-major split of the backward pass was tried here too:
+// the queue, its fill and the second pixel-major loop cost more instructions than the idle lanes of this loop,
+// profiles/r2b_*.) Traversal record of one batch (TRAV_WORDS words, written with REC): [0,32) every pixel's hit mask, [32,64)
+// the staged voxel ids, [64] the slot count, [65] the first E row of the batch in the E record, [71] its number of rows; E
+// row i holds, for every pixel of the block, exp(-tau) of its i-th hit in the batch (1 where it has none or missed).
 template <int K, bool STATS, bool REC>
-__global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
+__global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
                                                         const uint32_t* __restrict__ tile_order,
@@ -195,16 +361,18 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                                                         float* __restrict__ image, float* __restrict__ depth,
                                                         float* __restrict__ T_final, unsigned int* __restrict__ w_max,
                                                         unsigned long long* __restrict__ stats, uint32_t* __restrict__ trav,
-                                                        const uint32_t* __restrict__ trav_off, uint32_t* __restrict__ trav_count) {
+                                                        const uint32_t* __restrict__ trav_off, uint32_t* __restrict__ trav_count,
+                                                        float* __restrict__ trav_E, uint32_t* __restrict__ trav_ectl, uint32_t e_cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    WarpStage& S = reinterpret_cast<WarpStage*>(smem_raw)[warp];
+    FwdWarp& S = reinterpret_cast<FwdWarp*>(smem_raw)[warp];
     const int tile = (int)tile_order[blockIdx.x];
     const int tile_x = tile % c.tiles_x, tile_y = tile / c.tiles_x;
     const int wbx0 = tile_x * SVR_TILE + (warp & 1) * 8, wby0 = tile_y * SVR_TILE + (warp >> 1) * 4;
     const int px = wbx0 + (lane & 7), py = wby0 + (lane >> 3);
     const bool inimg = px < c.W && py < c.H;
     const size_t pix = (size_t)py * c.W + px;
+    const unsigned int lt = (1u << lane) - 1u;
 
     RayF ray;
     int oct = -1;
@@ -217,10 +385,8 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
     }
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dep = 0.f;
     unsigned int n_hit = 0, n_test = 0, n_surv = 0, n_read = 0;   // STATS only
-    // Traversal record for svr_backward (TRAV_WORDS words per batch: 32 hit masks, 32 voxel ids, the slot count): the
-    // backward pass replays the batches and skips its own cull and test phases. This warp's records are contiguous.
     uint32_t* rec_out = nullptr;
-    uint32_t n_rec = 0;
+    uint32_t n_rec = 0, e_pos = 0, e_left = 0;
     if (REC) {
         const uint32_t r0 = trav_off[tile], cap = (trav_off[tile + 1] - r0) >> 3;
         rec_out = trav + ((size_t)r0 + (size_t)warp * cap) * TRAV_WORDS;
@@ -232,19 +398,19 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
         bool alive = inimg && (oct == so) && (T >= T_min);
         unsigned int alive_mask = __ballot_sync(FULL, alive);
         if (alive_mask == 0u) continue;                               // no pixel of this warp uses this list
-        // Double-buffered staging: the ring is two halves of 32 slots. While one half is walked, the records of the
-        // next batch are already on their way into the other half (cp.async: no registers held, no stall on the load).
+        // Staging: double-buffered (the ring is two halves of 32 slots: while one half is walked, the records of the next
+        // batch are already on their way into the other half; cp.async: no registers held, no stall on the load). The list
+        // itself (rectangle + voxel id per entry) is read two chunks of 32 entries ahead into registers, so the cull does not
+        // wait for it.
         uint32_t base = start;
+        Chunk ca = load_chunk(rects_sorted, vals, base, end, lane), cb = load_chunk(rects_sorted, vals, base + 32u, end, lane);
         auto stage = [&](int half) -> int {
             int cnt = 0;
             while (cnt < 32 && base < end) {
-                const uint32_t idx = base + lane;
-                if (lane < 2) asm volatile("prefetch.global.L1 [%0];" ::"l"(rects_sorted + min(base + 64u + 16u * lane, end - 1u)));   // two chunks ahead
-                unsigned int M = 0u;
-                uint32_t vid = 0u;
-                if (idx < end) { M = block_cover_mask(__ldg(rects_sorted + idx), wbx0, wby0) & alive_mask; vid = __ldg(vals + idx); }
+                unsigned int M = block_cover_mask(ca.rc, wbx0, wby0) & alive_mask;
+                const uint32_t vid = ca.vid;
                 unsigned int m = __ballot_sync(FULL, M != 0u);
-                const int rank = __popc(m & ((1u << lane) - 1u));
+                const int rank = __popc(m & lt);
                 int adv = 32;
                 if (__popc(m) > 32 - cnt) {                            // more survivors than free slots: take the first ones
                     if (rank >= 32 - cnt) M = 0u;
@@ -258,9 +424,12 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
                     cp_async16(&S.r1[slot], rec + 3); cp_async16(&S.col[slot], rec + 4);
                     S.M[slot] = M;
                 }
-                if (STATS) { n_read += (idx < end && (int)lane < adv); n_surv += (M != 0u); }
+                if (STATS) { n_read += (base + lane < end && (int)lane < adv); n_surv += (M != 0u); }
                 cnt += __popc(m);
                 base += adv;
+                if (adv == 32) ca = cb;
+                else ca = load_chunk(rects_sorted, vals, base, end, lane);
+                cb = load_chunk(rects_sorted, vals, base + 32u, end, lane);
             }
             asm volatile("cp.async.commit_group;" ::: "memory");
             return cnt;
@@ -274,59 +443,53 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
             const int n = count;
             unsigned int cand = transpose32(lane < n ? S.M[head + lane] : 0u, lane);
             if (!alive) cand = 0u;
-            {
-                // two loops: (1) every lane slab-tests its own candidates against a slightly dilated box (centre hi
-                // parts only) and records the hits; (2) every lane integrates and composites its own hits. A lane that
-                // misses no longer sits idle through another lane's K samples, and the hit loop is as long as the
-                // pixel with the most HITS, not the most candidates.
-                unsigned int hits = 0u;
-                if (STATS) n_test += __popc(cand);
-                while (__any_sync(FULL, cand != 0u)) {
-                    if (cand) {
-                        const int k = __ffs(cand) - 1;
-                        cand &= cand - 1;
-                        const float4 a = S.g0[(head + k) & (RING - 1)];
-                        // dilated half edge (voxel_record_dev): a bound on what the lo parts and the rounding can move, so no
-                        // true hit is lost
-                        const float hd = S.col[(head + k) & (RING - 1)].w;
-                        const float cx = a.x * ray.inv[0], cy = a.y * ray.inv[1], cz = a.z * ray.inv[2];
-                        const float wx = hd * ray.ainv[0], wy = hd * ray.ainv[1], wz = hd * ray.ainv[2];
-                        const float s0 = fmaxf(fmaxf(cx - wx, cy - wy), fmaxf(cz - wz, 0.f));
-                        const float s1 = fminf(fminf(cx + wx, cy + wy), cz + wz);
-                        if (s1 > s0) hits |= 1u << k;
+            // two loops: (1) every lane slab-tests its own candidates against a slightly dilated box (centre hi parts only)
+            // and records the hits; (2) every lane integrates and composites its own hits. A lane that misses does not sit
+            // idle through another lane's K samples, and the hit loop is as long as the pixel with the most HITS.
+            unsigned int hits = test_candidates<true>(cand, S.g0 + head, S.col + head, ray.inv, n_test);
+            float* eg = nullptr;
+            if (REC && __any_sync(FULL, hits != 0u)) {
+                uint32_t* r = rec_out + (size_t)n_rec * TRAV_WORDS;
+                r[lane] = hits;
+                if (lane < n) r[32 + lane] = __float_as_uint(S.g1[head + lane].w);    // the staged voxel ids
+                const uint32_t rows = __reduce_max_sync(FULL, (unsigned int)__popc(hits));
+                if (e_left < rows) {                                   // next chunk of the E record
+                    const uint32_t grab = rows > ECHUNK ? rows : ECHUNK;
+                    if (lane == 0) e_pos = atomicAdd(trav_ectl, grab);
+                    e_pos = __shfl_sync(FULL, e_pos, 0);
+                    e_left = grab;
+                }
+                if (e_pos + rows <= e_cap) eg = trav_E + (size_t)e_pos * 32u + lane;
+                else if (lane == 0) trav_ectl[1] = 1u;                  // E record full: the backward pass recomputes E
+                if (lane == 0) { r[64] = (uint32_t)n; r[65] = e_pos; r[71] = rows; }
+                e_pos += rows;
+                e_left -= rows;
+                ++n_rec;
+            }
+            while (__any_sync(FULL, hits != 0u)) {
+                float E = 1.f;
+                if (hits) {
+                    const int slot = head + __ffs(hits) - 1;
+                    hits &= hits - 1;
+                    const float4 a = S.g0[slot], bq = S.g1[slot];
+                    float s0, s1, t_ref, D[3];
+                    if (slab(ray, a, bq, s0, s1, t_ref, D)) {               // the precise test decides
+                        const uint32_t vid = __float_as_uint(bq.w);
+                        unsigned int wm_old = 0u;
+                        if (w_max != nullptr) wm_old = w_max[vid];            // stale read is safe: w_max only grows
+                        const float4 ra = S.r0[slot], rb = S.r1[slot], col = S.col[slot];
+                        const float tau = integrate<K>(ray, D, a.w, s0, s1, ra, rb);
+                        E = ex2f(-1.4426950408889634f * tau);
+                        const float w = T * (1.f - E);
+                        T *= E;
+                        C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
+                        if (STATS) ++n_hit;
+                        Dep = fmaf(w, t_ref + 0.5f * (s0 + s1), Dep);
+                        if (w_max != nullptr && __float_as_uint(w) > wm_old) atomicMax(w_max + vid, __float_as_uint(w));
+                        if (T < T_min) { alive = false; hits = 0u; }          // R8: stop after the voxel that crosses T_min
                     }
                 }
-                if (REC) {
-                    uint32_t* r = rec_out + (size_t)n_rec * TRAV_WORDS;
-                    r[lane] = hits;
-                    if (lane < n) r[32 + lane] = __float_as_uint(S.g1[(head + lane) & (RING - 1)].w);    // the staged voxel ids
-                    if (lane == 0) r[64] = (uint32_t)n;
-                    ++n_rec;
-                }
-                while (__any_sync(FULL, hits != 0u)) {
-                    if (hits) {
-                        const int slot = (head + __ffs(hits) - 1) & (RING - 1);
-                        hits &= hits - 1;
-                        const float4 a = S.g0[slot], bq = S.g1[slot];
-                        float s0, s1, t_ref, D[3];
-                        if (slab(ray, a, bq, s0, s1, t_ref, D)) {               // the precise test decides
-                            const uint32_t vid = __float_as_uint(bq.w);
-                            unsigned int wm_old = 0u;
-                            if (w_max != nullptr) wm_old = w_max[vid];            // stale read is safe: w_max only grows
-                            const float4 ra = S.r0[slot], rb = S.r1[slot], col = S.col[slot];
-                            float dtau[8];
-                            float tau = integrate<K, false>(ray, D, a.w, s0, s1, ra, rb, dtau);
-                            float E = ex2f(-1.4426950408889634f * tau);
-                            float w = T * (1.f - E);
-                            T *= E;
-                            C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
-                            if (STATS) ++n_hit;
-                            Dep = fmaf(w, t_ref + 0.5f * (s0 + s1), Dep);
-                            if (w_max != nullptr && __float_as_uint(w) > wm_old) atomicMax(w_max + vid, __float_as_uint(w));
-                            if (T < T_min) { alive = false; hits = 0u; }          // R8: stop after the voxel that crosses T_min
-                        }
-                    }
-                }
+                if (REC && eg != nullptr) { *eg = E; eg += 32; }              // a whole row per step: no partial sectors
             }
             __syncwarp();
             head ^= 32;
@@ -357,62 +520,23 @@ __global__ void __launch_bounds__(256, 4) composite_kernel(CamDev c, const float
 
 
 // ================================================================================================
-// Hit-packed backward compositing (row a9). The lane-centric walk above keeps only ~12 of 32 lanes busy
-// in the expensive part of the backward pass (K samples + exp + the monomial sums) and needs a quad
-// exchange before every reduction. Here only the cheap part stays pixel-centric; the expensive part runs
-// on a compacted hit queue:
-//   1. cull + stage as above (32 voxel records in list order, warp-private);
-//   2. test: every lane pops its own pixel's candidates among the staged voxels and slab-tests them
-//      against a slightly dilated box (centre hi parts only, ray in registers), recording a hit bitmask;
-//   3. queue: the 32x32 hit matrix is transposed so that lane k knows which pixels hit slot k; a warp scan
-//      gives every slot its queue offset; every pixel lane then writes its own hits to their slot-major
-//      positions (slot offset + its rank among the slot's pixels);
-//   4. hit rounds: 32 hits per round, one per lane, all lanes busy in the precise slab test and the K
-//      samples. The sequential per-pixel state (T, P = G . C) lives in shared memory; hits of the same
-//      pixel inside a round (match_any) are chained in slot order by a short loop of shuffles, so every
-//      pixel composites front to back in exactly the list order:
-//          dL/dtau_k = G . (T_k c_k + C_k - C_final) = T_k (G . c_k) + P_k - G . C_final.
-//   5. reduce: hits of one voxel are contiguous lanes, so two steps of a segmented shuffle sum give every
-//      fragment of up to 4 consecutive hits of a voxel one set of three red.global.add.v4.f32: a voxel that
-//      covers 7 of the warp's pixels leaves as 2 reduction sets instead of 7.
-// With the traversal record the kernel is bound by the shared-memory pipe (loads of the per-pixel and per-slot data and
-// the shuffles): the per-pixel data are 4-byte columns (32 pixels = 32 banks: any set of pixels loads in one
-// conflict-free wavefront, 12 per hit round instead of ~24 for four 16-byte rows), and the per-pixel constant of dL/dtau is
-// folded into the chained scalar P.
-constexpr int QCAP = 512;          // queue entries per warp (a batch is cut so that its hits fit)
-#ifndef SVR_RED_STEPS
-#define SVR_RED_STEPS 3
-#endif
-constexpr int RED_STEPS = SVR_RED_STEPS;   // fragments of up to 2^RED_STEPS consecutive hits of one voxel share a reduction set
-                                           // (C4 backward: 1 step 2.14 ms, 2 steps 1.66 ms, 3 steps 1.64 ms)
-constexpr int NSLOT = 32;          // staged voxels per batch
-#ifndef BWD_CTAS
-#define BWD_CTAS 4
-#endif
-
-struct WarpWork {
-    float4 g0[NSLOT];   // gh.xyz, h
-    float4 g1[NSLOT];   // gl.xyz, voxel id bits
-    float4 r0[NSLOT];   // log2(e) * (c0, cx, cy, cz)
-    float4 r1[NSLOT];   // log2(e) * (cxy, cxz, cyz, cxyz)
-    float4 col[NSLOT];  // r, g, b, cover mask M of this warp's 8x4 block
-    float A[12][32];    // per pixel, 4-byte columns: 32 pixels = 32 banks, so a load of any set of pixels is one
-                        // conflict-free wavefront: dh.xyz, dl.xyz, 1/dh.xyz, G.xyz (G = dL/dC)
-    float T[32];        //   transmittance
-    float Pp[32];       //   P = G . C (+ gD . D with the depth head) - G . C_final (- the heads' constants)
-    float PD[32];       //   gD = dL/dDepth (kernels with HEADS only)
-    uint2 Hs[32];       // per slot of the batch: pixels that hit it, queue offset
-    unsigned short q[QCAP];
+// Backward compositing (row a9): see the file comment, steps 5'. REPLAY: the forward pass recorded the batches (no cull, no
+// test); if it also recorded every hit's E = exp(-tau) (and the kernel has no depth head, whose chain needs t_mid too), the
+// hit-major E sweep is skipped as well. The record is a stream known in advance: the header of batch b + 2 is loaded into
+// registers and the voxel records of batch b + 1 are gathered (cp.async) into the other half of the staging buffer while
+// batch b is worked on.
+struct BwdBase {
+    float4 g0[BWD_BUFS * NSLOT];   // gh.xyz, h                            (two halves: replay double-buffers the gather)
+    float4 g1[BWD_BUFS * NSLOT];   // gl.xyz, voxel id bits
+    float4 r0[BWD_BUFS * NSLOT];   // log2(e) * (c0, cx, cy, cz)
+    float4 r1[BWD_BUFS * NSLOT];   // log2(e) * (cxy, cxz, cyz, cxyz)
+    float4 col[BWD_BUFS * NSLOT];  // r, g, b, cover mask M of this warp's 8x4 block (non-replay) / dilated half edge
+    float A[12][32];        // per pixel, 4-byte columns: dh.xyz, dl.xyz, 1/dh.xyz, G.xyz (G = dL/dC)
+    unsigned int wms[NSLOT];// per slot: max blending weight seen by this warp (float bits)
+    WarpQ Q;
 };
-
-__device__ __forceinline__ int warp_incl_scan_i(int v, int lane) {
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(FULL, v, o);
-        if (lane >= o) v += t;
-    }
-    return v;
-}
+template <bool HEADS> struct BwdWarp : BwdBase {};
+template <> struct BwdWarp<true> : BwdBase { float TM[QCAP]; };   // t_mid per queue entry (depth head)
 
 template <int K, bool HEADS, bool REPLAY>
 __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
@@ -424,10 +548,11 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                                                                float* __restrict__ grad_rgb, const float* __restrict__ dL_ddepth,
                                                                const float* __restrict__ dL_dT, const float* __restrict__ depth_in,
                                                                const float* __restrict__ T_in, const uint32_t* __restrict__ trav,
-                                                               const uint32_t* __restrict__ trav_off, const uint32_t* __restrict__ trav_count) {
+                                                               const uint32_t* __restrict__ trav_off, const uint32_t* __restrict__ trav_count,
+                                                               const float* __restrict__ trav_E, const uint32_t* __restrict__ trav_ectl) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    WarpWork& S = reinterpret_cast<WarpWork*>(smem_raw)[warp];
+    BwdWarp<HEADS>& S = reinterpret_cast<BwdWarp<HEADS>*>(smem_raw)[warp];
     const int tile = (int)tile_order[blockIdx.x];
     const int tile_x = tile % c.tiles_x, tile_y = tile / c.tiles_x;
     const int wbx0 = tile_x * SVR_TILE + (warp & 1) * 8, wby0 = tile_y * SVR_TILE + (warp >> 1) * 4;
@@ -435,155 +560,175 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     const bool inimg = px < c.W && py < c.H;
     const size_t pix = (size_t)py * c.W + px;
     const unsigned int lt = (1u << lane) - 1u;
-    const int swl = lane;                                             // this pixel's row in the tables
 
     int oct = -1;
-    float dh[3], inv[3], ainv[3];
+    float inv[3];
+    float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
+    float gdep = 0.f;
     {
         RayF ray;
-        float4 g = make_float4(0.f, 0.f, 0.f, 0.f);
-        float gdep = 0.f;
         if (inimg) {
             setup_ray(c, px, py, ray);
             oct = pixel_octant_dev(c, px, py);
-            g = make_float4(dL[pix * 3], dL[pix * 3 + 1], dL[pix * 3 + 2], 0.f);
-            g.w = g.x * image_in[pix * 3] + g.y * image_in[pix * 3 + 1] + g.z * image_in[pix * 3 + 2];
+            G = make_float4(dL[pix * 3], dL[pix * 3 + 1], dL[pix * 3 + 2], 0.f);
+            G.w = G.x * image_in[pix * 3] + G.y * image_in[pix * 3 + 1] + G.z * image_in[pix * 3 + 2];
             if (HEADS) {
                 // dL/dtau_k = T_k (G . c_k + gD t_k) + P_k - (G . C_final + gD D_final + gT T_K): the heads only add constants
                 gdep = dL_ddepth ? dL_ddepth[pix] : 0.f;
-                g.w += gdep * (depth_in ? depth_in[pix] : 0.f) + (dL_dT ? dL_dT[pix] * T_in[pix] : 0.f);
+                G.w += gdep * (depth_in ? depth_in[pix] : 0.f) + (dL_dT ? dL_dT[pix] * T_in[pix] : 0.f);
             }
         } else {
 #pragma unroll
             for (int a = 0; a < 3; ++a) { ray.dh[a] = 0.f; ray.dl[a] = 0.f; ray.inv[a] = 0.f; ray.ainv[a] = 0.f; }
         }
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { dh[a] = ray.dh[a]; inv[a] = ray.inv[a]; ainv[a] = ray.ainv[a]; }
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { S.A[a][swl] = ray.dh[a]; S.A[3 + a][swl] = ray.dl[a]; S.A[6 + a][swl] = ray.inv[a]; }
-        S.A[9][swl] = g.x; S.A[10][swl] = g.y; S.A[11][swl] = g.z;
-        if (HEADS) S.PD[swl] = gdep;
-        S.T[swl] = 1.f;
-        S.Pp[swl] = -g.w;                        // the per-pixel constant of dL/dtau rides in P
+        for (int a = 0; a < 3; ++a) { inv[a] = ray.inv[a]; S.A[a][lane] = ray.dh[a]; S.A[3 + a][lane] = ray.dl[a]; S.A[6 + a][lane] = ray.inv[a]; }
+        S.A[9][lane] = G.x; S.A[10][lane] = G.y; S.A[11][lane] = G.z;
+        S.wms[lane] = 0u;
     }
     __syncwarp();
-    float Tpix = 1.f;
-    // steps 3-5 for the staged slots [head, head + n); returns the number of slots consumed (a batch is cut where the
-    // queue is full)
-    auto run_batch = [&](const unsigned int hits, int n, const int head) -> int {
-        // ---- 3. queue: slot-major positions from the transposed hit matrix ----
-        int nh;
-        {
-            const unsigned int H = transpose32(hits, lane);         // lane k: pixels that hit slot k
-            const int cnt = __popc(H);
-            const int inc = warp_incl_scan_i(cnt, lane);
-            n = min(n, __popc(__ballot_sync(FULL, inc <= QCAP)));  // cut the batch where the queue is full
-            nh = __shfl_sync(FULL, inc, n - 1);
-            S.Hs[lane] = make_uint2(H, (unsigned int)(inc - cnt));
-            __syncwarp();
-            unsigned int m = (n < 32) ? (hits & ((1u << n) - 1u)) : hits;
-            while (__any_sync(FULL, m != 0u)) {
-                if (m) {
-                    const int k = __ffs(m) - 1;
-                    m &= m - 1;
-                    const uint2 hk = S.Hs[k];
-                    S.q[hk.y + __popc(hk.x & lt)] = (unsigned short)((k << 5) | swl);
+    // per-pixel chain state, in this pixel's lane: transmittance and P = G . C (+ gD . D) - the per-pixel constant of dL/dtau
+    float T = 1.f, P = -G.w;
+    const bool haveE = REPLAY && !HEADS && trav_E != nullptr && trav_ectl[1] == 0u;
+
+    // steps 4-5' for the n slots staged at `buf`; hits = this pixel's hit bits; misc = the record's words 64.. (lane i: word 64 + i)
+    auto run_batch = [&](const int buf, const unsigned int hits, const int n, const uint32_t misc) {
+        const float4 *g0 = S.g0 + buf, *g1 = S.g1 + buf, *r0 = S.r0 + buf, *r1 = S.r1 + buf, *colp = S.col + buf;
+        int j = 0;
+        for (int k0 = 0; k0 < n; ++j) {
+            const unsigned int hsub = hits >> k0;
+            // E rows of this batch: row i = every pixel's i-th hit of the batch; this pixel's hits in this sub-batch start at
+            // row popc(its hits in earlier slots). The first EROWS of them are fetched into registers here, in one go (a load
+            // inside the chain loop would make every step wait for it: loads share scoreboards); later rows: slow path.
+            const float* eg = nullptr;
+            float e[EROWS];
+            if (haveE) {
+                const uint32_t ord = (uint32_t)__popc(hits & ((1u << k0) - 1u)), rows_total = __shfl_sync(FULL, misc, 7);
+                eg = trav_E + ((size_t)__shfl_sync(FULL, misc, 1) + ord) * 32u + lane;
+#pragma unroll
+                for (int u = 0; u < EROWS; ++u) e[u] = (ord + (uint32_t)u < rows_total) ? __ldg(eg + 32 * u) : 1.f;
+                eg += 32 * EROWS;
+            }
+            const QLayout L = queue_layout(hsub, n - k0, S.Q, lane);
+            const unsigned int mine = (L.n < 32) ? (hsub & ((1u << L.n) - 1u)) : hsub;
+            if (L.nh > 0) {
+                __syncwarp();
+                if (!haveE) {
+                    queue_fill(mine, S.Q, L, lane);
+                    __syncwarp();
+                    if constexpr (HEADS) sweep_E<K, true>(g0 + k0, g1 + k0, r0 + k0, r1 + k0, S.A, S.Q, L, S.TM, lane);
+                    else sweep_E<K, false>(g0 + k0, g1 + k0, r0 + k0, r1 + k0, S.A, S.Q, L, nullptr, lane);
+                    __syncwarp();
+                }
+                // ---- pixel-major chain: eqs. 2-4 front to back, dL/dtau and w of every hit into the queue ----
+#ifdef SVR_DBG_SKIP
+                if (SVR_DBG_SKIP < 2)
+#endif
+                {
+                    unsigned int m = mine;
+                    auto chain = [&](const float e_rec) {
+                        const int k = __ffs(m) - 1;
+                        m &= m - 1;
+                        const uint2 hk = S.Q.Hs[k];
+                        const int st = q_st((int)hk.y + __popc(hk.x & lt), L);
+                        if (haveE) S.Q.q[st] = (unsigned short)((k << 5) | lane);
+                        const float E = haveE ? e_rec : S.Q.E[st];
+                        const float4 col = colp[k0 + k];
+                        float gc = G.x * col.x + G.y * col.y + G.z * col.z;
+                        if constexpr (HEADS) gc = fmaf(gdep, S.TM[st], gc);
+                        const bool live = T >= T_min;                // R8: a ray stops after the voxel that crosses T_min
+                        const float w = live ? T * (1.f - E) : 0.f;
+                        T = live ? T * E : T;
+                        P = fmaf(w, gc, P);
+                        S.Q.X[st] = live ? fmaf(T, gc, P) : 0.f;
+                        S.Q.E[st] = w;
+                    };
+                    bool more = __any_sync(FULL, m != 0u);
+#pragma unroll
+                    for (int u = 0; u < EROWS; ++u) {
+                        if (more) {
+                            if (m) chain(e[u]);
+                            more = __any_sync(FULL, m != 0u);
+                        }
+                    }
+                    while (more) {                                       // more than EROWS hits of one pixel in a sub-batch
+                        float e_rec = 1.f;
+                        if (haveE && m) e_rec = __ldg(eg);
+                        eg += 32;
+                        if (m) chain(e_rec);
+                        more = __any_sync(FULL, m != 0u);
+                    }
+                }
+                __syncwarp();
+                // ---- hit-major: gradients of this lane's C consecutive entries, summed in registers per voxel ----
+#ifdef SVR_DBG_SKIP
+                if (SVR_DBG_SKIP < 1)
+#endif
+                {
+                    float acc[11];
+#pragma unroll
+                    for (int m = 0; m < 11; ++m) acc[m] = 0.f;
+                    float wq = 0.f;
+                    int cur = -1;
+                    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), bq = a, ra = a, rb = a;
+                    auto flush = [&]() {
+                        if (wq > 0.f || acc[0] != 0.f) {
+                            const uint32_t vid = __float_as_uint(bq.w);
+                            red_add_v4(grad_coef + (size_t)vid * 8, acc[0], acc[1], acc[2], acc[3]);
+                            red_add_v4(grad_coef + (size_t)vid * 8 + 4, acc[4], acc[5], acc[6], acc[7]);
+                            red_add_v4(grad_rgb + (size_t)vid * 4, acc[8], acc[9], acc[10], 0.f);
+                            if (w_max != nullptr) atomicMax(&S.wms[k0 + cur], __float_as_uint(wq));
+                        }
+                    };
+                    for (int cc = 0; cc < L.C; ++cc) {
+                        const bool valid = lane * L.C + cc < L.nh;
+                        const int st = q_row(cc, lane);
+                        const unsigned int u = valid ? (unsigned int)S.Q.q[st] : 0u;
+                        const int k = valid ? (int)(u >> 5) : cur;
+                        if (k != cur) {                                  // next voxel: send the finished fragment
+                            flush();
+#pragma unroll
+                            for (int m = 0; m < 11; ++m) acc[m] = 0.f;
+                            wq = 0.f;
+                            cur = k;
+                            a = g0[k0 + k]; bq = g1[k0 + k]; ra = r0[k0 + k]; rb = r1[k0 + k];
+                        }
+                        if (valid) {
+                            const float w = S.Q.E[st], dLdtau = S.Q.X[st];
+                            if (w > 0.f || dLdtau != 0.f) {
+                                const int i = (int)(u & 31u);
+                                RayF rr;
+#pragma unroll
+                                for (int ax = 0; ax < 3; ++ax) {
+                                    rr.dh[ax] = S.A[ax][i]; rr.dl[ax] = S.A[3 + ax][i]; rr.inv[ax] = S.A[6 + ax][i];
+                                    rr.ainv[ax] = fabsf(rr.inv[ax]);
+                                }
+                                float s0, s1, t_ref, D[3];
+                                if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
+                                    integrate_bwd<K>(rr, D, a.w, s0, s1, ra, rb, dLdtau, acc);
+                                    acc[8] = fmaf(w, S.A[9][i], acc[8]);
+                                    acc[9] = fmaf(w, S.A[10][i], acc[9]);
+                                    acc[10] = fmaf(w, S.A[11][i], acc[10]);
+                                    wq = fmaxf(wq, w);
+                                }
+                            }
+                        }
+                    }
+                    flush();
+                }
+                __syncwarp();
+                // eq. 5: one atomicMax per voxel of the sub-batch (its hits all lie in this sub-batch); no guard read: a load
+                // that is waited for here costs more than the reductions it would save
+                if (w_max != nullptr && lane >= k0 && lane < k0 + L.n) {
+                    const unsigned int wv = S.wms[lane];
+                    if (wv != 0u) {
+                        S.wms[lane] = 0u;
+                        atomicMax(w_max + __float_as_uint(g1[lane].w), wv);
+                    }
                 }
             }
+            k0 += L.n;
         }
-        __syncwarp();
-        // ---- 4. hit rounds: one hit per lane ----
-        for (int r = 0; r < nh; r += 32) {
-            const bool valid = r + lane < nh;
-            const unsigned int e = valid ? (unsigned int)S.q[r + lane] : 0xFFFFu;
-            const int k = (int)(e >> 5);                         // slot inside the batch (2047 = no entry)
-            const int i = (int)(e & 31u);                        // swizzled pixel id
-            const int slot = (head + k) & (NSLOT - 1);
-            // hits of the same pixel inside this round are chained in slot (= lane) order; issued first so that
-            // the match latency hides behind the samples
-            const unsigned int peers = __match_any_sync(FULL, valid ? (unsigned int)i : 32u + (unsigned int)lane);
-            // hits of one voxel are contiguous lanes (a run): RED_STEPS steps of a segmented sum towards lower lanes,
-            // then every lane that starts a fragment of 2^RED_STEPS lanes of its run sends the fragment's sums
-            const int kprev = __shfl_up_sync(FULL, k, 1);
-            const unsigned int heads = __ballot_sync(FULL, lane == 0 || kprev != k);
-            const unsigned int above = (heads >> lane) >> 1;
-            const int rem = above ? __ffs(above) - 1 : 31 - lane;     // lanes after this one in its run
-            const int run_pos = lane - (31 - __clz(heads & (lt | (1u << lane))));
-            const bool frag_head = valid && (run_pos & ((1 << RED_STEPS) - 1)) == 0;
-            const uint32_t vid = valid ? __float_as_uint(S.g1[slot].w) : 0u;
-            // w_max only grows, so a stale guard read is safe; issued here so that its latency hides behind the samples
-            unsigned int wm_old = 0xFFFFFFFFu;
-            if (frag_head && w_max != nullptr) wm_old = w_max[vid];
-            float tau = 0.f, dtau[8], gc = 0.f;
-            float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int m = 0; m < 8; ++m) dtau[m] = 0.f;
-            if (valid) {
-                const float4 a = S.g0[slot], bq = S.g1[slot];
-                RayF rr;
-#pragma unroll
-                for (int ax = 0; ax < 3; ++ax) {
-                    rr.dh[ax] = S.A[ax][i]; rr.dl[ax] = S.A[3 + ax][i]; rr.inv[ax] = S.A[6 + ax][i];
-                    rr.ainv[ax] = fabsf(rr.inv[ax]);
-                }
-                const float4 col = S.col[slot];
-                G = make_float4(S.A[9][i], S.A[10][i], S.A[11][i], 0.f);
-                gc = G.x * col.x + G.y * col.y + G.z * col.z;
-                float s0, s1, t_ref, D[3];
-                if (slab(rr, a, bq, s0, s1, t_ref, D)) {           // the precise test decides
-                    const float4 ra = S.r0[slot], rb = S.r1[slot];
-                    tau = integrate<K, true>(rr, D, a.w, s0, s1, ra, rb, dtau);
-                    if (HEADS) gc = fmaf(S.PD[i], t_ref + 0.5f * (s0 + s1), gc);
-                }
-            }
-            const float E = ex2f(-1.4426950408889634f * tau);
-            const unsigned int lower = peers & lt;
-            const int level = __popc(lower);
-            const int pred = lower ? 31 - __clz(lower) : lane;
-            const int maxL = (int)__reduce_max_sync(FULL, (unsigned int)level);
-            float2 st = make_float2(0.f, 0.f);
-            if (valid && level == 0) st = make_float2(S.T[i], S.Pp[i]);
-            float w = 0.f;
-            bool live = false;
-            for (int L = 0; L <= maxL; ++L) {
-                if (L > 0) {
-                    const float t0 = __shfl_sync(FULL, st.x, pred), t1 = __shfl_sync(FULL, st.y, pred);
-                    if (level == L) st = make_float2(t0, t1);
-                }
-                if (level == L) {
-                    live = valid && st.x >= T_min;                // R8: a ray stops after the voxel that crosses T_min
-                    w = live ? st.x * (1.f - E) : 0.f;
-                    st.x = live ? st.x * E : st.x;
-                    st.y = fmaf(w, gc, st.y);
-                }
-            }
-            if (valid && (peers >> lane) == 1u) { S.T[i] = st.x; S.Pp[i] = st.y; }    // last hit of its pixel in this round
-            // ---- 5. reduce ----
-            float v[11];
-            {
-                const float dLdtau = live ? fmaf(st.x, gc, st.y) : 0.f;
-#pragma unroll
-                for (int m = 0; m < 8; ++m) v[m] = dLdtau * dtau[m];
-                v[8] = w * G.x; v[9] = w * G.y; v[10] = w * G.z;
-            }
-            float wq = w;
-#pragma unroll
-            for (int s = 0; s < RED_STEPS; ++s) {
-                const int step = 1 << s;
-                const float take = (step <= rem) ? 1.f : 0.f;
-#pragma unroll
-                for (int m = 0; m < 11; ++m) v[m] = fmaf(take, __shfl_down_sync(FULL, v[m], step), v[m]);
-                wq = fmaxf(wq, take * __shfl_down_sync(FULL, wq, step));
-            }
-            if (frag_head && wq > 0.f) {
-                red_add_v4(grad_coef + (size_t)vid * 8, v[0], v[1], v[2], v[3]);
-                red_add_v4(grad_coef + (size_t)vid * 8 + 4, v[4], v[5], v[6], v[7]);
-                red_add_v4(grad_rgb + (size_t)vid * 4, v[8], v[9], v[10], 0.f);
-                if (__float_as_uint(wq) > wm_old) atomicMax(w_max + vid, __float_as_uint(wq));
-            }
-            __syncwarp();                                          // pixel state is reused by the next round
-        }
-        return n;
     };
 
     if (REPLAY) {
@@ -591,21 +736,87 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
         const uint32_t r0 = trav_off[tile], cap = (trav_off[tile + 1] - r0) >> 3;
         const uint32_t* rec = trav + ((size_t)r0 + (size_t)warp * cap) * TRAV_WORDS;
         const uint32_t n_rec = trav_count[tile * 8 + warp];
-        for (uint32_t rb = 0; rb < n_rec; ++rb, rec += TRAV_WORDS) {
-            const int n = (int)__ldg(rec + 64);
-            const unsigned int hits = __ldg(rec + lane);
-            if (__ballot_sync(FULL, hits != 0u) == 0u) continue;       // nothing hit in this batch
+        if (n_rec == 0u) return;
+        struct Hdr { unsigned int hits; uint32_t vid, misc; };
+        auto load_hdr = [&](const uint32_t* r) {
+            Hdr h;
+            h.hits = __ldg(r + lane); h.vid = __ldg(r + 32 + lane); h.misc = __ldg(r + 64 + (lane & 7));
+            return h;
+        };
+        auto gather = [&](const Hdr& h, int buf) {
+            const int n = (int)__shfl_sync(FULL, h.misc, 0);
             if (lane < n) {
-                const float4* pr = packed + 5 * (size_t)__ldg(rec + 32 + lane);
-                const float4 t0 = __ldg(pr), t1 = __ldg(pr + 1), t2 = __ldg(pr + 2), t3 = __ldg(pr + 3), t4 = __ldg(pr + 4);
-                const uint32_t vid = __float_as_uint(t1.w);
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
-                S.g0[lane] = t0; S.g1[lane] = t1; S.r0[lane] = t2; S.r1[lane] = t3; S.col[lane] = t4;
+                const float4* pr = packed + 5 * (size_t)h.vid;
+                const int slot = buf + lane;
+                cp_async16(&S.g0[slot], pr); cp_async16(&S.g1[slot], pr + 1); cp_async16(&S.r0[slot], pr + 2);
+                cp_async16(&S.r1[slot], pr + 3); cp_async16(&S.col[slot], pr + 4);
+                // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the DRAM fill
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)h.vid * 8));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)h.vid * 4));
             }
-            __syncwarp();
-            for (int k0 = 0; k0 < n;) k0 += run_batch(hits >> k0, n - k0, k0);
-            __syncwarp();
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            if (haveE) {                                                // its E rows: into L2
+                const uint32_t rows = __shfl_sync(FULL, h.misc, 7), eb = __shfl_sync(FULL, h.misc, 1);
+                if ((uint32_t)lane < rows) asm volatile("prefetch.global.L2 [%0];" ::"l"(trav_E + ((size_t)eb + lane) * 32u));
+            }
+        };
+        // header b + 2: into L2 (3 lines); header b + 1: loaded at the top of batch b, its voxel records gathered while batch b
+        // is worked on. Only (hits, misc) of two headers live in registers across a batch.
+        auto prefetch_hdr = [&](const uint32_t* r) {
+            if (lane < 3) asm volatile("prefetch.global.L2 [%0];" ::"l"(r + 32 * lane));
+        };
+        unsigned int hits_a, hits_b = 0u;
+        uint32_t misc_a, misc_b = 0u;
+        if (SVR_BWD_DB) {
+            {
+                const Hdr h0 = load_hdr(rec);
+                gather(h0, 0);
+                hits_a = h0.hits; misc_a = h0.misc;
+                if (n_rec > 1u) prefetch_hdr(rec + TRAV_WORDS);
+            }
+            for (uint32_t rb = 0; rb < n_rec; ++rb) {
+                const int buf = (int)(rb & 1u) * NSLOT;
+                if (rb + 1u < n_rec) {
+                    const Hdr h1 = load_hdr(rec + (size_t)(rb + 1u) * TRAV_WORDS);
+                    if (rb + 2u < n_rec) prefetch_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
+                    gather(h1, buf ^ NSLOT);
+                    hits_b = h1.hits; misc_b = h1.misc;
+                    asm volatile("cp.async.wait_group 1;" ::: "memory");
+                } else {
+                    asm volatile("cp.async.wait_group 0;" ::: "memory");
+                }
+                __syncwarp();
+                run_batch(buf, hits_a, (int)__shfl_sync(FULL, misc_a, 0), misc_a);
+                __syncwarp();
+                hits_a = hits_b; misc_a = misc_b;
+            }
+        } else {
+            // single buffer: the records of batch b + 1 are pulled into L2 while batch b is worked on and gathered after it
+            auto prefetch_records = [&](const Hdr& h) {
+                const int n = (int)__shfl_sync(FULL, h.misc, 0);
+                if (lane < n) {
+                    const char* pr = reinterpret_cast<const char*>(packed + 5 * (size_t)h.vid);
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pr));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pr + 64));
+                }
+            };
+            Hdr h1 = load_hdr(rec);
+            gather(h1, 0);
+            hits_a = h1.hits; misc_a = h1.misc;
+            if (n_rec > 1u) prefetch_hdr(rec + TRAV_WORDS);
+            for (uint32_t rb = 0; rb < n_rec; ++rb) {
+                const bool next = rb + 1u < n_rec;
+                if (next) {
+                    h1 = load_hdr(rec + (size_t)(rb + 1u) * TRAV_WORDS);
+                    if (rb + 2u < n_rec) prefetch_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
+                    prefetch_records(h1);
+                }
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                __syncwarp();
+                run_batch(0, hits_a, (int)__shfl_sync(FULL, misc_a, 0), misc_a);
+                __syncwarp();
+                if (next) { gather(h1, 0); hits_a = h1.hits; misc_a = h1.misc; }
+            }
         }
         return;
     }
@@ -613,13 +824,13 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
     for (int so = 0; so < 8; ++so) {
         const uint32_t start = ranges[(tile * 8 + so) * 2], end = ranges[(tile * 8 + so) * 2 + 1];
         if (start == end) continue;
-        bool alive = inimg && (oct == so) && (Tpix >= T_min);
+        bool alive = inimg && (oct == so) && (T >= T_min);
         unsigned int alive_mask = __ballot_sync(FULL, alive);
         if (alive_mask == 0u) continue;                               // no pixel of this warp uses this list
-        int head = 0, count = 0;                                      // ring state (warp-uniform)
         uint32_t base = start;
-        while (true) {
+        while (base < end) {
             // ---- 1. cull + stage until 32 survivors are waiting or the list is exhausted ----
+            int count = 0;
             while (count < NSLOT && base < end) {
                 const uint32_t idx = base + lane;
                 unsigned int M = 0u;
@@ -638,9 +849,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     const float4 t0 = __ldg(rec), t1 = __ldg(rec + 1), t2 = __ldg(rec + 2), t3 = __ldg(rec + 3);
                     float4 t4 = __ldg(rec + 4);
                     t4.w = __uint_as_float(M);
-                    const int slot = (head + count + rank) & (NSLOT - 1);
+                    const int slot = count + rank;
                     const uint32_t vid = __float_as_uint(t1.w);
-                    // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the DRAM fill
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
                     S.g0[slot] = t0; S.g1[slot] = t1; S.r0[slot] = t2; S.r1[slot] = t3; S.col[slot] = t4;
@@ -651,63 +861,41 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
             if (count == 0) break;
             __syncwarp();
             // ---- 2. test: every lane walks its own pixel's candidates (conservative slab test) ----
-            int n = count;
-            unsigned int hits = 0u;
-            {
-                unsigned int cand = transpose32(lane < n ? __float_as_uint(S.col[(head + lane) & (NSLOT - 1)].w) : 0u, lane);
-                if (!alive) cand = 0u;
-                while (__any_sync(FULL, cand != 0u)) {
-                    if (cand) {
-                        const int k = __ffs(cand) - 1;
-                        cand &= cand - 1;
-                        const float4 a = S.g0[(head + k) & (NSLOT - 1)];
-                        // box dilated by a bound on what the lo parts and the rounding can move: never loses a true hit
-                        const float hd = fmaf(fabsf(a.x) + fabsf(a.y) + fabsf(a.z), 4.8e-7f, a.w * 1.000002f);
-                        const float cx = a.x * inv[0], cy = a.y * inv[1], cz = a.z * inv[2];
-                        const float wx = hd * ainv[0], wy = hd * ainv[1], wz = hd * ainv[2];
-                        const float s0 = fmaxf(fmaxf(cx - wx, cy - wy), fmaxf(cz - wz, 0.f));
-                        const float s1 = fminf(fminf(cx + wx, cy + wy), cz + wz);
-                        if (s1 > s0) hits |= 1u << k;
-                    }
-                }
-            }
-            n = run_batch(hits, n, head);
-            head = (head + n) & (NSLOT - 1);
-            count -= n;
-            Tpix = S.T[swl];
-            alive = inimg && (oct == so) && (Tpix >= T_min);
+            unsigned int cand = transpose32(lane < count ? __float_as_uint(S.col[lane].w) : 0u, lane);
+            if (!alive) cand = 0u;
+            unsigned int n_test = 0;
+            const unsigned int hits = test_candidates<false>(cand, S.g0, S.col, inv, n_test);
+            if (__any_sync(FULL, hits != 0u)) run_batch(0, hits, count, 0u);
+            __syncwarp();
+            alive = inimg && (oct == so) && (T >= T_min);
             alive_mask = __ballot_sync(FULL, alive);
             if (alive_mask == 0u) break;                              // whole warp terminated
         }
     }
 }
 
-template <typename KernelT>
-SvrStatus set_smem_once(SvrContext* ctx, KernelT kernel, size_t smem, bool* done) {
-    if (!*done) {
-        SVR_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        *done = true;
-    }
-    return SVR_OK;
-}
-
 }  // namespace
+
+// A cudaFuncAttribute is per device: set it on every launch path once per (kernel, device) (a second context on another GPU
+// must get it too); the call is cheap next to a launch, so it is simply repeated.
+#define SVR_SET_SMEM(ctx, kernel, smem) SVR_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem)))
 
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
                          float* w_max, unsigned long long* stats, bool record) {
     if (f->n_tiles == 0) return SVR_OK;
-    StageScope scope__(ctx, ST_FORWARD);
-    const size_t smem = sizeof(WarpStage) * WARPS;
+    const size_t smem = sizeof(FwdWarp) * WARPS;
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
     const bool rec = record && f->trav != nullptr;
+    if (rec && f->trav_ectl) SVR_CUDA(ctx, cudaMemsetAsync(f->trav_ectl, 0, 2 * sizeof(uint32_t), ctx->stream));
+    StageScope scope__(ctx, ST_FORWARD);
 #define SVR_FWD_GO(KK, SS, RR)                                                                                       \
     do {                                                                                                             \
-        static bool done = false;                                                                                    \
-        SVR_TRY(set_smem_once(ctx, composite_kernel<KK, SS, RR>, smem, &done));                                      \
+        SVR_SET_SMEM(ctx, (composite_kernel<KK, SS, RR>), smem);                                                     \
         composite_kernel<KK, SS, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, image, depth, \
-                                                                             T_final, wm, stats, f->trav, f->trav_off, f->trav_count);       \
+                                                                             T_final, wm, stats, f->trav, f->trav_off, f->trav_count, \
+                                                                             f->trav_E, f->trav_ectl, f->trav_E ? f->trav_E_cap : 0u);       \
     } while (0)
 #define SVR_FWD(KK)                                                                                                  \
     do {                                                                                                             \
@@ -734,20 +922,20 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
                           const float* depth, const float* T_final) {
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, ST_BACKWARD);
-    const size_t smem = sizeof(WarpWork) * WARPS;
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
     // replay the forward pass's traversal record when there is one for this termination threshold
     const bool replay = f->trav != nullptr && f->trav_valid && f->trav_T_min == T_min && (ctx->debug_flags & 16) == 0;
     const bool heads = dL_ddepth != nullptr || dL_dT != nullptr;
+    const float* eg = (ctx->debug_flags & 32) ? nullptr : f->trav_E;       // debug flag 32: ignore the recorded E values
 #define SVR_BWD_GO(KK, HH, RR)                                                                                       \
     do {                                                                                                             \
-        static bool done = false;                                                                                    \
-        SVR_TRY(set_smem_once(ctx, backward_packed_kernel<KK, HH, RR>, smem, &done));                                \
+        const size_t smem = sizeof(BwdWarp<HH>) * WARPS;                                                             \
+        SVR_SET_SMEM(ctx, (backward_packed_kernel<KK, HH, RR>), smem);                                               \
         backward_packed_kernel<KK, HH, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(                                  \
             f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, wm, dL, image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth, T_final,         \
-            f->trav, f->trav_off, f->trav_count);                                                                    \
+            f->trav, f->trav_off, f->trav_count, eg, f->trav_ectl);                                                  \
     } while (0)
 #define SVR_BWD(KK)                                                                                                  \
     do {                                                                                                             \

@@ -104,20 +104,38 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
     void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed,
-                    f->trav, f->trav_off, f->trav_count};
+                    f->trav, f->trav_off, f->trav_count, f->trav_E, f->trav_ectl};
     for (void* p : ptrs)
         if (p) svr_free(ctx, p, 0);
     return SVR_OK;
 }
 
 // Traversal scratch (svr_forward records, svr_backward replays): at most E/4 + 80 n_tiles records of SVR_TRAV_WORDS words
-// (sum over tiles of 8 warps x (ceil(len / 32) + 9)). Debug flag 16 disables it (backward then culls and tests itself).
+// (sum over tiles of 8 warps x (ceil(len / 32) + 9)), plus the E record: exp(-tau) of every queued ray-voxel hit, in units of
+// 32 floats handed out by a device-side cursor. Its size follows the previous recorded view (units per list entry, read back
+// asynchronously after each recording forward pass) with 25 % slack; when it is too small, or the budget has no room for
+// it, the forward pass sets a flag and the backward pass recomputes E (same result, slower). Debug flag 16 disables the
+// traversal record (backward then culls and tests itself).
 SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
     if (ctx->debug_flags & 16) return SVR_OK;
     const size_t cap = (size_t)E / 4 + 80 * (size_t)f->n_tiles + 8;
     SVR_TRY(svr_alloc(ctx, (void**)&f->trav, sizeof(uint32_t) * SVR_TRAV_WORDS * cap));
     SVR_TRY(svr_alloc(ctx, (void**)&f->trav_off, sizeof(uint32_t) * (size_t)(f->n_tiles + 1)));
     SVR_TRY(svr_alloc(ctx, (void**)&f->trav_count, sizeof(uint32_t) * 8 * (size_t)f->n_tiles));
+    SVR_TRY(svr_alloc(ctx, (void**)&f->trav_ectl, 256));
+    if (ctx->e_last_entries > 0 && cudaEventQuery(ctx->ectl_ev) == cudaSuccess) {
+        const uint32_t used = reinterpret_cast<const uint32_t*>(ctx->host_pinned + 4)[0];
+        ctx->e_units_per_entry = (double)used / (double)ctx->e_last_entries;
+        ctx->e_last_entries = 0;
+    }
+    const double per_entry = ctx->e_units_per_entry > 0.0 ? 1.25 * ctx->e_units_per_entry : 0.5;
+    double units = per_entry * (double)E + 64.0 * (double)f->n_tiles + 1024.0;
+    if (units > 4.0e9) units = 4.0e9;
+    f->trav_E_cap = (uint32_t)units;
+    if (svr_alloc(ctx, (void**)&f->trav_E, sizeof(float) * 32 * ((size_t)f->trav_E_cap + 64)) != SVR_OK) {   // + 64 rows: read-ahead
+        f->trav_E = nullptr;            // no room under the budget: the backward pass recomputes E
+        f->trav_E_cap = 0;
+    }
     return SVR_OK;
 }
 
@@ -150,6 +168,7 @@ SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t wor
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->upload_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->lists_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->sort_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ectl_ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         // no usable CUDA device: fail loudly, there is no other path
         fprintf(stderr, "svr_create: CUDA error: %s\n", cudaGetErrorString(e));
@@ -174,6 +193,7 @@ void svr_destroy(SvrContext* ctx) {
     if (ctx->upload_ev) cudaEventDestroy(ctx->upload_ev);
     if (ctx->lists_ev) cudaEventDestroy(ctx->lists_ev);
     if (ctx->sort_ev) cudaEventDestroy(ctx->sort_ev);
+    if (ctx->ectl_ev) cudaEventDestroy(ctx->ectl_ev);
     if (ctx->aux) cudaStreamDestroy(ctx->aux);
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
@@ -386,7 +406,16 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     const bool record = opts->record != 0 && frame->trav != nullptr;
     SvrStatus st = launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max, nullptr, record);
-    if (st == SVR_OK && record) { frame->trav_valid = true; frame->trav_T_min = opts->T_min; }
+    if (st == SVR_OK && record) {
+        frame->trav_valid = true;
+        frame->trav_T_min = opts->T_min;
+        if (frame->trav_ectl && frame->n_entries > 0) {
+            // how much of the E record this view used: sizes the next frame's (alloc_traversal); never waited for
+            SVR_CUDA(ctx, cudaMemcpyAsync(ctx->host_pinned + 4, frame->trav_ectl, 8, cudaMemcpyDeviceToHost, ctx->stream));
+            SVR_CUDA(ctx, cudaEventRecord(ctx->ectl_ev, ctx->stream));
+            ctx->e_last_entries = frame->n_entries;
+        }
+    }
     return st;
 }
 

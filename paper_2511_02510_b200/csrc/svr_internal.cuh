@@ -11,7 +11,7 @@
 
 #define SVR_TILE 16
 #define SVR_MAX_K 4
-#define SVR_TRAV_WORDS 68     // traversal record: 32 hit masks, 32 voxel ids, slot count (+ padding to 16 bytes)
+#define SVR_TRAV_WORDS 72     // traversal record: 32 hit masks, 32 voxel ids, slot count, 6 sub-batch E offsets (+ padding to 16 bytes)
 
 enum SvrStage {
     ST_TILE_MASKS = 0, ST_RECTS, ST_SCAN, ST_EMIT, ST_SORT, ST_RANGES, ST_COLORS, ST_FORWARD, ST_LOSS, ST_BACKWARD,
@@ -43,12 +43,14 @@ struct SvrContext {
     size_t loss_ws_bytes = 0;
     // second stream: work that does not depend on the render (the loss's source phase, the host path's upload)
     cudaStream_t aux = nullptr;
-    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr, lists_ev = nullptr, sort_ev = nullptr;
+    cudaEvent_t fork_ev = nullptr, loss_ready_ev = nullptr, upload_ev = nullptr, lists_ev = nullptr, sort_ev = nullptr, ectl_ev = nullptr;
     bool loss_prepared = false;   // svr_loss_prepare queued a source phase that the next svr_loss_grad may consume
     const float* loss_prep_target = nullptr;
     int loss_prep_W = 0, loss_prep_H = 0;
     float loss_prep_q = 0.f;
-    uint64_t* host_pinned = nullptr;  // 64-byte pinned readback slot
+    uint64_t* host_pinned = nullptr;  // 64-byte pinned readback slot (words 4..5: the last forward's E-record cursor / flag)
+    double e_units_per_entry = 0.0;   // E-record units (32 floats) used per list entry by the last recorded view: sizes the next one
+    int64_t e_last_entries = 0;       // list entries of the frame whose cursor is in flight to host_pinned[4]
     cudaEvent_t readback_ev = nullptr; // marks the readback copy: the host waits for it, not for the work queued behind it
 };
 
@@ -121,6 +123,9 @@ struct SvrFrame {
     uint32_t* trav = nullptr;        // [trav_cap, SVR_TRAV_WORDS] records
     uint32_t* trav_off = nullptr;    // [n_tiles + 1] first record of each tile
     uint32_t* trav_count = nullptr;  // [n_tiles * 8] records written per warp
+    float* trav_E = nullptr;         // [trav_E_cap * 32] exp(-tau) of every queued hit, handed out to warps in chunks
+    uint32_t* trav_ectl = nullptr;   // [2] chunk cursor (units of 32 floats), overflow flag
+    uint32_t trav_E_cap = 0;         // capacity of trav_E in units of 32 floats
     mutable bool trav_valid = false; // a forward pass has recorded this frame's traversal ...
     mutable float trav_T_min = 0.f;  // ... with this termination threshold
     size_t bytes = 0;
