@@ -352,7 +352,7 @@ struct FwdWarp {
 // profiles/r2b_*.) Traversal record of one batch (TRAV_WORDS words, written with REC): [0,32) every pixel's hit mask, [32,64)
 // the staged voxel ids, [64] the slot count, [65] the first E row of the batch in the E record, [71] its number of rows; E
 // row i holds, for every pixel of the block, exp(-tau) of its i-th hit in the batch (1 where it has none or missed).
-template <int K, bool STATS, bool REC>
+template <int K, bool STATS, bool REC, bool WMAX>
 __global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
@@ -447,7 +447,7 @@ __global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, cons
             // and records the hits; (2) every lane integrates and composites its own hits. A lane that misses does not sit
             // idle through another lane's K samples, and the hit loop is as long as the pixel with the most HITS.
             unsigned int hits = test_candidates<true>(cand, S.g0 + head, S.col + head, ray.inv, n_test);
-            float* eg = nullptr;
+            uint32_t eoff = 0xFFFFFFFFu;                                  // this lane's word in the E record (none: no room / no hits)
             if (REC && __any_sync(FULL, hits != 0u)) {
                 uint32_t* r = rec_out + (size_t)n_rec * TRAV_WORDS;
                 r[lane] = hits;
@@ -459,7 +459,7 @@ __global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, cons
                     e_pos = __shfl_sync(FULL, e_pos, 0);
                     e_left = grab;
                 }
-                if (e_pos + rows <= e_cap) eg = trav_E + (size_t)e_pos * 32u + lane;
+                if (e_pos + rows <= e_cap) eoff = e_pos * 32u + lane;     // (e_cap < 2^27 rows: the offset fits 32 bits)
                 else if (lane == 0) trav_ectl[1] = 1u;                  // E record full: the backward pass recomputes E
                 if (lane == 0) { r[64] = (uint32_t)n; r[65] = e_pos; r[71] = rows; }
                 e_pos += rows;
@@ -476,7 +476,7 @@ __global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, cons
                     if (slab(ray, a, bq, s0, s1, t_ref, D)) {               // the precise test decides
                         const uint32_t vid = __float_as_uint(bq.w);
                         unsigned int wm_old = 0u;
-                        if (w_max != nullptr) wm_old = w_max[vid];            // stale read is safe: w_max only grows
+                        if (WMAX) wm_old = w_max[vid];                        // stale read is safe: w_max only grows
                         const float4 ra = S.r0[slot], rb = S.r1[slot], col = S.col[slot];
                         const float tau = integrate<K>(ray, D, a.w, s0, s1, ra, rb);
                         E = ex2f(-1.4426950408889634f * tau);
@@ -485,11 +485,11 @@ __global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, cons
                         C0 = fmaf(w, col.x, C0); C1 = fmaf(w, col.y, C1); C2 = fmaf(w, col.z, C2);
                         if (STATS) ++n_hit;
                         Dep = fmaf(w, t_ref + 0.5f * (s0 + s1), Dep);
-                        if (w_max != nullptr && __float_as_uint(w) > wm_old) atomicMax(w_max + vid, __float_as_uint(w));
+                        if (WMAX && __float_as_uint(w) > wm_old) atomicMax(w_max + vid, __float_as_uint(w));
                         if (T < T_min) { alive = false; hits = 0u; }          // R8: stop after the voxel that crosses T_min
                     }
                 }
-                if (REC && eg != nullptr) { *eg = E; eg += 32; }              // a whole row per step: no partial sectors
+                if (REC && eoff != 0xFFFFFFFFu) { trav_E[eoff] = E; eoff += 32u; }   // a whole row per step: no partial sectors
             }
             __syncwarp();
             head ^= 32;
@@ -543,9 +543,9 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                                                                const uint2* __restrict__ rects_sorted,
                                                                const uint32_t* __restrict__ ranges,
                                                                const uint32_t* __restrict__ tile_order, float T_min,
-                                                               unsigned int* __restrict__ w_max, const float* __restrict__ dL,
-                                                               const float* __restrict__ image_in, float* __restrict__ grad_coef,
-                                                               float* __restrict__ grad_rgb, const float* __restrict__ dL_ddepth,
+                                                               const bool want_wmax, const float* __restrict__ dL,
+                                                               const float* __restrict__ image_in, float* __restrict__ grow,
+                                                               const float* __restrict__ dL_ddepth,
                                                                const float* __restrict__ dL_dT, const float* __restrict__ depth_in,
                                                                const float* __restrict__ T_in, const uint32_t* __restrict__ trav,
                                                                const uint32_t* __restrict__ trav_off, const uint32_t* __restrict__ trav_count,
@@ -674,10 +674,11 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     auto flush = [&]() {
                         if (wq > 0.f || acc[0] != 0.f) {
                             const uint32_t vid = __float_as_uint(bq.w);
-                            red_add_v4(grad_coef + (size_t)vid * 8, acc[0], acc[1], acc[2], acc[3]);
-                            red_add_v4(grad_coef + (size_t)vid * 8 + 4, acc[4], acc[5], acc[6], acc[7]);
-                            red_add_v4(grad_rgb + (size_t)vid * 4, acc[8], acc[9], acc[10], 0.f);
-                            if (w_max != nullptr) atomicMax(&S.wms[k0 + cur], __float_as_uint(wq));
+                            float* row = grow + (size_t)vid * 16;             // the voxel's 64-byte scratch row
+                            red_add_v4(row, acc[0], acc[1], acc[2], acc[3]);
+                            red_add_v4(row + 4, acc[4], acc[5], acc[6], acc[7]);
+                            red_add_v4(row + 8, acc[8], acc[9], acc[10], 0.f);
+                            if (want_wmax) atomicMax(&S.wms[k0 + cur], __float_as_uint(wq));
                         }
                     };
                     for (int cc = 0; cc < L.C; ++cc) {
@@ -719,11 +720,11 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                 __syncwarp();
                 // eq. 5: one atomicMax per voxel of the sub-batch (its hits all lie in this sub-batch); no guard read: a load
                 // that is waited for here costs more than the reductions it would save
-                if (w_max != nullptr && lane >= k0 && lane < k0 + L.n) {
+                if (want_wmax && lane >= k0 && lane < k0 + L.n) {
                     const unsigned int wv = S.wms[lane];
                     if (wv != 0u) {
                         S.wms[lane] = 0u;
-                        atomicMax(w_max + __float_as_uint(g1[lane].w), wv);
+                        atomicMax(reinterpret_cast<unsigned int*>(grow + (size_t)__float_as_uint(g1[lane].w) * 16 + 12), wv);
                     }
                 }
             }
@@ -750,9 +751,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                 const int slot = buf + lane;
                 cp_async16(&S.g0[slot], pr); cp_async16(&S.g1[slot], pr + 1); cp_async16(&S.r0[slot], pr + 2);
                 cp_async16(&S.r1[slot], pr + 3); cp_async16(&S.col[slot], pr + 4);
-                // pull the voxel's gradient lines into L2 now: a reduction that misses L2 waits for the DRAM fill
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)h.vid * 8));
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)h.vid * 4));
+                // pull the voxel's gradient row into L2 now: a reduction that misses L2 waits for the DRAM fill
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(grow + (size_t)h.vid * 16));
             }
             asm volatile("cp.async.commit_group;" ::: "memory");
             if (haveE) {                                                // its E rows: into L2
@@ -851,8 +851,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     t4.w = __uint_as_float(M);
                     const int slot = count + rank;
                     const uint32_t vid = __float_as_uint(t1.w);
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_coef + (size_t)vid * 8));
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grad_rgb + (size_t)vid * 4));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(grow + (size_t)vid * 16));
                     S.g0[slot] = t0; S.g1[slot] = t1; S.r0[slot] = t2; S.r1[slot] = t3; S.col[slot] = t4;
                 }
                 count += __popc(m);
@@ -890,12 +889,17 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
     const bool rec = record && f->trav != nullptr;
     if (rec && f->trav_ectl) SVR_CUDA(ctx, cudaMemsetAsync(f->trav_ectl, 0, 2 * sizeof(uint32_t), ctx->stream));
     StageScope scope__(ctx, ST_FORWARD);
-#define SVR_FWD_GO(KK, SS, RR)                                                                                       \
+#define SVR_FWD_GO2(KK, SS, RR, WW)                                                                                  \
     do {                                                                                                             \
-        SVR_SET_SMEM(ctx, (composite_kernel<KK, SS, RR>), smem);                                                     \
-        composite_kernel<KK, SS, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, image, depth, \
+        SVR_SET_SMEM(ctx, (composite_kernel<KK, SS, RR, WW>), smem);                                                 \
+        composite_kernel<KK, SS, RR, WW><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, image, depth, \
                                                                              T_final, wm, stats, f->trav, f->trav_off, f->trav_count, \
                                                                              f->trav_E, f->trav_ectl, f->trav_E ? f->trav_E_cap : 0u);       \
+    } while (0)
+#define SVR_FWD_GO(KK, SS, RR)                                                                                       \
+    do {                                                                                                             \
+        if (wm) SVR_FWD_GO2(KK, SS, RR, true);                                                                       \
+        else SVR_FWD_GO2(KK, SS, RR, false);                                                                         \
     } while (0)
 #define SVR_FWD(KK)                                                                                                  \
     do {                                                                                                             \
@@ -912,19 +916,19 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
     }
 #undef SVR_FWD
 #undef SVR_FWD_GO
+#undef SVR_FWD_GO2
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;
 }
 
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
-                          float* grad_coef, float* grad_rgb, float* w_max, const float* dL_ddepth, const float* dL_dT,
+                          float* grad_row, bool want_wmax, const float* dL_ddepth, const float* dL_dT,
                           const float* depth, const float* T_final) {
     if (f->n_tiles == 0) return SVR_OK;
     StageScope scope__(ctx, ST_BACKWARD);
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
-    unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
     // replay the forward pass's traversal record when there is one for this termination threshold
     const bool replay = f->trav != nullptr && f->trav_valid && f->trav_T_min == T_min && (ctx->debug_flags & 16) == 0;
     const bool heads = dL_ddepth != nullptr || dL_dT != nullptr;
@@ -934,7 +938,7 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
         const size_t smem = sizeof(BwdWarp<HH>) * WARPS;                                                             \
         SVR_SET_SMEM(ctx, (backward_packed_kernel<KK, HH, RR>), smem);                                               \
         backward_packed_kernel<KK, HH, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(                                  \
-            f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, wm, dL, image, grad_coef, grad_rgb, dL_ddepth, dL_dT, depth, T_final,         \
+            f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, want_wmax, dL, image, grad_row, dL_ddepth, dL_dT, depth, T_final,         \
             f->trav, f->trav_off, f->trav_count, eg, f->trav_ectl);                                                  \
     } while (0)
 #define SVR_BWD(KK)                                                                                                  \
@@ -976,7 +980,7 @@ SvrStatus launch_gather_rects(SvrContext* ctx, SvrFrame* f) {
     StageScope scope__(ctx, ST_PACK);
     if (f->n_entries > 0) {
         gather_rects_kernel<<<(unsigned int)((f->n_entries + 255) / 256), 256, 0, ctx->stream>>>(
-            f->vals, f->n_entries, reinterpret_cast<const uint2*>(f->rects), reinterpret_cast<uint2*>(f->rects_sorted));
+            f->vals, f->n_entries, reinterpret_cast<const uint2*>(f->rects_tight ? f->rects_tight : f->rects), reinterpret_cast<uint2*>(f->rects_sorted));
         ctx->launches += 1;
     }
     SVR_CUDA(ctx, cudaGetLastError());

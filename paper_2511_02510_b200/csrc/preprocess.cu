@@ -50,8 +50,12 @@ __device__ __forceinline__ uint32_t sat_query(const uint32_t* __restrict__ sat, 
 }
 
 // ---- B1: pixel rectangle of a voxel ---------------------------------------------------------------
-__device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c, uint2 q) {
+// *tight (optional) = the pixels whose CENTRE lies in the projected bounding box grown by 1/64 px: only their rays can hit the
+// voxel (the projection of a box in front of the camera is inside the bounding box of its projected corners; 1/64 px is far
+// above the fp32 error of the projection, ~3e-4 px). The compositing cull uses it; the lists are built from the B1 rectangle.
+__device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c, uint2 q, ushort4* tight = nullptr) {
     const ushort4 culled = make_ushort4(0xFFFF, 0xFFFF, 0, 0);
+    if (tight) *tight = culled;
     int L = q.y >> 16;
     float e = __fmul_rn(s.root_edge, __int_as_float((127 - L) << 23));
     float lo[3], hi[3];
@@ -85,6 +89,7 @@ __device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c
             allB = allB && (__fadd_rn(b0, __fmul_rn(cyh, Z[k])) >= 0.0f);
         }
         if (allL || allR || allT || allB) return culled;
+        if (tight) *tight = make_ushort4(0, 0, (unsigned short)(c.W - 1), (unsigned short)(c.H - 1));
         return make_ushort4(0, 0, (unsigned short)(c.W - 1), (unsigned short)(c.H - 1));
     }
     float u0 = 0.f, u1 = 0.f, v0 = 0.f, v1 = 0.f;
@@ -101,6 +106,12 @@ __device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c
     r.z = (unsigned short)(int)floorf(fminf(u1, __fsub_rn(Wf, 1.0f)));
     r.y = (unsigned short)(int)floorf(fmaxf(v0, 0.0f));
     r.w = (unsigned short)(int)floorf(fminf(v1, __fsub_rn(Hf, 1.0f)));
+    if (tight) {
+        const float g = 0.5f + 1.0f / 64.0f, h = 0.5f - 1.0f / 64.0f;
+        const int x0 = max((int)ceilf(u0 - g), (int)r.x), x1 = min((int)floorf(u1 - h), (int)r.z);
+        const int y0 = max((int)ceilf(v0 - g), (int)r.y), y1 = min((int)floorf(v1 - h), (int)r.w);
+        if (x0 <= x1 && y0 <= y1) *tight = make_ushort4((unsigned short)x0, (unsigned short)y0, (unsigned short)x1, (unsigned short)y1);
+    }
     return r;
 }
 
@@ -338,9 +349,9 @@ __global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, 
 // Consumed scratch entries are re-zeroed, so the scratch buffers stay all-zero between calls.
 template <int DEG>
 __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
-                                                             const float4* __restrict__ rgbm, float4* __restrict__ grad_coef,
-                                                             float4* __restrict__ grad_rgb, float4* __restrict__ grad_raw,
-                                                             float* __restrict__ grad_sh) {
+                                                             const float4* __restrict__ rgbm, float4* __restrict__ grow,
+                                                             float4* __restrict__ grad_raw, float* __restrict__ grad_sh,
+                                                             float* __restrict__ w_max) {
     constexpr int NB = (DEG + 1) * (DEG + 1);
     constexpr int ROW = NB * 3;
     __shared__ float Ysm[4][32][NB + 1];
@@ -353,10 +364,17 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
     if (v < s.n) { ushort4 r = rects[v]; vis = r.x <= r.z; }
     bool sh_active = false;
     if (vis) {
-        float4 ga = grad_coef[2 * v], gb = grad_coef[2 * v + 1];
+        // the voxel's 64-byte scratch row: coefficient gradient (8), colour gradient (3), -, max blending weight, -
+        float4 ga = grow[4 * v], gb = grow[4 * v + 1];
+        const float4 g = grow[4 * v + 2];
+        const float wv = grow[4 * v + 3].x;
+        if (wv != 0.f) {                                              // eq. 5: merge into the caller's w_max
+            grow[4 * v + 3] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (w_max != nullptr) w_max[v] = fmaxf(w_max[v], wv);
+        }
         if (ga.x != 0.f || ga.y != 0.f || ga.z != 0.f || ga.w != 0.f || gb.x != 0.f || gb.y != 0.f || gb.z != 0.f || gb.w != 0.f) {
-            grad_coef[2 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
-            grad_coef[2 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+            grow[4 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
+            grow[4 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
             const float g0 = ga.x, gx = ga.y, gy = ga.z, gz = ga.w, gxy = gb.x, gxz = gb.y, gyz = gb.z, gxyz = gb.w;
             float4 ra = grad_raw[2 * v], rb = grad_raw[2 * v + 1];
             ra.x += ((g0 - gx) - (gy + gz)) + ((gxy + gxz) + (gyz - gxyz));
@@ -370,9 +388,8 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
             grad_raw[2 * v] = ra;
             grad_raw[2 * v + 1] = rb;
         }
-        float4 g = grad_rgb[v];
         if (g.x != 0.f || g.y != 0.f || g.z != 0.f) {
-            grad_rgb[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+            grow[4 * v + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
             unsigned mask = __float_as_uint(rgbm[v].w);
             float gv0 = (mask & 1u) ? g.x : 0.f, gv1 = (mask & 2u) ? g.y : 0.f, gv2 = (mask & 4u) ? g.z : 0.f;
             sh_active = (gv0 != 0.f || gv1 != 0.f || gv2 != 0.f);
@@ -459,7 +476,8 @@ template <int DEG>
 __global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamDev c, const uint8_t* __restrict__ masks,
                                                                 ushort4* __restrict__ rects, uint32_t* __restrict__ bcount,
                                                                 int* __restrict__ bigdiff, unsigned long long* __restrict__ totals,
-                                                                float4* __restrict__ rgbm, float4* __restrict__ vrec) {
+                                                                float4* __restrict__ rgbm, float4* __restrict__ vrec,
+                                                                ushort4* __restrict__ rects_tight) {
     const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     ushort4 r = make_ushort4(1, 0, 0, 0);      // "not visible"
@@ -474,10 +492,12 @@ __global__ void __launch_bounds__(256) rect_bucket_count_kernel(SceneDev s, CamD
             if (DEG >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(psh + 12 * (DEG + 1) * (DEG + 1) - 4));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(s.raw + v * 8));
         }
-        r = voxel_rect(s, c, q);
+        ushort4 rt;
+        r = voxel_rect(s, c, q, &rt);
         rects[v] = r;
         vis = r.x <= r.z;
         if (vis) {
+            rects_tight[v] = rt;
             const float4 col = voxel_color_dev<DEG>(s, c, q, v);
             rgbm[v] = col;
             voxel_record_dev(s, c, q, (uint32_t)v, col, vrec);
@@ -983,20 +1003,19 @@ SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
     return SVR_OK;
 }
 
-SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw, float* grad_sh) {
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row, float* grad_raw, float* grad_sh, float* w_max) {
     StageScope scope__(ctx, ST_SH_BACKWARD);
     if (f->scene.n == 0) return SVR_OK;
     unsigned int g = blocks_for(f->scene.n, 128);
     const ushort4* r = reinterpret_cast<const ushort4*>(f->rects);
     const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
-    float4* gc = reinterpret_cast<float4*>(grad_coef);
-    float4* gr = reinterpret_cast<float4*>(grad_rgb);
+    float4* gc = reinterpret_cast<float4*>(grad_row);
     float4* graw = reinterpret_cast<float4*>(grad_raw);
     switch (f->scene.sh_degree) {
-        case 0: voxel_backward_kernel<0><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
-        case 1: voxel_backward_kernel<1><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
-        case 2: voxel_backward_kernel<2><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
-        default: voxel_backward_kernel<3><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, gr, graw, grad_sh); break;
+        case 0: voxel_backward_kernel<0><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
+        case 1: voxel_backward_kernel<1><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
+        case 2: voxel_backward_kernel<2><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
+        default: voxel_backward_kernel<3><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
     }
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
@@ -1012,10 +1031,10 @@ SvrStatus launch_bucket_count(SvrContext* ctx, SvrFrame* f, uint32_t* bcount, in
         ushort4* r = reinterpret_cast<ushort4*>(f->rects);
         float4* col = reinterpret_cast<float4*>(f->rgbm);
         switch (f->scene.sh_degree) {
-            case 0: rect_bucket_count_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
-            case 1: rect_bucket_count_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
-            case 2: rect_bucket_count_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
-            default: rect_bucket_count_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed)); break;
+            case 0: rect_bucket_count_kernel<0><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed), reinterpret_cast<ushort4*>(f->rects_tight)); break;
+            case 1: rect_bucket_count_kernel<1><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed), reinterpret_cast<ushort4*>(f->rects_tight)); break;
+            case 2: rect_bucket_count_kernel<2><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed), reinterpret_cast<ushort4*>(f->rects_tight)); break;
+            default: rect_bucket_count_kernel<3><<<g, 256, 0, ctx->stream>>>(f->scene, f->cam, f->tile_masks, r, bcount, bigdiff, totals, col, reinterpret_cast<float4*>(f->packed), reinterpret_cast<ushort4*>(f->rects_tight)); break;
         }
         ctx->launches += 1;
     }
@@ -1044,16 +1063,13 @@ SvrStatus launch_bucket_scatter(SvrContext* ctx, SvrFrame* f, uint32_t* cursor, 
 SvrStatus launch_bucket_sort(SvrContext* ctx, SvrFrame* f, uint64_t* ent, const uint32_t* nonempty, const unsigned long long* totals,
                              unsigned int* work, int vb) {
     StageScope scope__(ctx, ST_SORT);
-    static bool attr_set = false;
     const int smem_small = 2 * SORT_CAP_SMALL * (int)sizeof(uint64_t) + (128 / 32) * 256 * (int)sizeof(uint16_t);
     const int smem_mid = 2 * SORT_CAP * (int)sizeof(uint64_t) + (SORT_THREADS2 / 32) * 256 * (int)sizeof(uint16_t);
     const int smem_big = 2 * SORT_CAP_BIG * (int)sizeof(uint64_t) + (1024 / 32) * 256 * (int)sizeof(uint16_t);
-    if (!attr_set) {
-        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<128, SORT_CAP_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_small));
-        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<SORT_THREADS2, SORT_CAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_mid));
-        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<1024, SORT_CAP_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_big));
-        attr_set = true;
-    }
+    // a function attribute is per device: set on every call (cheap), so a second context on another GPU gets it too
+    SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<128, SORT_CAP_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_small));
+    SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<SORT_THREADS2, SORT_CAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_mid));
+    SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_sort_kernel<1024, SORT_CAP_BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_big));
     // three block shapes so that the fixed cost of a pass (counter reset, scan) scales with the bucket; work[0..2] = fetch counters
     const int cb = 3 * f->scene.max_level;
     // The three classes are independent: the largest and the smallest run on the second stream beside the middle one

@@ -103,7 +103,7 @@ void fill_cam(const SvrCamera* cam, CamDev* c) {
 }
 
 SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
-    void* ptrs[] = {f->rects, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed,
+    void* ptrs[] = {f->rects, f->rects_tight, f->tile_masks, f->sat, f->offsets, f->rgbm, f->keys, f->vals, f->ranges, f->rects_sorted, f->tile_order, f->packed,
                     f->trav, f->trav_off, f->trav_count, f->trav_E, f->trav_ectl};
     for (void* p : ptrs)
         if (p) svr_free(ctx, p, 0);
@@ -130,7 +130,7 @@ SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
     }
     const double per_entry = ctx->e_units_per_entry > 0.0 ? 1.25 * ctx->e_units_per_entry : 0.5;
     double units = per_entry * (double)E + 64.0 * (double)f->n_tiles + 1024.0;
-    if (units > 4.0e9) units = 4.0e9;
+    if (units > 1.3e8) units = 1.3e8;      // word offsets into the record are 32-bit (rows * 32 < 2^32)
     f->trav_E_cap = (uint32_t)units;
     if (svr_alloc(ctx, (void**)&f->trav_E, sizeof(float) * 32 * ((size_t)f->trav_E_cap + 64)) != SVR_OK) {   // + 64 rows: read-ahead
         f->trav_E = nullptr;            // no room under the budget: the backward pass recomputes E
@@ -275,6 +275,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 #define CUDAF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(svr_fail(ctx, SVR_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e__))); } while (0)
 
     TRYF(A.get((void**)&f->rects, sizeof(uint16_t) * 4 * (size_t)n));
+    if (bucketed) TRYF(A.get((void**)&f->rects_tight, sizeof(uint16_t) * 4 * (size_t)n));
     TRYF(A.get((void**)&f->tile_masks, (size_t)f->n_tiles));
     if (!bucketed) TRYF(A.get((void**)&f->sat, sizeof(uint32_t) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1)));
     TRYF(A.get((void**)&f->rgbm, sizeof(float) * 4 * (size_t)n));
@@ -445,20 +446,17 @@ SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRe
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     const int64_t n = frame->scene.n;
     if (n == 0) return SVR_OK;
-    if (ctx->grad_rgb_cap < n) {
-        if (ctx->grad_rgb) svr_free(ctx, ctx->grad_rgb, sizeof(float) * 4 * (size_t)ctx->grad_rgb_cap);
-        if (ctx->grad_coef) svr_free(ctx, ctx->grad_coef, sizeof(float) * 8 * (size_t)ctx->grad_rgb_cap);
-        ctx->grad_rgb = ctx->grad_coef = nullptr;
-        ctx->grad_rgb_cap = 0;
-        SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_rgb, sizeof(float) * 4 * (size_t)n));
-        SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_coef, sizeof(float) * 8 * (size_t)n));
-        ctx->grad_rgb_cap = n;
-        SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_rgb, 0, sizeof(float) * 4 * (size_t)n, ctx->stream));
-        SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_coef, 0, sizeof(float) * 8 * (size_t)n, ctx->stream));
+    if (ctx->grad_cap < n) {
+        if (ctx->grad_row) svr_free(ctx, ctx->grad_row, 0);
+        ctx->grad_row = nullptr;
+        ctx->grad_cap = 0;
+        SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_row, sizeof(float) * 16 * (size_t)n));
+        ctx->grad_cap = n;
+        SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_row, 0, sizeof(float) * 16 * (size_t)n, ctx->stream));
     }
-    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_coef, ctx->grad_rgb, w_max, dL_ddepth, dL_dT,
+    SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_row, w_max != nullptr, dL_ddepth, dL_dT,
                             depth, T_final));
-    return launch_sh_backward(ctx, frame, ctx->grad_coef, ctx->grad_rgb, grad_raw_density, grad_sh);
+    return launch_sh_backward(ctx, frame, ctx->grad_row, grad_raw_density, grad_sh, w_max);
 }
 
 SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,

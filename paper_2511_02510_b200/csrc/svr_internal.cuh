@@ -36,9 +36,10 @@ struct SvrContext {
     int64_t launches = 0;
     std::string err;
     // persistent scratch
-    float* grad_rgb = nullptr;    // [n_cap,4] per-voxel colour-gradient scratch, kept all-zero between calls
-    float* grad_coef = nullptr;   // [n_cap,8] per-voxel density-coefficient-gradient scratch, same
-    int64_t grad_rgb_cap = 0;
+    // [n_cap,16] per-voxel gradient scratch, one 64-byte row per voxel (one DRAM access): [0,8) density-coefficient gradient,
+    // [8,11) colour gradient, [12] max blending weight (float bits); kept all-zero between calls by the finalize kernel
+    float* grad_row = nullptr;
+    int64_t grad_cap = 0;
     void* loss_ws = nullptr;      // loss workspace (see loss.cu)
     size_t loss_ws_bytes = 0;
     // second stream: work that does not depend on the render (the loss's source phase, the host path's upload)
@@ -109,6 +110,7 @@ struct SvrFrame {
     int64_t n_entries = 0;
     // device buffers (pool-allocated)
     uint16_t* rects = nullptr;       // [n,4]
+    uint16_t* rects_tight = nullptr; // [n,4] pixels whose centre can see the voxel (visible voxels only; bucketed list build)
     uint8_t* tile_masks = nullptr;   // [n_tiles]
     uint32_t* sat = nullptr;         // [(tiles_y+1)*(tiles_x+1)] summed-area table of popcount(mask)
     uint32_t* offsets = nullptr;     // [n+1] exclusive scan of counts
@@ -188,10 +190,9 @@ SvrStatus launch_gather_rects(SvrContext* ctx, SvrFrame* f);
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth,
                          float* T_final, float* w_max, unsigned long long* stats, bool record);
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
-                          float* grad_coef, float* grad_rgb, float* w_max, const float* dL_ddepth, const float* dL_dT,
+                          float* grad_row, bool want_wmax, const float* dL_ddepth, const float* dL_dT,
                           const float* depth, const float* T_final);
-SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_coef, float* grad_rgb, float* grad_raw,
-                             float* grad_sh);
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row, float* grad_raw, float* grad_sh, float* w_max);
 SvrStatus launch_loss_prepare(SvrContext* ctx, const float* target, int W, int H, float q);
 SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma,
                            float eps, float q, int sobel_source, float* dL, float* loss);
