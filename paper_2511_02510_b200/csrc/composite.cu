@@ -72,8 +72,7 @@ __constant__ unsigned int QINV[17] = {0, 65536, 32768, 21846, 16384, 13108, 1092
 
 struct WarpQ {              // hit queue of one sub-batch; per-entry arrays indexed by st(e)
     uint2 Hs[32];           // per slot: pixels that hit it, queue offset
-    float E[QCAP];          // forward: exp(-tau); backward: exp(-tau), replaced by the blending weight w
-    float X[QCAP];          // forward: t_mid; backward: dL/dtau
+    float2 WD[QCAP];        // x: exp(-tau) from the hit-major sweep, replaced by the blending weight w; y: dL/dtau
     unsigned short q[QCAP]; // (slot << 5) | pixel
 };
 
@@ -296,7 +295,7 @@ __device__ __forceinline__ void sweep_E(const float4* g0, const float4* g1, cons
                 E = ex2f(-1.4426950408889634f * tau);
                 tm = t_ref + 0.5f * (s0 + s1);
             }
-            Q.E[st] = E;
+            Q.WD[st].x = E;
             if (WANT_TM) tm_out[st] = tm;
         }
     }
@@ -632,7 +631,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                         const uint2 hk = S.Q.Hs[k];
                         const int st = q_st((int)hk.y + __popc(hk.x & lt), L);
                         if (haveE) S.Q.q[st] = (unsigned short)((k << 5) | lane);
-                        const float E = haveE ? e_rec : S.Q.E[st];
+                        const float E = haveE ? e_rec : S.Q.WD[st].x;
                         const float4 col = colp[k0 + k];
                         float gc = G.x * col.x + G.y * col.y + G.z * col.z;
                         if constexpr (HEADS) gc = fmaf(gdep, S.TM[st], gc);
@@ -640,8 +639,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                         const float w = live ? T * (1.f - E) : 0.f;
                         T = live ? T * E : T;
                         P = fmaf(w, gc, P);
-                        S.Q.X[st] = live ? fmaf(T, gc, P) : 0.f;
-                        S.Q.E[st] = w;
+                        S.Q.WD[st] = make_float2(w, live ? fmaf(T, gc, P) : 0.f);
                     };
                     bool more = __any_sync(FULL, m != 0u);
 #pragma unroll
@@ -695,7 +693,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                             a = g0[k0 + k]; bq = g1[k0 + k]; ra = r0[k0 + k]; rb = r1[k0 + k];
                         }
                         if (valid) {
-                            const float w = S.Q.E[st], dLdtau = S.Q.X[st];
+                            const float2 wd = S.Q.WD[st];
+                            const float w = wd.x, dLdtau = wd.y;
                             if (w > 0.f || dLdtau != 0.f) {
                                 const int i = (int)(u & 31u);
                                 RayF rr;
