@@ -15,8 +15,13 @@ Steps in the paper's order (reading R10 where the paper is silent):
 
 Pins (tests/test_oracle_pins.py): gamma = 0 => w~ = 1 and the gradient is sign(r)/(3|P|) (P:141);
 mean(w~) = 1 (eq. 8); constant target => s = 0; ramp image I = a x + b y => interior Sobel (8a, 8b);
-eq. 9 at t0, (t0+t1)/2, t1 gives 0, gamma_max/2, gamma_max. PARITY UNPINNED: Sobel source, grey
-conversion, border rule, percentile q, rho = L1 and the channel mean (paper silent).
+eq. 9 at t0, (t0+t1)/2, t1 gives 0, gamma_max/2, gamma_max; eq. 7 BY VALUE: a one-step target has Sobel
+magnitude {0, 4a}, so w_edge / w_flat = (eps / (1 + eps))^gamma and w~ in closed form; the
+nearest-rank rule sorted[ceil(q |P|) - 1] on a dot lattice whose magnitudes are {0, sqrt(2) a, 2a} with the
+rank boundary exactly at q |P| (floor(q |P|) or the maximum give another answer). The definitions the paper
+leaves open (Sobel source, grey conversion, border rule, the percentile q, rho = L1 and the channel mean) are
+the readings R10 of DESIGN.md: the pins fix that the code computes those readings, not that the paper meant them.
+q is used as given: callers that mirror the C ABI pass the binary32 value of the percentile.
 """
 from __future__ import annotations
 

@@ -198,8 +198,24 @@ def test_mirror_symmetry(orc):
     np.testing.assert_allclose(b["w_max"], a["w_max"], rtol=0, atol=1e-6)
 
 
+def _n_straddlers(scene, cam):
+    """voxels that cross the camera plane (some corner behind z = 1e-6, some in front): the oracle's bucketed mode sends
+    them to every block"""
+    e = scene.root_edge / 2.0 ** scene.ijkl[:, 3].astype(np.float64)
+    lo = scene.root_lo.astype(np.float64) + scene.ijkl[:, :3] * e[:, None]
+    zmin, zmax = np.full(scene.n, np.inf), np.full(scene.n, -np.inf)
+    for k in range(8):
+        z = (lo + e[:, None] * np.array([k & 1, (k >> 1) & 1, (k >> 2) & 1])) @ cam.R[2].astype(np.float64) + float(cam.t[2])
+        zmin, zmax = np.minimum(zmin, z), np.maximum(zmax, z)
+    return int(((zmin < 1e-6) & (zmax > 0)).sum())
+
+
 def test_bucketed_equals_pure(orc):
-    for cfg in (make_config("C1"), make_config("C2", n_voxels=3000, res_scale=0.25, n_cams=1)):
+    """The bucketed mode (the reference of every C3-C5 parity test) reproduces the pure mode, including on a reduced C4 whose
+    camera sits among background cells that cross the camera plane (the 'zmin < 1e-6 -> every block' branch)."""
+    c4 = make_config("C4", n_voxels=6000, res_scale=0.1, n_cams=1)
+    assert _n_straddlers(c4.scene, c4.cameras[0]) >= 5
+    for cfg in (make_config("C1"), make_config("C2", n_voxels=3000, res_scale=0.25, n_cams=1), c4):
         cam = cfg.cameras[0]
         a = orc.render(cfg.scene, cam, cfg.K, mode="pure")
         b = orc.render(cfg.scene, cam, cfg.K, mode="bucketed")
@@ -446,11 +462,64 @@ def test_sobel_of_a_ramp(orc):
     np.testing.assert_allclose(m[1:-1, 1:-1], math.hypot(8 * a, 8 * b), rtol=1e-12)
 
 
-def test_sh_quadrature_golden_fixture():
-    """tests/golden/sh_l1_axes.txt: band-1 values on the axes, sqrt(3/(4 pi)) (textbook), cited in the file."""
+def test_sh_quadrature_golden_fixture(orc):
+    """tests/golden/sh_l1_axes.txt: band-1 value on its own axis sqrt(3/(4 pi)) and Y_0 = 1/(2 sqrt(pi)) (textbook table of the
+    real SH basis, cited in the file) against the ORACLE's basis evaluated on the three axes (index i = l(l+1)+m: y, z, x)."""
     vals = [float(x) for x in open(os.path.join(GOLDEN, "sh_l1_axes.txt")).read().split("\n") if x and not x.startswith("#")]
-    assert abs(vals[0] - math.sqrt(3 / (4 * math.pi))) < 1e-15
-    assert abs(vals[1] - 0.5 / math.sqrt(math.pi)) < 1e-15
+    Y = orc.sh_basis(1, np.eye(3))                                     # rows: dir = +x, +y, +z
+    np.testing.assert_allclose(Y[:, 0], vals[1], rtol=0, atol=1e-15)
+    np.testing.assert_allclose([Y[1, 1], Y[2, 2], Y[0, 3]], vals[0], rtol=0, atol=1e-15)   # Y_1,-1(y), Y_1,0(z), Y_1,1(x)
+    assert abs(Y[0, 1]) + abs(Y[0, 2]) + abs(Y[1, 2]) + abs(Y[1, 3]) + abs(Y[2, 1]) + abs(Y[2, 3]) < 1e-15
+
+
+def test_lf_weights_closed_form_on_a_step_edge(orc):
+    """eq. 7 by VALUE (w = (eps + 1 - s)^gamma, eps = 1e-3; eq. 8). A two-level target with one vertical step
+    of height a has Sobel magnitude exactly 4a on the two columns beside the step and 0 elsewhere (kernel column sums 1+2+1).
+    With 10 % of the pixels on the edge the 0.99-quantile is 4a, so s = 1 on the edge and 0 on the flats:
+    w_edge / w_flat = (eps / (1 + eps))^gamma and w~ = w / mean(w) in closed form."""
+    H, W, a, gamma, eps = 12, 20, 0.375, 0.6, 1e-3
+    I = np.zeros((H, W, 3))
+    I[:, 9:] = a
+    m = orc.sobel_magnitude(I)
+    np.testing.assert_allclose(m[:, 8:10], 4 * a, rtol=1e-15)
+    assert np.count_nonzero(m) == 2 * H
+    from oracle.loss import lf_weights
+    wt = lf_weights(I, gamma, eps, 0.99)
+    w_e, w_f = eps ** gamma, (1.0 + eps) ** gamma
+    mean = (2 * H * w_e + (W - 2) * H * w_f) / (W * H)
+    np.testing.assert_allclose(wt[:, 8:10], w_e / mean, rtol=1e-13)
+    np.testing.assert_allclose(np.delete(wt, [8, 9], axis=1), w_f / mean, rtol=1e-13)
+    np.testing.assert_allclose(wt[0, 8] / wt[0, 0], (eps / (1.0 + eps)) ** gamma, rtol=1e-13)
+    # the same through the loss: L = mean over pixels of w~ |r|, r = 0.1 everywhere
+    L, dL, _ = orc.lf_loss_and_grad(I + 0.1, I, gamma, eps, 0.99)
+    assert abs(L - 0.1) < 1e-15                                       # mean(w~) = 1
+    np.testing.assert_allclose(dL[:, 8, 0], (w_e / mean) / (3 * W * H), rtol=1e-13)
+
+
+def test_lf_quantile_is_nearest_rank(orc):
+    """R10: m_q = sorted[ceil(q |P|) - 1]. A 20 x 20 lattice of 25 isolated dots of height a: each dot gives 4 pixels with
+    |grad| = 2a (edge neighbours: kernel weight 2), 4 with sqrt(2) a (corner neighbours: gx = gy = a) and a zero at its centre:
+    100 pixels at 2a, 100 at sqrt(2) a, 200 zeros. With q = 0.75 (exact in binary), q |P| = 300: the nearest rank is sorted[299]
+    = sqrt(2) a, so BOTH rings saturate (s = 1); floor(q |P|) = sorted[300] or the maximum would give 2a and s = 0.707 on the
+    corner ring."""
+    a, gamma, eps = 0.5, 0.6, 1e-3
+    I = np.zeros((20, 20, 3))
+    I[1::4, 1::4] = a
+    m = orc.sobel_magnitude(I)
+    vals, counts = np.unique(np.round(m.reshape(-1), 12), return_counts=True)
+    np.testing.assert_allclose(vals, [0.0, math.sqrt(2) * a, 2 * a], rtol=1e-12)
+    assert counts.tolist() == [200, 100, 100]
+    from oracle.loss import lf_weights
+    wt = lf_weights(I, gamma, eps, 0.75)
+    w_ring, w_flat = eps ** gamma, (1.0 + eps) ** gamma
+    mean = (200 * w_ring + 200 * w_flat) / 400
+    np.testing.assert_allclose(wt[m > 0], w_ring / mean, rtol=1e-12)  # corner ring saturated too: m_q = sqrt(2) a
+    np.testing.assert_allclose(wt[m == 0], w_flat / mean, rtol=1e-12)
+    # one rank higher (q |P| = 301 > 300) the quantile moves to 2a and the corner ring gets s = 1/sqrt(2)
+    wt2 = lf_weights(I, gamma, eps, 0.7501)
+    w_corner = (eps + 1.0 - 1.0 / math.sqrt(2)) ** gamma
+    mean2 = (100 * w_ring + 100 * w_corner + 200 * w_flat) / 400
+    np.testing.assert_allclose(wt2[np.isclose(m, math.sqrt(2) * a)], w_corner / mean2, rtol=1e-12)
 
 
 # ---------------------------------------------------------------------------------------------
