@@ -78,7 +78,22 @@ typedef struct {
     int32_t sobel_source;     /* 0 = target image (default reading), 1 = render */
 } SvrLossOpts;
 
+/* Context: device, stream, workspace. Workspace blocks (per-view lists, records, scratch) are cached by the context and
+ * reused from view to view; their backing store is
+ *   svr_create:                 a PRIVATE stream-ordered memory pool of the context (cudaMemPoolCreate; the device's default
+ *                               pool and its release threshold are not touched),
+ *   svr_create_with_allocator:  the caller's allocator, e.g. PyTorch's caching allocator ("PyTorch is used only for device
+ *                               memory and streams"): alloc_fn(bytes, user) returns device memory usable on `cuda_stream`
+ *                               (NULL on failure), free_fn(ptr, user) takes it back; both are called from the thread that
+ *                               calls the library, only for blocks the cache does not hold already. Both or neither.
+ * `workspace_budget_bytes` (0 = unlimited) bounds the bytes in live + cached blocks. Limits checked by svr_preprocess:
+ * root_edge a positive power of two (SVR_ERR_INVALID_ARG otherwise); image up to 65535 pixels a side and
+ * (ceil(W/16)+1)(ceil(H/16)+1) <= 51200 tile-grid points, about 14 Mpixel (SVR_ERR_UNSUPPORTED beyond). */
+typedef void* (*SvrAllocFn)(size_t bytes, void* user);
+typedef void (*SvrFreeFn)(void* ptr, void* user);
 SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t workspace_budget_bytes);
+SvrStatus svr_create_with_allocator(SvrContext** out, int device, void* cuda_stream, SvrAllocFn alloc_fn, SvrFreeFn free_fn, void* user,
+                                    size_t workspace_budget_bytes);
 void svr_destroy(SvrContext* ctx);
 const char* svr_last_error(const SvrContext* ctx);
 /* High-water mark of the context's workspace pool, bytes (peak VRAM the library itself held). */

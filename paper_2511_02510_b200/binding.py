@@ -19,12 +19,16 @@ _SO = os.path.join(_HERE, "libsvr.so")
 SVR_OK, SVR_ERR_INVALID_ARG, SVR_ERR_CUDA, SVR_ERR_WORKSPACE, SVR_ERR_UNSUPPORTED = range(5)
 _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR_WORKSPACE", 4: "SVR_ERR_UNSUPPORTED"}
 
-EXPORTS = ["svr_create", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
+EXPORTS = ["svr_create", "svr_create_with_allocator", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare", "svr_ssim_loss_grad", "svr_tv_loss_grad",
            "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_measure_peaks", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
            "svr_gather_corners", "svr_scatter_add_corners"]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)     # SvrAllocFn
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)            # SvrFreeFn
 
 
 class SvrError(RuntimeError):
@@ -67,6 +71,7 @@ def _load():
                           "(nvcc, sm_100a). There is no CPU or PyTorch fallback.")
     lib = C.CDLL(_SO)
     lib.svr_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.c_size_t]
+    lib.svr_create_with_allocator.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, ALLOC_FN, FREE_FN, C.c_void_p, C.c_size_t]
     lib.svr_destroy.argtypes = [C.c_void_p]
     lib.svr_destroy.restype = None
     lib.svr_last_error.argtypes = [C.c_void_p]
@@ -233,14 +238,34 @@ class Frame:
 class Context:
     """One library context bound to a device and a stream (default: torch's current stream)."""
 
-    def __init__(self, device: int = 0, stream: Optional[torch.cuda.Stream] = None, workspace_budget_bytes: int = 0):
+    def __init__(self, device: int = 0, stream: Optional[torch.cuda.Stream] = None, workspace_budget_bytes: int = 0,
+                 torch_allocator: bool = False):
+        """torch_allocator: the library's workspace blocks come from PyTorch's caching allocator (svr_create_with_allocator)
+        instead of the context's private CUDA memory pool."""
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2511_02510_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
         torch.cuda.set_device(device)
         self.device = device
         self.stream = stream if stream is not None else torch.cuda.current_stream(device)
         h = C.c_void_p()
-        st = _lib.svr_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream), workspace_budget_bytes)
+        if torch_allocator:
+            cs = self.stream.cuda_stream
+            self.alloc_calls = 0
+
+            def _alloc(nbytes, _user):
+                self.alloc_calls += 1
+                try:
+                    return torch.cuda.caching_allocator_alloc(int(nbytes), device, cs)
+                except RuntimeError:
+                    return None
+
+            def _free(ptr, _user):
+                torch.cuda.caching_allocator_delete(ptr)
+
+            self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)       # keep the thunks alive with the context
+            st = _lib.svr_create_with_allocator(C.byref(h), device, C.c_void_p(cs), self._alloc_cb, self._free_cb, None, workspace_budget_bytes)
+        else:
+            st = _lib.svr_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream), workspace_budget_bytes)
         if st != SVR_OK:
             raise SvrError(st, "svr_create failed")
         self.handle = h

@@ -590,6 +590,7 @@ __global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __rest
             local_ne += (cnt != 0u && cnt <= (uint32_t)SORT_CAP_SMALL);
         }
     }
+    atomicAdd(&totals[0], (unsigned long long)local);     // E in 64 bits (the caller zeroed totals): >= 2^31 is refused on the host
     // block-wide exclusive scans of (local, local_ne, local_big, local_mid)
     uint32_t inc = local, inc2 = local_ne, inc3 = local_big, inc4 = local_mid;
 #pragma unroll
@@ -609,7 +610,7 @@ __global__ void __launch_bounds__(1024) bucket_scan_kernel(const uint8_t* __rest
             if (lane >= o) { a += t; a2 += t2; a3 += t3; a4 += t4; }
         }
         wsum[lane] = a - w; wsum2[lane] = a2 - w2; wsum3[lane] = a3 - w3; wsum4[lane] = a4 - w4;
-        if (lane == 31) { totals[0] = a; totals[3] = a2 + a3 + a4; totals[5] = a3; totals[6] = a3 + a4; n_big_buckets = a3; n_mid_buckets = a4; }
+        if (lane == 31) { totals[3] = a2 + a3 + a4; totals[5] = a3; totals[6] = a3 + a4; n_big_buckets = a3; n_mid_buckets = a4; }
     }
     __syncthreads();
     // work list by size class, largest first: [ > SORT_CAP | > SORT_CAP_SMALL | rest ]
@@ -1040,6 +1041,8 @@ SvrStatus launch_bucket_count(SvrContext* ctx, SvrFrame* f, uint32_t* bcount, in
     }
     {
         StageScope scope__(ctx, ST_SCAN);
+        // more than 48 KB of dynamic shared memory above 12 288 grid points (about 3 Mpixel): opt in (per device, every call)
+        SVR_CUDA(ctx, cudaFuncSetAttribute(bucket_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SVR_SCAN_SMEM_MAX));
         bucket_scan_kernel<<<1, 1024, sizeof(int) * (size_t)(f->cam.tiles_x + 1) * (f->cam.tiles_y + 1), ctx->stream>>>(f->tile_masks, bigdiff, f->cam.tiles_x, f->cam.tiles_y, bcount, f->ranges,
                                                         nonempty, totals);
         ctx->launches += 1;

@@ -403,6 +403,7 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     if (n_cams < 1 || n_cams > MAX_CAMS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_cams must be 1..%d", MAX_CAMS);
     if (opts->n_bins < 1 || opts->n_bins > MAX_BINS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_bins must be 1..%d", MAX_BINS);
     if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    { int ex = 0; if (!(vox->root_edge > 0.f) || std::frexp(vox->root_edge, &ex) != 0.5f) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "root_edge must be a positive power of two"); }
     *n_removed_host = 0;
     const int64_t n = vox->n;
     const int B = opts->n_bins;
@@ -528,6 +529,7 @@ SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrC
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n_cams < 1 || n_cams > MAX_CAMS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_cams must be 1..%d", MAX_CAMS);
     if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    { int ex = 0; if (!(vox->root_edge > 0.f) || std::frexp(vox->root_edge, &ex) != 0.5f) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "root_edge must be a positive power of two"); }
     if (opts->max_splits < 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "max_splits must be >= 0");
     *n_split_host = 0;
     if (z_percentiles_host) z_percentiles_host[0] = z_percentiles_host[1] = 0.0f;

@@ -23,6 +23,18 @@ SvrStatus svr_fail(SvrContext* ctx, SvrStatus st, const char* fmt, ...) {
 // slack, so the per-view buffers, whose sizes follow the entry count E, are reused from view to view even though E
 // changes; the first time a size is seen costs a cudaMallocAsync (milliseconds when the pool has to grow). Everything
 // is ordered on the context's one stream, so reuse needs no extra synchronisation.
+static cudaError_t backing_alloc(SvrContext* ctx, void** p, size_t cap) {
+    if (ctx->alloc_fn) {
+        *p = ctx->alloc_fn(cap, ctx->alloc_user);
+        return *p ? cudaSuccess : cudaErrorMemoryAllocation;
+    }
+    return cudaMallocFromPoolAsync(p, cap, ctx->pool, ctx->stream);
+}
+static void backing_free(SvrContext* ctx, void* p) {
+    if (ctx->free_fn) ctx->free_fn(p, ctx->alloc_user);      // stream-ordered reuse is the caller's allocator's business: it was
+    else cudaFreeAsync(p, ctx->stream);                      // told the stream (svr_create_with_allocator's contract)
+}
+
 SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes) {
     *p = nullptr;
     if (bytes == 0) bytes = 256;
@@ -46,11 +58,11 @@ SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes) {
     } else {
         // make room under the budget by dropping cached blocks first
         while (ctx->budget && ctx->in_use + ctx->cached + cap > ctx->budget && !ctx->free_blocks.empty()) {
-            cudaFreeAsync(ctx->free_blocks.back().first, ctx->stream);
+            backing_free(ctx, ctx->free_blocks.back().first);
             ctx->cached -= ctx->free_blocks.back().second;
             ctx->free_blocks.pop_back();
         }
-        SVR_CUDA(ctx, cudaMallocAsync(p, cap, ctx->stream));
+        SVR_CUDA(ctx, backing_alloc(ctx, p, cap));
     }
     ctx->live[*p] = cap;
     ctx->in_use += cap;
@@ -66,7 +78,7 @@ void svr_free(SvrContext* ctx, void* p, size_t /*bytes*/) {
     ctx->live.erase(it);
     ctx->in_use -= cap;
     if (ctx->free_blocks.size() >= 48) {         // bounded list: drop the oldest cached block
-        cudaFreeAsync(ctx->free_blocks.front().first, ctx->stream);
+        backing_free(ctx, ctx->free_blocks.front().first);
         ctx->cached -= ctx->free_blocks.front().second;
         ctx->free_blocks.erase(ctx->free_blocks.begin());
     }
@@ -144,20 +156,33 @@ SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
 extern "C" {
 
 SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t workspace_budget_bytes) {
-    if (!out) return SVR_ERR_INVALID_ARG;
+    return svr_create_with_allocator(out, device, cuda_stream, nullptr, nullptr, nullptr, workspace_budget_bytes);
+}
+
+SvrStatus svr_create_with_allocator(SvrContext** out, int device, void* cuda_stream, SvrAllocFn alloc_fn, SvrFreeFn free_fn, void* user,
+                                    size_t workspace_budget_bytes) {
+    if (!out || ((alloc_fn == nullptr) != (free_fn == nullptr))) return SVR_ERR_INVALID_ARG;
     *out = nullptr;
     SvrContext* ctx = new (std::nothrow) SvrContext();
     if (!ctx) return SVR_ERR_CUDA;
     ctx->device = device;
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     ctx->budget = workspace_budget_bytes;
+    ctx->alloc_fn = alloc_fn;
+    ctx->free_fn = free_fn;
+    ctx->alloc_user = user;
     cudaError_t e = cudaSetDevice(device);
-    if (e == cudaSuccess) {
-        cudaMemPool_t pool;
-        e = cudaDeviceGetDefaultMemPool(&pool, device);
+    if (e == cudaSuccess && !alloc_fn) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = device;
+        e = cudaMemPoolCreate(&ctx->pool, &props);
         if (e == cudaSuccess) {
-            uint64_t thr = UINT64_MAX;   // keep freed workspace cached in the pool between frames
-            e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+            uint64_t thr = UINT64_MAX;   // keep freed workspace in THIS pool between frames (the device's default pool is untouched)
+            e = cudaMemPoolSetAttribute(ctx->pool, cudaMemPoolAttrReleaseThreshold, &thr);
         }
     }
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->host_pinned), 64);
@@ -184,8 +209,8 @@ void svr_destroy(SvrContext* ctx) {
     cudaSetDevice(ctx->device);
     if (ctx->aux) cudaStreamSynchronize(ctx->aux);
     cudaStreamSynchronize(ctx->stream);
-    for (auto& b : ctx->free_blocks) cudaFreeAsync(b.first, ctx->stream);
-    for (auto& b : ctx->live) cudaFreeAsync(b.first, ctx->stream);
+    for (auto& b : ctx->free_blocks) backing_free(ctx, b.first);
+    for (auto& b : ctx->live) backing_free(ctx, b.first);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     if (ctx->readback_ev) cudaEventDestroy(ctx->readback_ev);
     if (ctx->fork_ev) cudaEventDestroy(ctx->fork_ev);
@@ -198,6 +223,7 @@ void svr_destroy(SvrContext* ctx) {
     cudaStreamSynchronize(ctx->stream);
     for (const StagePending& p : ctx->pending) { cudaEventDestroy(p.e0); cudaEventDestroy(p.e1); }
     for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
+    if (ctx->pool) { cudaStreamSynchronize(ctx->stream); cudaMemPoolDestroy(ctx->pool); }
     delete ctx;
 }
 
@@ -214,6 +240,18 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "image size must be 1..65535");
     if (vox->max_level < 1 || vox->max_level > 16) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "max_level must be 1..16");
     if (vox->n > 0 && (!vox->ijkl || !vox->raw_density || !vox->sh)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null voxel arrays");
+    {
+        int ex = 0;      // R1: cell bounds must be exact in fp32, and the kernels form 1/edge by exponent arithmetic
+        if (!(vox->root_edge > 0.f) || std::frexp(vox->root_edge, &ex) != 0.5f)
+            return svr_fail(ctx, SVR_ERR_INVALID_ARG, "root_edge must be a positive power of two (got %g)", (double)vox->root_edge);
+    }
+    {
+        // the bucket scan keeps a (tiles_x + 1) x (tiles_y + 1) int table in one block's shared memory
+        const size_t pts = (size_t)((cam->W + SVR_TILE - 1) / SVR_TILE + 1) * (size_t)((cam->H + SVR_TILE - 1) / SVR_TILE + 1);
+        if (pts * sizeof(int) > SVR_SCAN_SMEM_MAX)
+            return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "image of %d x %d pixels has %zu tile-grid points (limit %zu: about 14 Mpixel)", cam->W,
+                            cam->H, pts, (size_t)SVR_SCAN_SMEM_MAX / sizeof(int));
+    }
     SVR_CUDA(ctx, cudaSetDevice(ctx->device));
 
     SvrFrame* f = new (std::nothrow) SvrFrame();
@@ -496,6 +534,10 @@ SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCa
         if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "D2H copy: %s", cudaGetErrorString(e));
     }
     if (f) svr_frame_release(ctx, f);
+    if (st != SVR_OK) {                   // the upload and the loss's target phase may still be using buf on the second stream
+        cudaStreamSynchronize(ctx->aux);
+        ctx->loss_prepared = false;
+    }
     svr_free(ctx, buf, bytes);
     return st;
 }

@@ -11,6 +11,7 @@
 
 #define SVR_TILE 16
 #define SVR_MAX_K 4
+#define SVR_SCAN_SMEM_MAX (200 * 1024)   // dynamic shared memory the one-block bucket scan may use for its tile-grid table
 #define SVR_TRAV_WORDS 72     // traversal record: 32 hit masks, 32 voxel ids, slot count, 6 sub-batch E offsets (+ padding to 16 bytes)
 
 enum SvrStage {
@@ -29,6 +30,12 @@ struct SvrContext {
     int64_t stage_calls[ST_COUNT] = {0};
     int device = 0;
     cudaStream_t stream = nullptr;
+    // backing store of the workspace blocks: the caller's allocator (svr_create_with_allocator) or a PRIVATE stream-ordered
+    // memory pool of this context (never the device's default pool, which the host application may share)
+    SvrAllocFn alloc_fn = nullptr;
+    SvrFreeFn free_fn = nullptr;
+    void* alloc_user = nullptr;
+    cudaMemPool_t pool = nullptr;
     size_t budget = 0;            // 0 = unlimited
     size_t in_use = 0, cached = 0, peak = 0;   // bytes in live blocks, in cached free blocks, and the peak of their sum
     std::vector<std::pair<void*, size_t>> free_blocks;   // cached free workspace blocks (pointer, capacity)

@@ -370,6 +370,60 @@ def test_error_behaviour(svr):
     frame.release()
 
 
+def test_two_contexts_and_torch_allocator(orc, svr):
+    """Boundary: (i) two contexts on one device with different budgets own separate private pools and both work;
+    (ii) svr_create_with_allocator: the workspace comes from PyTorch's caching allocator (torch's counters move, the callbacks are
+    called, results identical to the private-pool context)."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    sc, cam = cfg.scene, cfg.cameras[0]
+    vox = pkg.Voxels.from_scene(sc)
+    a = pkg.Context(0, workspace_budget_bytes=256 << 20)
+    b = pkg.Context(0, workspace_budget_bytes=64 << 10)           # too small for this scene
+    fa = a.svr_preprocess(vox, cam)
+    img_a, _, _ = a.svr_forward(fa, cfg.K, cfg.T_min)
+    with pytest.raises(pkg.SvrError) as ei:
+        b.svr_preprocess(vox, cam)
+    assert ei.value.status == 3
+    a.synchronize()
+    before = torch.cuda.memory_allocated()
+    t = pkg.Context(0, torch_allocator=True)
+    ft = t.svr_preprocess(vox, cam)
+    img_t, _, _ = t.svr_forward(ft, cfg.K, cfg.T_min)
+    t.synchronize()
+    assert t.alloc_calls > 0 and torch.cuda.memory_allocated() > before + (1 << 20)
+    np.testing.assert_array_equal(img_a.cpu().numpy(), img_t.cpu().numpy())
+    g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+    g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+    t.svr_backward(ft, cfg.K, torch.ones_like(img_t) / img_t.numel(), img_t, g_raw, g_sh, cfg.T_min)
+    t.synchronize()
+    assert float(g_raw.abs().sum()) > 0
+    fa.release(); ft.release()
+    a.close(); b.close(); t.close()
+    del img_t, ft
+    assert torch.cuda.memory_allocated() <= before + g_raw.numel() * 4 + g_sh.numel() * 4 + img_a.numel() * 4 * 4 + (1 << 20)     # the workspace went back
+
+
+def test_large_image_and_argument_limits(orc, svr):
+    """2560 x 1440: the bucket scan's tile-grid table needs more than 48 KB of shared memory (opt-in); lists stay bit-exact.
+    Beyond the documented limit the call is refused with SVR_ERR_UNSUPPORTED; a root_edge that is not a power of two with
+    SVR_ERR_INVALID_ARG."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    cam = look_at_camera((2.4, 1.1, 0.9), (0, 0, 0), 2560, 1440)
+    assert check_lists(orc, svr, cfg.scene, cam) > 20_000
+    vox = pkg.Voxels.from_scene(cfg.scene)
+    huge = pkg.make_camera(look_at_camera((2.4, 1.1, 0.9), (0, 0, 0), 8000, 8000))
+    with pytest.raises(pkg.SvrError) as ei:
+        ctx.svr_preprocess(vox, huge)
+    assert ei.value.status == 4 and "tile-grid" in str(ei.value)
+    from dataclasses import replace
+    bad = pkg.Voxels.from_scene(replace(cfg.scene, root_edge=1.5))
+    with pytest.raises(pkg.SvrError) as ei:
+        ctx.svr_preprocess(bad, cfg.cameras[0])
+    assert ei.value.status == 1 and "power of two" in str(ei.value)
+
+
 # ---------------------------------------------------------------------------------------------
 # reduced copies of C3..C5 in full (all pixels), full-size C3/C4 on sampled rays
 # ---------------------------------------------------------------------------------------------
