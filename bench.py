@@ -292,15 +292,23 @@ def main():
     torch.cuda.synchronize()
     torch.cuda.reset_peak_memory_stats(dev)
 
-    # ---- timed region: K steps of the whole path, stage timers on (CUDA events on the library's stream) ----
+    # ---- timed region: K steps of the whole path (no stage timers: `value` carries no event-record overhead) ----
     launches0 = ctx.kernel_launches
-    ctx.svr_get_stage_times(reset=True)
-    ctx.svr_set_stage_timing(True)
     ms_total, clocks = timed(step, args.steps, ClockSampler(local_rank))
-    stage = ctx.svr_get_stage_times(reset=True)
-    ctx.svr_set_stage_timing(False)
     launches = ctx.kernel_launches - launches0
     value = aggregate_value(rays, args.steps, world, ms_total)
+    # ---- the same K steps again with stage timers (CUDA events on the library's stream around every stage) ----
+    ctx.svr_get_stage_times(reset=True)
+    ctx.svr_set_stage_timing(True)
+    ms_staged, _ = timed(step, args.steps)
+    stage = ctx.svr_get_stage_times(reset=True)
+    ctx.svr_set_stage_timing(False)
+
+    # ---- one pass over the cameras with w_max cleared first (the first views after a prune / subdivide step pay the
+    # atomicMax of every voxel's first sighting; in steady state most hits only read) ----
+    w_max.zero_()
+    ms_cold, _ = timed(step, len(ccams))
+    ms_cold /= len(ccams)
 
     # ---- render-only FPS (preprocess + forward, w_max off) ----
     for i in range(3):
@@ -345,6 +353,7 @@ def main():
     staged = float(np.mean([s["entries_staged"] for s in stats]))
 
     peaks, peak_src = measured_peaks()
+    micro = ctx.svr_measure_peaks()        # FP32 FFMA / FFMA2 TFLOP/s, L2 red.v4 G/s, warp-instruction issue G/s (outside the timed regions)
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
     fp32_peak = n_sm * FP32_LANES_PER_SM * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12    # TFLOP/s
     stage_ms = {k: v[0] / args.steps for k, v in stage.items() if v[1] > 0}       # per step (a stage may launch twice)
@@ -352,15 +361,24 @@ def main():
     flop = {"forward_composite": FLOP_PER_FWD_HIT, "backward_composite": FLOP_PER_BWD_HIT}
     if dom in flop:
         achieved = hits * flop[dom] / (stage_ms[dom] * 1e-3) / 1e12
-        traffic = None      # DRAM bytes of one launch of this kernel from the committed ncu capture (full-size C4 only)
-        tpath = os.path.join(ROOT, "profiles", "r1q_traffic.csv")
+        # DRAM bytes and L2 reduction sectors of one launch of this kernel: NOT measured by this run, read from the committed ncu
+        # capture of this build (full-size C4 only)
+        traffic, red_sectors, tsrc = None, None, None
+        tpath = os.path.join(ROOT, "profiles", "r2_traffic.csv")
         if os.path.exists(tpath) and args.workload == "C4" and args.n_voxels is None and args.res_scale == 1.0:
             with open(tpath) as fh:
-                rows = dict(line.strip().split(",") for line in fh.readlines()[1:] if "," in line)
-            traffic = float(rows[dom]) if dom in rows else None
+                rows = {ln.split(",")[0]: ln.strip().split(",")[1:] for ln in fh.readlines()[1:] if "," in ln}
+            if dom in rows:
+                traffic, red_sectors, tsrc = float(rows[dom][0]), float(rows[dom][1]), "profiles/r2_traffic.csv (ncu --set full capture of this build, not this run)"
         roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                    "frac": achieved / fp32_peak, "traffic": traffic,
+                    "frac": achieved / fp32_peak, "traffic": traffic, "traffic_source": tsrc,
                     "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x sm_max_mhz, clocks {peak_src}",
+                    "peak_measured": micro["fp32_ffma_tflops"], "peak_measured_ffma2": micro["fp32_ffma2_tflops"],
+                    "frac_of_measured_peak": achieved / micro["fp32_ffma_tflops"],
+                    "issue_peak_measured_gwarp_inst_per_s": micro["issue_gwarp_inst_per_s"],
+                    "l2_red_v4_peak_measured_g_per_s": micro["l2_red_v4_gops"],
+                    "l2_red_sectors_per_launch": red_sectors,
+                    "l2_red_rate_g_per_s": (red_sectors / (stage_ms[dom] * 1e-3) / 1e9) if red_sectors else None,
                     "algorithmic": f"{hits:.4g} ray-voxel hits/view x {flop[dom]:.0f} flop",
                     "kernel_ms": stage_ms[dom], "slab_tests_per_hit": tests / max(hits, 1.0)}
     else:   # an HBM-bound stage dominates (not expected): report bytes moved by the sort
@@ -369,7 +387,7 @@ def main():
         roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": achieved / peaks["hbm_gbs"], "traffic": None, "kernel_ms": stage_ms[dom]}
 
-    line = {"metric": "fwd+bwd Mrays/s", "value": value, "unit": "Mrays/s", "n_gpus": world, "steps": args.steps,
+    line = {"metric": "fwd+bwd Mrays/s", "value": value, "unit": "Mrays/s", "render_fps": render_fps, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, args),
             "clocks": clocks,
@@ -377,9 +395,11 @@ def main():
                     "h2d_bytes_per_step": int(targets_host[0].numel() * 4 + 92), "d2h_bytes_per_step": 4,
                     "note": "svr_train_view_host: camera + target image from pinned host memory, loss read back"},
             "gpu_launches": int(launches),
-            "render_fps": render_fps,
             "roofline": roofline,
             "stage_ms_per_step": stage_ms,
+            "ms_per_step_with_stage_timers": ms_staged / args.steps,
+            "cold_w_max": {"ms_per_step": ms_cold, "what": "one pass over the cameras right after w_max was cleared (every voxel's first sighting "
+                                                           "takes the atomicMax path); `value` is the steady state between two adaptation steps"},
             "work_per_view": {"hits": hits, "slab_tests": tests, "entries_staged": staged,
                               "list_entries": float(np.mean([s["entries"] for s in stats])),
                               "warp_voxel_pairs": float(np.mean([s["warp_voxel_pairs"] for s in stats]))},

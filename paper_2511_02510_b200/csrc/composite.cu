@@ -5,30 +5,33 @@
 // (profiles/r1a_*), because the 8 blocks of a tile see very different numbers of voxels.
 //
 // Both kernels walk the tile's sorted (tile, octant) lists in BATCHES of up to 32 voxels that survive the
-// cull against the warp's pixel block, and split the work on a batch into a part that is parallel over
-// ray-voxel HITS (all 32 lanes busy whatever the shape of the voxels) and a part that is sequential per PIXEL
-// but cheap:
-//   1. cull: 32 entries at a time, lane i reads entry i's pixel rectangle (in list order, so the read is
-//      coalesced) and computes the 32-bit mask M of this warp's pixels it covers. M == 0 => skipped.
+// cull against the warp's pixel block:
+//   1. cull: 32 entries at a time, lane i reads entry i's TIGHT pixel rectangle (the pixels whose centre can see the voxel;
+//      in list order, so the read is coalesced, two chunks ahead in registers) and computes the 32-bit mask M of this
+//      warp's pixels it covers. M == 0 => skipped.
 //   2. stage: surviving lanes copy their voxel's 80-byte view record (voxel_record_dev, svr_internal.cuh),
-//      gathered by the voxel id read beside the rectangle, in list order, into warp-private shared memory.
+//      gathered by the voxel id read beside the rectangle, in list order, into warp-private shared memory (cp.async,
+//      double-buffered).
 //   3. test (pixel-major): the 32x32 bit matrix M[slot][pixel] is transposed with 5 shuffles, so every lane holds the
 //      slots that cover ITS pixel; it pops them and slab-tests them against a slightly dilated box -> hit bitmask.
-//   4. queue (layout): the hit matrix is transposed back (lane k: pixels that hit slot k), a warp scan gives every slot
-//      its offset: the hits of the batch form a slot-major queue of nh entries; entry e is worked on by lane e / C as its
-//      (e % C)-th item, C = ceil(nh / 32), and every per-entry array is indexed by st(e) = (e % C) * 32 + e / C: a lane's
+// Forward (composite_kernel):
+//   4. every lane pops its own hits front to back: precise slab test, K samples, eqs. 2-4, depth, w_max (eq. 5).
+//      With REC it writes the traversal record: per batch the staged voxel ids, every pixel's hit mask, and E = exp(-tau)
+//      of every hit in pixel-major rows (row i = every pixel's i-th hit of the batch).
+// Backward (backward_packed_kernel) replays the record (or culls and tests itself) and splits a batch into a part that is
+// sequential per PIXEL but cheap and a part that is parallel over ray-voxel HITS (all 32 lanes busy whatever the shape of
+// the voxels):
+//   4'. queue layout: the hit matrix is transposed back (lane k: pixels that hit slot k), a warp scan gives every slot its
+//      offset: the hits form a slot-major queue of nh entries; entry e is worked on by lane e / C as its (e % C)-th item,
+//      C = ceil(nh / 32), per-entry arrays are indexed by st(e) = row e % C, column (e / C + e % C) mod 32: a lane's
 //      accesses are conflict-free and its C entries are CONSECUTIVE hits, i.e. mostly hits of one voxel.
-//   5. forward, hit-major (F1): precise slab test + K-sample integration per entry -> E = exp(-tau), t_mid into the queue.
-//      forward, pixel-major (F2): every lane pops its own hits front to back: eqs. 2-4, depth, w_max (eq. 5).
-//      With REC the forward writes the traversal record: per batch the staged voxel ids, every pixel's hit mask and the
-//      E of every queue entry.
-//   5'. backward, pixel-major: with E from the record (or recomputed by the same hit-major sweep), every lane chains its
-//      own hits: T_k, P_k = G . C_k and from them dL/dtau_k = T_k (G . c_k) + P_k - G . C_final and w_k, into the queue.
-//      backward, hit-major: precise slab + K samples per entry with dL/dtau_k already known, so the gradient of the 8
-//      density coefficients and the colour is accumulated IN REGISTERS over the lane's consecutive entries and leaves as
-//      one set of three red.global.add.v4.f32 per (lane, voxel) fragment: no cross-lane reduction at all. (Round 1 reduced
-//      11 values per hit with a segmented shuffle sum and chained the pixel state through shuffles: 45 % of its
-//      instructions, profiles/r1q_*.)
+//   5'. pixel-major chain: with E from the record (or recomputed by a hit-major sweep), every lane chains its own hits:
+//      T_k, P_k = G . C_k and from them dL/dtau_k = T_k (G . c_k) + P_k - G . C_final and w_k, into the queue.
+//   6'. hit-major: precise slab + K samples per entry with dL/dtau_k already known, so the gradient of the 8 density
+//      coefficients and the colour is accumulated IN REGISTERS over the lane's consecutive entries and leaves as one set of
+//      three red.global.add.v4.f32 into the voxel's 64-byte scratch row per (lane, voxel) fragment: no cross-lane reduction.
+//      (Round 1 reduced 11 values per hit with a segmented shuffle sum and chained the pixel state through shuffles: 45 % of
+//      its instructions, profiles/r1q_*. The same split was tried for the forward pass and lost: profiles/r2b_*.)
 //
 // Density: the trilinear raw density is staged as polynomial coefficients (c0, cx, cy, cz, cxy, cxz, cyz,
 // cxyz), pre-multiplied by log2(e), so a sample costs 7 FMA + one EX2 instead of 7 lerps (14 ops) + MUL + EX2.
