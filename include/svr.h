@@ -215,6 +215,9 @@ typedef struct {
     float ema_alpha, m_low, m_high;
     float kappa, w_keep;
     float cap_fraction;
+    int32_t halo;             /* guard ii as a dilation ("keep-halo"): the protected set is the seeds (small footprint or
+                                 high w_max) dilated this many times over the face neighbours of the leaves (cells that touch on
+                                 one axis and overlap with positive area on the other two, any level difference); 0 = seeds only */
 } SvrPruneOpts;
 SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cams_host, int32_t n_cams,
                          const float* w_max, float* ema, uint8_t* state, const SvrPruneOpts* opts, uint8_t* keep,

@@ -16,15 +16,18 @@ Steps (one adaptation step, all voxels of the scene, statistics gathered over th
      "We prune v in V_b when w_max <= tau_b": inside score x_t = [w_max > tau_b].
   4. guard i: m_t = (1 - alpha) m_{t-1} + alpha x_t (float32); s_t = out if m_t < m_low, in if
      m_t > m_high, else s_{t-1}.
-  5. guard ii: protected if h_v < kappa * delta_v ("small relative to the local ray footprint") or
-     w_max >= w_keep ("high w_max").
+  5. guard ii (P:171 'Contour/detail dilation ("keep-halo")'): SEEDS are the voxels with h_v < kappa * delta_v ("small relative
+     to the local ray footprint") or w_max >= w_keep ("high w_max"); protected = the seeds dilated `halo` times over the
+     face-neighbour relation of the leaves (halo = 0: the seeds alone). Two leaves are face neighbours when their cells touch on
+     one axis and overlap with positive area on the other two (any level difference); edge or corner contact does not count.
   6. guard iii: at most R = floor(cap_fraction * N) voxels leave per step: the candidates (state out, not
      protected) with the smallest w_max, ties by lower index.
 Returns the new EMA, the new state, the keep mask, the thresholds and the bins.
 
 Pins (tests/test_oracle_pins.py): the quantile against a sort written out; eq. 11 F_b(tau_b) >= q_b > F_b(tau_b^-);
 the hysteresis on a hand-computed sequence; cap and protection invariants; one bin and no guards = a global quantile
-cut. PARITY UNPINNED (paper silent): the depth proxy, the bin edges, q_b's form, the inside score, kappa / w_keep
+cut; the keep-halo: a row of three cells, a gap of one empty cell, diagonal contact, a coarse cell beside fine ones, and the
+neighbour pairs against the O(n^2) geometric definition on a random octree. PARITY UNPINNED (paper silent): the depth proxy, the bin edges, q_b's form, the inside score, kappa / w_keep
 protection, the cap's choice among candidates.
 """
 from __future__ import annotations
@@ -45,6 +48,7 @@ class PruneOpts:
     kappa: float = 1.0
     w_keep: float = 0.5
     cap_fraction: float = 0.05
+    halo: int = 0            # dilation steps of the keep-halo (guard ii)
 
 
 def voxel_centres_f32(scene) -> np.ndarray:
@@ -105,6 +109,50 @@ def bin_quantiles(w_max: np.ndarray, bins: np.ndarray, opts: PruneOpts):
     return tau, q
 
 
+def face_neighbour_pairs(scene):
+    """All pairs (a, b) of leaves that share part of a face, listed once from the side of the finer (or equal) leaf a: b is the
+    leaf that covers the cell of a's size adjacent to one of a's six faces, i.e. that cell itself or one of its ancestors
+    (leaves are disjoint, so at most one of them is a leaf; a coarser-to-finer contact appears from the finer side)."""
+    ijkl = scene.ijkl.astype(np.int64)
+    n = scene.n
+    key_of = lambda L, x, y, z: (L << 48) | (x << 32) | (y << 16) | z          # level, ix, iy, iz: 16 bits each
+    keys = key_of(ijkl[:, 3], ijkl[:, 0], ijkl[:, 1], ijkl[:, 2])
+    order = np.argsort(keys, kind="stable")
+    skeys = keys[order]
+    A, B = [], []
+    for axis in range(3):
+        for step in (-1, 1):
+            c = ijkl[:, :3].copy()
+            c[:, axis] += step
+            inside = (c[:, axis] >= 0) & (c[:, axis] < (1 << ijkl[:, 3]))      # the adjacent cell lies in the root cube
+            for up in range(0, 17):                                            # the cell itself, its parent, grandparent, ...
+                L = ijkl[:, 3] - up
+                ok = inside & (L >= 0)
+                if not ok.any():
+                    break
+                k = key_of(np.maximum(L, 0), c[:, 0] >> up, c[:, 1] >> up, c[:, 2] >> up)
+                pos = np.searchsorted(skeys, k)
+                hit = ok & (pos < n) & (skeys[np.minimum(pos, n - 1)] == k)
+                a = np.flatnonzero(hit)
+                A.append(a)
+                B.append(order[pos[a]])
+    return np.concatenate(A), np.concatenate(B)
+
+
+def keep_halo(scene, seed: np.ndarray, steps: int) -> np.ndarray:
+    """Guard ii: the seed set dilated `steps` times over the face-neighbour relation."""
+    prot = np.asarray(seed, dtype=bool).copy()
+    if steps <= 0:
+        return prot
+    a, b = face_neighbour_pairs(scene)
+    for _ in range(steps):
+        new = prot.copy()
+        new[b[prot[a]]] = True
+        new[a[prot[b]]] = True
+        prot = new
+    return prot
+
+
 def prune_step(scene, cams, w_max: np.ndarray, ema: np.ndarray, state: np.ndarray, opts: PruneOpts):
     """One adaptation step. ema [n] float32 (m_{t-1}), state [n] uint8 (1 = in, 0 = out). Returns a dict."""
     w_max = np.asarray(w_max, dtype=np.float32)
@@ -116,7 +164,8 @@ def prune_step(scene, cams, w_max: np.ndarray, ema: np.ndarray, state: np.ndarra
     m = (one_minus * ema.astype(np.float32)).astype(np.float32) + (np.float32(opts.ema_alpha) * x).astype(np.float32)
     m = m.astype(np.float32)
     s = np.where(m < np.float32(opts.m_low), 0, np.where(m > np.float32(opts.m_high), 1, state)).astype(np.uint8)
-    protected = (half < (np.float32(opts.kappa) * delta).astype(np.float32)) | (w_max >= np.float32(opts.w_keep))
+    seed = (half < (np.float32(opts.kappa) * delta).astype(np.float32)) | (w_max >= np.float32(opts.w_keep))
+    protected = keep_halo(scene, seed, opts.halo)
     cand = (s == 0) & ~protected
     R = int(np.floor(np.float32(opts.cap_fraction) * np.float32(scene.n)))
     remove = np.zeros(scene.n, dtype=bool)
@@ -125,7 +174,7 @@ def prune_step(scene, cams, w_max: np.ndarray, ema: np.ndarray, state: np.ndarra
         order = np.lexsort((idx, w_max[idx]))                                   # by w_max, ties by lower index
         idx = idx[order[:R]]
     remove[idx] = True
-    return dict(z=z, delta=delta, bins=bins, tau=tau, q=q, ema=m, state=s, protected=protected, candidates=cand,
+    return dict(z=z, delta=delta, bins=bins, tau=tau, q=q, ema=m, state=s, seed=seed, protected=protected, candidates=cand,
                 keep=~remove, n_removed=int(remove.sum()), cap=R)
 
 

@@ -53,7 +53,7 @@ class SvrRenderOpts(C.Structure):
 
 class SvrPruneOpts(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("q_near", C.c_float), ("q_far", C.c_float), ("ema_alpha", C.c_float), ("m_low", C.c_float),
-                ("m_high", C.c_float), ("kappa", C.c_float), ("w_keep", C.c_float), ("cap_fraction", C.c_float)]
+                ("m_high", C.c_float), ("kappa", C.c_float), ("w_keep", C.c_float), ("cap_fraction", C.c_float), ("halo", C.c_int32)]
 
 
 class SvrSubdivOpts(C.Structure):

@@ -189,7 +189,8 @@ __global__ void __launch_bounds__(1024) select_digit_kernel(SelectState* __restr
 __global__ void __launch_bounds__(256) prune_state_kernel(SceneDev s, const float* __restrict__ w_max, const uint8_t* __restrict__ bins,
                                                           const float* __restrict__ delta, const SelectState* __restrict__ st,
                                                           SvrPruneOpts o, float* __restrict__ ema, uint8_t* __restrict__ state,
-                                                          uint8_t* __restrict__ cand, SelectState* __restrict__ st_cap) {
+                                                          uint8_t* __restrict__ cand, SelectState* __restrict__ st_cap,
+                                                          uint8_t* __restrict__ seed) {
     const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool c = false;
     if (v < s.n) {
@@ -206,9 +207,84 @@ __global__ void __launch_bounds__(256) prune_state_kernel(SceneDev s, const floa
         float x[3];
         const float half = voxel_half_and_centre(s, reinterpret_cast<const uint2*>(s.ijkl)[v], x);
         const bool prot = (half < __fmul_rn(o.kappa, delta[v])) || (w >= o.w_keep);
-        c = (sv == 0) && !prot;
-        cand[v] = c ? 1 : 0;
+        if (seed != nullptr) {                 // keep-halo: the seeds are dilated first, prune_cand_kernel decides afterwards
+            seed[v] = prot ? 1 : 0;
+        } else {
+            c = (sv == 0) && !prot;
+            cand[v] = c ? 1 : 0;
+        }
     }
+    const unsigned m = __ballot_sync(FULL, c);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(&st_cap->n_cand, (uint32_t)__popc(m));
+}
+
+// ---- guard ii as a dilation ("keep-halo"): face neighbours through a hash table of the leaves ----
+// key of a cell: level, ix, iy, iz (16 bits each); the table maps the key of every leaf to its index (open addressing, linear
+// probing, capacity a power of two >= 2 n).
+constexpr uint64_t HASH_EMPTY = ~0ull;
+__device__ __forceinline__ uint64_t cell_key(uint32_t L, uint32_t x, uint32_t y, uint32_t z) {
+    return ((uint64_t)L << 48) | ((uint64_t)x << 32) | ((uint64_t)y << 16) | (uint64_t)z;
+}
+__device__ __forceinline__ uint32_t hash_slot(uint64_t k, uint32_t mask) {
+    k ^= k >> 33; k *= 0xff51afd7ed558ccdull; k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ull; k ^= k >> 33;
+    return (uint32_t)k & mask;
+}
+__global__ void __launch_bounds__(256) halo_insert_kernel(SceneDev s, unsigned long long* __restrict__ hkeys, uint32_t* __restrict__ hvals,
+                                                          uint32_t mask) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+    const uint64_t k = cell_key(q.y >> 16, q.x & 0xFFFF, q.x >> 16, q.y & 0xFFFF);
+    uint32_t i = hash_slot(k, mask);
+    while (true) {
+        const unsigned long long old = atomicCAS(&hkeys[i], (unsigned long long)HASH_EMPTY, (unsigned long long)k);
+        if (old == HASH_EMPTY || old == k) { hvals[i] = (uint32_t)v; return; }
+        i = (i + 1) & mask;
+    }
+}
+__device__ __forceinline__ int64_t hash_find(const unsigned long long* __restrict__ hkeys, const uint32_t* __restrict__ hvals, uint32_t mask,
+                                             uint64_t k) {
+    uint32_t i = hash_slot(k, mask);
+    while (true) {
+        const unsigned long long cur = hkeys[i];
+        if (cur == k) return (int64_t)hvals[i];
+        if (cur == HASH_EMPTY) return -1;
+        i = (i + 1) & mask;
+    }
+}
+// One dilation step: out (initialised with a copy of in) |= neighbours of in. Every pair of face neighbours is visited from
+// the side of its finer (or equal) leaf a: b = the leaf covering the cell of a's size beside one of a's faces, i.e. that cell
+// or one of its ancestors (leaves are disjoint: at most one of them is a leaf).
+__global__ void __launch_bounds__(256) halo_dilate_kernel(SceneDev s, const unsigned long long* __restrict__ hkeys,
+                                                          const uint32_t* __restrict__ hvals, uint32_t mask, const uint8_t* __restrict__ in,
+                                                          uint8_t* __restrict__ out) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= s.n) return;
+    const uint2 q = reinterpret_cast<const uint2*>(s.ijkl)[v];
+    const int L = (int)(q.y >> 16);
+    const int c0[3] = {(int)(q.x & 0xFFFF), (int)(q.x >> 16), (int)(q.y & 0xFFFF)};
+    const bool mine = in[v] != 0;
+    bool got = false;
+    for (int face = 0; face < 6; ++face) {
+        int c[3] = {c0[0], c0[1], c0[2]};
+        c[face >> 1] += (face & 1) ? 1 : -1;
+        if (c[face >> 1] < 0 || c[face >> 1] >= (1 << L)) continue;              // outside the root cube
+        for (int up = 0; up <= L; ++up) {
+            const int64_t b = hash_find(hkeys, hvals, mask, cell_key((uint32_t)(L - up), (uint32_t)(c[0] >> up), (uint32_t)(c[1] >> up), (uint32_t)(c[2] >> up)));
+            if (b >= 0) {
+                if (mine) out[b] = 1;
+                got = got || in[b] != 0;
+                break;
+            }
+        }
+    }
+    if (got) out[v] = 1;
+}
+__global__ void __launch_bounds__(256) prune_cand_kernel(int64_t n, const uint8_t* __restrict__ state, const uint8_t* __restrict__ prot,
+                                                         uint8_t* __restrict__ cand, SelectState* __restrict__ st_cap) {
+    const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool c = false;
+    if (v < n) { c = state[v] == 0 && prot[v] == 0; cand[v] = c ? 1 : 0; }
     const unsigned m = __ballot_sync(FULL, c);
     if ((threadIdx.x & 31) == 0 && m) atomicAdd(&st_cap->n_cand, (uint32_t)__popc(m));
 }
@@ -402,6 +478,7 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n_cams < 1 || n_cams > MAX_CAMS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_cams must be 1..%d", MAX_CAMS);
     if (opts->n_bins < 1 || opts->n_bins > MAX_BINS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_bins must be 1..%d", MAX_BINS);
+    if (opts->halo < 0 || opts->halo > 8) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "halo must be 0..8 dilation steps");
     if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
     { int ex = 0; if (!(vox->root_edge > 0.f) || std::frexp(vox->root_edge, &ex) != 0.5f) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "root_edge must be a positive power of two"); }
     *n_removed_host = 0;
@@ -421,12 +498,17 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     uint8_t *bins = nullptr, *cand = nullptr;
     uint32_t *eq = nullptr, *eqp = nullptr, *hist = nullptr;
     SelectState* st = nullptr;      // st[0]: per-bin quantiles, st[1]: the cap
+    unsigned long long* hkeys = nullptr;     // keep-halo (opts->halo > 0): hash table of the leaves, two protection masks
+    uint32_t* hvals = nullptr;
+    uint8_t *prot_a = nullptr, *prot_b = nullptr;
+    size_t hkb = 0, hvb = 0;
     const size_t fb = sizeof(float) * (size_t)n, ub = (size_t)n, eb = sizeof(uint32_t) * (size_t)(n + 1);
     const size_t hb = sizeof(uint32_t) * (size_t)B * HBINS, sb = 2 * sizeof(SelectState) + 64;
     SvrStatus stt = SVR_OK;
     auto cleanup = [&]() {
         svr_free(ctx, z, fb); svr_free(ctx, delta, fb); svr_free(ctx, bins, ub); svr_free(ctx, cand, ub);
         svr_free(ctx, eq, eb); svr_free(ctx, eqp, eb); svr_free(ctx, hist, hb); svr_free(ctx, st, sb);
+        svr_free(ctx, hkeys, hkb); svr_free(ctx, hvals, hvb); svr_free(ctx, prot_a, ub); svr_free(ctx, prot_b, ub);
     };
 #define PTRY(call) do { stt = (call); if (stt != SVR_OK) { cleanup(); return stt; } } while (0)
 #define PCUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cleanup(); return svr_fail(ctx, SVR_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e__)); } } while (0)
@@ -448,7 +530,27 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         select_hist_kernel<<<g, 256, 0, ctx->stream>>>(n, w_max, bins, nullptr, st, shifts[p], (1u << bits[p]) - 1u, his[p], hist);
         select_digit_kernel<<<B, 1024, 0, ctx->stream>>>(st, hist, bits[p], p == 0, B, opts->q_near, opts->q_far, 0u);
     }
-    prune_state_kernel<<<g, 256, 0, ctx->stream>>>(s, w_max, bins, delta, st, *opts, ema, state, cand, st_cap);
+    if (opts->halo <= 0) {
+        prune_state_kernel<<<g, 256, 0, ctx->stream>>>(s, w_max, bins, delta, st, *opts, ema, state, cand, st_cap, nullptr);
+    } else {
+        // guard ii as a dilation: seeds -> `halo` dilation steps over the face neighbours -> candidates
+        uint32_t capn = 1024;
+        while ((int64_t)capn < 2 * n) capn <<= 1;
+        hkb = sizeof(unsigned long long) * (size_t)capn; hvb = sizeof(uint32_t) * (size_t)capn;
+        PTRY(svr_alloc(ctx, (void**)&hkeys, hkb)); PTRY(svr_alloc(ctx, (void**)&hvals, hvb));
+        PTRY(svr_alloc(ctx, (void**)&prot_a, ub)); PTRY(svr_alloc(ctx, (void**)&prot_b, ub));
+        PCUDA(cudaMemsetAsync(hkeys, 0xFF, hkb, ctx->stream));
+        prune_state_kernel<<<g, 256, 0, ctx->stream>>>(s, w_max, bins, delta, st, *opts, ema, state, cand, st_cap, prot_a);
+        halo_insert_kernel<<<g, 256, 0, ctx->stream>>>(s, hkeys, hvals, capn - 1u);
+        for (int it = 0; it < opts->halo; ++it) {
+            PCUDA(cudaMemcpyAsync(prot_b, prot_a, ub, cudaMemcpyDeviceToDevice, ctx->stream));
+            halo_dilate_kernel<<<g, 256, 0, ctx->stream>>>(s, hkeys, hvals, capn - 1u, prot_a, prot_b);
+            uint8_t* t = prot_a; prot_a = prot_b; prot_b = t;
+            ctx->launches += 1;
+        }
+        prune_cand_kernel<<<g, 256, 0, ctx->stream>>>(n, state, prot_a, cand, st_cap);
+        ctx->launches += 2;
+    }
     // guard iii: the cap-th smallest candidate
     for (int p = 0; p < 3; ++p) {
         select_hist_kernel<<<g, 256, 0, ctx->stream>>>(n, w_max, nullptr, cand, st_cap, shifts[p], (1u << bits[p]) - 1u, his[p], hist);

@@ -568,8 +568,8 @@ def _prune_inputs(name, n, seed):
     return cfg, w
 
 
-@pytest.mark.parametrize("name,n", [("C1", 512), ("C2", 50_000), ("C4", 300_000)])
-def test_prune_step_bit_exact_over_steps(orc, svr, name, n):
+@pytest.mark.parametrize("name,n,halo", [("C1", 512, 0), ("C2", 50_000, 0), ("C4", 300_000, 0), ("C1", 512, 1), ("C2", 50_000, 2), ("C4", 300_000, 1)])
+def test_prune_step_bit_exact_over_steps(orc, svr, name, n, halo):
     """Keep mask, state and thresholds identical to the oracle, EMA bit-identical, over several adaptation steps with
     changing w_max (so that the hysteresis takes every branch) and a cap that binds."""
     from oracle.prune import PruneOpts, prune_step
@@ -577,8 +577,9 @@ def test_prune_step_bit_exact_over_steps(orc, svr, name, n):
     cfg, w0 = _prune_inputs(name, n, 11)
     sc = cfg.scene
     vox = pkg.Voxels.from_scene(sc)
-    po = PruneOpts(n_bins=6, q_near=0.45, q_far=0.2, ema_alpha=0.4, m_low=0.35, m_high=0.65, kappa=0.4, w_keep=0.7, cap_fraction=0.03)
-    go = pkg.SvrPruneOpts(po.n_bins, po.q_near, po.q_far, po.ema_alpha, po.m_low, po.m_high, po.kappa, po.w_keep, po.cap_fraction)
+    po = PruneOpts(n_bins=6, q_near=0.45, q_far=0.2, ema_alpha=0.4, m_low=0.35, m_high=0.65, kappa=0.4, w_keep=0.7, cap_fraction=0.03,
+                   halo=halo)        # halo > 0: guard ii as a dilation over the face neighbours ("keep-halo")
+    go = pkg.SvrPruneOpts(po.n_bins, po.q_near, po.q_far, po.ema_alpha, po.m_low, po.m_high, po.kappa, po.w_keep, po.cap_fraction, po.halo)
     ema_ref, st_ref = np.ones(sc.n, np.float32), np.ones(sc.n, np.uint8)
     ema = torch.ones(sc.n, dtype=torch.float32, device="cuda")
     state = torch.ones(sc.n, dtype=torch.uint8, device="cuda")

@@ -618,6 +618,82 @@ def test_prune_guards_and_global_cut():
     assert np.array_equal(~r3["keep"], wp <= wp.min())
 
 
+def _cells_scene(cells):
+    """Scene of the given (ix, iy, iz, level) leaves in [0,1]^3 (parameters irrelevant to the keep-halo)."""
+    ijkl = np.array(cells, dtype=np.uint16)
+    n = ijkl.shape[0]
+    return Scene(np.zeros(3, np.float32), 1.0, 6, 0, ijkl, np.zeros((n, 8), np.float32), np.zeros((n, 1, 3), np.float32))
+
+
+def _touching_brute_force(ijkl, lmax=8):
+    """O(n^2) geometric definition of the face-neighbour relation in integer coordinates at level lmax: the cells touch on one
+    axis and overlap with positive length on the other two."""
+    size = 1 << (lmax - ijkl[:, 3].astype(np.int64))
+    lo = ijkl[:, :3].astype(np.int64) * size[:, None]
+    hi = lo + size[:, None]
+    pairs = set()
+    for a in range(ijkl.shape[0]):
+        for b in range(a + 1, ijkl.shape[0]):
+            for ax in range(3):
+                o1, o2 = (ax + 1) % 3, (ax + 2) % 3
+                touch = hi[a, ax] == lo[b, ax] or hi[b, ax] == lo[a, ax]
+                over = min(hi[a, o1], hi[b, o1]) > max(lo[a, o1], lo[b, o1]) and min(hi[a, o2], hi[b, o2]) > max(lo[a, o2], lo[b, o2])
+                if touch and over:
+                    pairs.add((a, b))
+    return pairs
+
+
+def test_keep_halo_dilation():
+    """Guard ii as a dilation: hand cases, then the neighbour pairs against the geometric definition."""
+    from oracle.prune import face_neighbour_pairs, keep_halo
+    # a row of three level-2 cells: only the middle one is a seed -> all three protected after one step
+    row = _cells_scene([(0, 1, 1, 2), (1, 1, 1, 2), (2, 1, 1, 2)])
+    assert keep_halo(row, [False, True, False], 1).tolist() == [True, True, True]
+    assert keep_halo(row, [True, False, False], 1).tolist() == [True, True, False]      # one step reaches one cell ...
+    assert keep_halo(row, [True, False, False], 2).tolist() == [True, True, True]       # ... two steps reach two
+    assert keep_halo(row, [True, False, False], 0).tolist() == [True, False, False]
+    # no protection across a gap of one empty cell, none across an edge or a corner
+    gap = _cells_scene([(0, 1, 1, 2), (2, 1, 1, 2), (1, 2, 1, 2), (1, 2, 2, 2)])          # cell (1,1,1) is empty
+    assert keep_halo(gap, [True, False, False, False], 1).tolist() == [True, False, False, False]   # (1,2,1) touches (0,1,1) by an edge only
+    # a level-1 cell beside the four level-2 cells on its +x face, and four more one cell further
+    fine = [(2, y, z, 2) for y in (0, 1) for z in (0, 1)] + [(3, y, z, 2) for y in (0, 1) for z in (0, 1)]
+    mixed = _cells_scene([(0, 0, 0, 1)] + fine)
+    assert keep_halo(mixed, [True] + [False] * 8, 1).tolist() == [True] + [True] * 4 + [False] * 4   # coarse seed: the touching four
+    one = [False] * 9
+    one[2] = True                                                                                     # fine seed (2,0,1): the coarse cell,
+    got = keep_halo(mixed, one, 1)                                                                   # its three face neighbours
+    want = [True, True, True, False, True, False, True, False, False]
+    #        coarse (2,0,0) (2,0,1)s (2,1,0) (2,1,1) (3,0,0) (3,0,1) (3,1,0) (3,1,1)
+    assert got.tolist() == want
+    # random octree: the pairs found through ancestor look-ups are exactly the geometric ones
+    cfg = make_config("C2", n_voxels=700)
+    a, b = face_neighbour_pairs(cfg.scene)
+    found = {(min(i, j), max(i, j)) for i, j in zip(a.tolist(), b.tolist())}
+    assert found == _touching_brute_force(cfg.scene.ijkl) and len(found) > 200
+    seed = np.random.default_rng(3).random(cfg.scene.n) < 0.05
+    prot = keep_halo(cfg.scene, seed, 1)
+    nb = np.zeros(cfg.scene.n, dtype=bool)
+    for i, j in found:
+        nb[i] |= seed[j]
+        nb[j] |= seed[i]
+    assert np.array_equal(prot, seed | nb)
+
+
+def test_prune_step_with_halo_protects_neighbours():
+    from oracle.prune import PruneOpts, prune_step
+    cfg, w = _prune_case()
+    n = cfg.scene.n
+    m0, s0 = np.zeros(n, np.float32), np.zeros(n, np.uint8)
+    base = dict(n_bins=4, q_near=0.5, q_far=0.3, ema_alpha=1.0, m_low=0.5, m_high=0.5, kappa=0.0, w_keep=0.8, cap_fraction=1.0)
+    r0 = prune_step(cfg.scene, cfg.cameras, w, m0, s0, PruneOpts(**base, halo=0))
+    r1 = prune_step(cfg.scene, cfg.cameras, w, m0, s0, PruneOpts(**base, halo=1))
+    assert np.array_equal(r0["seed"], r1["seed"]) and np.array_equal(r0["protected"], r0["seed"])
+    assert np.all(r1["protected"][r1["seed"]]) and r1["protected"].sum() > r0["protected"].sum()
+    assert np.all(r1["keep"][r1["protected"]]) and r1["n_removed"] < r0["n_removed"]     # the halo saved some low-w_max neighbours
+    saved = r1["keep"] & ~r0["keep"]
+    assert saved.any() and not np.any(saved & r1["seed"])
+
+
 # ---------------------------------------------------------------------------------------------
 # priority-driven subdivision (PAPER.md Sec. IV-D, P:174-206, eqs. 13-16): pins of oracle/subdivide.py
 # ---------------------------------------------------------------------------------------------
