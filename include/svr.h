@@ -194,6 +194,19 @@ void svr_set_debug_flags(SvrContext* ctx, int flags);
 const char* svr_stage_name(int stage);
 SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset);
 
+/* ---- NEXT-3: rendered normals (Fig. 8 shows normal maps; eq. 17 P:212-230 names the depth-normal
+ * consistency terms that consume them; the paper gives no formula: DESIGN.md reading R16) ----
+ * Per-voxel normal n_v = -g / |g|, g = gradient of the voxel's trilinear raw-density field at the cell centre (0 where g = 0),
+ * world space; rendered normal N(p) = sum_k w_k n_{v_k} with the blending weights of eqs. 2-4, zero background, not
+ * re-normalised (|N| <= 1 - T_K). svr_render_normals writes normal[H,W,3] (and T_final[H,W] if not NULL) for a frame of
+ * svr_preprocess; svr_backward_normals adds d sum(dL_dnormal . N) / d raw to grad_raw_density[n,8] (through the weights and
+ * through n_v). Both reuse the compositing kernels with n_v in the colour slot of the view records (restored before they
+ * return to the stream), so they cost one forward / backward pass each; svr_backward_normals replays the traversal recorded
+ * by svr_forward when there is one. */
+SvrStatus svr_render_normals(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* normal, float* T_final);
+SvrStatus svr_backward_normals(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dnormal,
+                               const float* normal, float* grad_raw_density);
+
 /* ---- NEXT-1: depth-aware quantile pruning, the consumer of w_max (eqs. 11-12) ----
  * One adaptation step over all voxels, statistics gathered over `n_cams` views (reading R11):
  *  1. depth proxy z_v = min over cameras with positive depth of the camera-space depth of the voxel centre

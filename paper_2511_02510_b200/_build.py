@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsvr.so")
-SOURCES = ["svr_api.cu", "preprocess.cu", "sort.cu", "composite.cu", "loss.cu", "prune.cu", "adam.cu", "ssim.cu", "peaks.cu"]
+SOURCES = ["svr_api.cu", "preprocess.cu", "sort.cu", "composite.cu", "loss.cu", "prune.cu", "adam.cu", "ssim.cu", "peaks.cu", "normals.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC"]
 

@@ -21,7 +21,7 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 
 EXPORTS = ["svr_create", "svr_create_with_allocator", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare", "svr_ssim_loss_grad", "svr_tv_loss_grad",
-           "svr_backward", "svr_backward_heads", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
+           "svr_backward", "svr_backward_heads", "svr_render_normals", "svr_backward_normals", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_measure_peaks", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
            "svr_gather_corners", "svr_scatter_add_corners"]
@@ -96,6 +96,8 @@ def _load():
     lib.svr_backward_heads.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 9
     lib.svr_train_view_host.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.POINTER(SvrCamera), C.POINTER(SvrRenderOpts),
                                         C.POINTER(SvrLossOpts), C.c_float] + [C.c_void_p] * 6
+    lib.svr_render_normals.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts), C.c_void_p, C.c_void_p]
+    lib.svr_backward_normals.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 3
     lib.svr_frame_lists.argtypes = [C.c_void_p] + [C.POINTER(C.c_void_p)] * 2 + [C.POINTER(C.c_int64)] + [C.POINTER(C.c_void_p)] * 3
     lib.svr_frame_colors.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
     lib.svr_copy_to_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]
@@ -402,6 +404,20 @@ class Context:
         o = SvrRenderOpts(K, T_min, 1)
         self._check(_lib.svr_backward_heads(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(dL_ddepth), _p(dL_dT), _p(image),
                                             _p(depth), _p(T_final), _p(grad_raw), _p(grad_sh), _p(w_max)))
+
+    # ---- NEXT-3: rendered normals (R16) -------------------------------------------------
+    def svr_render_normals(self, frame: "Frame", K: int, T_min: float = 1e-5):
+        dev = frame.vox.raw.device
+        normal = torch.empty((frame.H, frame.W, 3), dtype=torch.float32, device=dev)
+        Tf = torch.empty((frame.H, frame.W), dtype=torch.float32, device=dev)
+        o = SvrRenderOpts(K, T_min, 0)
+        self._check(_lib.svr_render_normals(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(normal), _p(Tf)))
+        return normal, Tf
+
+    def svr_backward_normals(self, frame: "Frame", K: int, dL_dnormal: torch.Tensor, normal: torch.Tensor, grad_raw: torch.Tensor,
+                             T_min: float = 1e-5):
+        o = SvrRenderOpts(K, T_min, 0)
+        self._check(_lib.svr_backward_normals(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL_dnormal), _p(normal), _p(grad_raw)))
 
     def svr_train_view_host(self, vox: Voxels, cam, K: int, gamma: float, target_host: torch.Tensor, grad_raw, grad_sh,
                             w_max=None, T_min: float = 1e-5, eps: float = 1e-3, percentile: float = 0.99,

@@ -35,6 +35,18 @@ static void backing_free(SvrContext* ctx, void* p) {
     else cudaFreeAsync(p, ctx->stream);                      // told the stream (svr_create_with_allocator's contract)
 }
 
+// the per-voxel gradient scratch rows of the backward passes (all-zero between calls)
+SvrStatus svr_ensure_grad_rows(SvrContext* ctx, int64_t n) {
+    if (ctx->grad_cap >= n) return SVR_OK;
+    if (ctx->grad_row) svr_free(ctx, ctx->grad_row, 0);
+    ctx->grad_row = nullptr;
+    ctx->grad_cap = 0;
+    SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_row, sizeof(float) * 16 * (size_t)n));
+    ctx->grad_cap = n;
+    SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_row, 0, sizeof(float) * 16 * (size_t)n, ctx->stream));
+    return SVR_OK;
+}
+
 SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes) {
     *p = nullptr;
     if (bytes == 0) bytes = 256;
@@ -484,14 +496,7 @@ SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRe
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     const int64_t n = frame->scene.n;
     if (n == 0) return SVR_OK;
-    if (ctx->grad_cap < n) {
-        if (ctx->grad_row) svr_free(ctx, ctx->grad_row, 0);
-        ctx->grad_row = nullptr;
-        ctx->grad_cap = 0;
-        SVR_TRY(svr_alloc(ctx, (void**)&ctx->grad_row, sizeof(float) * 16 * (size_t)n));
-        ctx->grad_cap = n;
-        SVR_CUDA(ctx, cudaMemsetAsync(ctx->grad_row, 0, sizeof(float) * 16 * (size_t)n, ctx->stream));
-    }
+    SVR_TRY(svr_ensure_grad_rows(ctx, n));
     SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_row, w_max != nullptr, dL_ddepth, dL_dT,
                             depth, T_final));
     return launch_sh_backward(ctx, frame, ctx->grad_row, grad_raw_density, grad_sh, w_max);

@@ -173,6 +173,7 @@ struct StageScope {
 // ---- workspace pool --------------------------------------------------------------------------
 SvrStatus svr_alloc(SvrContext* ctx, void** p, size_t bytes);
 void svr_free(SvrContext* ctx, void* p, size_t bytes);
+SvrStatus svr_ensure_grad_rows(SvrContext* ctx, int64_t n);
 
 // ---- stage launchers (each counts its kernel launches into ctx->launches) --------------------
 SvrStatus launch_tile_masks(SvrContext* ctx, SvrFrame* f, bool with_sat);

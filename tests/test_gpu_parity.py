@@ -691,6 +691,37 @@ def test_backward_heads(orc, svr, name, n, scale):
     frame.release()
 
 
+def test_rendered_normals_and_their_gradient(orc, svr):
+    """NEXT-3: N = sum_k w_k n_v (R16) and d sum(G . N) / d raw against oracle/normals.py; the colour render is unchanged by
+    the normal passes (the records' colour slot is restored), with and without a recorded traversal."""
+    from oracle import normals
+    pkg, ctx, torch = svr
+    for cfg, mode in [(make_config("C1"), "pure"), (make_config("C2", n_voxels=20_000, res_scale=0.5, n_cams=1), "bucketed"),
+                      (make_config("C4", n_voxels=100_000, res_scale=0.2, n_cams=1), "bucketed")]:
+        sc, cam = cfg.scene, cfg.cameras[0]
+        vox = pkg.Voxels.from_scene(sc)
+        N_ref, T_ref = normals.render_normals(orc, sc, cam, cfg.K, mode=mode)
+        rng = np.random.default_rng(8)
+        G = rng.normal(0, 1.0 / (cam.W * cam.H), size=(cam.H, cam.W, 3)).astype(np.float32)
+        g_ref = normals.backward_normals(orc, sc, cam, cfg.K, G.astype(np.float64), mode=mode)
+        for record in (True, False):
+            frame = ctx.svr_preprocess(vox, cam)
+            img0, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min, record=record)
+            img0 = img0.clone()
+            N, Tf = ctx.svr_render_normals(frame, cfg.K, cfg.T_min)
+            ctx.synchronize()
+            assert max_rel(N.cpu().numpy(), N_ref) <= IMG_TOL and max_rel(Tf.cpu().numpy(), T_ref) <= IMG_TOL, (cfg.name, record)
+            assert float(np.abs(N_ref).max()) > 0.05
+            g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+            ctx.svr_backward_normals(frame, cfg.K, torch.from_numpy(G).cuda(), N, g_raw, cfg.T_min)
+            ctx.synchronize()
+            assert rel_l2(g_raw.cpu().numpy(), g_ref) <= GRAD_TOL, (cfg.name, record, rel_l2(g_raw.cpu().numpy(), g_ref))
+            img1, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min, record=False)
+            ctx.synchronize()
+            np.testing.assert_array_equal(img0.cpu().numpy(), img1.cpu().numpy())      # the colours are back in the records
+            frame.release()
+
+
 # ---------------------------------------------------------------------------------------------
 # NEXT-4 (part): fused Adam against oracle/adam.py, bit-identical
 # ---------------------------------------------------------------------------------------------

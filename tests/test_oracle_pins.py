@@ -695,6 +695,55 @@ def test_prune_step_with_halo_protects_neighbours():
 
 
 # ---------------------------------------------------------------------------------------------
+# rendered normals (NEXT-3; reading R16): pins of oracle/normals.py
+# ---------------------------------------------------------------------------------------------
+def test_normals_linear_field_and_shared_normal(orc):
+    from oracle import normals
+    sc = tiny_scene(7, n=8, sh_degree=1)
+    # corner raws sampled from a linear field a + b . x: the centre gradient of the trilinear interpolant is b exactly
+    b = np.array([0.7, -1.3, 0.4])
+    e = sc.root_edge / 2.0 ** sc.ijkl[:, 3].astype(np.float64)
+    lo = sc.root_lo.astype(np.float64) + sc.ijkl[:, :3] * e[:, None]
+    corners = np.array([[c & 1, (c >> 1) & 1, (c >> 2) & 1] for c in range(8)], dtype=np.float64)
+    raw = -1.0 + ((lo[:, None, :] + corners[None, :, :] * e[:, None, None]) @ b)
+    np.testing.assert_allclose(normals.voxel_gradients(sc, raw), np.broadcast_to(b, (sc.n, 3)), rtol=1e-12, atol=1e-12)
+    n = normals.voxel_normals(sc, raw)
+    np.testing.assert_allclose(n, np.broadcast_to(-b / np.linalg.norm(b), (sc.n, 3)), rtol=1e-12)
+    assert np.all(normals.voxel_normals(sc, np.full((sc.n, 8), 0.3)) == 0.0)            # constant field: no normal
+    # every voxel has the same normal: N(p) = (sum_k w_k) n = (1 - T_K) n on every ray (eqs. 2-4: sum w + T_K = 1)
+    cam = look_at_camera((2.3, 0.9, 1.4), (0.0, 0.1, 0.0), 24, 18)
+    N, Tf = normals.render_normals(orc, sc, cam, 3, raw=raw)
+    np.testing.assert_allclose(N, (1.0 - Tf)[..., None] * (-b / np.linalg.norm(b)), rtol=0, atol=1e-13)
+    assert (1.0 - Tf).max() > 0.3
+    # general scene: |N| <= 1 - T_K, and N equals the weighted sum over the dumped hits of one ray
+    N2, Tf2 = normals.render_normals(orc, sc, cam, 3)
+    assert np.all(np.linalg.norm(N2, axis=-1) <= 1.0 - Tf2 + 1e-12)
+    nv = normals.voxel_normals(sc)
+    for (x, y) in [(12, 9), (5, 11), (17, 6)]:
+        d = orc.ray_dump(sc, cam, 3, x, y)
+        np.testing.assert_allclose(N2[y, x], (d["w"][:, None] * nv[d["vox"]]).sum(0), rtol=0, atol=1e-13)
+
+
+def test_normals_gradient_matches_finite_differences(orc):
+    from oracle import normals
+    sc = tiny_scene(11, n=8, sh_degree=0)
+    cam = look_at_camera((2.2, -0.8, 1.1), (0.0, 0.0, 0.1), 16, 12)
+    rng = np.random.default_rng(2)
+    G = rng.normal(0, 1, size=(cam.H, cam.W, 3))
+    raw0 = sc.raw.astype(np.float64)
+    g = normals.backward_normals(orc, sc, cam, 2, G, raw=raw0)
+    assert np.abs(g).max() > 1e-3
+    L = lambda r: float((G * normals.render_normals(orc, sc, cam, 2, raw=r)[0]).sum())
+    h = 1e-6
+    for (v, c) in [(0, 0), (1, 5), (3, 2), (4, 7), (6, 1), (7, 3)]:
+        rp, rm = raw0.copy(), raw0.copy()
+        rp[v, c] += h
+        rm[v, c] -= h
+        fd = (L(rp) - L(rm)) / (2 * h)
+        assert abs(fd - g[v, c]) <= 2e-6 * max(1.0, abs(fd)), (v, c, fd, g[v, c])
+
+
+# ---------------------------------------------------------------------------------------------
 # priority-driven subdivision (Sec. IV-D, eqs. 13-16): pins of oracle/subdivide.py
 # ---------------------------------------------------------------------------------------------
 def test_subdivide_eligibility_priority_budget():
