@@ -155,6 +155,7 @@ SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
     const double per_entry = ctx->e_units_per_entry > 0.0 ? 1.25 * ctx->e_units_per_entry : 0.5;
     double units = per_entry * (double)E + 64.0 * (double)f->n_tiles + 1024.0;
     if (units > 1.3e8) units = 1.3e8;      // word offsets into the record are 32-bit (rows * 32 < 2^32)
+    if (ctx->debug_flags & 128) units = 64.0;       // test hook: an E record that is far too small (exercises the overflow flag)
     f->trav_E_cap = (uint32_t)units;
     if (svr_alloc(ctx, (void**)&f->trav_E, sizeof(float) * 32 * ((size_t)f->trav_E_cap + 64)) != SVR_OK) {   // + 64 rows: read-ahead
         f->trav_E = nullptr;            // no room under the budget: the backward pass recomputes E

@@ -854,3 +854,20 @@ def test_backward_with_and_without_traversal_record(orc, svr):
         outs.append(w_max.cpu().numpy())
         frame.release()
     np.testing.assert_array_equal(outs[0], outs[1])              # replayed and recomputed traversals are the same traversal
+    # the two fall-backs of the replaying kernel: recorded E values ignored (flag 32), and an E record that overflowed (flag 128):
+    # the forward pass sets a device flag and the backward pass recomputes exp(-tau) with its hit-major sweep
+    for flag in (32, 128):
+        ctx.svr_set_debug_flags(flag)
+        try:
+            frame = ctx.svr_preprocess(vox, cam)
+            image, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min, record=True)
+            g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+            g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+            w_max = torch.zeros(sc.n, dtype=torch.float32, device="cuda")
+            ctx.svr_backward(frame, cfg.K, torch.from_numpy(G).cuda(), image, g_raw, g_sh, cfg.T_min, w_max=w_max)
+            ctx.synchronize()
+            assert rel_l2(g_raw.cpu().numpy(), r_raw) <= GRAD_TOL and rel_l2(g_sh.cpu().numpy(), r_sh) <= GRAD_TOL, flag
+            np.testing.assert_array_equal(w_max.cpu().numpy(), outs[0])
+            frame.release()
+        finally:
+            ctx.svr_set_debug_flags(0)
