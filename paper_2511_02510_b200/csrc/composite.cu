@@ -55,10 +55,23 @@ constexpr int NSLOT = 32;          // staged voxels per batch
 #endif
 constexpr int QCAP = SVR_QCAP;     // queue entries per warp (a batch is cut into sub-batches whose hits fit)
 constexpr int CMAX = QCAP / 32;
-static_assert(QCAP >= 256 && QCAP <= 512 && QCAP % 32 == 0, "a batch has at most 1024 hits: at most SVR_TRAV_SUB sub-batches");
+static_assert(QCAP >= 64 && QCAP <= 512 && QCAP % 32 == 0, "queue entries per lane C = QCAP / 32 <= 16 (QINV); a slot has at most 32 hits");
 constexpr int RING = 64;           // forward staging slots per warp (two halves of 32)
+#ifndef FWD_CTAW
+#define FWD_CTAW 4      // warps per CTA: the eight warps of a tile are independent (no CTA barrier), so a tile may span several CTAs
+#endif
+#ifndef BWD_CTAW
+#define BWD_CTAW 4      // replay backward; the recomputing fallback keeps whole tiles (measured: 4 is 6 % slower there)
+#endif
+#define BWD_CW(REPLAY) ((REPLAY) ? BWD_CTAW : 8)
+#ifndef BWD_MINB
+#define BWD_MINB(REPLAY) ((REPLAY) ? 5 : BWD_CTAS)     // replay: 5 x 4 warps, 94 registers (6 x 4 at 80 registers measured 3 % slower)
+#endif
 #ifndef FWD_CTAS
 #define FWD_CTAS 4
+#endif
+#ifndef FWD_MINB
+#define FWD_MINB (FWD_CTAS * (8 / FWD_CTAW))
 #endif
 #ifndef SVR_BWD_DB
 #define SVR_BWD_DB 1              // replaying backward: 1 = gather of the next batch double-buffered (3 CTAs/SM), 0 = single buffer,
@@ -67,7 +80,10 @@ constexpr int RING = 64;           // forward staging slots per warp (two halves
 #define BWD_CTAS (SVR_BWD_DB ? 3 : 4)
 #endif
 constexpr int BWD_BUFS = SVR_BWD_DB ? 2 : 1;
-constexpr int EROWS = 8;            // E rows a backward lane fetches into registers at the start of a sub-batch
+#ifndef EROWS_N
+#define EROWS_N 8
+#endif
+constexpr int EROWS = EROWS_N;            // E rows a backward lane fetches into registers at the start of a sub-batch
 constexpr uint32_t ECHUNK = 16;    // the E record is handed out to warps in chunks of (at least) 16 rows of 32 floats
 
 // ceil(65536 / C): (pos * QINV[C]) >> 16 == pos / C for pos < 512, C <= 16
@@ -355,7 +371,7 @@ struct FwdWarp {
 // the staged voxel ids, [64] the slot count, [65] the first E row of the batch in the E record, [71] its number of rows; E
 // row i holds, for every pixel of the block, exp(-tau) of its i-th hit in the batch (1 where it has none or missed).
 template <int K, bool STATS, bool REC, bool WMAX>
-__global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
+__global__ void __launch_bounds__(32 * FWD_CTAW, FWD_MINB) composite_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
                                                         const uint2* __restrict__ rects_sorted,
                                                         const uint32_t* __restrict__ ranges,
                                                         const uint32_t* __restrict__ tile_order,
@@ -366,9 +382,10 @@ __global__ void __launch_bounds__(256, FWD_CTAS) composite_kernel(CamDev c, cons
                                                         const uint32_t* __restrict__ trav_off, uint32_t* __restrict__ trav_count,
                                                         float* __restrict__ trav_E, uint32_t* __restrict__ trav_ectl, uint32_t e_cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    FwdWarp& S = reinterpret_cast<FwdWarp*>(smem_raw)[warp];
-    const int tile = (int)tile_order[blockIdx.x];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = (int)(blockIdx.x % (8 / FWD_CTAW)) * FWD_CTAW + (tid >> 5);      // warp of the tile: 0..7
+    FwdWarp& S = reinterpret_cast<FwdWarp*>(smem_raw)[tid >> 5];
+    const int tile = (int)tile_order[blockIdx.x / (8 / FWD_CTAW)];
     const int tile_x = tile % c.tiles_x, tile_y = tile / c.tiles_x;
     const int wbx0 = tile_x * SVR_TILE + (warp & 1) * 8, wby0 = tile_y * SVR_TILE + (warp >> 1) * 4;
     const int px = wbx0 + (lane & 7), py = wby0 + (lane >> 3);
@@ -534,14 +551,13 @@ struct BwdBase {
     float4 r1[BWD_BUFS * NSLOT];   // log2(e) * (cxy, cxz, cyz, cxyz)
     float4 col[BWD_BUFS * NSLOT];  // r, g, b, cover mask M of this warp's 8x4 block (non-replay) / dilated half edge
     float A[12][32];        // per pixel, 4-byte columns: dh.xyz, dl.xyz, 1/dh.xyz, G.xyz (G = dL/dC)
-    unsigned int wms[NSLOT];// per slot: max blending weight seen by this warp (float bits)
     WarpQ Q;
 };
 template <bool HEADS> struct BwdWarp : BwdBase {};
 template <> struct BwdWarp<true> : BwdBase { float TM[QCAP]; };   // t_mid per queue entry (depth head)
 
 template <int K, bool HEADS, bool REPLAY>
-__global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
+__global__ void __launch_bounds__(32 * BWD_CW(REPLAY), BWD_MINB(REPLAY)) backward_packed_kernel(CamDev c, const float4* __restrict__ packed, const uint32_t* __restrict__ vals,
                                                                const uint2* __restrict__ rects_sorted,
                                                                const uint32_t* __restrict__ ranges,
                                                                const uint32_t* __restrict__ tile_order, float T_min,
@@ -553,9 +569,11 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                                                                const uint32_t* __restrict__ trav_off, const uint32_t* __restrict__ trav_count,
                                                                const float* __restrict__ trav_E, const uint32_t* __restrict__ trav_ectl) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    BwdWarp<HEADS>& S = reinterpret_cast<BwdWarp<HEADS>*>(smem_raw)[warp];
-    const int tile = (int)tile_order[blockIdx.x];
+    const int tid = threadIdx.x, lane = tid & 31;
+    constexpr int CW = BWD_CW(REPLAY);
+    const int warp = (int)(blockIdx.x % (8 / CW)) * CW + (tid >> 5);                  // warp of the tile: 0..7
+    BwdWarp<HEADS>& S = reinterpret_cast<BwdWarp<HEADS>*>(smem_raw)[tid >> 5];
+    const int tile = (int)tile_order[blockIdx.x / (8 / CW)];
     const int tile_x = tile % c.tiles_x, tile_y = tile / c.tiles_x;
     const int wbx0 = tile_x * SVR_TILE + (warp & 1) * 8, wby0 = tile_y * SVR_TILE + (warp >> 1) * 4;
     const int px = wbx0 + (lane & 7), py = wby0 + (lane >> 3);
@@ -586,7 +604,6 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
 #pragma unroll
         for (int a = 0; a < 3; ++a) { inv[a] = ray.inv[a]; S.A[a][lane] = ray.dh[a]; S.A[3 + a][lane] = ray.dl[a]; S.A[6 + a][lane] = ray.inv[a]; }
         S.A[9][lane] = G.x; S.A[10][lane] = G.y; S.A[11][lane] = G.z;
-        S.wms[lane] = 0u;
     }
     __syncwarp();
     // per-pixel chain state, in this pixel's lane: transmittance and P = G . C (+ gD . D) - the per-pixel constant of dL/dtau
@@ -661,6 +678,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                     }
                 }
                 __syncwarp();
+                // the slot headers are not read again in this sub-batch: Hs[k].x now collects slot k's max blending weight
+                if (want_wmax) { S.Q.Hs[lane].x = 0u; __syncwarp(); }
                 // ---- hit-major: gradients of this lane's C consecutive entries, summed in registers per voxel ----
 #ifdef SVR_DBG_SKIP
                 if (SVR_DBG_SKIP < 1)
@@ -679,7 +698,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                             red_add_v4(row, acc[0], acc[1], acc[2], acc[3]);
                             red_add_v4(row + 4, acc[4], acc[5], acc[6], acc[7]);
                             red_add_v4(row + 8, acc[8], acc[9], acc[10], 0.f);
-                            if (want_wmax) atomicMax(&S.wms[k0 + cur], __float_as_uint(wq));
+                            if (want_wmax) atomicMax(&S.Q.Hs[cur].x, __float_as_uint(wq));
                         }
                     };
                     for (int cc = 0; cc < L.C; ++cc) {
@@ -723,9 +742,8 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
                 // eq. 5: one atomicMax per voxel of the sub-batch (its hits all lie in this sub-batch); no guard read: a load
                 // that is waited for here costs more than the reductions it would save
                 if (want_wmax && lane >= k0 && lane < k0 + L.n) {
-                    const unsigned int wv = S.wms[lane];
+                    const unsigned int wv = S.Q.Hs[lane - k0].x;
                     if (wv != 0u) {
-                        S.wms[lane] = 0u;
                         atomicMax(reinterpret_cast<unsigned int*>(grow + (size_t)__float_as_uint(g1[lane].w) * 16 + 12), wv);
                     }
                 }
@@ -884,7 +902,7 @@ __global__ void __launch_bounds__(256, BWD_CTAS) backward_packed_kernel(CamDev c
 SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, float* image, float* depth, float* T_final,
                          float* w_max, unsigned long long* stats, bool record) {
     if (f->n_tiles == 0) return SVR_OK;
-    const size_t smem = sizeof(FwdWarp) * WARPS;
+    const size_t smem = sizeof(FwdWarp) * FWD_CTAW;
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
     unsigned int* wm = reinterpret_cast<unsigned int*>(w_max);
@@ -894,7 +912,7 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
 #define SVR_FWD_GO2(KK, SS, RR, WW)                                                                                  \
     do {                                                                                                             \
         SVR_SET_SMEM(ctx, (composite_kernel<KK, SS, RR, WW>), smem);                                                 \
-        composite_kernel<KK, SS, RR, WW><<<f->n_tiles, 256, smem, ctx->stream>>>(f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, image, depth, \
+        composite_kernel<KK, SS, RR, WW><<<f->n_tiles * (8 / FWD_CTAW), 32 * FWD_CTAW, smem, ctx->stream>>>(f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, image, depth, \
                                                                              T_final, wm, stats, f->trav, f->trav_off, f->trav_count, \
                                                                              f->trav_E, f->trav_ectl, f->trav_E ? f->trav_E_cap : 0u);       \
     } while (0)
@@ -937,9 +955,9 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
     const float* eg = (ctx->debug_flags & 32) ? nullptr : f->trav_E;       // debug flag 32: ignore the recorded E values
 #define SVR_BWD_GO(KK, HH, RR)                                                                                       \
     do {                                                                                                             \
-        const size_t smem = sizeof(BwdWarp<HH>) * WARPS;                                                             \
+        const size_t smem = sizeof(BwdWarp<HH>) * BWD_CW(RR);                                                             \
         SVR_SET_SMEM(ctx, (backward_packed_kernel<KK, HH, RR>), smem);                                               \
-        backward_packed_kernel<KK, HH, RR><<<f->n_tiles, 256, smem, ctx->stream>>>(                                  \
+        backward_packed_kernel<KK, HH, RR><<<f->n_tiles * (8 / BWD_CW(RR)), 32 * BWD_CW(RR), smem, ctx->stream>>>(                             \
             f->cam, pk, f->vals, rs, f->ranges, f->tile_order, T_min, want_wmax, dL, image, grad_row, dL_ddepth, dL_dT, depth, T_final,         \
             f->trav, f->trav_off, f->trav_count, eg, f->trav_ectl);                                                  \
     } while (0)
