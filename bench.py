@@ -172,7 +172,7 @@ def workload_config(cfg, args):
     cam = cfg.cameras[0]
     name = cfg.name + (" (voxels stored in Morton order: NOT the metric's config)" if args.scene_order == "morton" else "")
     return {"workload": f"{name}: {cfg.scene.n} voxels, {cam.W}x{cam.H}, {len(cfg.cameras)} cameras round-robin, K={cfg.K}, "
-                        f"SH degree {cfg.scene.sh_degree}, T_min={cfg.T_min}, gamma={cfg.gamma}, backward emits w_max",
+                        f"SH degree {cfg.scene.sh_degree}, T_min={cfg.T_min}, gamma={cfg.gamma}, backward emits w_max and writes the gradients (grad_overwrite)",
             "seed": cfg.seed, "rays_per_step": cam.W * cam.H,
             "l2": "inputs larger than L2 (scene parameters 928 MB at full size); no explicit flush",
             "parallelism": f"replicas x{args.gpus} (no data-path collective)"}
@@ -253,7 +253,8 @@ def main():
         fr = ctx.svr_preprocess(vox, ccams[k])
         ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, depth=depth, T_final=Tf)
         ctx.svr_loss_grad(image, targets[k], cfg.gamma, dL=dL, loss=loss)
-        ctx.svr_backward(fr, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=w_max if cfg.emit_wmax_in_backward else None)
+        ctx.svr_backward(fr, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=w_max if cfg.emit_wmax_in_backward else None,
+                         overwrite=True)     # one view per step: gradients written, not summed (no zero fill between steps)
         fr.release()
 
     def render_step(i):
@@ -265,7 +266,7 @@ def main():
     def e2e_step(i):
         k = camera_index(i, rank, len(ccams))
         return ctx.svr_train_view_host(vox, ccams[k], cfg.K, cfg.gamma, targets_host[k], g_raw, g_sh,
-                                       w_max=w_max if cfg.emit_wmax_in_backward else None, T_min=cfg.T_min)
+                                       w_max=w_max if cfg.emit_wmax_in_backward else None, T_min=cfg.T_min, overwrite=True)
 
     def barrier():
         if world > 1:

@@ -48,7 +48,7 @@ class SvrCamera(C.Structure):
 
 
 class SvrRenderOpts(C.Structure):
-    _fields_ = [("K", C.c_int32), ("T_min", C.c_float), ("record", C.c_int32)]
+    _fields_ = [("K", C.c_int32), ("T_min", C.c_float), ("record", C.c_int32), ("grad_overwrite", C.c_int32)]
 
 
 class SvrPruneOpts(C.Structure):
@@ -390,18 +390,19 @@ class Context:
         return dL, loss
 
     def svr_backward(self, frame: Frame, K: int, dL: torch.Tensor, image: torch.Tensor, grad_raw: torch.Tensor,
-                     grad_sh: torch.Tensor, T_min: float = 1e-5, w_max: Optional[torch.Tensor] = None):
+                     grad_sh: torch.Tensor, T_min: float = 1e-5, w_max: Optional[torch.Tensor] = None, overwrite: bool = False):
+        """overwrite=False: gradients accumulate (+=); True: grad_raw / grad_sh are written for all voxels (SvrRenderOpts.grad_overwrite)."""
         _dev(dL, torch.float32, "dL")
         _dev(image, torch.float32, "image")
         _dev(grad_raw, torch.float32, "grad_raw")
         _dev(grad_sh, torch.float32, "grad_sh")
-        o = SvrRenderOpts(K, T_min, 1)
+        o = SvrRenderOpts(K, T_min, 1, 1 if overwrite else 0)
         self._check(_lib.svr_backward(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(image), _p(grad_raw),
                                       _p(grad_sh), _p(w_max)))
 
     def svr_backward_heads(self, frame: "Frame", K: int, dL, image, grad_raw, grad_sh, T_min: float = 1e-5, w_max=None,
-                           dL_ddepth=None, dL_dT=None, depth=None, T_final=None):
-        o = SvrRenderOpts(K, T_min, 1)
+                           dL_ddepth=None, dL_dT=None, depth=None, T_final=None, overwrite: bool = False):
+        o = SvrRenderOpts(K, T_min, 1, 1 if overwrite else 0)
         self._check(_lib.svr_backward_heads(self.handle, C.c_void_p(frame.handle), C.byref(o), _p(dL), _p(dL_ddepth), _p(dL_dT), _p(image),
                                             _p(depth), _p(T_final), _p(grad_raw), _p(grad_sh), _p(w_max)))
 
@@ -421,10 +422,10 @@ class Context:
 
     def svr_train_view_host(self, vox: Voxels, cam, K: int, gamma: float, target_host: torch.Tensor, grad_raw, grad_sh,
                             w_max=None, T_min: float = 1e-5, eps: float = 1e-3, percentile: float = 0.99,
-                            sobel_source: int = 0, image_host: Optional[torch.Tensor] = None) -> float:
+                            sobel_source: int = 0, image_host: Optional[torch.Tensor] = None, overwrite: bool = False) -> float:
         c = cam if isinstance(cam, SvrCamera) else make_camera(cam)
         assert not target_host.is_cuda and target_host.dtype == torch.float32 and target_host.is_contiguous()
-        ro, lo = SvrRenderOpts(K, T_min, 1), SvrLossOpts(eps, percentile, sobel_source)
+        ro, lo = SvrRenderOpts(K, T_min, 1, 1 if overwrite else 0), SvrLossOpts(eps, percentile, sobel_source)
         loss = C.c_float()
         self._check(_lib.svr_train_view_host(self.handle, C.byref(vox.c), C.byref(c), C.byref(ro), C.byref(lo), gamma,
                                              _p(target_host), _p(grad_raw), _p(grad_sh), _p(w_max),

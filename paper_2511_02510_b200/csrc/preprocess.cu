@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(256) voxel_color_kernel(SceneDev s, CamDev c, 
 //     coef = A raw (see composite.cu) => grad_raw += A^T grad_coef;
 // (ii) grad_sh[v,i,ch] += Y_i(dir_v) * grad_rgb[v,ch] * [c_v,ch > 0] (zero sub-gradient at the clamp).
 // Consumed scratch entries are re-zeroed, so the scratch buffers stay all-zero between calls.
-template <int DEG>
+template <int DEG, bool OVERWRITE>
 __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev c, const ushort4* __restrict__ rects,
                                                              const float4* __restrict__ rgbm, float4* __restrict__ grow,
                                                              float4* __restrict__ grad_raw, float* __restrict__ grad_sh,
@@ -362,7 +362,7 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
     const int64_t v = v0 + lane;
     bool vis = false;
     if (v < s.n) { ushort4 r = rects[v]; vis = r.x <= r.z; }
-    bool sh_active = false;
+    bool sh_active = false, raw_done = false;
     if (vis) {
         // the voxel's 64-byte scratch row: coefficient gradient (8), colour gradient (3), -, max blending weight, -
         float4 ga = grow[4 * v], gb = grow[4 * v + 1];
@@ -376,7 +376,8 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
             grow[4 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
             grow[4 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
             const float g0 = ga.x, gx = ga.y, gy = ga.z, gz = ga.w, gxy = gb.x, gxz = gb.y, gyz = gb.z, gxyz = gb.w;
-            float4 ra = grad_raw[2 * v], rb = grad_raw[2 * v + 1];
+            float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
+            if (!OVERWRITE) { ra = grad_raw[2 * v]; rb = grad_raw[2 * v + 1]; }
             ra.x += ((g0 - gx) - (gy + gz)) + ((gxy + gxz) + (gyz - gxyz));
             ra.y += (gx - gxy) - (gxz - gxyz);
             ra.z += (gy - gxy) - (gyz - gxyz);
@@ -387,6 +388,7 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
             rb.w += gxyz;
             grad_raw[2 * v] = ra;
             grad_raw[2 * v + 1] = rb;
+            raw_done = true;
         }
         if (g.x != 0.f || g.y != 0.f || g.z != 0.f) {
             grow[4 * v + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -403,10 +405,15 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
             }
         }
     }
+    if (OVERWRITE && v < s.n && !raw_done) {                          // no gradient from this view: zeros, written not summed
+        grad_raw[2 * v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        grad_raw[2 * v + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     const unsigned amask = __ballot_sync(0xffffffffu, sh_active);
-    if (amask == 0u) return;
+    if (!OVERWRITE && amask == 0u) return;
     __syncwarp();
-    // cooperative read-modify-write of the warp's contiguous grad_sh block, skipping untouched voxels
+    // the warp's contiguous grad_sh block, cooperatively: read-modify-write skipping untouched voxels, or (OVERWRITE) plain
+    // stores of every voxel's row
     const int nvox = (int)min((int64_t)32, s.n - v0);
     if constexpr (ROW % 4 == 0) {
         float4* p4 = reinterpret_cast<float4*>(grad_sh + v0 * ROW);
@@ -421,12 +428,16 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
                 const int e = e0 + 32 * u;
                 vvs[u] = e / (ROW / 4);
                 on[u] = e < total && ((amask >> vvs[u]) & 1u);
-                if (on[u]) t[u] = p4[e];
+                t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (!OVERWRITE && on[u]) t[u] = p4[e];
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                if (!on[u]) continue;
                 const int e = e0 + 32 * u, vv = vvs[u];
+                if (!on[u]) {
+                    if (OVERWRITE && e < total) p4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    continue;
+                }
                 const int f0 = (e - vv * (ROW / 4)) * 4;
                 float tv[4] = {t[u].x, t[u].y, t[u].z, t[u].w};
 #pragma unroll
@@ -441,9 +452,12 @@ __global__ void __launch_bounds__(128) voxel_backward_kernel(SceneDev s, CamDev 
         float* p = grad_sh + v0 * ROW;
         for (int e = lane; e < nvox * ROW; e += 32) {
             int vv = e / ROW;
-            if (!((amask >> vv) & 1u)) continue;
+            if (!((amask >> vv) & 1u)) {
+                if (OVERWRITE) p[e] = 0.f;
+                continue;
+            }
             int idx = e - vv * ROW;
-            p[e] = fmaf(Ysm[warp][vv][idx / 3], gsm[warp][vv][idx % 3], p[e]);
+            p[e] = fmaf(Ysm[warp][vv][idx / 3], gsm[warp][vv][idx % 3], OVERWRITE ? 0.f : p[e]);
         }
     }
 }
@@ -1004,7 +1018,8 @@ SvrStatus launch_voxel_colors(SvrContext* ctx, SvrFrame* f) {
     return SVR_OK;
 }
 
-SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row, float* grad_raw, float* grad_sh, float* w_max) {
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row, float* grad_raw, float* grad_sh, float* w_max,
+                             bool overwrite) {
     StageScope scope__(ctx, ST_SH_BACKWARD);
     if (f->scene.n == 0) return SVR_OK;
     unsigned int g = blocks_for(f->scene.n, 128);
@@ -1012,12 +1027,18 @@ SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row
     const float4* rgbm = reinterpret_cast<const float4*>(f->rgbm);
     float4* gc = reinterpret_cast<float4*>(grad_row);
     float4* graw = reinterpret_cast<float4*>(grad_raw);
+#define SVR_VB(DD)                                                                                                           \
+    do {                                                                                                                     \
+        if (overwrite) voxel_backward_kernel<DD, true><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max);  \
+        else voxel_backward_kernel<DD, false><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max);           \
+    } while (0)
     switch (f->scene.sh_degree) {
-        case 0: voxel_backward_kernel<0><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
-        case 1: voxel_backward_kernel<1><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
-        case 2: voxel_backward_kernel<2><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
-        default: voxel_backward_kernel<3><<<g, 128, 0, ctx->stream>>>(f->scene, f->cam, r, rgbm, gc, graw, grad_sh, w_max); break;
+        case 0: SVR_VB(0); break;
+        case 1: SVR_VB(1); break;
+        case 2: SVR_VB(2); break;
+        default: SVR_VB(3); break;
     }
+#undef SVR_VB
     ctx->launches += 1;
     SVR_CUDA(ctx, cudaGetLastError());
     return SVR_OK;

@@ -500,7 +500,7 @@ SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRe
     SVR_TRY(svr_ensure_grad_rows(ctx, n));
     SVR_TRY(launch_backward(ctx, frame, opts->K, opts->T_min, dL_dimage, image, ctx->grad_row, w_max != nullptr, dL_ddepth, dL_dT,
                             depth, T_final));
-    return launch_sh_backward(ctx, frame, ctx->grad_row, grad_raw_density, grad_sh, w_max);
+    return launch_sh_backward(ctx, frame, ctx->grad_row, grad_raw_density, grad_sh, w_max, opts->grad_overwrite != 0);
 }
 
 SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,

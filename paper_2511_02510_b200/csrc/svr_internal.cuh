@@ -200,7 +200,8 @@ SvrStatus launch_forward(SvrContext* ctx, const SvrFrame* f, int K, float T_min,
 SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min, const float* dL, const float* image,
                           float* grad_row, bool want_wmax, const float* dL_ddepth, const float* dL_dT,
                           const float* depth, const float* T_final);
-SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row, float* grad_raw, float* grad_sh, float* w_max);
+SvrStatus launch_sh_backward(SvrContext* ctx, const SvrFrame* f, float* grad_row, float* grad_raw, float* grad_sh, float* w_max,
+                             bool overwrite);
 SvrStatus launch_loss_prepare(SvrContext* ctx, const float* target, int W, int H, float q);
 SvrStatus launch_loss_grad(SvrContext* ctx, const float* render, const float* target, int W, int H, float gamma,
                            float eps, float q, int sobel_source, float* dL, float* loss);

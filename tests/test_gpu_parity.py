@@ -101,6 +101,15 @@ def check_backward(orc, svr, cfg, cam, vox, frame, image, G, mode="bucketed"):
     r_raw, r_sh = orc.backward(sc, cam, cfg.K, dL.cpu().numpy().astype(np.float64), mode=mode)
     e_raw, e_sh = rel_l2(g_raw.cpu().numpy(), r_raw), rel_l2(g_sh.cpu().numpy(), r_sh)
     assert e_raw <= GRAD_TOL and e_sh <= GRAD_TOL, (e_raw, e_sh)
+    # SvrRenderOpts.grad_overwrite: the same gradients WRITTEN over whatever the buffers held (every voxel, zeros included)
+    o_raw, o_sh = torch.full_like(g_raw, 7.0), torch.full_like(g_sh, float("nan"))
+    ctx.svr_backward(frame, cfg.K, dL, image, o_raw, o_sh, cfg.T_min, w_max=None, overwrite=True)
+    ctx.synchronize()
+    assert not torch.isnan(o_sh).any() and torch.equal(o_raw == 0, g_raw == 0) and torch.equal(o_sh == 0, g_sh == 0)
+    o_raw, o_sh = o_raw.cpu().numpy(), o_sh.cpu().numpy()
+    assert rel_l2(o_raw, r_raw) <= GRAD_TOL and rel_l2(o_sh, r_sh) <= GRAD_TOL
+    # (two launches differ by the order of the float reductions only)
+    assert rel_l2(o_raw, g_raw.cpu().numpy()) <= 1e-5 and rel_l2(o_sh, g_sh.cpu().numpy()) <= 1e-5
     return e_raw, e_sh, w_max
 
 
