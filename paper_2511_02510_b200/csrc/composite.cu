@@ -788,19 +788,24 @@ __global__ void __launch_bounds__(32 * BWD_CW(REPLAY), BWD_MINB(REPLAY)) backwar
         unsigned int hits_a, hits_b = 0u;
         uint32_t misc_a, misc_b = 0u;
         if (SVR_BWD_DB) {
+            // three headers deep: header b + 3 into L2, header b + 2 into registers (consumed one batch later, so its round
+            // trip to L2 is not waited for), voxel records of batch b + 1 gathered, batch b worked on
+            Hdr hn;
+            hn.hits = 0u; hn.vid = 0u; hn.misc = 0u;
             {
                 const Hdr h0 = load_hdr(rec);
+                if (n_rec > 1u) hn = load_hdr(rec + TRAV_WORDS);
+                if (n_rec > 2u) prefetch_hdr(rec + 2 * TRAV_WORDS);
                 gather(h0, 0);
                 hits_a = h0.hits; misc_a = h0.misc;
-                if (n_rec > 1u) prefetch_hdr(rec + TRAV_WORDS);
             }
             for (uint32_t rb = 0; rb < n_rec; ++rb) {
                 const int buf = (int)(rb & 1u) * NSLOT;
                 if (rb + 1u < n_rec) {
-                    const Hdr h1 = load_hdr(rec + (size_t)(rb + 1u) * TRAV_WORDS);
-                    if (rb + 2u < n_rec) prefetch_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
-                    gather(h1, buf ^ NSLOT);
-                    hits_b = h1.hits; misc_b = h1.misc;
+                    gather(hn, buf ^ NSLOT);
+                    hits_b = hn.hits; misc_b = hn.misc;
+                    if (rb + 2u < n_rec) hn = load_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
+                    if (rb + 3u < n_rec) prefetch_hdr(rec + (size_t)(rb + 3u) * TRAV_WORDS);
                     asm volatile("cp.async.wait_group 1;" ::: "memory");
                 } else {
                     asm volatile("cp.async.wait_group 0;" ::: "memory");
