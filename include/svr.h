@@ -68,7 +68,10 @@ typedef struct {
     float T_min;              /* a ray stops after the first voxel that leaves T < T_min (R8); 0 = never */
     int32_t record;           /* svr_forward: != 0 records the traversal (per warp and batch: staged list entries, slots
                                  each pixel hit) in the frame; a following svr_backward with the same T_min replays it and
-                                 skips its own cull and test phases (training). 0: render only (about 4% faster).
+                                 skips its own cull and test phases (training). 0: render only (about 9% faster).
+                                 The record's buffers are allocated by the frame's first recording pass (a render-only
+                                 frame never holds them); if the workspace budget has no room for them the pass does not
+                                 record and svr_backward walks the lists itself (same result, slower).
                                  Ignored by svr_backward: without a record it culls and tests itself. */
     int32_t grad_overwrite;   /* svr_backward / svr_backward_heads: 0 = gradients ACCUMULATE (+=) into grad_raw_density and
                                  grad_sh (several views sum into one buffer; the caller zeroes). != 0: both arrays are

@@ -136,20 +136,37 @@ SvrStatus release_frame_buffers(SvrContext* ctx, SvrFrame* f) {
 
 // Traversal scratch (svr_forward records, svr_backward replays): at most E/4 + 80 n_tiles records of SVR_TRAV_WORDS words
 // (sum over tiles of 8 warps x (ceil(len / 32) + 9)), plus the E record: exp(-tau) of every queued ray-voxel hit, in units of
-// 32 floats handed out by a device-side cursor. Its size follows the previous recorded view (units per list entry, read back
-// asynchronously after each recording forward pass) with 25 % slack; when it is too small, or the budget has no room for
-// it, the forward pass sets a flag and the backward pass recomputes E (same result, slower). Debug flag 16 disables the
-// traversal record (backward then culls and tests itself).
-SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
+// 32 floats handed out by a device-side cursor. Its size follows the recorded views so far (largest number of units per list
+// entry, read back asynchronously after each recording forward pass) with 25 % slack; when it is too small, or the budget has
+// no room for it, the forward pass sets a flag and the backward pass recomputes E (same result, slower). Debug flag 16 disables
+// the traversal record (backward then culls and tests itself).
+// The small parts are allocated at preprocess time (the list build fills trav_off):
+SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t /*E*/) {
     if (ctx->debug_flags & 16) return SVR_OK;
-    const size_t cap = (size_t)E / 4 + 80 * (size_t)f->n_tiles + 8;
-    SVR_TRY(svr_alloc(ctx, (void**)&f->trav, sizeof(uint32_t) * SVR_TRAV_WORDS * cap));
     SVR_TRY(svr_alloc(ctx, (void**)&f->trav_off, sizeof(uint32_t) * (size_t)(f->n_tiles + 1)));
     SVR_TRY(svr_alloc(ctx, (void**)&f->trav_count, sizeof(uint32_t) * 8 * (size_t)f->n_tiles));
     SVR_TRY(svr_alloc(ctx, (void**)&f->trav_ectl, 256));
+    return SVR_OK;
+}
+
+// the records and the E rows, by the first recording forward pass of the frame. Returns false (no record: the backward pass then
+// walks the lists itself) when the budget has no room for the records.
+bool alloc_traversal_record(SvrContext* ctx, const SvrFrame* f) {
+    if (f->trav) return true;
+    if ((ctx->debug_flags & 16) || !f->trav_off || f->n_entries <= 0) return false;
+    const int64_t E = f->n_entries;
+    const size_t cap = (size_t)E / 4 + 80 * (size_t)f->n_tiles + 8;
+    if (svr_alloc(ctx, (void**)&f->trav, sizeof(uint32_t) * SVR_TRAV_WORDS * cap) != SVR_OK) {
+        f->trav = nullptr;
+        ctx->err.clear();
+        return false;
+    }
     if (ctx->e_last_entries > 0 && cudaEventQuery(ctx->ectl_ev) == cudaSuccess) {
         const uint32_t used = reinterpret_cast<const uint32_t*>(ctx->host_pinned + 4)[0];
-        ctx->e_units_per_entry = (double)used / (double)ctx->e_last_entries;
+        // the largest ratio seen, not the last one: the sizes of a camera's buffers then repeat from epoch to epoch and the
+        // workspace cache serves them (sizes that follow the previous VIEW made multi-GB blocks miss the cache on C5: 100 ms)
+        const double r = (double)used / (double)ctx->e_last_entries;
+        if (r > ctx->e_units_per_entry) ctx->e_units_per_entry = r;
         ctx->e_last_entries = 0;
     }
     const double per_entry = ctx->e_units_per_entry > 0.0 ? 1.25 * ctx->e_units_per_entry : 0.5;
@@ -160,8 +177,9 @@ SvrStatus alloc_traversal(SvrContext* ctx, SvrFrame* f, int64_t E) {
     if (svr_alloc(ctx, (void**)&f->trav_E, sizeof(float) * 32 * ((size_t)f->trav_E_cap + 64)) != SVR_OK) {   // + 64 rows: read-ahead
         f->trav_E = nullptr;            // no room under the budget: the backward pass recomputes E
         f->trav_E_cap = 0;
+        ctx->err.clear();
     }
-    return SVR_OK;
+    return true;
 }
 
 }  // namespace
@@ -456,7 +474,8 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
                       float* T_final, float* w_max) {
     if (!ctx || !frame || !opts || !image) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
-    const bool record = opts->record != 0 && frame->trav != nullptr;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    const bool record = opts->record != 0 && alloc_traversal_record(ctx, frame);
     SvrStatus st = launch_forward(ctx, frame, opts->K, opts->T_min, image, depth, T_final, w_max, nullptr, record);
     if (st == SVR_OK && record) {
         frame->trav_valid = true;

@@ -129,12 +129,13 @@ struct SvrFrame {
     float* packed = nullptr;         // [n,20] per-voxel view record, visible voxels only (composite.cu voxel_record_kernel)
     uint32_t* tile_order = nullptr;  // [2*n_tiles]: tile ids by descending list length, then the lengths
     // traversal scratch written by svr_forward, replayed by svr_backward (composite.cu)
-    uint32_t* trav = nullptr;        // [trav_cap, SVR_TRAV_WORDS] records
+    // (trav and trav_E are allocated by the first RECORDING forward pass: a render-only frame never holds them)
+    mutable uint32_t* trav = nullptr;        // [trav_cap, SVR_TRAV_WORDS] records
     uint32_t* trav_off = nullptr;    // [n_tiles + 1] first record of each tile
     uint32_t* trav_count = nullptr;  // [n_tiles * 8] records written per warp
-    float* trav_E = nullptr;         // [trav_E_cap * 32] exp(-tau) of every queued hit, handed out to warps in chunks
+    mutable float* trav_E = nullptr;         // [trav_E_cap * 32] exp(-tau) of every queued hit, handed out to warps in chunks
     uint32_t* trav_ectl = nullptr;   // [2] chunk cursor (units of 32 floats), overflow flag
-    uint32_t trav_E_cap = 0;         // capacity of trav_E in units of 32 floats
+    mutable uint32_t trav_E_cap = 0;         // capacity of trav_E in units of 32 floats
     mutable bool trav_valid = false; // a forward pass has recorded this frame's traversal ...
     mutable float trav_T_min = 0.f;  // ... with this termination threshold
     size_t bytes = 0;

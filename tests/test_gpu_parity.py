@@ -880,3 +880,40 @@ def test_backward_with_and_without_traversal_record(orc, svr):
             frame.release()
         finally:
             ctx.svr_set_debug_flags(0)
+
+
+@pytest.mark.gpu
+def test_render_only_frames_hold_no_traversal_record(orc, svr):
+    """The traversal records and the E rows are allocated by the first RECORDING forward pass of a frame: a render-only frame never
+    holds them (workspace peak of a fresh context), a recording pass after a render-only pass on the same frame still records, and a
+    budget with room for the lists but not for the record degrades to the self-walking backward pass instead of failing."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    sc, cam = cfg.scene, cfg.cameras[1]
+    peaks = {}
+    for record in (False, True):
+        c = pkg.Context(0)
+        vox = pkg.Voxels.from_scene(sc)
+        frame = c.svr_preprocess(vox, cam)
+        c.svr_forward(frame, cfg.K, cfg.T_min, record=record)
+        c.synchronize()
+        peaks[record] = c.workspace_peak_bytes
+        frame.release()
+        c.close()
+    assert peaks[False] < peaks[True], peaks
+    G = np.random.default_rng(8).normal(0, 1.0 / (cam.W * cam.H), size=(cam.H, cam.W, 3)).astype(np.float32)
+    r_raw, r_sh = orc.backward(sc, cam, cfg.K, G.astype(np.float64), mode="bucketed")
+    # a budget just above the render-only peak: the record does not fit
+    for budget in (0, peaks[False] + (peaks[True] - peaks[False]) // 8):
+        c = pkg.Context(0, workspace_budget_bytes=budget)
+        vox = pkg.Voxels.from_scene(sc)
+        frame = c.svr_preprocess(vox, cam)
+        c.svr_forward(frame, cfg.K, cfg.T_min, record=False)
+        image, _, _ = c.svr_forward(frame, cfg.K, cfg.T_min, record=True)
+        g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+        g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+        c.svr_backward(frame, cfg.K, torch.from_numpy(G).cuda(), image, g_raw, g_sh, cfg.T_min)
+        c.synchronize()
+        assert rel_l2(g_raw.cpu().numpy(), r_raw) <= GRAD_TOL and rel_l2(g_sh.cpu().numpy(), r_sh) <= GRAD_TOL, budget
+        frame.release()
+        c.close()
