@@ -917,3 +917,28 @@ def test_render_only_frames_hold_no_traversal_record(orc, svr):
         assert rel_l2(g_raw.cpu().numpy(), r_raw) <= GRAD_TOL and rel_l2(g_sh.cpu().numpy(), r_sh) <= GRAD_TOL, budget
         frame.release()
         c.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", list(range(12)))
+def test_fuzz_random_scenes_cameras_and_sizes(orc, svr, seed):
+    """Seeded random cases off the beaten track of C1-C5: tiny mixed-level scenes and reduced C2 scenes, cameras anywhere between
+    inside the root cube and four radii out, ragged image sizes down to less than one tile, narrow to very wide fields of view, every
+    K and SH degree. Lists bit-exact; images, w_max and gradients within the parity tolerances (both gradient modes)."""
+    pkg, ctx, torch = svr
+    rng = np.random.Generator(np.random.PCG64(9000 + seed))
+    cfg = make_config("C1")
+    if seed % 3 == 2:
+        cfg = make_config("C2", n_voxels=int(rng.integers(300, 4000)))
+    else:
+        cfg.scene = tiny_scene(700 + seed, n=int(rng.integers(3, 9)), sh_degree=seed % 4)
+    cfg.K = int(rng.integers(1, 5))
+    d = rng.normal(size=3)
+    pos = d / np.linalg.norm(d) * float(rng.choice([0.15, 0.6, 1.3, 2.5, 4.0]))
+    target = rng.uniform(-0.3, 0.3, size=3)
+    W, H = int(rng.integers(5, 150)), int(rng.integers(5, 110))
+    cam = look_at_camera(tuple(pos), tuple(target), W, H, hfov_deg=float(rng.uniform(25, 110)))
+    check_lists(orc, svr, cfg.scene, cam)
+    vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam)
+    check_backward(orc, svr, cfg, cam, vox, frame, image, random_image_grad(cam, seed))
+    frame.release()
