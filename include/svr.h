@@ -147,6 +147,32 @@ SvrStatus svr_loss_prepare(SvrContext* ctx, const float* target, int32_t W, int3
 SvrStatus svr_ssim_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H,
                              float lambda, int32_t accumulate, float* dL_dimage, float* loss);
 
+/* svr_ssim_loss_grad for callers that cannot allocate device memory. svr_ssim_loss_grad needs a context (a memory pool and two
+ * streams are created with it) and takes 36 bytes of scratch per pixel from that pool. That is not possible everywhere this
+ * library is used: inside a host application whose own allocator already holds the GPU's memory, so that an allocation made
+ * behind its back may fail or push it over its limit; under a fixed per-process memory reservation that has to be known
+ * before the run starts; or in a loop that cannot afford the device-wide stall an allocation or a free can cause. This entry
+ * point takes no context and calls no cudaMalloc / cudaFree / pool or other allocating routine, on any call. Its scratch is
+ * an array inside the library image, sized for SVR_SSIM_STATIC_MAX_PIXELS pixels (256 + 36 * 2^20 bytes = 36 MiB): every GPU
+ * that loads libsvr.so holds it from load until the process exits, whether or not this function is ever called.
+ *  - Same result as svr_ssim_loss_grad (the same kernels): dL_dimage[H,W,3] = lambda * dL_SSIM/d render, or += it when
+ *    accumulate != 0; *loss (device float) = L_SSIM. render / target / dL_dimage / loss are DEVICE pointers of the caller on
+ *    `device`; `cuda_stream` is a cudaStream_t of that device (NULL = the default stream). Asynchronous on that stream.
+ *  - W * H > SVR_SSIM_STATIC_MAX_PIXELS (also returned by svr_ssim_static_max_pixels) is refused with SVR_ERR_UNSUPPORTED
+ *    before anything is launched; null pointers, an empty image or device outside 0..63 give SVR_ERR_INVALID_ARG; CUDA
+ *    failures SVR_ERR_CUDA. svr_static_last_error returns the calling thread's message for the last failed call.
+ *  - The FIRST call on each device does a one-time, synchronous set-up (looks up the device address of the scratch array,
+ *    uploads the 11 window weights, raises one kernel's shared-memory limit); make that call before any stream capture
+ *    begins. Later calls only enqueue a 8-byte memset and two kernels.
+ *  - Every call on a device uses the same array, which keeps the previous call's contents; the function clears the one
+ *    accumulator that must start at zero. Two calls whose kernels can overlap on the GPU (different streams with no
+ *    ordering between them, from one host thread or several) race on the array and both results are garbage: order them. */
+#define SVR_SSIM_STATIC_MAX_PIXELS 1048576
+SvrStatus svr_ssim_loss_grad_static(int device, void* cuda_stream, const float* render, const float* target, int32_t W,
+                                    int32_t H, float lambda, int32_t accumulate, float* dL_dimage, float* loss);
+int64_t svr_ssim_static_max_pixels(void);
+const char* svr_static_last_error(void);
+
 /* (4) backward compositing: gradients of sum(dL_dimage * image) w.r.t. corner raw densities and SH
  * coefficients. `image` is svr_forward's output for this frame (the suffix colour is image - prefix).
  * grad_raw_density[n,8] and grad_sh[n,(D+1)^2,3] ACCUMULATE (+=; caller zeroes) so several views sum

@@ -6,7 +6,7 @@ imported before the library exists; there is no fallback path: a missing library
 missing GPU raises at Context().
 """
 _NAMES = ["Context", "Frame", "Voxels", "SvrCamera", "SvrError", "SvrLossOpts", "SvrPruneOpts", "SvrRenderOpts", "SvrSubdivOpts", "SvrVoxels", "EXPORTS",
-          "make_camera", "svr_gamma_schedule", "lib"]
+          "make_camera", "svr_gamma_schedule", "svr_ssim_loss_grad_static", "svr_ssim_static_max_pixels", "lib"]
 __all__ = list(_NAMES)
 
 

@@ -21,6 +21,7 @@ _STATUS = {0: "SVR_OK", 1: "SVR_ERR_INVALID_ARG", 2: "SVR_ERR_CUDA", 3: "SVR_ERR
 
 EXPORTS = ["svr_create", "svr_create_with_allocator", "svr_destroy", "svr_last_error", "svr_workspace_peak_bytes", "svr_kernel_launches",
            "svr_preprocess", "svr_frame_refresh_colors", "svr_frame_release", "svr_forward", "svr_loss_grad", "svr_loss_prepare", "svr_ssim_loss_grad", "svr_tv_loss_grad",
+           "svr_ssim_loss_grad_static", "svr_ssim_static_max_pixels", "svr_static_last_error",
            "svr_backward", "svr_backward_heads", "svr_render_normals", "svr_backward_normals", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_measure_peaks", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
            "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
@@ -90,6 +91,10 @@ def _load():
                                   C.POINTER(SvrLossOpts), C.c_void_p, C.c_void_p]
     lib.svr_ssim_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_int32,
                                        C.c_void_p, C.c_void_p]
+    lib.svr_ssim_loss_grad_static.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_int32,
+                                              C.c_void_p, C.c_void_p]
+    lib.svr_ssim_static_max_pixels.restype = C.c_int64
+    lib.svr_static_last_error.restype = C.c_char_p
     lib.svr_tv_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_void_p, C.c_void_p]
     lib.svr_loss_prepare.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(SvrLossOpts)]
     lib.svr_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(SvrRenderOpts)] + [C.c_void_p] * 5
@@ -494,3 +499,26 @@ class Context:
 
 def svr_gamma_schedule(t: float, T: float, t0_frac: float = 0.3, t1_frac: float = 0.6, gamma_max: float = 0.6) -> float:
     return float(_lib.svr_gamma_schedule(t, T, t0_frac, t1_frac, gamma_max))
+
+
+def svr_ssim_static_max_pixels() -> int:
+    return int(_lib.svr_ssim_static_max_pixels())
+
+
+def svr_ssim_loss_grad_static(render: torch.Tensor, target: torch.Tensor, dL: torch.Tensor, loss: torch.Tensor, lam: float = 1.0,
+                              accumulate: bool = False, stream: Optional[torch.cuda.Stream] = None):
+    """svr_ssim_loss_grad without a Context and without any allocation, for callers that cannot allocate device memory (see
+    include/svr.h): the scratch is a fixed array inside libsvr.so, good for images of up to svr_ssim_static_max_pixels()
+    pixels. Nothing is allocated here either, so the outputs are the caller's: dL [H,W,3] (written, or added to when
+    `accumulate`) and loss [1], float32 on the inputs' device. Runs on `stream` (default: torch's current stream of that
+    device). All calls on a device share the one scratch array: keep them ordered on the GPU."""
+    for t, name in ((render, "render"), (target, "target"), (dL, "dL"), (loss, "loss")):
+        _dev(t, torch.float32, name)
+    H, W = int(render.shape[0]), int(render.shape[1])
+    dev = render.device.index if render.device.index is not None else torch.cuda.current_device()
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    st = _lib.svr_ssim_loss_grad_static(dev, C.c_void_p(s.cuda_stream), _p(render), _p(target), W, H, lam, 1 if accumulate else 0,
+                                        _p(dL), _p(loss))
+    if st != SVR_OK:
+        raise SvrError(st, _lib.svr_static_last_error().decode())
+    return dL, loss

@@ -12,6 +12,9 @@
 // relative error of 1e-4 in flat regions. Everything else is fp32. HBM-bound, per pixel: the first kernel reads 24 B (R, I)
 // and writes 36 B (three maps), the second reads 36 + 24 B and writes 12 B (+ 12 B read when accumulating): 132 B.
 #include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
 
 #include "svr_internal.cuh"
 
@@ -180,4 +183,99 @@ extern "C" SvrStatus svr_ssim_loss_grad(SvrContext* ctx, const float* render, co
     if (e != cudaSuccess) st = svr_fail(ctx, SVR_ERR_CUDA, "ssim: %s", cudaGetErrorString(e));
     svr_free(ctx, ws, bytes);
     return st;
+}
+
+// ---- svr_ssim_loss_grad_static: the same two kernels, for callers that must not allocate ----
+//
+// svr_ssim_loss_grad above takes its three derivative maps (36 B per pixel) from the context's workspace pool, and getting a
+// context at all means a memory pool and streams have been created. Some users of this library cannot do either at the point
+// where they need L_SSIM: a plug-in running inside a host process whose own allocator has already claimed the device memory
+// (a raw allocation from here can fail although that allocator still has room), code under a hard per-process memory
+// reservation where every byte has to be accounted for before the run starts, and loops that cannot tolerate the device-wide
+// stall an allocation or a free may cause. For them the scratch below is part of the library image: it is reserved on every
+// GPU that loads libsvr.so, from load until the process exits, and this entry point makes no allocation call of any kind.
+//
+// g_ssim_static_scratch is a DEVICE array. In host code its name only stands for the symbol; it is not an address a kernel can
+// use. The host side therefore asks the runtime for the device address once per device (cudaGetSymbolAddress, with that device
+// current) and hands that pointer to the kernels.
+namespace {
+
+constexpr int64_t kStaticMaxPixels = SVR_SSIM_STATIC_MAX_PIXELS;
+constexpr size_t kStaticMapFloats = (size_t)kStaticMaxPixels * 3;
+constexpr size_t kStaticBytes = 256 + 3 * kStaticMapFloats * sizeof(float);   // accumulator block + dm1, dq11, dq12 at the limit
+constexpr int kStaticMaxDevices = 64;
+
+static __device__ __align__(256) unsigned char g_ssim_static_scratch[kStaticBytes];
+
+std::mutex g_static_mu;                                   // guards the per-device set-up table
+unsigned char* g_static_ptr[kStaticMaxDevices] = {};      // device address of the scratch on device d (nullptr: not set up yet)
+thread_local char g_static_err[256] = "";
+
+SvrStatus static_fail(SvrStatus st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_static_err, sizeof(g_static_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define SVR_STATIC_CUDA(call)                                                                                              \
+    do {                                                                                                                   \
+        cudaError_t e__ = (call);                                                                                          \
+        if (e__ != cudaSuccess) return static_fail(SVR_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__));         \
+    } while (0)
+
+// Once per device, with that device current: resolve the scratch symbol to its device address, upload the window, raise the
+// dynamic shared memory limit of the first kernel. Synchronous.
+SvrStatus static_setup(int device, unsigned char** out) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (g_static_ptr[device]) { *out = g_static_ptr[device]; return SVR_OK; }
+    unsigned char* ptr = nullptr;
+    SVR_STATIC_CUDA(cudaGetSymbolAddress((void**)&ptr, g_ssim_static_scratch));
+    if (!ptr) return static_fail(SVR_ERR_CUDA, "cudaGetSymbolAddress returned a null scratch address on device %d", device);
+    double g[11], sum = 0.0;
+    for (int k = 0; k < 11; ++k) { g[k] = exp(-(double)((k - 5) * (k - 5)) / (2.0 * 1.5 * 1.5)); sum += g[k]; }
+    for (int k = 0; k < 11; ++k) g[k] /= sum;
+    SVR_STATIC_CUDA(cudaMemcpyToSymbol(c_g, g, sizeof(g), 0, cudaMemcpyHostToDevice));
+    const int smem_stats = 5 * TH * OUTF * (int)sizeof(double) + 2 * TH * ROWF * (int)sizeof(float);
+    SVR_STATIC_CUDA(cudaFuncSetAttribute(ssim_stats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_stats));
+    g_static_ptr[device] = ptr;
+    *out = ptr;
+    return SVR_OK;
+}
+
+}  // namespace
+
+extern "C" int64_t svr_ssim_static_max_pixels(void) { return kStaticMaxPixels; }
+
+extern "C" const char* svr_static_last_error(void) { return g_static_err; }
+
+extern "C" SvrStatus svr_ssim_loss_grad_static(int device, void* cuda_stream, const float* render, const float* target, int32_t W,
+                                               int32_t H, float lambda, int32_t accumulate, float* dL_dimage, float* loss) {
+    g_static_err[0] = 0;
+    if (!render || !target || !dL_dimage || !loss) return static_fail(SVR_ERR_INVALID_ARG, "null argument");
+    if (W <= 0 || H <= 0) return static_fail(SVR_ERR_INVALID_ARG, "empty image");
+    if (device < 0 || device >= kStaticMaxDevices) return static_fail(SVR_ERR_INVALID_ARG, "device %d outside 0..%d", device, kStaticMaxDevices - 1);
+    const int64_t pixels = (int64_t)W * (int64_t)H;
+    if (pixels > kStaticMaxPixels)
+        return static_fail(SVR_ERR_UNSUPPORTED,
+                           "image %d x %d = %lld pixels is over the %lld-pixel limit of the built-in scratch array; use svr_ssim_loss_grad",
+                           W, H, (long long)pixels, (long long)kStaticMaxPixels);
+    SVR_STATIC_CUDA(cudaSetDevice(device));
+    unsigned char* ws = nullptr;
+    SVR_TRY(static_setup(device, &ws));
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    const size_t nf = (size_t)pixels * 3;
+    SsimAcc* acc = reinterpret_cast<SsimAcc*>(ws);
+    float* dm1 = reinterpret_cast<float*>(ws + 256);
+    float *dq11 = dm1 + nf, *dq12 = dq11 + nf;
+    // the array keeps what the previous call left in it: the index sum has to start at zero, the maps are fully rewritten
+    // over the W x H pixels the second kernel reads (its halo reads outside the image are zero by construction)
+    SVR_STATIC_CUDA(cudaMemsetAsync(acc, 0, sizeof(SsimAcc), stream));
+    const int smem_stats = 5 * TH * OUTF * (int)sizeof(double) + 2 * TH * ROWF * (int)sizeof(float);
+    const dim3 grid((unsigned int)((W + TS - 1) / TS), (unsigned int)((H + TS - 1) / TS));
+    ssim_stats_kernel<<<grid, 256, smem_stats, stream>>>(render, target, W, H, dm1, dq11, dq12, acc);
+    ssim_grad_kernel<<<grid, 256, 0, stream>>>(render, target, W, H, dm1, dq11, dq12, acc, lambda, accumulate, dL_dimage, loss);
+    SVR_STATIC_CUDA(cudaGetLastError());
+    return SVR_OK;
 }
