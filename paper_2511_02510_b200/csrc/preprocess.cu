@@ -50,9 +50,16 @@ __device__ __forceinline__ uint32_t sat_query(const uint32_t* __restrict__ sat, 
 }
 
 // ---- B1: pixel rectangle of a voxel ---------------------------------------------------------------
-// *tight (optional) = the pixels whose CENTRE lies in the projected bounding box grown by 1/64 px: only their rays can hit the
-// voxel (the projection of a box in front of the camera is inside the bounding box of its projected corners; 1/64 px is far
-// above the fp32 error of the projection, ~3e-4 px). The compositing cull uses it; the lists are built from the B1 rectangle.
+// *tight (optional) = the pixels whose CENTRE lies in the projected bounding box grown by a margin m: only their rays can hit
+// the voxel (the projection of a box in front of the camera is inside the bounding box of its projected corners).
+// m = max(1/64 px, bound on the fp32 error of the projected corner), per axis. The bound follows the rounding of the chain
+// above: each camera-space coordinate is 3 products and 3 sums of magnitude <= Mg = |P|_1 + |t|_inf (|R_ij| <= 1), plus the
+// rounding of lo / hi themselves, so |dX|, |dY|, |dZ| <= d = 2^-21 Mg; the quotient, the scaling and the offset add
+// 2^-21 (|u| + |cx|); together |du| <= 1.01 (fx + |u - cx|) d / zmin + 2^-21 (|u| + |cx|). Typical views (C4: fx ~ 1000,
+// z ~ 2.5, Mg ~ 6) give ~1e-3 px, so the margin stays 1/64 px; it grows for voxels within a few z_near of a camera
+// inside the scene and for large fx (4K images: up to a few 0.1 px), where a fixed 1/64 px would drop true hits. The result
+// is clamped to the B1 rectangle, whose own margin is at least 0.5 px. The compositing cull uses it; the lists are built from
+// the B1 rectangle.
 __device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c, uint2 q, ushort4* tight = nullptr) {
     const ushort4 culled = make_ushort4(0xFFFF, 0xFFFF, 0, 0);
     if (tight) *tight = culled;
@@ -107,9 +114,14 @@ __device__ __forceinline__ ushort4 voxel_rect(const SceneDev& s, const CamDev& c
     r.y = (unsigned short)(int)floorf(fmaxf(v0, 0.0f));
     r.w = (unsigned short)(int)floorf(fminf(v1, __fsub_rn(Hf, 1.0f)));
     if (tight) {
-        const float g = 0.5f + 1.0f / 64.0f, h = 0.5f - 1.0f / 64.0f;
-        const int x0 = max((int)ceilf(u0 - g), (int)r.x), x1 = min((int)floorf(u1 - h), (int)r.z);
-        const int y0 = max((int)ceilf(v0 - g), (int)r.y), y1 = min((int)floorf(v1 - h), (int)r.w);
+        const float Mg = fmaxf(fabsf(lo[0]), fabsf(hi[0])) + fmaxf(fabsf(lo[1]), fabsf(hi[1])) + fmaxf(fabsf(lo[2]), fabsf(hi[2])) +
+                         fmaxf(fmaxf(fabsf(c.t[0]), fabsf(c.t[1])), fabsf(c.t[2]));
+        const float p21 = 4.76837158e-7f;                                   // 2^-21
+        const float dz = 1.01f * p21 * Mg / zmin;                           // zmin >= z_near > 0 here
+        const float mu = fmaxf(1.0f / 64.0f, (c.fx + fmaxf(fabsf(u0 - c.cx), fabsf(u1 - c.cx))) * dz + p21 * (fmaxf(fabsf(u0), fabsf(u1)) + fabsf(c.cx)));
+        const float mv = fmaxf(1.0f / 64.0f, (c.fy + fmaxf(fabsf(v0 - c.cy), fabsf(v1 - c.cy))) * dz + p21 * (fmaxf(fabsf(v0), fabsf(v1)) + fabsf(c.cy)));
+        const int x0 = max((int)ceilf(u0 - (0.5f + mu)), (int)r.x), x1 = min((int)floorf(u1 - (0.5f - mu)), (int)r.z);
+        const int y0 = max((int)ceilf(v0 - (0.5f + mv)), (int)r.y), y1 = min((int)floorf(v1 - (0.5f - mv)), (int)r.w);
         if (x0 <= x1 && y0 <= y1) *tight = make_ushort4((unsigned short)x0, (unsigned short)y0, (unsigned short)x1, (unsigned short)y1);
     }
     return r;

@@ -942,3 +942,26 @@ def test_fuzz_random_scenes_cameras_and_sizes(orc, svr, seed):
     vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam)
     check_backward(orc, svr, cfg, cam, vox, frame, image, random_image_grad(cam, seed))
     frame.release()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", [0, 1, 2])
+def test_4k_wide_image_camera_inside_scene(orc, svr, case):
+    """The compositing cull tests pixel centres against the fp32-projected bounding box grown by a margin (preprocess.cu,
+    voxel_rect). The fp32 projection error grows with fx / z, so the cases that can lose true hits are wide images (large fx)
+    seen from inside the scene, with small voxels a few z_near from the camera: 4K-wide strips, camera on the C2 shell.
+    Lists bit-exact; image, depth, T, w_max and gradients within the parity tolerances."""
+    pkg, ctx, torch = svr
+    rng = np.random.Generator(np.random.PCG64(4096 + case))
+    cfg = make_config("C2", n_voxels=20_000)
+    d = rng.normal(size=3)
+    pos = d / np.linalg.norm(d) * float([0.6, 0.55, 0.3][case])            # on / just inside the shell of radius 0.6
+    target = pos + rng.normal(size=3)
+    W, H = [(4096, 24), (3840, 37), (4000, 18)][case]
+    cam = look_at_camera(tuple(pos), tuple(target), W, H, hfov_deg=[50.0, 35.0, 90.0][case])
+    check_lists(orc, svr, cfg.scene, cam)
+    vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam)
+    # a one-signed dL/dimage: with the camera inside a voxel, ~1e5 pixels sum into one gradient row, and a random-sign G makes
+    # that sum cancel to where two launches' float reduction orders differ by more than check_backward's 1e-5 side check
+    check_backward(orc, svr, cfg, cam, vox, frame, image, np.abs(random_image_grad(cam, 40 + case)) / (W * H))
+    frame.release()
