@@ -67,8 +67,10 @@ typedef struct {
     int32_t K;                /* 1..4 midpoint samples per ray segment (R5) */
     float T_min;              /* a ray stops after the first voxel that leaves T < T_min (R8); 0 = never */
     int32_t record;           /* svr_forward: != 0 records the traversal (per warp and batch: staged list entries, slots
-                                 each pixel hit) in the frame; a following svr_backward with the same T_min replays it and
-                                 skips its own cull and test phases (training). 0: render only (about 9% faster).
+                                 each pixel hit, exp(-tau) per hit) in the frame; a following svr_backward /
+                                 svr_backward_heads / svr_backward_normals with the SAME K and T_min replays it and skips its
+                                 own cull and test phases (training); with another K or T_min it ignores the record and
+                                 walks the lists itself. 0: render only (about 9% faster).
                                  The record's buffers are allocated by the frame's first recording pass (a render-only
                                  frame never holds them); if the workspace budget has no room for them the pass does not
                                  record and svr_backward walks the lists itself (same result, slower).

@@ -954,8 +954,9 @@ SvrStatus launch_backward(SvrContext* ctx, const SvrFrame* f, int K, float T_min
     StageScope scope__(ctx, ST_BACKWARD);
     const uint2* rs = reinterpret_cast<const uint2*>(f->rects_sorted);
     const float4* pk = reinterpret_cast<const float4*>(f->packed);
-    // replay the forward pass's traversal record when there is one for this termination threshold
-    const bool replay = f->trav != nullptr && f->trav_valid && f->trav_T_min == T_min && (ctx->debug_flags & 16) == 0;
+    // replay the forward pass's traversal record when there is one for this termination threshold and sample count (the
+    // recorded E = exp(-tau) values, and through them the slot where a ray stopped, belong to the K they were integrated with)
+    const bool replay = f->trav != nullptr && f->trav_valid && f->trav_T_min == T_min && f->trav_K == K && (ctx->debug_flags & 16) == 0;
     const bool heads = dL_ddepth != nullptr || dL_dT != nullptr;
     const float* eg = (ctx->debug_flags & 32) ? nullptr : f->trav_E;       // debug flag 32: ignore the recorded E values
 #define SVR_BWD_GO(KK, HH, RR)                                                                                       \

@@ -159,6 +159,8 @@ bool alloc_traversal_record(SvrContext* ctx, const SvrFrame* f) {
     if (svr_alloc(ctx, (void**)&f->trav, sizeof(uint32_t) * SVR_TRAV_WORDS * cap) != SVR_OK) {
         f->trav = nullptr;
         ctx->err.clear();
+        (void)cudaGetLastError();       // a real out-of-memory leaves the runtime's last error set: the launch check after the
+                                        // forward kernel would report it although rendering without a record is fine
         return false;
     }
     if (ctx->e_last_entries > 0 && cudaEventQuery(ctx->ectl_ev) == cudaSuccess) {
@@ -178,6 +180,7 @@ bool alloc_traversal_record(SvrContext* ctx, const SvrFrame* f) {
         f->trav_E = nullptr;            // no room under the budget: the backward pass recomputes E
         f->trav_E_cap = 0;
         ctx->err.clear();
+        (void)cudaGetLastError();       // as above
     }
     return true;
 }
@@ -480,6 +483,7 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
     if (st == SVR_OK && record) {
         frame->trav_valid = true;
         frame->trav_T_min = opts->T_min;
+        frame->trav_K = opts->K;
         if (frame->trav_ectl && frame->n_entries > 0) {
             // how much of the E record this view used: sizes the next frame's (alloc_traversal); never waited for
             SVR_CUDA(ctx, cudaMemcpyAsync(ctx->host_pinned + 4, frame->trav_ectl, 8, cudaMemcpyDeviceToHost, ctx->stream));

@@ -138,6 +138,7 @@ struct SvrFrame {
     mutable uint32_t trav_E_cap = 0;         // capacity of trav_E in units of 32 floats
     mutable bool trav_valid = false; // a forward pass has recorded this frame's traversal ...
     mutable float trav_T_min = 0.f;  // ... with this termination threshold
+    mutable int trav_K = 0;          // ... and this sample count (the recorded E = exp(-tau) and the termination point depend on it)
     size_t bytes = 0;
 };
 

@@ -882,6 +882,27 @@ def test_backward_with_and_without_traversal_record(orc, svr):
             ctx.svr_set_debug_flags(0)
 
 
+def test_backward_ignores_a_record_made_with_another_K(orc, svr):
+    """The traversal record holds exp(-tau) per hit, which depends on the sample count K: after forward(K=2, record) and a
+    render-only forward(K=3), svr_backward(K=3) must not chain T and w from the K=2 values. It has to fall back to walking
+    the lists itself and give the oracle's K=3 gradients."""
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000)
+    sc, cam = cfg.scene, cfg.cameras[1]
+    vox = pkg.Voxels.from_scene(sc)
+    G = np.random.default_rng(16).normal(0, 1.0 / (cam.W * cam.H), size=(cam.H, cam.W, 3)).astype(np.float32)
+    r_raw, r_sh = orc.backward(sc, cam, 3, G.astype(np.float64), mode="bucketed")
+    frame = ctx.svr_preprocess(vox, cam)
+    ctx.svr_forward(frame, 2, cfg.T_min, record=True)
+    image, _, _ = ctx.svr_forward(frame, 3, cfg.T_min, record=False)
+    g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+    g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+    ctx.svr_backward(frame, 3, torch.from_numpy(G).cuda(), image, g_raw, g_sh, cfg.T_min)
+    ctx.synchronize()
+    assert rel_l2(g_raw.cpu().numpy(), r_raw) <= GRAD_TOL and rel_l2(g_sh.cpu().numpy(), r_sh) <= GRAD_TOL
+    frame.release()
+
+
 @pytest.mark.gpu
 def test_render_only_frames_hold_no_traversal_record(orc, svr):
     """The traversal records and the E rows are allocated by the first RECORDING forward pass of a frame: a render-only frame never
