@@ -81,11 +81,19 @@ extern "C" SvrStatus svr_measure_peaks(SvrContext* ctx, float* out_host) {
     const int n_sm = prop.multiProcessorCount;
     const int blocks = n_sm * 8;                       // 2048 threads per SM: full occupancy
     const unsigned int rows = 1u << 20;                // 32 MB table: resident in the 126 MB L2
+    SVR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));          // time on an idle stream: earlier work must not sit inside the first interval
     float* table = nullptr;
     SVR_TRY(svr_alloc(ctx, (void**)&table, sizeof(float) * 8 * (size_t)rows + 256));
     float* sink = table + (size_t)rows * 8;
-    cudaEvent_t e[2];
-    for (auto& ev : e) SVR_CUDA(ctx, cudaEventCreate(&ev));
+    cudaEvent_t e[2] = {nullptr, nullptr};
+    // every exit below goes through this: the events are destroyed and the table goes back to the workspace
+    auto done = [&](cudaError_t err, const char* what) -> SvrStatus {
+        for (auto& ev : e) if (ev) cudaEventDestroy(ev);
+        svr_free(ctx, table, 0);
+        return err == cudaSuccess ? SVR_OK : svr_fail(ctx, SVR_ERR_CUDA, "svr_measure_peaks: %s: %s", what, cudaGetErrorString(err));
+    };
+    for (auto& ev : e) { const cudaError_t err = cudaEventCreate(&ev); if (err != cudaSuccess) return done(err, "cudaEventCreate"); }
+#define PEAK_CUDA(call, what) do { const cudaError_t err__ = (call); if (err__ != cudaSuccess) return done(err__, what); } while (0)
     auto timed = [&](auto launch, float* ms_best) -> cudaError_t {
         *ms_best = 1e30f;
         for (int rep = 0; rep < 4; ++rep) {            // first repetition warms up
@@ -101,19 +109,18 @@ extern "C" SvrStatus svr_measure_peaks(SvrContext* ctx, float* out_host) {
         return cudaGetLastError();
     };
     float ms = 0.f;
-    SVR_CUDA(ctx, cudaMemsetAsync(table, 0, sizeof(float) * 8 * (size_t)rows + 256, ctx->stream));
-    SVR_CUDA(ctx, timed([&] { ffma_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(sink, 0.999f, 0.001f); }, &ms));
+    PEAK_CUDA(cudaMemsetAsync(table, 0, sizeof(float) * 8 * (size_t)rows + 256, ctx->stream), "clearing the table");
+    PEAK_CUDA(timed([&] { ffma_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(sink, 0.999f, 0.001f); }, &ms), "ffma_peak_kernel");
     const double fma_per_launch = (double)blocks * 256.0 * PEAK_ITERS * 8.0;
     out_host[0] = (float)(2.0 * fma_per_launch / (ms * 1e-3) / 1e12);
-    SVR_CUDA(ctx, timed([&] { ffma2_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(sink, 0.999f, 0.001f); }, &ms));
+    PEAK_CUDA(timed([&] { ffma2_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(sink, 0.999f, 0.001f); }, &ms), "ffma2_peak_kernel");
     out_host[1] = (float)(4.0 * fma_per_launch / (ms * 1e-3) / 1e12);
     const int reps = 256;
-    SVR_CUDA(ctx, timed([&] { red_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(table, rows, reps); }, &ms));
+    PEAK_CUDA(timed([&] { red_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(table, rows, reps); }, &ms), "red_peak_kernel");
     out_host[2] = (float)((double)blocks * 256.0 * reps / (ms * 1e-3) / 1e9);
-    SVR_CUDA(ctx, timed([&] { issue_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(reinterpret_cast<unsigned int*>(sink), 0x5bd1e995u); }, &ms));
+    PEAK_CUDA(timed([&] { issue_peak_kernel<<<blocks, 256, 0, ctx->stream>>>(reinterpret_cast<unsigned int*>(sink), 0x5bd1e995u); }, &ms), "issue_peak_kernel");
     out_host[3] = (float)((double)blocks * 8.0 * PEAK_ITERS * 8.0 * 2.0 / (ms * 1e-3) / 1e9);
-    for (auto& ev : e) cudaEventDestroy(ev);
-    svr_free(ctx, table, 0);
+#undef PEAK_CUDA
     ctx->launches += 16;
-    return SVR_OK;
+    return done(cudaSuccess, "");
 }

@@ -480,6 +480,9 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
     if (opts->n_bins < 1 || opts->n_bins > MAX_BINS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_bins must be 1..%d", MAX_BINS);
     if (opts->halo < 0 || opts->halo > 8) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "halo must be 0..8 dilation steps");
     if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
+    // the keep-halo hash table has 2^k >= 2 n slots addressed with 32-bit masks: 2^31 slots at most
+    if (opts->halo > 0 && vox->n > ((int64_t)1 << 30))
+        return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "keep-halo (halo > 0) supports at most 2^30 voxels, got %lld", (long long)vox->n);
     { int ex = 0; if (!(vox->root_edge > 0.f) || std::frexp(vox->root_edge, &ex) != 0.5f) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "root_edge must be a positive power of two"); }
     *n_removed_host = 0;
     const int64_t n = vox->n;
@@ -534,8 +537,9 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
         prune_state_kernel<<<g, 256, 0, ctx->stream>>>(s, w_max, bins, delta, st, *opts, ema, state, cand, st_cap, nullptr);
     } else {
         // guard ii as a dilation: seeds -> `halo` dilation steps over the face neighbours -> candidates
-        uint32_t capn = 1024;
-        while ((int64_t)capn < 2 * n) capn <<= 1;
+        uint64_t capn64 = 1024;
+        while (capn64 < 2 * (uint64_t)n) capn64 <<= 1;          // <= 2^31: n <= 2^30 was checked above
+        const uint32_t capn = (uint32_t)capn64;
         hkb = sizeof(unsigned long long) * (size_t)capn; hvb = sizeof(uint32_t) * (size_t)capn;
         PTRY(svr_alloc(ctx, (void**)&hkeys, hkb)); PTRY(svr_alloc(ctx, (void**)&hvals, hvb));
         PTRY(svr_alloc(ctx, (void**)&prot_a, ub)); PTRY(svr_alloc(ctx, (void**)&prot_b, ub));

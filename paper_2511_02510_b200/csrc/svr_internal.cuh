@@ -12,7 +12,7 @@
 #define SVR_TILE 16
 #define SVR_MAX_K 4
 #define SVR_SCAN_SMEM_MAX (200 * 1024)   // dynamic shared memory the one-block bucket scan may use for its tile-grid table
-#define SVR_TRAV_WORDS 72     // traversal record: 32 hit masks, 32 voxel ids, slot count, 6 sub-batch E offsets (+ padding to 16 bytes)
+#define SVR_TRAV_WORDS 72     // traversal record: [0..31] hit masks, [32..63] voxel ids, [64] slot count, [65] first E row of the batch, [71] its E row count; [66..70] unused (the record is a multiple of 16 bytes)
 
 enum SvrStage {
     ST_TILE_MASKS = 0, ST_RECTS, ST_SCAN, ST_EMIT, ST_SORT, ST_RANGES, ST_COLORS, ST_FORWARD, ST_LOSS, ST_BACKWARD,
