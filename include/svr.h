@@ -228,8 +228,8 @@ int svr_num_stages(void);
 /* Experiments / tests only: bit 3 (8) selects the first list-build design (per-voxel scan + global radix sort, the
  * fallback when Morton code + voxel id exceed 64 bits); bit 4 (16): no traversal record (svr_backward walks the lists itself);
  * bit 5 (32): svr_backward ignores the recorded exp(-tau) values and recomputes them; bit 7 (128): the first recording svr_forward of a frame allocates an E
- * record of 64 rows only, so that it overflows and sets the flag that makes the backward pass recompute;
- * bit 10 (1024) prints stream idle gaps per stage. */
+ * record of 64 rows only, so that it overflows and sets the flag that makes the backward pass recompute.
+ * Other bits are ignored. */
 void svr_set_debug_flags(SvrContext* ctx, int flags);
 const char* svr_stage_name(int stage);
 SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset);

@@ -276,8 +276,6 @@ class Context:
         if st != SVR_OK:
             raise SvrError(st, "svr_create failed")
         self.handle = h
-        if os.environ.get("SVR_DEBUG_FLAGS"):      # measurement experiments only (A/B of kernel variants)
-            _lib.svr_set_debug_flags(self.handle, int(os.environ["SVR_DEBUG_FLAGS"]))
 
     def close(self):
         if self.handle:

@@ -45,6 +45,7 @@ __global__ void __launch_bounds__(256) adam_kernel(float* __restrict__ theta, fl
 
 extern "C" SvrStatus svr_adam_step(SvrContext* ctx, float* theta, float* grad, float* m, float* v, int64_t n, float lr, float beta1,
                                    float beta2, float eps, int32_t step, int32_t zero_grad) {
+    SVR_NVTX();
     if (!ctx || !theta || !grad || !m || !v) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n < 0 || step < 1) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n must be >= 0 and step >= 1");
     if (((uintptr_t)theta | (uintptr_t)grad | (uintptr_t)m | (uintptr_t)v) & 15)
@@ -82,6 +83,7 @@ __global__ void __launch_bounds__(256) scatter_corners_kernel(const float* __res
 }  // namespace
 
 extern "C" SvrStatus svr_gather_corners(SvrContext* ctx, const float* grid, const uint32_t* corner_index, int64_t n, float* raw_density) {
+    SVR_NVTX();
     if (!ctx || !grid || !corner_index || !raw_density) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n < 0 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
     if (n == 0) return SVR_OK;
@@ -94,6 +96,7 @@ extern "C" SvrStatus svr_gather_corners(SvrContext* ctx, const float* grid, cons
 
 extern "C" SvrStatus svr_scatter_add_corners(SvrContext* ctx, const float* grad_raw_density, const uint32_t* corner_index, int64_t n,
                                              float* grad_grid) {
+    SVR_NVTX();
     if (!ctx || !grad_raw_density || !corner_index || !grad_grid) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n < 0 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
     if (n == 0) return SVR_OK;
@@ -157,6 +160,7 @@ __global__ void tv_finish_kernel(const double* __restrict__ acc, int64_t n, floa
 
 extern "C" SvrStatus svr_tv_loss_grad(SvrContext* ctx, const float* raw_density, int64_t n, float lambda, float* grad_raw_density,
                                       float* loss) {
+    SVR_NVTX();
     if (!ctx || !raw_density || !grad_raw_density || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n < 1 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
     if (((uintptr_t)raw_density | (uintptr_t)grad_raw_density) & 15) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "arrays must be 16-byte aligned");

@@ -48,42 +48,19 @@ namespace {
 
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int TRAV_WORDS = SVR_TRAV_WORDS;   // words of one traversal record (forward -> backward), see composite_kernel
-constexpr int WARPS = 8;
 constexpr int NSLOT = 32;          // staged voxels per batch
-#ifndef SVR_QCAP
-#define SVR_QCAP 256
-#endif
-constexpr int QCAP = SVR_QCAP;     // queue entries per warp (a batch is cut into sub-batches whose hits fit)
-constexpr int CMAX = QCAP / 32;
+constexpr int QCAP = 256;          // queue entries per warp (a batch is cut into sub-batches whose hits fit)
 static_assert(QCAP >= 64 && QCAP <= 512 && QCAP % 32 == 0, "queue entries per lane C = QCAP / 32 <= 16 (QINV); a slot has at most 32 hits");
 constexpr int RING = 64;           // forward staging slots per warp (two halves of 32)
-#ifndef FWD_CTAW
-#define FWD_CTAW 4      // warps per CTA: the eight warps of a tile are independent (no CTA barrier), so a tile may span several CTAs
-#endif
-#ifndef BWD_CTAW
-#define BWD_CTAW 4      // replay backward; the recomputing fallback keeps whole tiles (measured: 4 is 6 % slower there)
-#endif
-#define BWD_CW(REPLAY) ((REPLAY) ? BWD_CTAW : 8)
-#ifndef BWD_MINB
-#define BWD_MINB(REPLAY) ((REPLAY) ? 5 : BWD_CTAS)     // replay: 5 x 4 warps, 94 registers (6 x 4 at 80 registers measured 3 % slower)
-#endif
-#ifndef FWD_CTAS
-#define FWD_CTAS 4
-#endif
-#ifndef FWD_MINB
-#define FWD_MINB (FWD_CTAS * (8 / FWD_CTAW))
-#endif
-#ifndef SVR_BWD_DB
-#define SVR_BWD_DB 1              // replaying backward: 1 = gather of the next batch double-buffered (3 CTAs/SM), 0 = single buffer,
-#endif                            // next batch only prefetched into L2 (4 CTAs/SM)
-#ifndef BWD_CTAS
-#define BWD_CTAS (SVR_BWD_DB ? 3 : 4)
-#endif
-constexpr int BWD_BUFS = SVR_BWD_DB ? 2 : 1;
-#ifndef EROWS_N
-#define EROWS_N 8
-#endif
-constexpr int EROWS = EROWS_N;            // E rows a backward lane fetches into registers at the start of a sub-batch
+// Launch configuration (measured alternatives: DESIGN.md section 6). The eight warps of a tile are independent (no CTA barrier),
+// so a tile may span several CTAs.
+#define FWD_CTAW 4                                      // forward: warps per CTA
+#define FWD_MINB 8                                      // forward: CTAs per SM (63 registers)
+#define BWD_CTAW 4                                      // replaying backward: warps per CTA
+#define BWD_CW(REPLAY) ((REPLAY) ? BWD_CTAW : 8)        // the self-walking fallback keeps whole tiles (4 is 6 % slower there)
+#define BWD_MINB(REPLAY) ((REPLAY) ? 5 : 3)             // replay: 5 x 4 warps, 94 registers (6 x 4 at 80 registers: 3 % slower)
+constexpr int BWD_BUFS = 2;        // replaying backward: the gather of the next batch is double-buffered
+constexpr int EROWS = 8;           // E rows a backward lane fetches into registers at the start of a sub-batch
 constexpr uint32_t ECHUNK = 16;    // the E record is handed out to warps in chunks of (at least) 16 rows of 32 floats
 
 // ceil(65536 / C): (pos * QINV[C]) >> 16 == pos / C for pos < 512, C <= 16
@@ -468,6 +445,10 @@ __global__ void __launch_bounds__(32 * FWD_CTAW, FWD_MINB) composite_kernel(CamD
             unsigned int hits = test_candidates<true>(cand, S.g0 + head, S.col + head, ray.inv, n_test);
             uint32_t eoff = 0xFFFFFFFFu;                                  // this lane's word in the E record (none: no room / no hits)
             if (REC && __any_sync(FULL, hits != 0u)) {
+                // capacity of this warp's slice of the record (launch_traversal_offsets sizes it as ceil(len / 32) + 9 per list
+                // set; re-read here rather than kept in a register). Writing past it would corrupt the next warp's records or
+                // the heap, silently: stop the kernel instead (no sanitizer run covers this path on the target machines).
+                if (n_rec >= ((trav_off[tile + 1] - trav_off[tile]) >> 3)) __trap();
                 uint32_t* r = rec_out + (size_t)n_rec * TRAV_WORDS;
                 r[lane] = hits;
                 if (lane < n) r[32 + lane] = __float_as_uint(S.g1[head + lane].w);    // the staged voxel ids
@@ -640,9 +621,6 @@ __global__ void __launch_bounds__(32 * BWD_CW(REPLAY), BWD_MINB(REPLAY)) backwar
                     __syncwarp();
                 }
                 // ---- pixel-major chain: eqs. 2-4 front to back, dL/dtau and w of every hit into the queue ----
-#ifdef SVR_DBG_SKIP
-                if (SVR_DBG_SKIP < 2)
-#endif
                 {
                     unsigned int m = mine;
                     auto chain = [&](const float e_rec) {
@@ -681,9 +659,6 @@ __global__ void __launch_bounds__(32 * BWD_CW(REPLAY), BWD_MINB(REPLAY)) backwar
                 // the slot headers are not read again in this sub-batch: Hs[k].x now collects slot k's max blending weight
                 if (want_wmax) { S.Q.Hs[lane].x = 0u; __syncwarp(); }
                 // ---- hit-major: gradients of this lane's C consecutive entries, summed in registers per voxel ----
-#ifdef SVR_DBG_SKIP
-                if (SVR_DBG_SKIP < 1)
-#endif
                 {
                     float acc[11];
 #pragma unroll
@@ -787,61 +762,32 @@ __global__ void __launch_bounds__(32 * BWD_CW(REPLAY), BWD_MINB(REPLAY)) backwar
         };
         unsigned int hits_a, hits_b = 0u;
         uint32_t misc_a, misc_b = 0u;
-        if (SVR_BWD_DB) {
-            // three headers deep: header b + 3 into L2, header b + 2 into registers (consumed one batch later, so its round
-            // trip to L2 is not waited for), voxel records of batch b + 1 gathered, batch b worked on
-            Hdr hn;
-            hn.hits = 0u; hn.vid = 0u; hn.misc = 0u;
-            {
-                const Hdr h0 = load_hdr(rec);
-                if (n_rec > 1u) hn = load_hdr(rec + TRAV_WORDS);
-                if (n_rec > 2u) prefetch_hdr(rec + 2 * TRAV_WORDS);
-                gather(h0, 0);
-                hits_a = h0.hits; misc_a = h0.misc;
-            }
-            for (uint32_t rb = 0; rb < n_rec; ++rb) {
-                const int buf = (int)(rb & 1u) * NSLOT;
-                if (rb + 1u < n_rec) {
-                    gather(hn, buf ^ NSLOT);
-                    hits_b = hn.hits; misc_b = hn.misc;
-                    if (rb + 2u < n_rec) hn = load_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
-                    if (rb + 3u < n_rec) prefetch_hdr(rec + (size_t)(rb + 3u) * TRAV_WORDS);
-                    asm volatile("cp.async.wait_group 1;" ::: "memory");
-                } else {
-                    asm volatile("cp.async.wait_group 0;" ::: "memory");
-                }
-                __syncwarp();
-                run_batch(buf, hits_a, (int)__shfl_sync(FULL, misc_a, 0), misc_a);
-                __syncwarp();
-                hits_a = hits_b; misc_a = misc_b;
-            }
-        } else {
-            // single buffer: the records of batch b + 1 are pulled into L2 while batch b is worked on and gathered after it
-            auto prefetch_records = [&](const Hdr& h) {
-                const int n = (int)__shfl_sync(FULL, h.misc, 0);
-                if (lane < n) {
-                    const char* pr = reinterpret_cast<const char*>(packed + 5 * (size_t)h.vid);
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pr));
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pr + 64));
-                }
-            };
-            Hdr h1 = load_hdr(rec);
-            gather(h1, 0);
-            hits_a = h1.hits; misc_a = h1.misc;
-            if (n_rec > 1u) prefetch_hdr(rec + TRAV_WORDS);
-            for (uint32_t rb = 0; rb < n_rec; ++rb) {
-                const bool next = rb + 1u < n_rec;
-                if (next) {
-                    h1 = load_hdr(rec + (size_t)(rb + 1u) * TRAV_WORDS);
-                    if (rb + 2u < n_rec) prefetch_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
-                    prefetch_records(h1);
-                }
+        // three headers deep: header b + 3 into L2, header b + 2 into registers (consumed one batch later, so its round
+        // trip to L2 is not waited for), voxel records of batch b + 1 gathered, batch b worked on
+        Hdr hn;
+        hn.hits = 0u; hn.vid = 0u; hn.misc = 0u;
+        {
+            const Hdr h0 = load_hdr(rec);
+            if (n_rec > 1u) hn = load_hdr(rec + TRAV_WORDS);
+            if (n_rec > 2u) prefetch_hdr(rec + 2 * TRAV_WORDS);
+            gather(h0, 0);
+            hits_a = h0.hits; misc_a = h0.misc;
+        }
+        for (uint32_t rb = 0; rb < n_rec; ++rb) {
+            const int buf = (int)(rb & 1u) * NSLOT;
+            if (rb + 1u < n_rec) {
+                gather(hn, buf ^ NSLOT);
+                hits_b = hn.hits; misc_b = hn.misc;
+                if (rb + 2u < n_rec) hn = load_hdr(rec + (size_t)(rb + 2u) * TRAV_WORDS);
+                if (rb + 3u < n_rec) prefetch_hdr(rec + (size_t)(rb + 3u) * TRAV_WORDS);
+                asm volatile("cp.async.wait_group 1;" ::: "memory");
+            } else {
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
-                __syncwarp();
-                run_batch(0, hits_a, (int)__shfl_sync(FULL, misc_a, 0), misc_a);
-                __syncwarp();
-                if (next) { gather(h1, 0); hits_a = h1.hits; misc_a = h1.misc; }
             }
+            __syncwarp();
+            run_batch(buf, hits_a, (int)__shfl_sync(FULL, misc_a, 0), misc_a);
+            __syncwarp();
+            hits_a = hits_b; misc_a = misc_b;
         }
         return;
     }

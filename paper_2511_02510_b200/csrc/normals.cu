@@ -106,6 +106,7 @@ SvrStatus swap_normals(SvrContext* ctx, const SvrFrame* f, float4* saved, int en
 extern "C" {
 
 SvrStatus svr_render_normals(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* normal, float* T_final) {
+    SVR_NVTX();
     if (!ctx || !frame || !opts || !normal) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     if (frame->packed == nullptr && frame->scene.n > 0) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "frame has no view records");
@@ -128,6 +129,7 @@ SvrStatus svr_render_normals(SvrContext* ctx, const SvrFrame* frame, const SvrRe
 
 SvrStatus svr_backward_normals(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dnormal,
                                const float* normal, float* grad_raw_density) {
+    SVR_NVTX();
     if (!ctx || !frame || !opts || !dL_dnormal || !normal || !grad_raw_density) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     const int64_t n = frame->scene.n;

@@ -74,6 +74,7 @@ __global__ void __launch_bounds__(256) red_peak_kernel(float* table, unsigned in
 }  // namespace
 
 extern "C" SvrStatus svr_measure_peaks(SvrContext* ctx, float* out_host) {
+    SVR_NVTX();
     if (!ctx || !out_host) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     SVR_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaDeviceProp prop;

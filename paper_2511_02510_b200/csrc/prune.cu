@@ -474,6 +474,7 @@ extern "C" {
 SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cams_host, int32_t n_cams, const float* w_max,
                          float* ema, uint8_t* state, const SvrPruneOpts* opts, uint8_t* keep, float* tau_host,
                          int64_t* n_removed_host) {
+    SVR_NVTX();
     if (!ctx || !vox || !cams_host || !w_max || !ema || !state || !opts || !keep || !n_removed_host)
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n_cams < 1 || n_cams > MAX_CAMS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_cams must be 1..%d", MAX_CAMS);
@@ -588,6 +589,7 @@ SvrStatus svr_prune_step(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 
 SvrStatus svr_compact_rows(SvrContext* ctx, const uint8_t* keep, int64_t n, const void* src, void* dst, int64_t row_bytes,
                            int64_t* n_out_host) {
+    SVR_NVTX();
     if (!ctx || !keep || !src || !dst) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n < 0 || n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "row count out of range");
     if (row_bytes < 1 || (row_bytes > 2 && row_bytes % 4 != 0)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "row_bytes must be 1, 2 or a multiple of 4");
@@ -631,6 +633,7 @@ SvrStatus svr_compact_rows(SvrContext* ctx, const uint8_t* keep, int64_t n, cons
 SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cams_host, int32_t n_cams,
                                const float* usefulness, const SvrSubdivOpts* opts, uint8_t* split, float* priority,
                                float* z_percentiles_host, int64_t* n_split_host) {
+    SVR_NVTX();
     if (!ctx || !vox || !cams_host || !usefulness || !opts || !split || !n_split_host)
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (n_cams < 1 || n_cams > MAX_CAMS) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "n_cams must be 1..%d", MAX_CAMS);
@@ -711,6 +714,7 @@ SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrC
 
 SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8_t* split, uint16_t* ijkl_out, float* raw_out,
                               float* sh_out, int64_t* n_out_host) {
+    SVR_NVTX();
     if (!ctx || !vox || !split || !ijkl_out || !raw_out || !sh_out) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (vox->n < 0 || vox->n >= ((int64_t)1 << 28)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
     if (n_out_host) *n_out_host = 0;

@@ -150,6 +150,7 @@ __global__ void __launch_bounds__(256) ssim_grad_kernel(const float* __restrict_
 
 extern "C" SvrStatus svr_ssim_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H, float lambda,
                                         int32_t accumulate, float* dL_dimage, float* loss) {
+    SVR_NVTX();
     if (!ctx || !render || !target || !dL_dimage || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (W <= 0 || H <= 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "empty image");
     SVR_CUDA(ctx, cudaSetDevice(ctx->device));

@@ -190,11 +190,13 @@ bool alloc_traversal_record(SvrContext* ctx, const SvrFrame* f) {
 extern "C" {
 
 SvrStatus svr_create(SvrContext** out, int device, void* cuda_stream, size_t workspace_budget_bytes) {
+    SVR_NVTX();
     return svr_create_with_allocator(out, device, cuda_stream, nullptr, nullptr, nullptr, workspace_budget_bytes);
 }
 
 SvrStatus svr_create_with_allocator(SvrContext** out, int device, void* cuda_stream, SvrAllocFn alloc_fn, SvrFreeFn free_fn, void* user,
                                     size_t workspace_budget_bytes) {
+    SVR_NVTX();
     if (!out || ((alloc_fn == nullptr) != (free_fn == nullptr))) return SVR_ERR_INVALID_ARG;
     *out = nullptr;
     SvrContext* ctx = new (std::nothrow) SvrContext();
@@ -266,6 +268,7 @@ size_t svr_workspace_peak_bytes(const SvrContext* ctx) { return ctx ? ctx->peak 
 int64_t svr_kernel_launches(const SvrContext* ctx) { return ctx ? ctx->launches : 0; }
 
 SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam, SvrFrame** out) {
+    SVR_NVTX();
     if (!ctx || !vox || !cam || !out) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     *out = nullptr;
     if (vox->n < 0 || vox->n >= ((int64_t)1 << 31)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "voxel count out of range");
@@ -461,6 +464,7 @@ SvrStatus svr_preprocess(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera*
 }
 
 SvrStatus svr_frame_refresh_colors(SvrContext* ctx, SvrFrame* frame) {
+    SVR_NVTX();
     if (!ctx || !frame) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     frame->trav_valid = false;      // termination depends on the densities: the next forward pass records again
     SVR_TRY(launch_voxel_colors(ctx, frame));
@@ -475,6 +479,7 @@ void svr_frame_release(SvrContext* ctx, SvrFrame* frame) {
 
 SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* image, float* depth,
                       float* T_final, float* w_max) {
+    SVR_NVTX();
     if (!ctx || !frame || !opts || !image) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     SVR_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -495,6 +500,7 @@ SvrStatus svr_forward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpt
 }
 
 SvrStatus svr_loss_prepare(SvrContext* ctx, const float* target, int32_t W, int32_t H, const SvrLossOpts* opts) {
+    SVR_NVTX();
     if (!ctx || !target || !opts) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (W <= 0 || H <= 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "empty image");
     if (!(opts->percentile > 0.f && opts->percentile <= 1.f)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "percentile must be in (0,1]");
@@ -504,6 +510,7 @@ SvrStatus svr_loss_prepare(SvrContext* ctx, const float* target, int32_t W, int3
 
 SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* target, int32_t W, int32_t H, float gamma,
                         const SvrLossOpts* opts, float* dL_dimage, float* loss) {
+    SVR_NVTX();
     if (!ctx || !render || !target || !opts || !dL_dimage || !loss) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (W <= 0 || H <= 0) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "empty image");
     if (!(opts->percentile > 0.f && opts->percentile <= 1.f)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "percentile must be in (0,1]");
@@ -513,6 +520,7 @@ SvrStatus svr_loss_grad(SvrContext* ctx, const float* render, const float* targe
 SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
                              const float* dL_ddepth, const float* dL_dT, const float* image, const float* depth, const float* T_final,
                              float* grad_raw_density, float* grad_sh, float* w_max) {
+    SVR_NVTX();
     if (!ctx || !frame || !opts || !dL_dimage || !image || !grad_raw_density || !grad_sh)
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if ((dL_ddepth && !depth) || (dL_dT && !T_final))
@@ -528,12 +536,14 @@ SvrStatus svr_backward_heads(SvrContext* ctx, const SvrFrame* frame, const SvrRe
 
 SvrStatus svr_backward(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, const float* dL_dimage,
                        const float* image, float* grad_raw_density, float* grad_sh, float* w_max) {
+    SVR_NVTX();
     return svr_backward_heads(ctx, frame, opts, dL_dimage, nullptr, nullptr, image, nullptr, nullptr, grad_raw_density, grad_sh, w_max);
 }
 
 SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCamera* cam_host, const SvrRenderOpts* ropts,
                               const SvrLossOpts* lopts, float gamma, const float* target_host, float* grad_raw_density,
                               float* grad_sh, float* w_max, float* loss_host, float* image_host) {
+    SVR_NVTX();
     if (!ctx || !vox || !cam_host || !ropts || !lopts || !target_host || !loss_host)
         return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     const size_t npix = (size_t)cam_host->W * cam_host->H;
@@ -573,6 +583,7 @@ SvrStatus svr_train_view_host(SvrContext* ctx, const SvrVoxels* vox, const SvrCa
 
 SvrStatus svr_frame_lists(const SvrFrame* frame, const uint64_t** keys, const uint32_t** vals, int64_t* n_entries,
                           const uint32_t** ranges, const uint16_t** rects, const uint8_t** tile_masks) {
+    SVR_NVTX();
     if (!frame) return SVR_ERR_INVALID_ARG;
     if (keys) *keys = frame->keys;
     if (vals) *vals = frame->vals;
@@ -584,6 +595,7 @@ SvrStatus svr_frame_lists(const SvrFrame* frame, const uint64_t** keys, const ui
 }
 
 SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm) {
+    SVR_NVTX();
     if (!frame || !rgbm) return SVR_ERR_INVALID_ARG;
     *rgbm = frame->rgbm;
     return SVR_OK;
@@ -591,6 +603,7 @@ SvrStatus svr_frame_colors(const SvrFrame* frame, const float** rgbm) {
 
 SvrStatus svr_forward_stats(SvrContext* ctx, const SvrFrame* frame, const SvrRenderOpts* opts, float* image,
                             uint64_t* stats_host) {
+    SVR_NVTX();
     if (!ctx || !frame || !opts || !image || !stats_host) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     if (opts->K < 1 || opts->K > SVR_MAX_K) return svr_fail(ctx, SVR_ERR_UNSUPPORTED, "K must be 1..4");
     unsigned long long* d = nullptr;
@@ -623,20 +636,9 @@ const char* svr_stage_name(int stage) {
 }
 
 SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int reset) {
+    SVR_NVTX();
     if (!ctx) return SVR_ERR_INVALID_ARG;
     SVR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    if (ctx->debug_flags & 1024) {   // measurement experiment: idle time on the stream before each stage
-        static double gap_ms[ST_COUNT] = {0};
-        static long gap_n = 0;
-        for (size_t i = 1; i < ctx->pending.size(); ++i) {
-            float t = 0.f;
-            if (cudaEventElapsedTime(&t, ctx->pending[i - 1].e1, ctx->pending[i].e0) == cudaSuccess) gap_ms[ctx->pending[i].stage] += t;
-        }
-        gap_n += 1;
-        fprintf(stderr, "gaps before stage (ms, cumulative):");
-        for (int i = 0; i < ST_COUNT; ++i) fprintf(stderr, " %s=%.3f", svr_stage_name(i), gap_ms[i]);
-        fprintf(stderr, "\n");
-    }
     for (const StagePending& p : ctx->pending) {
         float t = 0.f;
         if (cudaEventElapsedTime(&t, p.e0, p.e1) == cudaSuccess) {
@@ -656,6 +658,7 @@ SvrStatus svr_get_stage_times(SvrContext* ctx, double* ms, int64_t* calls, int r
 }
 
 SvrStatus svr_copy_to_host(SvrContext* ctx, void* dst_host, const void* src_device, size_t bytes) {
+    SVR_NVTX();
     if (!ctx || !dst_host || !src_device) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
     SVR_CUDA(ctx, cudaMemcpyAsync(dst_host, src_device, bytes, cudaMemcpyDeviceToHost, ctx->stream));
     SVR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));

@@ -7,7 +7,17 @@
 #include <unordered_map>
 #include <utility>
 #include <vector>
+#include <nvtx3/nvToolsExt.h>      // header-only NVTX v3: a no-op function-pointer test unless a profiler has injected itself
 #include "svr.h"
+
+// One NVTX range per C-ABI call: ncu --nvtx / a timeline tool shows which call a kernel belongs to.
+struct SvrNvtxRange {
+    explicit SvrNvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~SvrNvtxRange() { nvtxRangePop(); }
+    SvrNvtxRange(const SvrNvtxRange&) = delete;
+    SvrNvtxRange& operator=(const SvrNvtxRange&) = delete;
+};
+#define SVR_NVTX() SvrNvtxRange nvtx_range__(__func__)
 
 #define SVR_TILE 16
 #define SVR_MAX_K 4
