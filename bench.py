@@ -44,6 +44,33 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
+def git_blob_hash(path: str) -> str:
+    """`git hash-object` of a file (sha1 over "blob <len>\\0" + content), computed here so that no git checkout is needed."""
+    import hashlib
+    with open(path, "rb") as f:
+        data = f.read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def ncu_counters(kernel: str):
+    """Counters of one launch of a compositing kernel on full-size C4 from the committed ncu capture (profiles/r3_counters.csv,
+    see r3_counters.md): DRAM bytes, L2 reduction sectors, executed FFMA / FADD / FMUL thread instructions per elapsed cycle.
+    They are NOT measured by this run; `stale` says whether composite.cu changed since the capture (git blob hash)."""
+    path = os.path.join(ROOT, "profiles", "r3_counters.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        lines = [ln.strip() for ln in fh if ln.strip() and not ln.startswith("#")]
+    cols = lines[0].split(",")
+    for ln in lines[1:]:
+        row = dict(zip(cols, ln.split(",")))
+        if row["kernel"] == kernel:
+            now = git_blob_hash(os.path.join(ROOT, "paper_2511_02510_b200", "csrc", "composite.cu"))
+            row["stale"] = now != row["composite_cu_blob"]
+            return row
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons sampled DURING the timed region."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -257,6 +284,19 @@ def main():
                          overwrite=True)     # one view per step: gradients written, not summed (no zero fill between steps)
         fr.release()
 
+    def step_accumulate(i):
+        """The ABI's default gradient mode: svr_backward ADDS into grad_raw / grad_sh, so a one-view step zero-fills both first."""
+        k = camera_index(i, rank, len(ccams))
+        ctx.svr_loss_prepare(targets[k])
+        fr = ctx.svr_preprocess(vox, ccams[k])
+        ctx.svr_forward(fr, cfg.K, cfg.T_min, image=image, depth=depth, T_final=Tf)
+        ctx.svr_loss_grad(image, targets[k], cfg.gamma, dL=dL, loss=loss)
+        g_raw.zero_()
+        g_sh.zero_()
+        ctx.svr_backward(fr, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=w_max if cfg.emit_wmax_in_backward else None,
+                         overwrite=False)
+        fr.release()
+
     def render_step(i):
         k = camera_index(i, rank, len(ccams))
         fr = ctx.svr_preprocess(vox, ccams[k])
@@ -308,6 +348,13 @@ def main():
     ms_staged, _ = timed(step, args.steps)
     stage = ctx.svr_get_stage_times(reset=True)
     ctx.svr_set_stage_timing(False)
+
+    # ---- the same steps in the ABI's default accumulate mode, zero fill of both gradient arrays included ----
+    with torch.cuda.stream(stream):         # torch's zero fills go on the library's stream
+        for i in range(3):
+            step_accumulate(i)
+    ms_acc, _ = timed(step_accumulate, args.steps)
+    value_accumulate = aggregate_value(rays, args.steps, world, ms_acc)
 
     # ---- one pass over the cameras with w_max cleared first (the first views after a prune / subdivide step pay the
     # atomicMax of every voxel's first sighting; in steady state most hits only read) ----
@@ -364,33 +411,44 @@ def main():
     stage_ms = {k: v[0] / args.steps for k, v in stage.items() if v[1] > 0}       # per step (a stage may launch twice)
     dom = max(stage_ms, key=stage_ms.get)
     flop = {"forward_composite": FLOP_PER_FWD_HIT, "backward_composite": FLOP_PER_BWD_HIT}
+    full_c4 = args.workload == "C4" and args.n_voxels is None and args.res_scale == 1.0
+
+    def alu_roofline(kernel):
+        """FP32 roofline entry of a compositing kernel: algorithmic flops per launch / live stage time, against the FP32 peak;
+        the counters of the committed ncu capture (DRAM traffic, executed-FP32 fraction) next to it when this is full-size C4."""
+        achieved = hits * flop[kernel] / (stage_ms[kernel] * 1e-3) / 1e12
+        c = ncu_counters(kernel) if full_c4 else None
+        traffic = float(c["dram_bytes_per_launch"]) if c else None
+        red_sectors = float(c["l2_red_sectors_per_launch"]) if c else None
+        # SURVEY 8(d) fraction (i): executed FP32 thread instructions per elapsed cycle, (2 ffma + fadd + fmul) / (SMs x 128 lanes x 2)
+        frac_exec = ((2.0 * float(c["ffma_per_cycle"]) + float(c["fadd_per_cycle"]) + float(c["fmul_per_cycle"])) / (n_sm * FP32_LANES_PER_SM * 2)) if c else None
+        return {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+                "frac": achieved / fp32_peak, "traffic": traffic,
+                "frac_executed_fp32": frac_exec,
+                "traffic_source": (f"profiles/r3_counters.csv (ncu --set full capture, not this run; composite.cu blob {c['composite_cu_blob'][:12]}, "
+                                   f"{'STALE: composite.cu changed since' if c['stale'] else 'matches this build'})") if c else None,
+                "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x sm_max_mhz, clocks {peak_src}",
+                "peak_measured": micro["fp32_ffma_tflops"], "peak_measured_ffma2": micro["fp32_ffma2_tflops"],
+                "frac_of_measured_peak": achieved / micro["fp32_ffma_tflops"],
+                "issue_peak_measured_gwarp_inst_per_s": micro["issue_gwarp_inst_per_s"],
+                "l2_red_v4_peak_measured_g_per_s": micro["l2_red_v4_gops"],
+                "l2_red_sectors_per_launch": red_sectors,
+                "l2_red_rate_g_per_s": (red_sectors / (stage_ms[kernel] * 1e-3) / 1e9) if red_sectors else None,
+                "algorithmic": f"{hits:.4g} ray-voxel hits/view x {flop[kernel]:.0f} flop",
+                "kernel_ms": stage_ms[kernel], "slab_tests_per_hit": tests / max(hits, 1.0)}
+
     if dom in flop:
-        achieved = hits * flop[dom] / (stage_ms[dom] * 1e-3) / 1e12
-        # DRAM bytes and L2 reduction sectors of one launch of this kernel: NOT measured by this run, read from the committed ncu
-        # capture of this build (full-size C4 only)
-        traffic, red_sectors, tsrc = None, None, None
-        tpath = os.path.join(ROOT, "profiles", "r2_traffic.csv")
-        if os.path.exists(tpath) and args.workload == "C4" and args.n_voxels is None and args.res_scale == 1.0:
-            with open(tpath) as fh:
-                rows = {ln.split(",")[0]: ln.strip().split(",")[1:] for ln in fh.readlines()[1:] if "," in ln}
-            if dom in rows:
-                traffic, red_sectors, tsrc = float(rows[dom][0]), float(rows[dom][1]), "profiles/r2_traffic.csv (ncu --set full capture of this build, not this run)"
-        roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                    "frac": achieved / fp32_peak, "traffic": traffic, "traffic_source": tsrc,
-                    "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x sm_max_mhz, clocks {peak_src}",
-                    "peak_measured": micro["fp32_ffma_tflops"], "peak_measured_ffma2": micro["fp32_ffma2_tflops"],
-                    "frac_of_measured_peak": achieved / micro["fp32_ffma_tflops"],
-                    "issue_peak_measured_gwarp_inst_per_s": micro["issue_gwarp_inst_per_s"],
-                    "l2_red_v4_peak_measured_g_per_s": micro["l2_red_v4_gops"],
-                    "l2_red_sectors_per_launch": red_sectors,
-                    "l2_red_rate_g_per_s": (red_sectors / (stage_ms[dom] * 1e-3) / 1e9) if red_sectors else None,
-                    "algorithmic": f"{hits:.4g} ray-voxel hits/view x {flop[dom]:.0f} flop",
-                    "kernel_ms": stage_ms[dom], "slab_tests_per_hit": tests / max(hits, 1.0)}
+        roofline = alu_roofline(dom)
     else:   # an HBM-bound stage dominates (not expected): report bytes moved by the sort
         bytes_ = staged * 170.0
         achieved = bytes_ / (stage_ms[dom] * 1e-3) / 1e9
         roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": achieved / peaks["hbm_gbs"], "traffic": None, "kernel_ms": stage_ms[dom]}
+    roofline_forward = alu_roofline("forward_composite") if "forward_composite" in stage_ms else None
+    # the driver's record keeps `roofline` whole: the half of the metric that is not `value` rides in it too
+    roofline["render_fps"] = render_fps
+    roofline["peak_vram_bytes"] = peak_vram
+    roofline["step_flop_frac"] = (hits * (FLOP_PER_FWD_HIT + FLOP_PER_BWD_HIT) / (ms_total / args.steps * 1e-3) / 1e12) / fp32_peak
 
     line = {"metric": "fwd+bwd Mrays/s", "value": value, "unit": "Mrays/s", "render_fps": render_fps, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -398,17 +456,20 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "Mrays/s", "ms_per_step": ms_e2e / args.steps,
                     "h2d_bytes_per_step": int(targets_host[0].numel() * 4 + 92), "d2h_bytes_per_step": 4,
-                    "note": "svr_train_view_host: camera + target image from pinned host memory, loss read back"},
+                    "note": "svr_train_view_host: camera + target image from pinned host memory, the 4-byte loss read back; the gradients and "
+                            "w_max stay on the device by design (they feed the device-side svr_adam_step / svr_prune_step)"},
             "gpu_launches": int(launches),
             "roofline": roofline,
-            "stage_ms_per_step": stage_ms,
+            "roofline_forward": roofline_forward,
+            "value_accumulate": {"value": value_accumulate, "unit": "Mrays/s", "ms_per_step": ms_acc / args.steps,
+                                 "what": "the same step with grad_overwrite = 0 (the ABI's default: gradients accumulate) and the zero "
+                                         "fill of grad_raw / grad_sh it needs before a one-view step"},
             "ms_per_step_with_stage_timers": ms_staged / args.steps,
             "cold_w_max": {"ms_per_step": ms_cold, "what": "one pass over the cameras right after w_max was cleared (every voxel's first sighting "
                                                            "takes the atomicMax path); `value` is the steady state between two adaptation steps"},
             "work_per_view": {"hits": hits, "slab_tests": tests, "entries_staged": staged,
                               "list_entries": float(np.mean([s["entries"] for s in stats])),
                               "warp_voxel_pairs": float(np.mean([s["warp_voxel_pairs"] for s in stats]))},
-            "peak_vram_bytes": peak_vram,
             "train_iteration": {"what": "step + svr_adam_step (zero_grad) over raw and sh; outside `value`",
                                 "ms": ms_iter / args.steps, "iterations_per_s": args.steps * world / (ms_iter * 1e-3)}}
 
@@ -526,9 +587,19 @@ def main():
         oracle.build()
         n_rays = args.cpu_baseline_rays
         dt = oracle_sample_run(cfg, cams[0], n_rays, 4242)
+        # every oracle call first bins the voxels and evaluates the per-view colours of all of them, whatever the number of
+        # rays: timed on its own with a one-ray sample, so that the sample-size dependence of `value` can be read off
+        dt_setup = oracle_sample_run(cfg, cams[0], 1, 4243)
         line["cpu_baseline"] = {"value": n_rays / dt / 1e6, "unit": "Mrays/s", "cores": oracle.num_threads(), "kind": "oracle",
                                 "sample": f"{n_rays} seeded rays of camera 0 (of {rays}), bucketed fp64 oracle, forward+backward, "
-                                          f"{dt:.1f} s"}
+                                          f"{dt:.1f} s of which {dt_setup:.1f} s are the per-call set-up (binning + per-view colours of all "
+                                          f"voxels, independent of the ray count)",
+                                "setup_s": dt_setup,
+                                "value_excluding_setup": n_rays / max(dt - dt_setup, 1e-9) / 1e6}
+    # last keys of the line (the driver's record keeps the tail): the rest of BASELINE.json's metric
+    line["stage_ms_per_step"] = stage_ms
+    line["peak_vram_bytes"] = peak_vram
+    line["render_fps"] = line.pop("render_fps")
     if rank == 0:
         print(json.dumps(line))
     ctx.close()
