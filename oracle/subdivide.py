@@ -109,3 +109,23 @@ def apply_splits(scene, split: np.ndarray):
     raw = np.concatenate([scene.raw[keep], child_raws(scene.raw[par]).reshape(-1, 8)])
     sh = np.concatenate([scene.sh[keep], np.repeat(scene.sh[par], 8, axis=0)])
     return ijkl, raw, sh
+
+
+def carry_rows(rows: np.ndarray, split: np.ndarray, mode: str) -> np.ndarray:
+    """Per-voxel side state through a split ("refresh the optimizer/scheduler after topology changes"; DESIGN.md
+    reading R17). `rows` [n, ...] is any per-voxel array (EMA, hysteresis state, w_max, usefulness, Adam moments). The new
+    array follows apply_splits' order: the unsplit voxels' rows in their order, then 8 rows per split voxel grouped by parent
+    in parent order, each the parent's row (mode "copy": statistics the children inherit) or zero (mode "zero": state that
+    restarts, e.g. Adam moments of parameters that did not exist before)."""
+    if mode not in ("copy", "zero"):
+        raise ValueError(mode)
+    split = np.asarray(split, dtype=bool)
+    keep = np.flatnonzero(~split)
+    par = np.flatnonzero(split)
+    out = np.empty((keep.size + 8 * par.size,) + rows.shape[1:], dtype=rows.dtype)
+    for j, i in enumerate(keep):
+        out[j] = rows[i]
+    for j, i in enumerate(par):
+        for o in range(8):
+            out[keep.size + 8 * j + o] = rows[i] if mode == "copy" else 0
+    return out

@@ -783,6 +783,39 @@ def test_subdivide_eligibility_priority_budget():
     assert np.array_equal(r2["priority"], P)                     # degenerate range: z~ = 0
 
 
+def test_subdivide_carry_rows_hand_case_and_alignment_with_the_new_topology():
+    """oracle/subdivide.carry_rows (reading R17): a hand case typed out, and the property that makes it usable: row j of
+    the carried array belongs to voxel j of apply_splits' new voxel set (an unsplit voxel keeps its own row; a child carries its
+    parent's row, identified through the child's cell index halved) - the rows of ijkl itself serve as the carried payload."""
+    from oracle import subdivide
+    rows = np.array([[10, 11], [20, 21], [30, 31], [40, 41]], dtype=np.float32)
+    split = np.array([False, True, False, True])
+    got = subdivide.carry_rows(rows, split, "copy")
+    want = np.array([[10, 11], [30, 31]] + [[20, 21]] * 8 + [[40, 41]] * 8, dtype=np.float32)
+    np.testing.assert_array_equal(got, want)
+    got0 = subdivide.carry_rows(rows, split, "zero")
+    np.testing.assert_array_equal(got0, np.array([[10, 11], [30, 31]] + [[0, 0]] * 16, dtype=np.float32))
+    assert got0.dtype == rows.dtype
+    np.testing.assert_array_equal(subdivide.carry_rows(rows, np.zeros(4, dtype=bool), "zero"), rows)      # no split: identity
+    state = np.array([1, 0, 1, 1], dtype=np.uint8)                                                        # 1-D, one byte per voxel
+    np.testing.assert_array_equal(subdivide.carry_rows(state, split, "copy"), np.array([1, 1] + [0] * 8 + [1] * 8, dtype=np.uint8))
+    with pytest.raises(ValueError):
+        subdivide.carry_rows(rows, split, "mean")
+    # alignment with apply_splits on a mixed-level scene
+    sc = tiny_scene(321, n=8, sh_degree=1)
+    rng = np.random.default_rng(5)
+    split = rng.random(sc.n) < 0.4
+    split[0], split[1] = True, False
+    ijkl_new, _, sh_new = subdivide.apply_splits(sc, split)
+    carried = subdivide.carry_rows(sc.ijkl, split, "copy").astype(np.int64)
+    n_keep = int((~split).sum())
+    np.testing.assert_array_equal(carried[:n_keep], ijkl_new[:n_keep])
+    ch = ijkl_new[n_keep:].astype(np.int64)
+    np.testing.assert_array_equal(ch[:, :3] // 2, carried[n_keep:, :3])
+    np.testing.assert_array_equal(ch[:, 3] - 1, carried[n_keep:, 3])
+    np.testing.assert_array_equal(subdivide.carry_rows(sc.sh, split, "copy"), sh_new)      # SH is carried by copy (R12)
+
+
 def test_subdivide_children_tile_parent_and_sample_its_field():
     from oracle.subdivide import apply_splits, child_raws
     from svr_inputs import tiny_scene
