@@ -528,6 +528,53 @@ def test_full_size_windows(orc, svr, name, cam_index):
     check_lists(orc, svr, sc, cam)
 
 
+@pytest.mark.parametrize("name,cam_index", [("C3", 5), ("C4", 3), ("C5", 2)])
+def test_full_size_whole_image(orc, svr, name, cam_index):
+    """One WHOLE image of the full-size scene, in the launch configuration bench.py times (recording forward + replaying
+    backward), against the bucketed oracle on every ray: image / depth / T_final on all pixels, w_max two-sided on ALL voxels
+    (BASELINE configs[3]: "backward also emits w_max for all voxels"), and grad_raw / grad_sh for the dense dL/dC that
+    svr_loss_grad gives for a noisy target. A camera other than test_full_size_windows' (which keeps the second kernel pair)."""
+    pkg, ctx, torch = svr
+    cfg = make_config(name)
+    cam, sc = cfg.cameras[cam_index], cfg.scene
+    vox = pkg.Voxels.from_scene(sc)
+    frame = ctx.svr_preprocess(vox, cam)
+    w_max = torch.zeros(sc.n, dtype=torch.float32, device="cuda")
+    image, depth, Tf = ctx.svr_forward(frame, cfg.K, cfg.T_min, w_max=w_max, record=True)
+    ctx.synchronize()
+    ref = orc.render(sc, cam, cfg.K, mode="bucketed")
+    wm = w_max.cpu().numpy()
+    errs = dict(image=max_rel(image.cpu().numpy(), ref["image"]), T=max_rel(Tf.cpu().numpy(), ref["T_final"]),
+                depth=max_rel(depth.cpu().numpy(), ref["depth"], cfg.orbit_radius), w_max=max_rel(wm, ref["w_max"]))
+    print(f"{name} whole image {cam.W}x{cam.H}, camera {cam_index}: {errs}; voxels seen {int((ref['w_max'] > 0).sum())} of {sc.n}")
+    for k, v in errs.items():
+        assert v <= IMG_TOL, (k, errs)
+    assert np.all(wm[ref["w_max"] == 0] <= 1e-6)
+    assert (ref["w_max"] > 0).sum() > sc.n // 20
+    target = noisy_target(ref["image"], cfg.seed + 31, cfg.target_noise)
+    dL, _ = ctx.svr_loss_grad(image, torch.from_numpy(target).cuda(), cfg.gamma)
+    g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
+    g_sh = torch.zeros((sc.n, sc.n_basis, 3), dtype=torch.float32, device="cuda")
+    wb = torch.zeros(sc.n, dtype=torch.float32, device="cuda")
+    ctx.svr_backward(frame, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=wb)
+    ctx.synchronize()
+    assert np.array_equal(wb.cpu().numpy(), wm)                         # the backward pass emits the forward's w_max
+    r_raw, r_sh = orc.backward(sc, cam, cfg.K, dL.cpu().numpy().astype(np.float64), mode="bucketed")
+    e_raw, e_sh = rel_l2(g_raw.cpu().numpy(), r_raw), rel_l2(g_sh.cpu().numpy(), r_sh)
+    print(f"{name} whole image gradients: relL2 raw {e_raw:.2e}, sh {e_sh:.2e}")
+    assert e_raw <= GRAD_TOL and e_sh <= GRAD_TOL, (e_raw, e_sh)
+    frame.release()
+
+
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+def test_lists_bit_exact_every_camera_full_size(orc, svr, name):
+    """Rectangles, tile masks, keys, voxel ids and ranges bit-exact against the binning oracle on EVERY camera of the full-size
+    configs (the other full-size tests look at one camera each)."""
+    cfg = make_config(name)
+    for cam in cfg.cameras:
+        check_lists(orc, svr, cfg.scene, cam)
+
+
 def test_train_view_host_matches_the_four_calls(orc, svr):
     """svr_train_view_host (the entry point bench.py's e2e number goes through: host target in, loss out) against the oracle
     chain and against svr_preprocess -> svr_forward -> svr_loss_grad -> svr_backward on device buffers: image and loss and w_max
