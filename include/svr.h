@@ -306,6 +306,19 @@ SvrStatus svr_subdivide_select(SvrContext* ctx, const SvrVoxels* vox, const SvrC
 SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8_t* split, uint16_t* ijkl_out,
                               float* raw_out, float* sh_out, int64_t* n_out_host);
 
+/* Per-voxel side state through a split ("refresh the optimizer/scheduler after topology changes"; reading R17):
+ * svr_subdivide_apply writes the new ijkl / raw / sh; every other per-voxel array the trainer keeps (svr_prune_step's ema and
+ * state, w_max, the usefulness score, Adam moments) goes through this call with the SAME split mask, once per array, and lands
+ * in the same order: dst = the unsplit voxels' rows in their order, then 8 rows per split voxel grouped by parent in parent
+ * order, each the parent's row (SVR_ROWS_COPY_PARENT: statistics the children inherit) or zero bytes (SVR_ROWS_ZERO: state that
+ * restarts, e.g. the Adam moments of the children's new parameters). src [n] rows, dst [n + 7 * n_split] rows of row_bytes
+ * (1, 2 or a multiple of 4) each, device, not overlapping. *n_out_host (may be NULL) = n + 7 * n_split (then the call
+ * synchronises). With svr_compact_rows (prune) this lets one adaptation cycle prune -> compact -> subdivide keep its state. */
+#define SVR_ROWS_COPY_PARENT 0
+#define SVR_ROWS_ZERO 1
+SvrStatus svr_subdivide_rows(SvrContext* ctx, const uint8_t* split, int64_t n, const void* src, void* dst, int64_t row_bytes,
+                             int32_t mode, int64_t* n_out_host);
+
 /* ---- NEXT-4 (part): fused Adam over a flat float32 parameter array ("Adam state per voxel", ref. [14] P:334) ----
  * m <- b1 m + (1-b1) g; v <- b2 v + (1-b2) g g; theta <- theta - (lr (m / c1)) / (sqrt(v / c2) + eps), c1 = 1 - b1^step,
  * c2 = 1 - b2^step (fp64 on the host, rounded once); float32, each operation rounded in this order. One pass over

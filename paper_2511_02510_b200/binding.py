@@ -24,7 +24,7 @@ EXPORTS = ["svr_create", "svr_create_with_allocator", "svr_destroy", "svr_last_e
            "svr_ssim_loss_grad_static", "svr_ssim_static_max_pixels", "svr_static_last_error",
            "svr_backward", "svr_backward_heads", "svr_render_normals", "svr_backward_normals", "svr_train_view_host", "svr_frame_lists", "svr_frame_colors", "svr_copy_to_host", "svr_gamma_schedule",
            "svr_forward_stats", "svr_measure_peaks", "svr_set_stage_timing", "svr_num_stages", "svr_stage_name", "svr_get_stage_times", "svr_set_debug_flags",
-           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_adam_step",
+           "svr_prune_step", "svr_compact_rows", "svr_subdivide_select", "svr_subdivide_apply", "svr_subdivide_rows", "svr_adam_step",
            "svr_gather_corners", "svr_scatter_add_corners"]
 
 
@@ -113,6 +113,7 @@ def _load():
     lib.svr_subdivide_select.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(SvrSubdivOpts),
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
     lib.svr_subdivide_apply.argtypes = [C.c_void_p, C.POINTER(SvrVoxels), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+    lib.svr_subdivide_rows.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.POINTER(C.c_int64)]
     lib.svr_adam_step.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, C.c_int32]
     lib.svr_gather_corners.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
     lib.svr_scatter_add_corners.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
@@ -481,6 +482,18 @@ class Context:
         assert int(n_out.value) == n_new, (int(n_out.value), n_new)
         return ijkl, raw, sh
 
+
+    def svr_subdivide_rows(self, split: torch.Tensor, src: torch.Tensor, n_split: int, zero: bool = False) -> torch.Tensor:
+        """A per-voxel array (first dimension = voxels) through the split `split`: unsplit rows, then 8 rows per split voxel,
+        each the parent's row (zero=False) or zeros (zero=True). n_split = number of set entries of `split`."""
+        _dev(split, torch.uint8, "split")
+        if not (src.is_cuda and src.is_contiguous()):
+            raise ValueError("src must be a contiguous CUDA tensor")
+        n = int(src.shape[0])
+        row_bytes = src.element_size() * (src.numel() // max(n, 1))
+        dst = torch.empty((n + 7 * int(n_split),) + tuple(src.shape[1:]), dtype=src.dtype, device=src.device)
+        self._check(_lib.svr_subdivide_rows(self.handle, _p(split), n, _p(src), _p(dst), row_bytes, 1 if zero else 0, None))
+        return dst
 
     def svr_adam_step(self, theta, grad, m, v, lr: float, beta1: float, beta2: float, eps: float, step: int, zero_grad: bool = True):
         """Fused Adam over flat float32 tensors (in place)."""

@@ -446,6 +446,24 @@ __global__ void __launch_bounds__(256) subdiv_sh_kernel(int64_t n, int words, co
     for (int o = 0; o < 8; ++o) sh_out[(base + o) * words + w] = val;
 }
 
+// per-voxel side-state rows through a split (R17): one thread per (voxel, word of type T); an unsplit voxel's row moves
+// to its new index, a split voxel's 8 children get the parent's row (zero == 0) or zeros
+template <typename T>
+__global__ void __launch_bounds__(256) subdiv_rows_kernel(int64_t n, int words, const uint8_t* __restrict__ split, const uint32_t* __restrict__ offs,
+                                                          const T* __restrict__ src, T* __restrict__ dst, int zero) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t v = i / words;
+    if (v >= n) return;
+    const int w = (int)(i - v * words);
+    const uint32_t r = offs[v];
+    if (!split[v]) { dst[((size_t)v - r) * words + w] = src[i]; return; }
+    T val = T();
+    if (!zero) val = src[i];
+    const size_t base = (size_t)(n - offs[n]) + 8 * (size_t)r;
+#pragma unroll
+    for (int o = 0; o < 8; ++o) dst[(base + o) * words + w] = val;
+}
+
 SceneDev scene_of(const SvrVoxels* vox) {
     SceneDev s{};
     s.n = vox->n; s.sh_degree = vox->sh_degree; s.n_basis = (vox->sh_degree + 1) * (vox->sh_degree + 1); s.max_level = vox->max_level;
@@ -744,6 +762,48 @@ SvrStatus svr_subdivide_apply(SvrContext* ctx, const SvrVoxels* vox, const uint8
             *n_out_host = n + 7 * (int64_t)n_split;
         }
         if (e != cudaSuccess) stt = svr_fail(ctx, SVR_ERR_CUDA, "subdivide: %s", cudaGetErrorString(e));
+    }
+    svr_free(ctx, counts, eb);
+    svr_free(ctx, offs, eb);
+    return stt;
+}
+
+SvrStatus svr_subdivide_rows(SvrContext* ctx, const uint8_t* split, int64_t n, const void* src, void* dst, int64_t row_bytes,
+                             int32_t mode, int64_t* n_out_host) {
+    SVR_NVTX();
+    if (!ctx || !split || !src || !dst) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "null argument");
+    if (n < 0 || n >= ((int64_t)1 << 28)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "row count out of range");
+    if (row_bytes < 1 || (row_bytes > 2 && row_bytes % 4 != 0)) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "row_bytes must be 1, 2 or a multiple of 4");
+    if (mode != SVR_ROWS_COPY_PARENT && mode != SVR_ROWS_ZERO) return svr_fail(ctx, SVR_ERR_INVALID_ARG, "mode must be SVR_ROWS_COPY_PARENT or SVR_ROWS_ZERO");
+    if (n_out_host) *n_out_host = 0;
+    if (n == 0) return SVR_OK;
+    SVR_CUDA(ctx, cudaSetDevice(ctx->device));
+    uint32_t *counts = nullptr, *offs = nullptr;
+    const size_t eb = sizeof(uint32_t) * (size_t)(n + 1);
+    SVR_TRY(svr_alloc(ctx, (void**)&counts, eb));
+    SvrStatus stt = svr_alloc(ctx, (void**)&offs, eb);
+    if (stt != SVR_OK) { svr_free(ctx, counts, eb); return stt; }
+    split_to_counts_kernel<<<nblocks(n + 1, 256), 256, 0, ctx->stream>>>(n, split, counts);
+    stt = launch_exclusive_scan(ctx, counts, offs, n + 1);
+    if (stt == SVR_OK) {
+        const int zero = mode == SVR_ROWS_ZERO;
+        if (row_bytes == 1)
+            subdiv_rows_kernel<uint8_t><<<nblocks(n, 256), 256, 0, ctx->stream>>>(n, 1, split, offs, (const uint8_t*)src, (uint8_t*)dst, zero);
+        else if (row_bytes == 2)
+            subdiv_rows_kernel<uint16_t><<<nblocks(n, 256), 256, 0, ctx->stream>>>(n, 1, split, offs, (const uint16_t*)src, (uint16_t*)dst, zero);
+        else {
+            const int words = (int)(row_bytes / 4);
+            subdiv_rows_kernel<uint32_t><<<nblocks(n * words, 256), 256, 0, ctx->stream>>>(n, words, split, offs, (const uint32_t*)src, (uint32_t*)dst, zero);
+        }
+        ctx->launches += 2;
+        cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess && n_out_host) {
+            uint32_t n_split = 0;
+            e = cudaMemcpyAsync(&n_split, offs + n, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+            *n_out_host = n + 7 * (int64_t)n_split;
+        }
+        if (e != cudaSuccess) stt = svr_fail(ctx, SVR_ERR_CUDA, "subdivide rows: %s", cudaGetErrorString(e));
     }
     svr_free(ctx, counts, eb);
     svr_free(ctx, offs, eb);

@@ -714,6 +714,120 @@ def test_subdivide_bit_exact_and_rerender(orc, svr, name, n, use_cur):
         f0.release(); f1.release()
 
 
+def test_subdivide_rows_bit_exact(orc, svr):
+    """svr_subdivide_rows against oracle/subdivide.carry_rows: every row width class (1, 2, 4 bytes, wide rows), both modes,
+    ragged sizes, no split / all split."""
+    from oracle.subdivide import carry_rows
+    pkg, ctx, torch = svr
+    rng = np.random.default_rng(206)
+    for n, p_split in [(1, 1.0), (7, 0.5), (1000, 0.0), (1000, 1.0), (33_333, 0.13)]:
+        split_np = rng.random(n) < p_split
+        split = torch.from_numpy(split_np.astype(np.uint8)).cuda()
+        arrays = [rng.normal(size=n).astype(np.float32), rng.integers(0, 2, n).astype(np.uint8), rng.normal(size=n).astype(np.float16),
+                  rng.normal(size=(n, 8)).astype(np.float32), rng.normal(size=(n, 16, 3)).astype(np.float32),
+                  rng.integers(0, 65535, (n, 4)).astype(np.int16)]
+        for arr in arrays:
+            for zero in (False, True):
+                got = ctx.svr_subdivide_rows(split, torch.from_numpy(arr).cuda(), int(split_np.sum()), zero=zero)
+                ctx.synchronize()
+                np.testing.assert_array_equal(got.cpu().numpy(), carry_rows(arr, split_np, "zero" if zero else "copy"))
+    with pytest.raises(RuntimeError):
+        ctx.svr_subdivide_rows(split, torch.zeros((n, 3), dtype=torch.uint8, device="cuda"), 0)      # 3-byte rows
+
+
+def test_adaptation_cycle_train_prune_compact_subdivide_train(orc, svr):
+    """One whole adaptation cycle with every per-voxel array carried through both topology changes: 20 training steps
+    (hot path + svr_adam_step) -> svr_prune_step -> svr_compact_rows on all rows -> svr_subdivide_select / _apply / _rows ->
+    lists bit-exact on the new scene -> 20 more steps on the carried Adam state. Each adaptation stage is checked against its
+    oracle fed the same inputs (stage-wise: the trained parameters and the gathered w_max come from the device)."""
+    from dataclasses import replace
+    from oracle.prune import PruneOpts, prune_step
+    from oracle.subdivide import SubdivOpts, apply_splits, carry_rows, select_splits
+    from svr_inputs.scenes import perturbed_copy
+    pkg, ctx, torch = svr
+    cfg = make_config("C2", n_voxels=20_000, res_scale=0.5, n_cams=4)
+    sc, cams = cfg.scene, cfg.cameras
+    targets = []
+    for cam in cams:                                                   # config recipe: renders of a perturbed copy of the scene
+        _, f, img, *_ = gpu_forward(svr, perturbed_copy(sc, cfg.seed + 1), cam, cfg.K, cfg.T_min)
+        targets.append(img.clone())
+        f.release()
+    vox = pkg.Voxels.from_scene(sc)
+    state = {"m_raw": torch.zeros_like(vox.raw), "v_raw": torch.zeros_like(vox.raw), "m_sh": torch.zeros_like(vox.sh), "v_sh": torch.zeros_like(vox.sh),
+             "ema": torch.ones(sc.n, dtype=torch.float32, device="cuda"), "st": torch.ones(sc.n, dtype=torch.uint8, device="cuda"),
+             "w_max": torch.zeros(sc.n, dtype=torch.float32, device="cuda")}
+
+    def train(vox, state, first_step, steps):
+        g_raw, g_sh = torch.empty_like(vox.raw), torch.empty_like(vox.sh)
+        losses = []
+        for i in range(steps):
+            k = i % len(cams)
+            frame = ctx.svr_preprocess(vox, cams[k])
+            image, _, _ = ctx.svr_forward(frame, cfg.K, cfg.T_min)
+            dL, loss = ctx.svr_loss_grad(image, targets[k], cfg.gamma)
+            ctx.svr_backward(frame, cfg.K, dL, image, g_raw, g_sh, cfg.T_min, w_max=state["w_max"], overwrite=True)
+            t = first_step + i
+            ctx.svr_adam_step(vox.raw.view(-1), g_raw.view(-1), state["m_raw"].view(-1), state["v_raw"].view(-1), 0.02, 0.9, 0.999, 1e-8, t, zero_grad=False)
+            ctx.svr_adam_step(vox.sh.view(-1), g_sh.view(-1), state["m_sh"].view(-1), state["v_sh"].view(-1), 0.005, 0.9, 0.999, 1e-8, t, zero_grad=False)
+            ctx.synchronize()
+            frame.release()
+            losses.append(float(loss.item()))
+        return losses
+
+    def host_scene(vox):
+        return replace(sc, ijkl=vox.ijkl.cpu().numpy().view(np.uint16), raw=vox.raw.cpu().numpy(), sh=vox.sh.cpu().numpy())
+
+    loss_a = train(vox, state, 1, 20)
+    assert np.isfinite(loss_a).all() and np.mean(loss_a[-4:]) < np.mean(loss_a[:4]), loss_a
+
+    # ---- prune (NEXT-1) and compaction of every row ----
+    po = PruneOpts(n_bins=6, q_near=0.3, q_far=0.1, ema_alpha=1.0, m_low=0.35, m_high=0.65, kappa=0.2, w_keep=0.7, cap_fraction=0.05, halo=1)
+    go = pkg.SvrPruneOpts(po.n_bins, po.q_near, po.q_far, po.ema_alpha, po.m_low, po.m_high, po.kappa, po.w_keep, po.cap_fraction, po.halo)
+    sc1 = host_scene(vox)
+    host = {k: v.cpu().numpy() for k, v in state.items()}
+    ref = prune_step(sc1, cams, host["w_max"], host["ema"], host["st"], po)
+    keep, _, n_removed = ctx.svr_prune_step(vox, cams, state["w_max"], state["ema"], state["st"], go)
+    np.testing.assert_array_equal(keep.cpu().numpy().astype(bool), ref["keep"])
+    assert n_removed == ref["n_removed"] > 0
+    host["ema"], host["st"] = ref["ema"], ref["state"]
+    np.testing.assert_array_equal(state["ema"].cpu().numpy(), host["ema"])
+    k_np = ref["keep"]
+    vox = pkg.Voxels(ctx.svr_compact_rows(keep, vox.ijkl).clone(), ctx.svr_compact_rows(keep, vox.raw).clone(), ctx.svr_compact_rows(keep, vox.sh).clone(),
+                     sc.sh_degree, sc.max_level, sc.root_lo, sc.root_edge)
+    state = {k: ctx.svr_compact_rows(keep, v).clone() for k, v in state.items()}
+    for k in state:
+        np.testing.assert_array_equal(state[k].cpu().numpy(), host[k][k_np])
+    np.testing.assert_array_equal(vox.raw.cpu().numpy(), sc1.raw[k_np])
+
+    # ---- subdivide (NEXT-2) with the side state carried through the split ----
+    sc2 = host_scene(vox)
+    so = SubdivOpts(kappa=0.05, beta=0.3, max_level=sc.max_level, max_splits=sc2.n // 20, use_current_percentiles=True)
+    gs = pkg.SvrSubdivOpts(so.kappa, so.beta, so.max_level, so.max_splits, 1, 0.0, 0.0)
+    P = state["w_max"].cpu().numpy()
+    sref = select_splits(sc2, cams, P, so)
+    split, _, _, n_split = ctx.svr_subdivide_select(vox, cams, state["w_max"], gs)
+    np.testing.assert_array_equal(split.cpu().numpy().astype(bool), sref["split"])
+    assert n_split == int(sref["split"].sum()) > 0
+    r_ijkl, r_raw, r_sh = apply_splits(sc2, sref["split"])
+    ijkl, raw, sh = ctx.svr_subdivide_apply(vox, split, n_split)
+    np.testing.assert_array_equal(ijkl.cpu().numpy().view(np.uint16), r_ijkl)
+    np.testing.assert_array_equal(raw.cpu().numpy(), r_raw)
+    np.testing.assert_array_equal(sh.cpu().numpy(), r_sh)
+    moments = ("m_raw", "v_raw", "m_sh", "v_sh")                       # the children's parameters are new: their moments restart
+    new_state = {k: ctx.svr_subdivide_rows(split, v, n_split, zero=k in moments) for k, v in state.items()}
+    for k, v in state.items():
+        np.testing.assert_array_equal(new_state[k].cpu().numpy(), carry_rows(v.cpu().numpy(), sref["split"], "zero" if k in moments else "copy"))
+    state = new_state
+    vox = pkg.Voxels(ijkl, raw, sh, sc.sh_degree, sc.max_level, sc.root_lo, sc.root_edge)
+    assert vox.n == sc.n - n_removed + 7 * n_split
+    check_lists(orc, svr, host_scene(vox), cams[1])                    # the new set is a valid octree for the hot path
+
+    # ---- train on: the carried Adam state keeps the loss falling across the topology change ----
+    loss_b = train(vox, state, 21, 20)
+    assert np.isfinite(loss_b).all(), loss_b
+    assert np.mean(loss_b[:4]) < np.mean(loss_a[:4]) and np.mean(loss_b[-4:]) < np.mean(loss_a[-4:]), (loss_a, loss_b)
+
+
 # ---------------------------------------------------------------------------------------------
 # NEXT-3: backward through the depth and transmittance heads against the oracle
 # ---------------------------------------------------------------------------------------------
