@@ -89,7 +89,7 @@ def check_forward(orc, svr, cfg, cam, mode="bucketed"):
     return vox, frame, image, ref, errs
 
 
-def check_backward(orc, svr, cfg, cam, vox, frame, image, G, mode="bucketed"):
+def check_backward(orc, svr, cfg, cam, vox, frame, image, G, mode="bucketed", order_tol=1e-5):
     pkg, ctx, torch = svr
     sc = cfg.scene
     g_raw = torch.zeros((sc.n, 8), dtype=torch.float32, device="cuda")
@@ -109,7 +109,7 @@ def check_backward(orc, svr, cfg, cam, vox, frame, image, G, mode="bucketed"):
     o_raw, o_sh = o_raw.cpu().numpy(), o_sh.cpu().numpy()
     assert rel_l2(o_raw, r_raw) <= GRAD_TOL and rel_l2(o_sh, r_sh) <= GRAD_TOL
     # (two launches differ by the order of the float reductions only)
-    assert rel_l2(o_raw, g_raw.cpu().numpy()) <= 1e-5 and rel_l2(o_sh, g_sh.cpu().numpy()) <= 1e-5
+    assert rel_l2(o_raw, g_raw.cpu().numpy()) <= order_tol and rel_l2(o_sh, g_sh.cpu().numpy()) <= order_tol
     return e_raw, e_sh, w_max
 
 
@@ -1143,7 +1143,9 @@ def test_4k_wide_image_camera_inside_scene(orc, svr, case):
     cam = look_at_camera(tuple(pos), tuple(target), W, H, hfov_deg=[50.0, 35.0, 90.0][case])
     check_lists(orc, svr, cfg.scene, cam)
     vox, frame, image, ref, errs = check_forward(orc, svr, cfg, cam)
-    # a one-signed dL/dimage: with the camera inside a voxel, ~1e5 pixels sum into one gradient row, and a random-sign G makes
-    # that sum cancel to where two launches' float reduction orders differ by more than check_backward's 1e-5 side check
-    check_backward(orc, svr, cfg, cam, vox, frame, image, np.abs(random_image_grad(cam, 40 + case)) / (W * H))
+    # The parity bar against the oracle stays 1e-3. check_backward's side check (two launches of the kernel agree to 1e-5:
+    # only the order of the float atomics differs) is relaxed to 1e-4 here: with the camera inside a voxel ~1e5 pixels add
+    # into the same gradient row, and the order noise of an fp32 sum of N terms is ~sqrt(N) 2^-24 = 2e-5 (measured 1.0-1.2e-5).
+    # A one-signed dL/dimage keeps those sums from cancelling.
+    check_backward(orc, svr, cfg, cam, vox, frame, image, np.abs(random_image_grad(cam, 40 + case)) / (W * H), order_tol=1e-4)
     frame.release()
